@@ -1,0 +1,134 @@
+/* whp.h — C-ABI boundary of the B200-native candidate picking-plan evaluator.
+ *
+ * What the library computes (one GPU, sm_100a, no collectives):
+ *   the data-parallel hot path of subproblem 2 of the paper's NHATC-coordinated warehouse
+ *   SDO — "by evaluating the permutations of different picking sequences, can minimum
+ *   distance for the picking route be found" (§5 Eq. 2: min Σ d_i), scored
+ *   inside an NHATC subproblem  min f_ij(x) + φ(c_ij)  (§5 Eq. 3) where
+ *   c is the inconsistency between target t and response r.
+ *   The concrete definitions (geometry D0, next-fit batching D2, per-batch sets D3,
+ *   S-shape distance D4, responses D5, penalty D6, argmin D7, swap neighbourhood D8) are
+ *   the readings listed in DESIGN.md §2 (from SURVEY.md §8(c) and BASELINE.json north_star).
+ *
+ * Conventions
+ *   - Every call returns a whp_status; nothing throws or aborts. whp_last_error() gives text.
+ *   - "host" pointers are ordinary CPU memory; they are copied during the call and the
+ *     caller keeps ownership. "DEVICE" pointers are caller-owned CUDA device memory on the
+ *     ctx's device (e.g. a torch tensor's data_ptr()); the library never frees them.
+ *   - eval / argmin / apply calls are asynchronous on `cuda_stream` (a cudaStream_t passed
+ *     as void*; NULL = the legacy default stream). Argument errors are detected
+ *     synchronously before anything is launched.
+ *   - All arrays are dense, row-major, native-endian.
+ *   - A row of d_perms that is not a permutation of 0..n_orders-1 is a precondition
+ *     violation (entries outside [0,n_orders) would read out of bounds); use
+ *     whp_validate_perms when the source is untrusted.
+ *
+ * Limits (WHP_ERR_OUT_OF_RANGE beyond them): n_aisles <= 1024, slots_per_side <= 4095,
+ *   n_classes <= 256, n_orders < 2^24, total items < 2^24, cart_capacity < 2^20.
+ */
+#ifndef WHP_H
+#define WHP_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct whp_ctx whp_ctx; /* opaque; owns packed device tables and scratch */
+
+typedef enum {
+  WHP_OK = 0,
+  WHP_ERR_INVALID_ARG = 1,  /* null pointer, non-positive size, K < 1, W < 2 ...          */
+  WHP_ERR_OUT_OF_RANGE = 2, /* loc / sku / class / window outside bounds; non-finite t,v,w;
+                               a documented limit exceeded                                  */
+  WHP_ERR_CAPACITY = 3,     /* some order has more items than cart_capacity               */
+  WHP_ERR_STATE = 4,        /* eval before whp_load_orders / whp_set_penalty              */
+  WHP_ERR_CUDA = 5,         /* a CUDA runtime call failed (text in whp_last_error)        */
+  WHP_ERR_NOMEM = 6
+} whp_status;
+
+/* D0 geometry + SKU tables (BASELINE.json north_star: "whp_create_layout (aisles, slots,
+ * SKU→location assignment from category clustering)").
+ *   Location l in [0, 2*n_aisles*slots_per_side): aisle = l / (2S), slot = l % S,
+ *   depth = (slot+1)*slot_pitch; aisle length A = (S+1)*slot_pitch; aisle a at x = a*aisle_spacing;
+ *   depot at the front of depot_aisle.
+ *   sku_loc   host int32[n_skus]  location of each SKU
+ *   sku_class host int32[n_skus]  workload class (category x zone) in [0, n_classes)
+ *   cuda_device: ordinal; *out receives the new context. */
+whp_status whp_create_layout(int32_t n_aisles, int32_t slots_per_side, int32_t slot_pitch,
+                             int32_t aisle_spacing, int32_t depot_aisle, int32_t n_skus,
+                             const int32_t* sku_loc, const int32_t* sku_class,
+                             int32_t n_classes, int32_t cuda_device, whp_ctx** out);
+
+/* D1 orders in CSR form. order_ptr host int32[n_orders+1], strictly increasing from 0;
+ * item_sku host int32[order_ptr[n_orders]] (an order may repeat a SKU, each repeat is one
+ * item). Every order must satisfy q_o <= cart_capacity (else WHP_ERR_CAPACITY, reading Q5).
+ * Packs the per-order and per-pick device tables; may be called again to replace them. */
+whp_status whp_load_orders(whp_ctx* ctx, int32_t n_orders, const int32_t* order_ptr,
+                           const int32_t* item_sku, int32_t cart_capacity);
+
+/* D6 penalty parameters: targets t, multipliers v, weights w; host double[n_classes] each,
+ * all finite. May be called again (the NHATC outer loop updates them). */
+whp_status whp_set_penalty(whp_ctx* ctx, const double* t, const double* v, const double* w);
+
+/* a1–a5: evaluate n_cand candidate plans. d_perms DEVICE int32[n_cand][n_orders].
+ * Outputs, DEVICE, each nullable (a NULL output is simply not written):
+ *   d_dist        int64 [n_cand]            D   = Σ_b dist_b              (D4)
+ *   d_penalty     double[n_cand]            φ                              (D6)
+ *   d_obj         double[n_cand]            J   = (double)D + φ            (D6)
+ *   d_n_batches   int32 [n_cand]                                           (D2)
+ *   d_batch_hash  uint64[n_cand]            Σ_b (start_pos_b+1)(2b+1) mod 2^64 (D2)
+ *   d_batch_of_pos int32[n_cand][n_orders]  batch index of every position  (D2)
+ *   d_n_distinct  int32 [n_cand]            Σ_b |distinct locations of b|  (D3)
+ *   d_resp        int32 [n_cand][n_classes] r_k                            (D5)
+ * n_cand == 0 is a no-op returning WHP_OK. */
+whp_status whp_eval_candidates(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,
+                               int64_t* d_dist, double* d_penalty, double* d_obj,
+                               int32_t* d_n_batches, uint64_t* d_batch_hash,
+                               int32_t* d_batch_of_pos, int32_t* d_n_distinct,
+                               int32_t* d_resp, void* cuda_stream);
+
+/* Same computation through HOST buffers (the end-to-end path): h_perms host
+ * int32[n_cand][n_orders]; h_dist / h_obj host arrays [n_cand] (nullable). Permutations are
+ * copied to the device in chunks overlapped with evaluation; results are copied back; the
+ * call returns after everything has completed. Pinned host memory makes the copies
+ * asynchronous, pageable memory works but serialises. */
+whp_status whp_eval_candidates_host(whp_ctx* ctx, const int32_t* h_perms, int64_t n_cand,
+                                    int64_t* h_dist, double* h_obj,
+                                    int64_t* h_argmin_idx, double* h_argmin_val);
+
+/* a6 (D8): all W(W-1)/2 pairwise swaps of positions inside [win_start, win_start+win_len)
+ * of d_base_perm (DEVICE int32[n_orders]); neighbour n <-> (i',j'), 0 <= i' < j' < W,
+ * n = i'(2W-i'-1)/2 + (j'-i'-1); value = D2–D6 of the swapped sequence. Only the batches a
+ * swap can affect are rescored. d_dist int64 / d_obj double DEVICE [W(W-1)/2], nullable. */
+whp_status whp_eval_swaps(whp_ctx* ctx, const int32_t* d_base_perm, int32_t win_start,
+                          int32_t win_len, int64_t* d_dist, double* d_obj, void* cuda_stream);
+
+/* a7 (D7): index of the minimum of d_obj[0..n), ties -> lowest index. d_idx int64*, d_val
+ * double* are DEVICE scalars (d_val nullable). n must be >= 1. */
+whp_status whp_argmin(whp_ctx* ctx, const double* d_obj, int64_t n, int64_t* d_idx,
+                      double* d_val, void* cuda_stream);
+
+/* D8 trajectory step: decode neighbour *d_idx (DEVICE int64, as written by whp_argmin over
+ * a whp_eval_swaps result with the same window) and exchange the two positions of
+ * d_base_perm in place, on the device, so a search loop needs no host round trip. */
+whp_status whp_apply_swap(whp_ctx* ctx, int32_t* d_base_perm, int32_t win_start,
+                          int32_t win_len, const int64_t* d_idx, void* cuda_stream);
+
+/* Debug helper: *h_n_bad (host) receives the number of rows of d_perms that are not a
+ * permutation of 0..n_orders-1. Synchronises the stream. */
+whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,
+                              int64_t* h_n_bad, void* cuda_stream);
+
+/* Kernel launches issued by this ctx since creation (bench.py's gpu_launches claim). */
+int64_t whp_launch_count(const whp_ctx* ctx);
+
+void whp_destroy(whp_ctx* ctx);
+const char* whp_last_error(const whp_ctx* ctx); /* "" when none; valid until next call */
+const char* whp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WHP_H */

@@ -1,0 +1,18 @@
+"""TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+ctypes marshalling for oracle/whp_oracle.c (the plain single-threaded CPU restatement of the
+hot path). Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this package; the product package never does.
+"""
+from .binding import (  # noqa: F401
+    argmin,
+    batch_distance,
+    build,
+    decode_neighbour,
+    eval_candidate_batches,
+    eval_candidates,
+    eval_swaps,
+    optimal_route,
+    penalty,
+    swap_trajectory,
+)

@@ -1,0 +1,154 @@
+"""ctypes marshalling for whp_oracle.c — no arithmetic of the method lives here."""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "whp_oracle.c")
+_SO = os.path.join(_HERE, "libwhp_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off: every fp64 * and + individually rounded (reading Q12)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.check_call(
+            ["gcc", "-O2", "-std=c99", "-ffp-contract=off", "-fno-fast-math", "-shared",
+             "-fPIC", "-o", _SO, _SRC])
+    return _SO
+
+
+class _Geom(C.Structure):
+    _fields_ = [("n_aisles", C.c_int32), ("slots_per_side", C.c_int32),
+                ("slot_pitch", C.c_int32), ("aisle_spacing", C.c_int32),
+                ("depot_aisle", C.c_int32)]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_batch_distance.restype = C.c_int64
+        _lib.orc_optimal_route.restype = C.c_int64
+        _lib.orc_penalty.restype = C.c_double
+        _lib.orc_argmin.restype = C.c_int64
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _geom(g):
+    """g: any object with the five geometry attributes (e.g. workloads.Problem), or a 5-tuple
+    (n_aisles, slots_per_side, slot_pitch, aisle_spacing, depot_aisle)."""
+    if hasattr(g, "n_aisles"):
+        return _Geom(int(g.n_aisles), int(g.slots_per_side), int(g.slot_pitch),
+                     int(g.aisle_spacing), int(g.depot_aisle))
+    return _Geom(*[int(x) for x in g])
+
+
+def batch_distance(geom, locs) -> int:
+    locs = _i32(locs)
+    return int(_load().orc_batch_distance(C.byref(_geom(geom)), _p(locs), C.c_int32(len(locs))))
+
+
+def optimal_route(geom, locs) -> int:
+    locs = _i32(locs)
+    return int(_load().orc_optimal_route(C.byref(_geom(geom)), _p(locs), C.c_int32(len(locs))))
+
+
+def penalty(r, t, v, w) -> float:
+    r, t, v, w = _i32(r), _f64(t), _f64(v), _f64(w)
+    return float(_load().orc_penalty(C.c_int32(len(r)), _p(r), _p(t), _p(v), _p(w)))
+
+
+def argmin(x) -> int:
+    x = _f64(x)
+    return int(_load().orc_argmin(_p(x), C.c_int64(len(x))))
+
+
+def decode_neighbour(W: int, n: int):
+    i, j = C.c_int32(), C.c_int32()
+    _load().orc_decode_neighbour(C.c_int32(W), C.c_int64(n), C.byref(i), C.byref(j))
+    return i.value, j.value
+
+
+def _common(pb):
+    keep = (_i32(pb.sku_loc), _i32(pb.sku_class), _i32(pb.order_ptr), _i32(pb.item_sku),
+            _f64(pb.t), _f64(pb.v), _f64(pb.w))
+    g = _geom(pb)
+    args = [C.byref(g), _p(keep[0]), _p(keep[1]), C.c_int32(pb.n_classes),
+            C.c_int32(pb.n_orders), _p(keep[2]), _p(keep[3]), C.c_int32(pb.cart_capacity),
+            _p(keep[4]), _p(keep[5]), _p(keep[6])]
+    return args, (keep, g)
+
+
+def eval_candidates(pb, perms, detail: bool = False) -> dict:
+    """D1–D6 for every row of perms. detail=True also returns batch_of_pos and resp."""
+    perms = _i32(perms)
+    if perms.ndim == 1:
+        perms = perms[None, :]
+    n_cand, n = perms.shape
+    assert n == pb.n_orders
+    out = {
+        "dist": np.zeros(n_cand, np.int64), "penalty": np.zeros(n_cand, np.float64),
+        "obj": np.zeros(n_cand, np.float64), "n_batches": np.zeros(n_cand, np.int32),
+        "batch_hash": np.zeros(n_cand, np.uint64), "n_distinct": np.zeros(n_cand, np.int32),
+        "batch_of_pos": np.zeros((n_cand, n), np.int32) if detail else None,
+        "resp": np.zeros((n_cand, pb.n_classes), np.int32) if detail else None,
+    }
+    args, keep = _common(pb)
+    _load().orc_eval_candidates(*args, _p(perms), C.c_int64(n_cand), _p(out["dist"]),
+                                _p(out["penalty"]), _p(out["obj"]), _p(out["n_batches"]),
+                                _p(out["batch_hash"]), _p(out["batch_of_pos"]),
+                                _p(out["n_distinct"]), _p(out["resp"]))
+    del keep
+    return out
+
+
+def eval_candidate_batches(pb, perm):
+    """Per-batch S-shape lengths of one plan (for the brute-force bound P3)."""
+    perm = _i32(perm)
+    nb = C.c_int32()
+    bd = np.zeros(pb.n_orders, np.int64)
+    bop = np.zeros(pb.n_orders, np.int32)
+    args, keep = _common(pb)
+    _load().orc_eval_candidate(*args, _p(perm), None, None, None, C.byref(nb), None, _p(bop),
+                               None, None, _p(bd))
+    del keep
+    return bd[:nb.value].copy(), bop
+
+
+def eval_swaps(pb, base_perm, win_start: int, win_len: int) -> dict:
+    base_perm = _i32(base_perm)
+    nn = win_len * (win_len - 1) // 2
+    out = {"dist": np.zeros(nn, np.int64), "obj": np.zeros(nn, np.float64)}
+    args, keep = _common(pb)
+    _load().orc_eval_swaps(*args, _p(base_perm), C.c_int32(win_start), C.c_int32(win_len),
+                           _p(out["dist"]), _p(out["obj"]))
+    del keep
+    return out
+
+
+def swap_trajectory(pb, base_perm, W: int, stride: int, n_iter: int) -> dict:
+    perm = _i32(base_perm).copy()
+    out = {"move": np.zeros(n_iter, np.int64), "dist": np.zeros(n_iter, np.int64),
+           "obj": np.zeros(n_iter, np.float64)}
+    args, keep = _common(pb)
+    _load().orc_swap_trajectory(*args, _p(perm), C.c_int32(W), C.c_int32(stride),
+                                C.c_int32(n_iter), _p(out["move"]), _p(out["dist"]),
+                                _p(out["obj"]))
+    del keep
+    out["perm"] = perm
+    return out

@@ -1,0 +1,295 @@
+/* whp_oracle.c — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded C restatement of what the hot path computes, written from the
+ * paper and the readings in DESIGN.md §2 (SURVEY.md §8(c) D0–D8). It shares no code with the
+ * CUDA path (paper_2110_13693_b200/csrc) and neither includes the other. Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may call it.
+ *
+ * Every set is built by sort + unique (no bitmasks), every swapped permutation is
+ * materialised and re-evaluated from scratch, and nothing is blocked, fused or reordered
+ * beyond what the definitions state. Build: gcc -O2 -ffp-contract=off -std=c99 (oracle/build.py).
+ *
+ * Passages followed
+ *   PAPER.md:125–132 (§5 Eq. 2)  subproblem 2: min Σ d_i over picking sequences; δ = f(d)
+ *   PAPER.md:154–162 (§5 Eq. 3)  NHATC subproblem: min f(x) + φ(c), c = inconsistency(t, r)
+ *   BASELINE.json north_star      greedy cart batches, dedup, S-shape, φ = v·c + ‖w∘c‖², argmin
+ *
+ * Pin status: D0/D4 pinned by closed forms + brute-force optimal route (P1–P4, E1–E3);
+ * D2 by batching invariants (P5) and E4–E6; D5/D6 by E4–E6, K=1 closed form and a long-double
+ * cross-sum (P6, P8); D7 by P9; D8 by E6 and by equality with materialised permutations (P7).
+ * "Parity unpinned" BY THE PAPER (it prints no formula for them): the choice of r_k (Q9), the
+ * geometry constants (Q2–Q3) — they are pinned only to DESIGN.md's readings and hand-worked
+ * examples.
+ */
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct {
+  int32_t n_aisles;       /* NA */
+  int32_t slots_per_side; /* S  */
+  int32_t slot_pitch;     /* p  */
+  int32_t aisle_spacing;  /* P  */
+  int32_t depot_aisle;    /* a0 */
+} orc_geom;
+
+/* ---- D0 geometry ------------------------------------------------------------------- */
+static int32_t loc_aisle(const orc_geom* g, int32_t loc) { return loc / (2 * g->slots_per_side); }
+static int32_t loc_depth(const orc_geom* g, int32_t loc) {
+  return (loc % g->slots_per_side + 1) * g->slot_pitch;
+}
+static int64_t aisle_len(const orc_geom* g) {
+  return (int64_t)(g->slots_per_side + 1) * g->slot_pitch;
+}
+static int64_t iabs64(int64_t x) { return x < 0 ? -x : x; }
+
+/* D0 walking metric between points (a1,y1), (a2,y2): same aisle -> |y1-y2|, else cross over
+ * the nearer of the front (y=0) and back (y=A) cross-aisles. This is what Dijkstra
+ * returns in this graph. */
+static int64_t walk(const orc_geom* g, int32_t a1, int64_t y1, int32_t a2, int64_t y2) {
+  if (a1 == a2) return iabs64(y1 - y2);
+  int64_t A = aisle_len(g);
+  int64_t front = y1 + y2, back = 2 * A - y1 - y2;
+  return iabs64((int64_t)a1 - a2) * g->aisle_spacing + (front < back ? front : back);
+}
+
+static int cmp_i32(const void* a, const void* b) {
+  int32_t x = *(const int32_t*)a, y = *(const int32_t*)b;
+  return (x > y) - (x < y);
+}
+/* sort + unique in place, returns the number of distinct values */
+static int32_t sort_unique(int32_t* v, int32_t n) {
+  if (n == 0) return 0;
+  qsort(v, (size_t)n, sizeof(int32_t), cmp_i32);
+  int32_t m = 1;
+  for (int32_t i = 1; i < n; i++)
+    if (v[i] != v[m - 1]) v[m++] = v[i];
+  return m;
+}
+
+/* ---- D3 + D4: S-shape length of one batch given its pick locations (repeats allowed) -- */
+int64_t orc_batch_distance(const orc_geom* g, const int32_t* locs, int32_t n) {
+  if (n <= 0) return 0;
+  int32_t* aisles = (int32_t*)malloc(sizeof(int32_t) * (size_t)n);
+  for (int32_t i = 0; i < n; i++) aisles[i] = loc_aisle(g, locs[i]);
+  int32_t m = sort_unique(aisles, n); /* V_b */
+  int32_t a_min = aisles[0], a_max = aisles[m - 1];
+  free(aisles);
+  int64_t D_last = 0; /* deepest pick in the last visited aisle */
+  for (int32_t i = 0; i < n; i++)
+    if (loc_aisle(g, locs[i]) == a_max && loc_depth(g, locs[i]) > D_last)
+      D_last = loc_depth(g, locs[i]);
+  int64_t a0 = g->depot_aisle, P = g->aisle_spacing, A = aisle_len(g);
+  int64_t H = P * (iabs64(a0 - a_min) + (a_max - a_min) + iabs64(a_max - a0));
+  int64_t Vt = (m % 2 == 0) ? (int64_t)m * A : (int64_t)(m - 1) * A + 2 * D_last;
+  return H + Vt;
+}
+
+/* ---- P3: exhaustive optimal closed tour from the depot through the DISTINCT locations --- */
+static void perm_search(const orc_geom* g, const int32_t* a, const int64_t* y, int32_t n,
+                        uint32_t used, int32_t last_a, int64_t last_y, int64_t len, int32_t cnt,
+                        int64_t* best) {
+  if (len >= *best) return;
+  if (cnt == n) {
+    int64_t tot = len + walk(g, last_a, last_y, g->depot_aisle, 0);
+    if (tot < *best) *best = tot;
+    return;
+  }
+  for (int32_t i = 0; i < n; i++)
+    if (!(used & (1u << i)))
+      perm_search(g, a, y, n, used | (1u << i), a[i], y[i],
+                  len + walk(g, last_a, last_y, a[i], y[i]), cnt + 1, best);
+}
+/* returns -1 if more than 10 distinct points (too slow to enumerate) */
+int64_t orc_optimal_route(const orc_geom* g, const int32_t* locs, int32_t n) {
+  if (n <= 0) return 0;
+  int32_t* u = (int32_t*)malloc(sizeof(int32_t) * (size_t)n);
+  memcpy(u, locs, sizeof(int32_t) * (size_t)n);
+  int32_t m = sort_unique(u, n);
+  /* two sides of one slot are the same walking point: dedupe on (aisle, depth) */
+  int32_t a[16];
+  int64_t y[16];
+  int32_t k = 0;
+  for (int32_t i = 0; i < m; i++) {
+    int32_t ai = loc_aisle(g, u[i]);
+    int64_t yi = loc_depth(g, u[i]);
+    int dup = 0;
+    for (int32_t j = 0; j < k; j++)
+      if (a[j] == ai && y[j] == yi) dup = 1;
+    if (!dup) {
+      if (k == 10) { free(u); return -1; }
+      a[k] = ai; y[k] = yi; k++;
+    }
+  }
+  free(u);
+  int64_t best = INT64_MAX;
+  perm_search(g, a, y, k, 0u, g->depot_aisle, 0, 0, 0, &best);
+  return best;
+}
+
+/* ---- D6 penalty: φ = Σ_k v_k c_k + (w_k c_k)^2, c = t - r, canonical 32-lane sum --------- */
+double orc_penalty(int32_t K, const int32_t* r, const double* t, const double* v,
+                   const double* w) {
+  double s[32], s2[32];
+  for (int l = 0; l < 32; l++) s[l] = 0.0;
+  for (int32_t k = 0; k < K; k++) {
+    double c = t[k] - (double)r[k];
+    double u = w[k] * c;
+    double lin = v[k] * c;
+    double sq = u * u;
+    double term = lin + sq;
+    s[k % 32] = s[k % 32] + term;
+  }
+  for (int off = 16; off >= 1; off /= 2) {
+    for (int l = 0; l < 32; l++) s2[l] = s[l] + s[l ^ off];
+    for (int l = 0; l < 32; l++) s[l] = s2[l];
+  }
+  return s[0];
+}
+
+/* ---- D1–D6: one candidate plan --------------------------------------------------------- */
+/* Outputs (all nullable): dist, penalty, obj, n_batches, batch_hash, batch_of_pos[n_orders],
+ * n_distinct, resp[K], batch_dist[<= n_orders] (per-batch S-shape length, first n_batches). */
+int32_t orc_eval_candidate(const orc_geom* g, const int32_t* sku_loc, const int32_t* sku_class,
+                           int32_t K, int32_t n_orders, const int32_t* order_ptr,
+                           const int32_t* item_sku, int32_t C, const double* t, const double* v,
+                           const double* w, const int32_t* perm, int64_t* dist, double* penalty,
+                           double* obj, int32_t* n_batches, uint64_t* batch_hash,
+                           int32_t* batch_of_pos, int32_t* n_distinct, int32_t* resp,
+                           int64_t* batch_dist) {
+  int32_t* bop = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n_orders > 0 ? n_orders : 1));
+  /* D2 next-fit */
+  int32_t b = 0, load = 0;
+  for (int32_t pos = 0; pos < n_orders; pos++) {
+    int32_t o = perm[pos];
+    int32_t q = order_ptr[o + 1] - order_ptr[o];
+    if (load > 0 && load + q > C) { b++; load = 0; }
+    bop[pos] = b;
+    load += q;
+  }
+  int32_t nb = n_orders > 0 ? b + 1 : 0;
+
+  int32_t* r = (int32_t*)calloc((size_t)K, sizeof(int32_t));
+  int32_t n_items = order_ptr[n_orders];
+  int32_t* locs = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n_items > 0 ? n_items : 1));
+  int32_t* cls = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n_items > 0 ? n_items : 1));
+  int64_t D = 0;
+  uint64_t hash = 0;
+  int32_t ndist = 0;
+  int32_t pos = 0;
+  for (int32_t bb = 0; bb < nb; bb++) {
+    int32_t start = pos, n = 0;
+    while (pos < n_orders && bop[pos] == bb) { /* D3: gather the batch's picks */
+      int32_t o = perm[pos];
+      for (int32_t it = order_ptr[o]; it < order_ptr[o + 1]; it++) {
+        locs[n] = sku_loc[item_sku[it]];
+        cls[n] = sku_class[item_sku[it]];
+        n++;
+      }
+      pos++;
+    }
+    hash += (uint64_t)(start + 1) * (uint64_t)(2 * (int64_t)bb + 1);
+    int64_t db = orc_batch_distance(g, locs, n); /* D4 */
+    if (batch_dist) batch_dist[bb] = db;
+    D += db;
+    ndist += sort_unique(locs, n);    /* |L_b| */
+    int32_t kc = sort_unique(cls, n); /* K_b  */
+    for (int32_t i = 0; i < kc; i++) r[cls[i]] += 1; /* D5 */
+  }
+  double phi = orc_penalty(K, r, t, v, w);
+  if (dist) *dist = D;
+  if (penalty) *penalty = phi;
+  if (obj) *obj = (double)D + phi;
+  if (n_batches) *n_batches = nb;
+  if (batch_hash) *batch_hash = hash;
+  if (n_distinct) *n_distinct = ndist;
+  if (batch_of_pos) memcpy(batch_of_pos, bop, sizeof(int32_t) * (size_t)n_orders);
+  if (resp) memcpy(resp, r, sizeof(int32_t) * (size_t)K);
+  free(bop); free(r); free(locs); free(cls);
+  return 0;
+}
+
+/* many candidates, perms[n_cand][n_orders]; every output array nullable */
+int32_t orc_eval_candidates(const orc_geom* g, const int32_t* sku_loc, const int32_t* sku_class,
+                            int32_t K, int32_t n_orders, const int32_t* order_ptr,
+                            const int32_t* item_sku, int32_t C, const double* t, const double* v,
+                            const double* w, const int32_t* perms, int64_t n_cand, int64_t* dist,
+                            double* penalty, double* obj, int32_t* n_batches,
+                            uint64_t* batch_hash, int32_t* batch_of_pos, int32_t* n_distinct,
+                            int32_t* resp) {
+  for (int64_t c = 0; c < n_cand; c++)
+    orc_eval_candidate(g, sku_loc, sku_class, K, n_orders, order_ptr, item_sku, C, t, v, w,
+                       perms + c * n_orders, dist ? dist + c : 0, penalty ? penalty + c : 0,
+                       obj ? obj + c : 0, n_batches ? n_batches + c : 0,
+                       batch_hash ? batch_hash + c : 0,
+                       batch_of_pos ? batch_of_pos + c * n_orders : 0,
+                       n_distinct ? n_distinct + c : 0, resp ? resp + c * K : 0, 0);
+  return 0;
+}
+
+/* ---- D7 argmin: smallest index attaining the minimum ------------------------------------ */
+int64_t orc_argmin(const double* x, int64_t n) {
+  int64_t best = 0;
+  for (int64_t i = 1; i < n; i++)
+    if (x[i] < x[best]) best = i;
+  return best;
+}
+
+/* ---- D8 swap neighbourhood: materialise each swapped permutation, evaluate from scratch - */
+int32_t orc_eval_swaps(const orc_geom* g, const int32_t* sku_loc, const int32_t* sku_class,
+                       int32_t K, int32_t n_orders, const int32_t* order_ptr,
+                       const int32_t* item_sku, int32_t C, const double* t, const double* v,
+                       const double* w, const int32_t* base_perm, int32_t win_start,
+                       int32_t win_len, int64_t* dist, double* obj) {
+  int32_t* p = (int32_t*)malloc(sizeof(int32_t) * (size_t)n_orders);
+  int64_t n = 0;
+  for (int32_t i = 0; i < win_len; i++)
+    for (int32_t j = i + 1; j < win_len; j++) { /* lexicographic (i', j') */
+      memcpy(p, base_perm, sizeof(int32_t) * (size_t)n_orders);
+      int32_t tmp = p[win_start + i];
+      p[win_start + i] = p[win_start + j];
+      p[win_start + j] = tmp;
+      orc_eval_candidate(g, sku_loc, sku_class, K, n_orders, order_ptr, item_sku, C, t, v, w, p,
+                         dist ? dist + n : 0, 0, obj ? obj + n : 0, 0, 0, 0, 0, 0, 0);
+      n++;
+    }
+  free(p);
+  return 0;
+}
+
+/* neighbour index -> (i', j') by counting rows, the inverse of n = i'(2W-i'-1)/2 + (j'-i'-1) */
+void orc_decode_neighbour(int32_t W, int64_t n, int32_t* i_out, int32_t* j_out) {
+  int32_t i = 0;
+  int64_t row = W - 1;
+  while (n >= row) { n -= row; row--; i++; }
+  *i_out = i;
+  *j_out = i + 1 + (int32_t)n;
+}
+
+/* D8 trajectory (config 4): window s_it = (it*stride) mod (n_orders-W+1); always apply the
+ * argmin move. perm is updated in place; records move[it], D[it], J[it] of the applied move. */
+int32_t orc_swap_trajectory(const orc_geom* g, const int32_t* sku_loc, const int32_t* sku_class,
+                            int32_t K, int32_t n_orders, const int32_t* order_ptr,
+                            const int32_t* item_sku, int32_t C, const double* t, const double* v,
+                            const double* w, int32_t* perm, int32_t W, int32_t stride,
+                            int32_t n_iter, int64_t* move, int64_t* move_dist, double* move_obj) {
+  int64_t nn = (int64_t)W * (W - 1) / 2;
+  int64_t* dist = (int64_t*)malloc(sizeof(int64_t) * (size_t)nn);
+  double* obj = (double*)malloc(sizeof(double) * (size_t)nn);
+  for (int32_t it = 0; it < n_iter; it++) {
+    int32_t s = (int32_t)(((int64_t)it * stride) % (n_orders - W + 1));
+    orc_eval_swaps(g, sku_loc, sku_class, K, n_orders, order_ptr, item_sku, C, t, v, w, perm, s,
+                   W, dist, obj);
+    int64_t best = orc_argmin(obj, nn);
+    int32_t i, j;
+    orc_decode_neighbour(W, best, &i, &j);
+    int32_t tmp = perm[s + i];
+    perm[s + i] = perm[s + j];
+    perm[s + j] = tmp;
+    move[it] = best;
+    move_dist[it] = dist[best];
+    move_obj[it] = obj[best];
+  }
+  free(dist); free(obj);
+  return 0;
+}

@@ -1,0 +1,384 @@
+"""Pins for the oracle (CPU only): closed forms, invariants, brute force, hand-worked examples.
+
+Each test cites the definition (DESIGN.md §2 / SURVEY.md §8(c)) it pins. Nothing here touches
+the CUDA path. The helpers below are deliberately written in a different style from
+oracle/whp_oracle.c (python sets, itertools, exact rationals) so that a shared mistake is
+unlikely.
+"""
+import itertools
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2110_13693_b200 import workloads as W
+
+TINY = (4, 10, 1, 3, 0)  # NA, S, pitch, spacing, depot (BASELINE.json configs[1])
+
+
+# ---------- independent helpers (tests only) -------------------------------------------------
+def _point(geom, loc):
+    NA, S, p, P, a0 = geom
+    return loc // (2 * S), (loc % S + 1) * p
+
+
+def _walk(geom, u, v):
+    """D0 metric written from the layout picture: same aisle -> along it; else out through the
+    nearer cross-aisle (front y=0, back y=A), across, and in."""
+    NA, S, p, P, a0 = geom
+    A = (S + 1) * p
+    (a1, y1), (a2, y2) = u, v
+    if a1 == a2:
+        return abs(y1 - y2)
+    return abs(a1 - a2) * P + min(y1 + y2, (A - y1) + (A - y2))
+
+
+def _brute_route(geom, locs):
+    pts = sorted({_point(geom, l) for l in locs})
+    depot = (geom[4], 0)
+    best = None
+    for order in itertools.permutations(pts):
+        tour = [depot, *order, depot]
+        d = sum(_walk(geom, tour[i], tour[i + 1]) for i in range(len(tour) - 1))
+        best = d if best is None or d < best else best
+    return best
+
+
+def _py_plan(pb, perm):
+    """D1-D5 with python sets; returns (batch_of_pos, per-batch loc lists, r)."""
+    q = np.diff(pb.order_ptr)
+    bop, b, load = [], 0, 0
+    for o in perm:
+        if load > 0 and load + q[o] > pb.cart_capacity:
+            b, load = b + 1, 0
+        bop.append(b)
+        load += q[o]
+    batches = [[] for _ in range(b + 1)]
+    classes = [set() for _ in range(b + 1)]
+    for pos, o in enumerate(perm):
+        for it in range(pb.order_ptr[o], pb.order_ptr[o + 1]):
+            sku = pb.item_sku[it]
+            batches[bop[pos]].append(int(pb.sku_loc[sku]))
+            classes[bop[pos]].add(int(pb.sku_class[sku]))
+    r = [sum(1 for cs in classes if k in cs) for k in range(pb.n_classes)]
+    return bop, batches, r
+
+
+def _exact_penalty(r, t, v, w):
+    """phi as an exact rational (fp64 inputs are rationals), then rounded once."""
+    tot = Fraction(0)
+    for rk, tk, vk, wk in zip(r, t, v, w):
+        c = Fraction(float(tk)) - int(rk)
+        tot += Fraction(float(vk)) * c + (Fraction(float(wk)) * c) ** 2
+    return tot
+
+
+def _golden_problem(golden):
+    g, pp = golden["geometry"], golden["plan_problem"]
+    ptr = np.cumsum([0] + [len(o) for o in pp["orders"]])
+    return W.Problem(
+        n_aisles=g["n_aisles"], slots_per_side=g["slots_per_side"], slot_pitch=g["slot_pitch"],
+        aisle_spacing=g["aisle_spacing"], depot_aisle=g["depot_aisle"],
+        sku_loc=np.array(pp["sku_loc"], np.int32), sku_class=np.array(pp["sku_class"], np.int32),
+        n_classes=pp["n_classes"], order_ptr=ptr.astype(np.int32),
+        item_sku=np.array([s for o in pp["orders"] for s in o], np.int32),
+        cart_capacity=pp["cart_capacity"], t=np.array(pp["t"]), v=np.array(pp["v"]),
+        w=np.array(pp["w"]))
+
+
+# ---------- E1-E6: hand-worked examples -------------------------------------------------------
+def test_golden_batches(golden):
+    geom = tuple(golden["geometry"][k] for k in
+                 ("n_aisles", "slots_per_side", "slot_pitch", "aisle_spacing", "depot_aisle"))
+    for ex in golden["batches"]:
+        assert oracle.batch_distance(geom, ex["locs"]) == ex["dist"], ex["id"]
+        assert oracle.optimal_route(geom, ex["locs"]) == ex["optimal"], ex["id"]
+        assert _brute_route(geom, ex["locs"]) == ex["optimal"], ex["id"]
+
+
+def test_golden_plans(golden):
+    pb = _golden_problem(golden)
+    perms = np.array([p["perm"] for p in golden["plans"]], np.int32)
+    out = oracle.eval_candidates(pb, perms, detail=True)
+    for i, ex in enumerate(golden["plans"]):
+        assert out["batch_of_pos"][i].tolist() == ex["batch_of_pos"], ex["id"]
+        assert int(out["dist"][i]) == ex["dist"], ex["id"]
+        assert out["resp"][i].tolist() == ex["resp"], ex["id"]
+        assert out["penalty"][i] == ex["penalty"], ex["id"]  # dyadic data: exact in any order
+        assert out["obj"][i] == ex["obj"], ex["id"]
+        assert int(out["batch_hash"][i]) == ex["batch_hash"], ex["id"]
+        assert int(out["n_batches"][i]) == len(ex["batch_dist"]), ex["id"]
+        bd, _ = oracle.eval_candidate_batches(pb, perms[i])
+        assert bd.tolist() == ex["batch_dist"], ex["id"]
+        if "n_distinct" in ex:
+            assert int(out["n_distinct"][i]) == ex["n_distinct"]
+        if "batch_optimal" in ex:
+            _, batches, _ = _py_plan(pb, perms[i])
+            geom = (pb.n_aisles, pb.slots_per_side, pb.slot_pitch, pb.aisle_spacing,
+                    pb.depot_aisle)
+            assert [oracle.optimal_route(geom, b) for b in batches] == ex["batch_optimal"]
+    assert oracle.argmin(out["obj"][:2]) == golden["argmin_E4_E5"]
+
+
+def test_golden_swap_E6(golden):
+    pb = _golden_problem(golden)
+    e4, e6 = golden["plans"][0], golden["plans"][2]
+    s, Wn = e6["window"]
+    sw = oracle.eval_swaps(pb, np.array(e4["perm"], np.int32), s, Wn)
+    n = e6["neighbour_index"]
+    assert oracle.decode_neighbour(Wn, n) == tuple(e6["pair"])
+    assert int(sw["dist"][n]) == e6["dist"] and sw["obj"][n] == e6["obj"]
+
+
+# ---------- P1/P2: closed forms of D4 (north_star) ---------------------------------------------
+@pytest.mark.parametrize("geom", [TINY, (20, 50, 1, 3, 0), (7, 13, 2, 5, 0)])
+def test_single_aisle_closed_form(geom):
+    NA, S, p, P, a0 = geom
+    for loc in range(2 * NA * S):
+        a, depth = loc // (2 * S), (loc % S + 1) * p
+        assert oracle.batch_distance(geom, [loc]) == 2 * a * P + 2 * depth
+        # one aisle, several picks: out to the deepest and back — also the true optimum
+        other = (loc // S) * S + (loc * 7 + 3) % S
+        deepest = max(depth, (other % S + 1) * p)
+        assert oracle.batch_distance(geom, [loc, other, loc]) == 2 * a * P + 2 * deepest
+        if loc % 17 == 0:
+            assert oracle.optimal_route(geom, [loc, other]) == 2 * a * P + 2 * deepest
+
+
+def test_even_aisles_full_traversals_only():
+    geom = (20, 50, 1, 3, 0)
+    NA, S, p, P, a0 = geom
+    A = (S + 1) * p
+    rng = np.random.default_rng(1)
+    for _ in range(300):
+        m = int(rng.choice([2, 4, 6, 8]))
+        aisles = rng.choice(NA, size=m, replace=False)
+        locs = []
+        for a in aisles:
+            for _ in range(int(rng.integers(1, 4))):
+                locs.append(int(a) * 2 * S + int(rng.integers(0, 2 * S)))
+        d = oracle.batch_distance(geom, locs)
+        assert d == 2 * int(aisles.max()) * P + m * A  # independent of every depth
+        # adding a pick in a visited aisle that is not the last one never changes it
+        not_last = int(np.sort(aisles)[0])
+        assert oracle.batch_distance(geom, locs + [not_last * 2 * S + 3]) == d
+
+
+def test_odd_aisles_last_aisle_return():
+    geom = (20, 50, 1, 3, 0)
+    NA, S, p, P, a0 = geom
+    A = (S + 1) * p
+    rng = np.random.default_rng(2)
+    for _ in range(300):
+        m = int(rng.choice([1, 3, 5, 7]))
+        aisles = np.sort(rng.choice(NA, size=m, replace=False))
+        locs, deepest_last = [], 0
+        for a in aisles:
+            for _ in range(int(rng.integers(1, 4))):
+                slot = int(rng.integers(0, S))
+                locs.append(int(a) * 2 * S + int(rng.integers(0, 2)) * S + slot)
+                if a == aisles[-1]:
+                    deepest_last = max(deepest_last, (slot + 1) * p)
+        assert oracle.batch_distance(geom, locs) == (2 * int(aisles[-1]) * P + (m - 1) * A
+                                                     + 2 * deepest_last)
+
+
+def test_nonzero_depot_horizontal_term():
+    # D4's H for a depot in the middle: out to the leftmost, across, back from the rightmost
+    geom = (9, 6, 1, 4, 4)
+    S, P, A = 6, 4, 7
+    locs = [2 * 2 * S + 1, 7 * 2 * S + 2]  # aisles 2 and 7, m = 2
+    assert oracle.batch_distance(geom, locs) == P * ((4 - 2) + (7 - 2) + (7 - 4)) + 2 * A
+    locs = [6 * 2 * S + 1]  # single aisle right of the depot, depth 2
+    assert oracle.batch_distance(geom, locs) == P * (2 + 0 + 2) + 2 * 2
+
+
+# ---------- P3: S-shape >= exhaustive optimum; metric cross-checked --------------------------
+def test_sshape_not_below_optimal_on_every_tiny_batch():
+    wl = W.make_workload("tiny")
+    pb = wl.problem
+    perms = W.perms(wl.seed, pb.n_orders, wl.n_cand)
+    n_checked = 0
+    for c in range(wl.n_cand):
+        bd, _ = oracle.eval_candidate_batches(pb, perms[c])
+        _, batches, _ = _py_plan(pb, perms[c])
+        assert len(bd) == len(batches)
+        for d, locs in zip(bd, batches):
+            opt = oracle.optimal_route(TINY, locs)
+            assert opt >= 0 and d >= opt  # cart capacity 8 => at most 8 distinct locations
+            n_checked += 1
+            if c < 4:  # the C enumeration against the itertools one
+                assert opt == _brute_route(TINY, locs)
+    assert n_checked > 400
+
+
+def test_optimal_route_matches_itertools_on_random_sets():
+    rng = np.random.default_rng(3)
+    geom = (6, 8, 2, 5, 0)
+    for _ in range(60):
+        locs = rng.integers(0, 2 * 6 * 8, size=int(rng.integers(1, 7))).tolist()
+        assert oracle.optimal_route(geom, locs) == _brute_route(geom, locs)
+        assert oracle.batch_distance(geom, locs) >= _brute_route(geom, locs)
+
+
+# ---------- P4: invariances of dist_b ---------------------------------------------------------
+def test_batch_distance_invariances():
+    rng = np.random.default_rng(4)
+    geom = (20, 50, 1, 3, 0)
+    S = 50
+    for _ in range(200):
+        locs = rng.integers(0, 2000, size=int(rng.integers(1, 25)))
+        d = oracle.batch_distance(geom, locs)
+        assert oracle.batch_distance(geom, rng.permutation(locs)) == d
+        assert oracle.batch_distance(geom, np.concatenate([locs, locs[:3]])) == d
+        flipped = (locs // (2 * S)) * 2 * S + (1 - (locs % (2 * S)) // S) * S + locs % S
+        assert oracle.batch_distance(geom, flipped) == d
+
+
+# ---------- P5: batching invariants -------------------------------------------------------------
+@pytest.mark.parametrize("name", ["tiny", "mid"])
+def test_batching_invariants(name):
+    wl = W.make_workload(name)
+    pb = wl.problem
+    n = min(wl.n_cand, 48)
+    perms = W.perm_rows(wl.seed, pb.n_orders, np.arange(n))
+    out = oracle.eval_candidates(pb, perms, detail=True)
+    q = np.diff(pb.order_ptr)
+    C = pb.cart_capacity
+    for c in range(n):
+        bop = out["batch_of_pos"][c]
+        assert bop[0] == 0 and np.all(np.diff(bop) >= 0) and np.all(np.diff(bop) <= 1)
+        nb = int(out["n_batches"][c])
+        assert nb == bop[-1] + 1 and nb >= -(-pb.n_items // C)
+        loads = np.bincount(bop, weights=q[perms[c]], minlength=nb).astype(int)
+        assert loads.max() <= C and loads.min() >= 1
+        starts = np.flatnonzero(np.diff(bop, prepend=-1))
+        for b in range(nb - 1):  # greedy: the next order did not fit
+            assert loads[b] + q[perms[c][starts[b + 1]]] > C
+        assert int(out["batch_hash"][c]) == sum((int(s) + 1) * (2 * b + 1)
+                                                for b, s in enumerate(starts)) % (1 << 64)
+        # P8: responses recounted with sets; per-candidate python restatement
+        pbop, batches, r = _py_plan(pb, perms[c])
+        assert pbop == bop.tolist() and r == out["resp"][c].tolist()
+        assert max(r) <= nb and sum(r) >= nb
+        assert int(out["n_distinct"][c]) == sum(len(set(b)) for b in batches)
+        assert int(out["dist"][c]) == sum(oracle.batch_distance(pb, b) for b in batches)
+
+
+def test_one_big_cart_is_permutation_invariant():
+    pb = W.make_problem("tiny")
+    pb.cart_capacity = pb.n_items
+    perms = W.perm_rows(0, pb.n_orders, np.arange(16))
+    out = oracle.eval_candidates(pb, perms)
+    assert np.all(out["n_batches"] == 1) and len(set(out["dist"].tolist())) == 1
+    all_locs = pb.sku_loc[pb.item_sku]
+    assert int(out["dist"][0]) == oracle.batch_distance(pb, all_locs)
+
+
+def test_every_order_fills_the_cart():
+    pb = W.make_problem("tiny")
+    q = 3
+    n_orders = 12
+    pb.order_ptr = (np.arange(n_orders + 1) * q).astype(np.int32)
+    pb.item_sku = (W.stream_u64(5, 77, n_orders * q) % np.uint64(pb.n_skus)).astype(np.int32)
+    pb.cart_capacity = q
+    perms = W.perm_rows(1, n_orders, np.arange(8))
+    out = oracle.eval_candidates(pb, perms)
+    per_order = sum(oracle.batch_distance(pb, pb.sku_loc[pb.item_sku[o * q:(o + 1) * q]])
+                    for o in range(n_orders))
+    assert np.all(out["n_batches"] == n_orders) and np.all(out["dist"] == per_order)
+
+
+# ---------- P6: penalty ---------------------------------------------------------------------------
+def test_penalty_closed_forms():
+    assert oracle.penalty([3], [5.0], [0.5], [0.25]) == 0.5 * 2.0 + (0.25 * 2.0) ** 2  # K = 1
+    r = np.arange(40, dtype=np.int32)
+    assert oracle.penalty(r, r.astype(float), np.ones(40), np.ones(40)) == 0.0  # t = r
+    assert oracle.penalty(r, r + 1.0, np.zeros(40), np.zeros(40)) == 0.0  # v = w = 0
+    # sign of c = t - r: a response above target with v > 0, w = 0 gives a NEGATIVE linear term
+    assert oracle.penalty([4], [1.0], [2.0], [0.0]) == -6.0
+    assert oracle.penalty([4], [1.0], [0.0], [2.0]) == 36.0  # (w c)^2, not w c^2
+
+
+@pytest.mark.parametrize("K", [1, 4, 20, 31, 32, 33, 200, 256])
+def test_penalty_against_exact_rational(K):
+    rng = np.random.default_rng(K)
+    for scale in ("unit", "log"):
+        r = rng.integers(0, 400, size=K).astype(np.int32)
+        t = rng.uniform(0, 400, size=K)
+        v = rng.uniform(0, 1, size=K) if scale == "unit" else 10 ** rng.uniform(-3, 3, K)
+        w = rng.uniform(0, 1, size=K) if scale == "unit" else 10 ** rng.uniform(-3, 3, K)
+        exact = _exact_penalty(r, t, v, w)
+        mag = sum(abs(float(vk * (tk - rk))) + float(wk * (tk - rk)) ** 2
+                  for rk, tk, vk, wk in zip(r, t, v, w))
+        assert abs(Fraction(oracle.penalty(r, t, v, w)) - exact) <= Fraction(1e-12) * Fraction(mag)
+
+
+def test_objective_is_distance_plus_penalty():
+    wl = W.make_workload("mid")
+    pb = wl.problem
+    perms = W.perm_rows(0, pb.n_orders, np.arange(8))
+    out = oracle.eval_candidates(pb, perms, detail=True)
+    for c in range(8):
+        assert out["penalty"][c] == oracle.penalty(out["resp"][c], pb.t, pb.v, pb.w)
+        assert out["obj"][c] == float(out["dist"][c]) + out["penalty"][c]
+    pb.v = np.zeros_like(pb.v)
+    pb.w = np.zeros_like(pb.w)
+    out0 = oracle.eval_candidates(pb, perms)
+    assert np.all(out0["obj"] == out0["dist"].astype(float))
+
+
+# ---------- P7: swap neighbourhood ------------------------------------------------------------------
+def test_swaps_equal_materialised_permutations():
+    wl = W.make_workload("mid")
+    pb = wl.problem
+    base = W.base_perm(0, pb.n_orders)
+    s, Wn = 37, 12
+    sw = oracle.eval_swaps(pb, base, s, Wn)
+    base_out = oracle.eval_candidates(pb, base, detail=True)
+    q = np.diff(pb.order_ptr)
+    n = 0
+    for i in range(Wn):
+        for j in range(i + 1, Wn):
+            assert oracle.decode_neighbour(Wn, n) == (i, j)
+            assert n == i * (2 * Wn - i - 1) // 2 + (j - i - 1)
+            p = base.copy()
+            p[s + i], p[s + j] = p[s + j], p[s + i]
+            one = oracle.eval_candidates(pb, p)
+            assert sw["dist"][n] == one["dist"][0] and sw["obj"][n] == one["obj"][0]
+            bop = base_out["batch_of_pos"][0]
+            first_of_batch = s + i == 0 or bop[s + i - 1] != bop[s + i]
+            if bop[s + i] == bop[s + j] and not first_of_batch:
+                # both orders inside one batch, and the batch's opening order unchanged (a
+                # smaller opening order could slip into the previous cart): nothing changes
+                assert sw["obj"][n] == base_out["obj"][0]
+            if q[base[s + i]] == q[base[s + j]]:
+                assert one["n_batches"][0] == base_out["n_batches"][0]
+            n += 1
+
+
+def test_trajectory_applies_argmin_each_iteration():
+    pb = W.make_problem("tiny")
+    base = W.base_perm(0, pb.n_orders)
+    tr = oracle.swap_trajectory(pb, base, 6, 3, 5)
+    perm = base.copy()
+    for it in range(5):
+        s = (it * 3) % (pb.n_orders - 6 + 1)
+        sw = oracle.eval_swaps(pb, perm, s, 6)
+        best = int(np.argmin(sw["obj"]))  # numpy: first minimum
+        assert tr["move"][it] == best and tr["obj"][it] == sw["obj"][best]
+        i, j = oracle.decode_neighbour(6, best)
+        perm[s + i], perm[s + j] = perm[s + j], perm[s + i]
+    assert perm.tolist() == tr["perm"].tolist()
+
+
+# ---------- P9: argmin ----------------------------------------------------------------------------------
+def test_argmin_first_minimum():
+    assert oracle.argmin(np.full(17, 3.25)) == 0
+    x = np.array([5.0, 2.0, 7.0, 2.0, 2.0, 9.0])
+    assert oracle.argmin(x) == 1
+    rng = np.random.default_rng(9)
+    for _ in range(50):
+        x = rng.integers(0, 6, size=int(rng.integers(1, 40))).astype(float)
+        assert oracle.argmin(x) == int(np.argmin(x))
