@@ -1,0 +1,269 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the candidate picking-plan evaluation path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+        --master-port P bench.py --gpus N --steps K --warmup W
+
+A step is one pass of the whole hot path (SURVEY.md §8(a) rows a1–a7) on the paper-scale
+workload (BASELINE.json configs[2] + configs[3], "paper" / "neighbourhood" in workloads.py):
+    whp_eval_candidates on 16,384 candidate plans (a1–a5)  -> whp_argmin (a7)
+    whp_eval_swaps on the 32,640-neighbour window of the trajectory plan (a6) -> whp_argmin
+    -> whp_apply_swap (the trajectory of configs[3] advances one iteration per step).
+`value` = candidate plans per second over the whole step, inputs resident in HBM. Multi-GPU:
+candidates are independent, so each rank evaluates its own 16,384 plans (weak scaling), no
+data-path collective; time = max over ranks. `--impl reference` times the oracle (oracle/, a
+plain single-threaded CPU program) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2110_13693_b200 import harness, workloads as W  # noqa: E402
+
+WORKLOAD = "paper"  # BASELINE.json configs[2] (the third listed): the config the metric is quoted on
+CPU_SAMPLE = 8192   # candidates the oracle is timed on for cpu_baseline (~12 s on one core)
+REF_SAMPLE = 512    # candidates per step of --impl reference
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the candidate kernel, from the
+# ncu --set full capture recorded in profiles/ (None until measured for the current kernel)
+NCU_TRAFFIC_BYTES = None
+
+
+def config_dict(pb, n_cand, world, wl_nb):
+    return {"workload": "paper-scale (BASELINE.json configs[3rd]): 400 aisles x 250 slots/side, "
+                        "100k SKUs, Zipf(1.0), K=200",
+            "n_orders": pb.n_orders, "n_items": pb.n_items, "cart_capacity": pb.cart_capacity,
+            "candidates_per_gpu": n_cand, "global_candidates": n_cand * world,
+            "neighbourhood": {"window": wl_nb.window, "stride": wl_nb.stride,
+                              "neighbours": wl_nb.window * (wl_nb.window - 1) // 2},
+            "parallelism": f"candidates sharded x{world}, tables replicated, no collective",
+            "l2": "permutation input 262 MB per step > 126 MB L2 (no flush needed)"}
+
+
+def run_reference(args):
+    """The oracle as it stands, single thread, on the box's host cores; rank 0 only."""
+    rank, _, world = harness.dist_env()
+    if rank != 0:
+        return 0
+    import oracle
+    wl = W.make_workload(WORKLOAD)
+    pb = wl.problem
+    wl_nb = W.make_workload("neighbourhood")
+    n = REF_SAMPLE
+    perms = W.perm_rows(wl.seed, pb.n_orders, np.arange(n))
+
+    def step():
+        out = oracle.eval_candidates(pb, perms)
+        return oracle.argmin(out["obj"])
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    value = n * args.steps / dt
+    line = {
+        "impl": "reference", "metric": "candidate_plans_per_s", "value": value,
+        "unit": "candidate plans/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "int64+f64", "data": "synthetic",
+        "picks_per_s": value * pb.n_items,
+        "config": config_dict(pb, wl.n_cand, 1, wl_nb),
+        "cpu_baseline": {"value": value, "unit": "candidate plans/s", "cores": 1,
+                         "kind": "oracle",
+                         "sample": f"{n} of the 16,384 paper-scale candidates per step "
+                                   "(a1-a5 + argmin; the swap neighbourhood is not in the sample)"},
+        "e2e": {"value": value, "unit": "candidate plans/s", "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: there is no CPU fallback "
+                           "(use --impl reference for the oracle arm)")
+    from paper_2110_13693_b200 import whp
+    rank, local_rank, world = harness.init_dist("nccl")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+
+    wl = W.make_workload(WORKLOAD)
+    wl_nb = W.make_workload("neighbourhood")
+    pb = wl.problem
+    n, n_cand = pb.n_orders, wl.n_cand
+    ctx = whp.Context.from_problem(pb, device=local_rank)
+    lo, hi = harness.weak_rows(n_cand, rank)
+    perms = W.perms_torch(wl.seed, n, lo, hi, dev)  # resident in HBM before the clock starts
+    dist = torch.zeros(n_cand, dtype=torch.int64, device=dev)
+    pen = torch.zeros(n_cand, dtype=torch.float64, device=dev)
+    obj = torch.zeros(n_cand, dtype=torch.float64, device=dev)
+    nbat = torch.zeros(n_cand, dtype=torch.int32, device=dev)
+    bhash = torch.zeros(n_cand, dtype=torch.int64, device=dev)
+    idx = torch.zeros(1, dtype=torch.int64, device=dev)
+    val = torch.zeros(1, dtype=torch.float64, device=dev)
+    Wn, stride = wl_nb.window, wl_nb.stride
+    nn = Wn * (Wn - 1) // 2
+    base = torch.from_numpy(W.base_perm(wl.seed + rank, n)).to(dev)
+    sdist = torch.zeros(nn, dtype=torch.int64, device=dev)
+    sobj = torch.zeros(nn, dtype=torch.float64, device=dev)
+    sidx = torch.zeros(1, dtype=torch.int64, device=dev)
+    it_counter = [0]
+    k_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+            for _ in range(args.steps)]
+    s_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+            for _ in range(args.steps)]
+
+    def step(timed_index=None):
+        if timed_index is not None:
+            k_ev[timed_index][0].record()
+        ctx.eval_candidates(perms, dist=dist, penalty=pen, obj=obj, n_batches=nbat,
+                            batch_hash=bhash)
+        if timed_index is not None:
+            k_ev[timed_index][1].record()
+        ctx.argmin(obj, idx, val)
+        s = (it_counter[0] * stride) % (n - Wn + 1)
+        if timed_index is not None:
+            s_ev[timed_index][0].record()
+        ctx.eval_swaps(base, s, Wn, dist=sdist, obj=sobj)
+        if timed_index is not None:
+            s_ev[timed_index][1].record()
+        ctx.argmin(sobj, sidx)
+        ctx.apply_swap(base, s, Wn, sidx)
+        it_counter[0] += 1
+
+    def timed_run():
+        sampler = harness.ClockSampler(local_rank, 50).start().wait_first() if rank == 0 else None
+        if sampler:
+            sampler.mark()  # warm-up and timed steps are both "under load"
+        for _ in range(args.warmup):
+            step()
+        torch.cuda.synchronize()
+        harness.barrier(world)
+        launches0 = ctx.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for k in range(args.steps):
+            step(k)
+        e1.record()
+        torch.cuda.synchronize()
+        harness.barrier(world)
+        ms = e0.elapsed_time(e1)
+        clocks = sampler.stop() if sampler else None
+        return ms, clocks, ctx.launch_count() - launches0
+
+    ms, clocks, launches = timed_run()
+    redo = harness.max_over_ranks(1.0 if (rank == 0 and harness.clocks_rejected(clocks)) else 0.0,
+                                  world, dev)
+    remeasured = False
+    if redo > 0:
+        ms, clocks, launches = timed_run()
+        remeasured = True
+    ms = harness.max_over_ranks(ms, world, dev)
+    k_ms = float(np.mean([a.elapsed_time(b) for a, b in k_ev]))
+    s_ms = float(np.mean([a.elapsed_time(b) for a, b in s_ev]))
+    k_ms_max = harness.max_over_ranks(k_ms, world, dev)
+    ms_per_step = ms / args.steps
+    value = n_cand * world / (ms_per_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry point (pinned host memory) ---------------
+    h_perms = torch.empty((n_cand, n), dtype=torch.int32).pin_memory()
+    h_perms.copy_(perms)
+    h_dist = torch.zeros(n_cand, dtype=torch.int64).pin_memory()
+    h_obj = torch.zeros(n_cand, dtype=torch.float64).pin_memory()
+    for _ in range(max(1, min(args.warmup, 2))):
+        ctx.eval_candidates_host(h_perms, h_dist, h_obj)
+    torch.cuda.synchronize()
+    harness.barrier(world)
+    e2e_steps = max(1, min(args.steps, 10))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e_idx, e_val = ctx.eval_candidates_host(h_perms, h_dist, h_obj)
+    torch.cuda.synchronize()
+    e2e_s = harness.max_over_ranks(time.perf_counter() - t0, world, dev)
+    harness.barrier(world)
+    e2e_value = n_cand * world * e2e_steps / e2e_s
+    torch.cuda.synchronize()
+    same = bool(np.array_equal(h_obj.numpy(), obj.cpu().numpy()) and e_idx == int(idx.item()))
+
+    # ---- roofline of the dominant kernel (candidate evaluation) -----------------------------
+    bytes_pc = harness.algorithmic_bytes_per_candidate(n, pb.n_items)
+    peaks = harness.measured_peaks(ROOT)
+    achieved = bytes_pc["survey"] * n_cand / (k_ms_max * 1e-3) / 1e9
+    roofline = {
+        "bound": "hbm", "kernel": "whp_eval_candidates", "achieved": achieved,
+        "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
+        "traffic": NCU_TRAFFIC_BYTES, "peak_source": peaks["source"] + ", burst copy figure",
+        "bytes_per_candidate": bytes_pc["survey"], "kernel_ms": k_ms_max,
+        "kernel_share_of_step": k_ms_max / ms_per_step,
+        "frac_packed_bytes": bytes_pc["packed"] * n_cand / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"],
+        "frac_hbm_compulsory": bytes_pc["hbm_compulsory"] * n_cand / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"],
+    }
+
+    if rank != 0:
+        return 0
+    # ---- CPU baseline: the oracle on a bounded sample, rank 0 at N=1 only -------------------
+    cpu = None
+    if world == 1:
+        import oracle
+        sample = W.perm_rows(wl.seed, n, np.arange(CPU_SAMPLE))
+        t0 = time.perf_counter()
+        ref = oracle.eval_candidates(pb, sample)
+        oracle.argmin(ref["obj"])
+        dt = time.perf_counter() - t0
+        agree = bool(np.array_equal(ref["obj"], obj[:CPU_SAMPLE].cpu().numpy())
+                     and np.array_equal(ref["dist"], dist[:CPU_SAMPLE].cpu().numpy()))
+        cpu = {"value": CPU_SAMPLE / dt, "unit": "candidate plans/s", "cores": 1,
+               "kind": "oracle", "seconds": dt,
+               "sample": f"first {CPU_SAMPLE} of the 16,384 candidates (a1-a5 + argmin), single "
+                         "thread, gcc -O2",
+               "gpu_results_equal_oracle_on_sample": agree}
+    line = {
+        "metric": "candidate_plans_per_s", "value": value, "unit": "candidate plans/s",
+        "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "int64+f64", "data": "synthetic",
+        "picks_per_s": value * pb.n_items,
+        "config": config_dict(pb, n_cand, world, wl_nb),
+        "neighbourhood": {"ms_per_iteration_eval_swaps": s_ms,
+                          "neighbours_per_s": nn / (s_ms * 1e-3)},
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "e2e": {"value": e2e_value, "unit": "candidate plans/s",
+                "h2d_bytes_per_step": int(h_perms.numel() * 4),
+                "d2h_bytes_per_step": int(n_cand * 16 + 16),
+                "api": "whp_eval_candidates_host (pinned host buffers, chunked copy/compute overlap)",
+                "matches_device_path": same},
+        "gpu_launches": int(launches),
+        "clocks": clocks, "remeasured_for_clocks": remeasured,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)  # timing rule: at least 3 warm-up steps
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,346 @@
+// whp_api.cu — the extern "C" boundary (include/whp.h): argument checking, table packing,
+// device memory owned by the context, and dispatch to the kernel launchers. No arithmetic of
+// the method happens on the host: the host only validates and packs inputs.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "whp_internal.cuh"
+
+namespace {
+
+whp_status fail(whp_ctx* c, whp_status s, const char* msg) {
+  if (c) c->err = msg;
+  return s;
+}
+whp_status cuda_fail(whp_ctx* c, cudaError_t e, const char* where) {
+  if (c) c->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return e == cudaErrorMemoryAllocation ? WHP_ERR_NOMEM : WHP_ERR_CUDA;
+}
+#define WHP_CUDA(c, call)                                        \
+  do {                                                           \
+    cudaError_t e_ = (call);                                     \
+    if (e_ != cudaSuccess) return cuda_fail((c), e_, #call);     \
+  } while (0)
+
+struct device_guard {
+  int prev = -1;
+  explicit device_guard(int dev) { cudaGetDevice(&prev); if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+  ~device_guard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+template <class T>
+void dfree(T*& p) { if (p) { cudaFree(p); p = nullptr; } }
+
+void free_orders(whp_ctx* c) {
+  dfree(c->d_order_rec); dfree(c->d_pick_rec);
+  dfree(c->base.bstart); dfree(c->base.bop); dfree(c->base.bdist); dfree(c->base.bclass);
+  dfree(c->base.resp); dfree(c->base.totals);
+  dfree(c->d_stage[0]); dfree(c->d_stage[1]);
+  c->stage_rows = 0;
+  c->have_orders = false;
+}
+
+}  // namespace
+
+whp_tables whp_make_tables(const whp_ctx* c) {
+  whp_tables T;
+  T.g = c->g;
+  T.n_orders = c->n_orders; T.n_items = c->n_items; T.C = c->C; T.K = c->K;
+  T.order_rec = c->d_order_rec; T.pick_rec = c->d_pick_rec; T.tvw = c->d_tvw;
+  return T;
+}
+
+extern "C" {
+
+const char* whp_version(void) { return "whp 0.1 (sm_100a)"; }
+
+const char* whp_last_error(const whp_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int64_t whp_launch_count(const whp_ctx* c) { return c ? c->launches : 0; }
+
+whp_status whp_create_layout(int32_t n_aisles, int32_t slots_per_side, int32_t slot_pitch,
+                             int32_t aisle_spacing, int32_t depot_aisle, int32_t n_skus,
+                             const int32_t* sku_loc, const int32_t* sku_class, int32_t n_classes,
+                             int32_t cuda_device, whp_ctx** out) {
+  if (!out) return WHP_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!sku_loc || !sku_class) return WHP_ERR_INVALID_ARG;
+  if (n_aisles < 1 || slots_per_side < 1 || slot_pitch < 1 || aisle_spacing < 1 || n_skus < 1 ||
+      n_classes < 1 || cuda_device < 0)
+    return WHP_ERR_INVALID_ARG;
+  if (n_aisles > WHP_MAX_AISLES || slots_per_side > WHP_MAX_SLOTS ||
+      n_classes > WHP_MAX_CLASSES || depot_aisle < 0 || depot_aisle >= n_aisles)
+    return WHP_ERR_OUT_OF_RANGE;
+  const int64_t n_loc = 2ll * n_aisles * slots_per_side;
+  for (int32_t s = 0; s < n_skus; ++s) {
+    if (sku_loc[s] < 0 || sku_loc[s] >= n_loc) return WHP_ERR_OUT_OF_RANGE;
+    if (sku_class[s] < 0 || sku_class[s] >= n_classes) return WHP_ERR_OUT_OF_RANGE;
+  }
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cuda_device >= n_dev) return WHP_ERR_CUDA;
+  whp_ctx* c = new (std::nothrow) whp_ctx();
+  if (!c) return WHP_ERR_NOMEM;
+  c->device = cuda_device;
+  c->g.n_aisles = n_aisles; c->g.slots_per_side = slots_per_side; c->g.slot_pitch = slot_pitch;
+  c->g.aisle_spacing = aisle_spacing; c->g.depot_aisle = depot_aisle;
+  c->g.aisle_len = (int64_t)(slots_per_side + 1) * slot_pitch;
+  c->n_skus = n_skus; c->K = n_classes;
+  c->h_sku_loc = (int32_t*)malloc(sizeof(int32_t) * (size_t)n_skus);
+  c->h_sku_class = (int32_t*)malloc(sizeof(int32_t) * (size_t)n_skus);
+  if (!c->h_sku_loc || !c->h_sku_class) { whp_destroy(c); return WHP_ERR_NOMEM; }
+  memcpy(c->h_sku_loc, sku_loc, sizeof(int32_t) * (size_t)n_skus);
+  memcpy(c->h_sku_class, sku_class, sizeof(int32_t) * (size_t)n_skus);
+  device_guard dg(cuda_device);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { whp_destroy(c); return WHP_ERR_CUDA; }
+  c->num_sms = prop.multiProcessorCount;
+  c->argmin_cap = c->num_sms * 4;
+  cudaError_t e = cudaMalloc(&c->d_tvw, sizeof(double) * 3 * (size_t)n_classes);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_argmin_part, 16 * (size_t)c->argmin_cap + 16);
+  if (e == cudaSuccess) e = cudaMemset(c->d_argmin_part, 0, 16 * (size_t)c->argmin_cap + 16);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_count, sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_h_idx, sizeof(int64_t));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_h_val, sizeof(double));
+  for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
+    e = cudaStreamCreateWithFlags(&c->s_copy[k], cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_copied[k], cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_done[k], cudaEventDisableTiming);
+  }
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->s_exec, cudaStreamNonBlocking);
+  if (e != cudaSuccess) { whp_status s = e == cudaErrorMemoryAllocation ? WHP_ERR_NOMEM : WHP_ERR_CUDA; whp_destroy(c); return s; }
+  *out = c;
+  return WHP_OK;
+}
+
+whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_ptr,
+                           const int32_t* item_sku, int32_t cart_capacity) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!order_ptr || !item_sku || n_orders < 1 || cart_capacity < 1)
+    return fail(c, WHP_ERR_INVALID_ARG, "null pointer or non-positive size");
+  if (n_orders >= (1 << 24) || cart_capacity >= (1 << 20))
+    return fail(c, WHP_ERR_OUT_OF_RANGE, "n_orders or cart_capacity beyond the documented limit");
+  if (order_ptr[0] != 0) return fail(c, WHP_ERR_INVALID_ARG, "order_ptr[0] must be 0");
+  for (int32_t o = 0; o < n_orders; ++o) {
+    const int64_t q = (int64_t)order_ptr[o + 1] - order_ptr[o];
+    if (q < 1) return fail(c, WHP_ERR_INVALID_ARG, "order_ptr must be strictly increasing");
+    if (q > cart_capacity) return fail(c, WHP_ERR_CAPACITY, "an order exceeds the cart capacity");
+    if (q > WHP_MAX_ORDER_ITEMS) return fail(c, WHP_ERR_OUT_OF_RANGE, "an order has more than 255 items");
+  }
+  const int32_t n_items = order_ptr[n_orders];
+  if (n_items >= WHP_MAX_ITEMS) return fail(c, WHP_ERR_OUT_OF_RANGE, "more than 2^24 items");
+  for (int32_t i = 0; i < n_items; ++i)
+    if (item_sku[i] < 0 || item_sku[i] >= c->n_skus) return fail(c, WHP_ERR_OUT_OF_RANGE, "item_sku out of range");
+  // pack (layout in whp_internal.cuh)
+  std::vector<uint32_t> orec((size_t)n_orders), prec((size_t)n_items);
+  const int32_t S = c->g.slots_per_side;
+  for (int32_t o = 0; o < n_orders; ++o)
+    orec[o] = ((uint32_t)order_ptr[o] << WHP_Q_BITS) | (uint32_t)(order_ptr[o + 1] - order_ptr[o]);
+  for (int32_t i = 0; i < n_items; ++i) {
+    const int32_t loc = c->h_sku_loc[item_sku[i]];
+    const uint32_t aisle = (uint32_t)(loc / (2 * S)), side = (uint32_t)((loc % (2 * S)) / S);
+    const uint32_t slot1 = (uint32_t)(loc % S) + 1u;
+    prec[i] = (aisle << WHP_PICK_AISLE_SHIFT) | (slot1 << WHP_PICK_SLOT_SHIFT) |
+              (side << WHP_PICK_LOC_SHIFT) | (uint32_t)c->h_sku_class[item_sku[i]];
+  }
+  device_guard dg(c->device);
+  WHP_CUDA(c, cudaDeviceSynchronize());  // nothing may still be reading the old tables
+  free_orders(c);
+  c->n_orders = n_orders; c->n_items = n_items; c->C = cart_capacity;
+  const size_t no = (size_t)n_orders;
+  WHP_CUDA(c, cudaMalloc(&c->d_order_rec, 4 * no));
+  WHP_CUDA(c, cudaMalloc(&c->d_pick_rec, 4 * (size_t)n_items));
+  WHP_CUDA(c, cudaMalloc(&c->base.bstart, 4 * (no + 1)));
+  WHP_CUDA(c, cudaMalloc(&c->base.bop, 4 * no));
+  WHP_CUDA(c, cudaMalloc(&c->base.bdist, 8 * (no + 1)));
+  WHP_CUDA(c, cudaMalloc(&c->base.bclass, 32 * no));
+  WHP_CUDA(c, cudaMalloc(&c->base.resp, 4 * (size_t)c->K));
+  WHP_CUDA(c, cudaMalloc(&c->base.totals, 16));
+  WHP_CUDA(c, cudaMemcpy(c->d_order_rec, orec.data(), 4 * no, cudaMemcpyHostToDevice));
+  WHP_CUDA(c, cudaMemcpy(c->d_pick_rec, prec.data(), 4 * (size_t)n_items, cudaMemcpyHostToDevice));
+  c->have_orders = true;
+  return WHP_OK;
+}
+
+whp_status whp_set_penalty(whp_ctx* c, const double* t, const double* v, const double* w) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!t || !v || !w) return fail(c, WHP_ERR_INVALID_ARG, "null pointer");
+  std::vector<double> tvw(3 * (size_t)c->K);
+  for (int32_t k = 0; k < c->K; ++k) {
+    if (!std::isfinite(t[k]) || !std::isfinite(v[k]) || !std::isfinite(w[k]))
+      return fail(c, WHP_ERR_OUT_OF_RANGE, "non-finite t, v or w");
+    tvw[k] = t[k]; tvw[c->K + k] = v[k]; tvw[2 * (size_t)c->K + k] = w[k];
+  }
+  device_guard dg(c->device);
+  WHP_CUDA(c, cudaDeviceSynchronize());
+  WHP_CUDA(c, cudaMemcpy(c->d_tvw, tvw.data(), sizeof(double) * tvw.size(), cudaMemcpyHostToDevice));
+  c->have_penalty = true;
+  return WHP_OK;
+}
+
+static whp_status ready(whp_ctx* c) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!c->have_orders) return fail(c, WHP_ERR_STATE, "whp_load_orders has not been called");
+  if (!c->have_penalty) return fail(c, WHP_ERR_STATE, "whp_set_penalty has not been called");
+  return WHP_OK;
+}
+
+whp_status whp_eval_candidates(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
+                               int64_t* d_dist, double* d_penalty, double* d_obj,
+                               int32_t* d_n_batches, uint64_t* d_batch_hash,
+                               int32_t* d_batch_of_pos, int32_t* d_n_distinct, int32_t* d_resp,
+                               void* cuda_stream) {
+  whp_status s = ready(c);
+  if (s != WHP_OK) return s;
+  if (n_cand < 0) return fail(c, WHP_ERR_INVALID_ARG, "n_cand < 0");
+  if (n_cand == 0) return WHP_OK;
+  if (!d_perms) return fail(c, WHP_ERR_INVALID_ARG, "d_perms is null");
+  device_guard dg(c->device);
+  whp_eval_out out{d_dist, d_penalty, d_obj, d_n_batches, d_batch_hash, d_batch_of_pos,
+                   d_n_distinct, d_resp};
+  WHP_CUDA(c, whp_launch_eval(c, d_perms, n_cand, out, (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
+whp_status whp_eval_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
+                          int32_t win_len, int64_t* d_dist, double* d_obj, void* cuda_stream) {
+  whp_status s = ready(c);
+  if (s != WHP_OK) return s;
+  if (!d_base_perm) return fail(c, WHP_ERR_INVALID_ARG, "d_base_perm is null");
+  if (win_len < 2) return fail(c, WHP_ERR_INVALID_ARG, "window shorter than 2");
+  if (win_start < 0 || (int64_t)win_start + win_len > c->n_orders)
+    return fail(c, WHP_ERR_OUT_OF_RANGE, "window outside the plan");
+  device_guard dg(c->device);
+  WHP_CUDA(c, whp_launch_swaps(c, d_base_perm, win_start, win_len, d_dist, d_obj,
+                               (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
+whp_status whp_argmin(whp_ctx* c, const double* d_obj, int64_t n, int64_t* d_idx, double* d_val,
+                      void* cuda_stream) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!d_obj || !d_idx || n < 1) return fail(c, WHP_ERR_INVALID_ARG, "null pointer or n < 1");
+  device_guard dg(c->device);
+  WHP_CUDA(c, whp_launch_argmin(c, d_obj, n, d_idx, d_val, (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
+whp_status whp_apply_swap(whp_ctx* c, int32_t* d_base_perm, int32_t win_start, int32_t win_len,
+                          const int64_t* d_idx, void* cuda_stream) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!c->have_orders) return fail(c, WHP_ERR_STATE, "whp_load_orders has not been called");
+  if (!d_base_perm || !d_idx) return fail(c, WHP_ERR_INVALID_ARG, "null pointer");
+  if (win_len < 2) return fail(c, WHP_ERR_INVALID_ARG, "window shorter than 2");
+  if (win_start < 0 || (int64_t)win_start + win_len > c->n_orders)
+    return fail(c, WHP_ERR_OUT_OF_RANGE, "window outside the plan");
+  device_guard dg(c->device);
+  WHP_CUDA(c, whp_launch_apply_swap(c, d_base_perm, win_start, win_len, d_idx,
+                                    (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
+whp_status whp_validate_perms(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
+                              int64_t* h_n_bad, void* cuda_stream) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!c->have_orders) return fail(c, WHP_ERR_STATE, "whp_load_orders has not been called");
+  if (!d_perms || !h_n_bad || n_cand < 0) return fail(c, WHP_ERR_INVALID_ARG, "bad argument");
+  *h_n_bad = 0;
+  if (n_cand == 0) return WHP_OK;
+  if (c->n_orders > (1 << 20)) return fail(c, WHP_ERR_OUT_OF_RANGE, "validate supports n_orders <= 2^20");
+  device_guard dg(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  WHP_CUDA(c, cudaMemsetAsync(c->d_count, 0, sizeof(unsigned long long), st));
+  WHP_CUDA(c, whp_launch_validate(c, d_perms, n_cand, st));
+  unsigned long long bad = 0;
+  WHP_CUDA(c, cudaMemcpyAsync(&bad, c->d_count, sizeof(bad), cudaMemcpyDeviceToHost, st));
+  WHP_CUDA(c, cudaStreamSynchronize(st));
+  *h_n_bad = (int64_t)bad;
+  return WHP_OK;
+}
+
+whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t n_cand,
+                                    int64_t* h_dist, double* h_obj, int64_t* h_argmin_idx,
+                                    double* h_argmin_val) {
+  whp_status s = ready(c);
+  if (s != WHP_OK) return s;
+  if (n_cand < 0) return fail(c, WHP_ERR_INVALID_ARG, "n_cand < 0");
+  if (n_cand == 0) return WHP_OK;
+  if (!h_perms) return fail(c, WHP_ERR_INVALID_ARG, "h_perms is null");
+  device_guard dg(c->device);
+  // staging: two device buffers of `rows` plans each (~32 MB), results for all plans
+  const int64_t row_bytes = 4ll * c->n_orders;
+  int64_t rows = (32ll << 20) / row_bytes;
+  if (rows < 1) rows = 1;
+  if (rows > n_cand) rows = n_cand;
+  if (c->stage_rows < rows) {
+    dfree(c->d_stage[0]); dfree(c->d_stage[1]);
+    WHP_CUDA(c, cudaMalloc(&c->d_stage[0], (size_t)(rows * row_bytes)));
+    WHP_CUDA(c, cudaMalloc(&c->d_stage[1], (size_t)(rows * row_bytes)));
+    c->stage_rows = rows;
+  }
+  rows = c->stage_rows < n_cand ? c->stage_rows : n_cand;
+  if (c->h_out_cap < n_cand) {
+    dfree(c->d_h_dist); dfree(c->d_h_obj);
+    WHP_CUDA(c, cudaMalloc(&c->d_h_dist, 8 * (size_t)n_cand));
+    WHP_CUDA(c, cudaMalloc(&c->d_h_obj, 8 * (size_t)n_cand));
+    c->h_out_cap = n_cand;
+  }
+  // pipeline: copy chunk k+1 (alternating copy streams) while chunk k is evaluated
+  int64_t chunk = 0;
+  for (int64_t lo = 0; lo < n_cand; lo += rows, ++chunk) {
+    const int b = (int)(chunk & 1);
+    const int64_t nr = (n_cand - lo < rows) ? n_cand - lo : rows;
+    if (chunk >= 2) WHP_CUDA(c, cudaStreamWaitEvent(c->s_copy[b], c->ev_done[b], 0));
+    WHP_CUDA(c, cudaMemcpyAsync(c->d_stage[b], h_perms + lo * c->n_orders,
+                                (size_t)(nr * row_bytes), cudaMemcpyHostToDevice, c->s_copy[b]));
+    WHP_CUDA(c, cudaEventRecord(c->ev_copied[b], c->s_copy[b]));
+    WHP_CUDA(c, cudaStreamWaitEvent(c->s_exec, c->ev_copied[b], 0));
+    whp_eval_out out{c->d_h_dist + lo, nullptr, c->d_h_obj + lo, nullptr, nullptr, nullptr,
+                     nullptr, nullptr};
+    WHP_CUDA(c, whp_launch_eval(c, c->d_stage[b], nr, out, c->s_exec));
+    WHP_CUDA(c, cudaEventRecord(c->ev_done[b], c->s_exec));
+  }
+  if (h_argmin_idx || h_argmin_val) {
+    WHP_CUDA(c, whp_launch_argmin(c, c->d_h_obj, n_cand, c->d_h_idx, c->d_h_val, c->s_exec));
+    if (h_argmin_idx)
+      WHP_CUDA(c, cudaMemcpyAsync(h_argmin_idx, c->d_h_idx, 8, cudaMemcpyDeviceToHost, c->s_exec));
+    if (h_argmin_val)
+      WHP_CUDA(c, cudaMemcpyAsync(h_argmin_val, c->d_h_val, 8, cudaMemcpyDeviceToHost, c->s_exec));
+  }
+  if (h_dist)
+    WHP_CUDA(c, cudaMemcpyAsync(h_dist, c->d_h_dist, 8 * (size_t)n_cand, cudaMemcpyDeviceToHost, c->s_exec));
+  if (h_obj)
+    WHP_CUDA(c, cudaMemcpyAsync(h_obj, c->d_h_obj, 8 * (size_t)n_cand, cudaMemcpyDeviceToHost, c->s_exec));
+  WHP_CUDA(c, cudaStreamSynchronize(c->s_exec));
+  return WHP_OK;
+}
+
+void whp_destroy(whp_ctx* c) {
+  if (!c) return;
+  {
+    device_guard dg(c->device);
+    cudaDeviceSynchronize();
+    free_orders(c);
+    dfree(c->d_tvw); dfree(c->d_argmin_part); dfree(c->d_count);
+    dfree(c->d_h_dist); dfree(c->d_h_obj); dfree(c->d_h_idx); dfree(c->d_h_val);
+    for (int k = 0; k < 2; ++k) {
+      if (c->s_copy[k]) cudaStreamDestroy(c->s_copy[k]);
+      if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]);
+      if (c->ev_done[k]) cudaEventDestroy(c->ev_done[k]);
+    }
+    if (c->s_exec) cudaStreamDestroy(c->s_exec);
+  }
+  free(c->h_sku_loc); free(c->h_sku_class);
+  delete c;
+}
+
+}  // extern "C"

@@ -1,0 +1,111 @@
+// whp_internal.cuh — context, packed table formats and launch prototypes shared by the .cu
+// files of libwhp.so. Not part of the public boundary (include/whp.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/whp.h"
+
+// ---- packed device tables -----------------------------------------------------
+// order record, 32 bit:  item_off[31:8] | q[7:0]            (q = number of items, 1..255)
+// pick  record, 32 bit:  aisle[30:21] | slot1[20:9] | side[8] | class[7:0]
+//   slot1 = slot + 1 (depth = slot1 * slot_pitch). The field order makes an unsigned max over
+//   the records of a batch return (a_max, deepest slot in a_max) in its top 22 bits (D3).
+#define WHP_Q_BITS 8
+#define WHP_Q_MASK 0xffu
+#define WHP_PICK_AISLE_SHIFT 21
+#define WHP_PICK_SLOT_SHIFT 9
+#define WHP_PICK_SLOT_MASK 0xfffu
+#define WHP_PICK_LOC_SHIFT 8 /* rec >> 8 identifies the location (aisle, slot, side) */
+#define WHP_PICK_CLASS_MASK 0xffu
+
+#define WHP_MAX_AISLES 1024
+#define WHP_MAX_SLOTS 4095
+#define WHP_MAX_CLASSES 256
+#define WHP_MAX_ITEMS (1 << 24)
+#define WHP_MAX_ORDER_ITEMS 255
+
+struct whp_geom {
+  int32_t n_aisles, slots_per_side, slot_pitch, aisle_spacing, depot_aisle;
+  int64_t aisle_len;  // A = (S+1)*p
+};
+
+// Read-only view of everything a kernel needs (passed by value).
+struct whp_tables {
+  whp_geom g;
+  int32_t n_orders, n_items, C, K;
+  const uint32_t* order_rec;  // [n_orders]
+  const uint32_t* pick_rec;   // [n_items]
+  const double* tvw;          // [3][K]: t, v, w
+};
+
+// Per-plan outputs of the candidate walker; any pointer may be null.
+struct whp_eval_out {
+  int64_t* dist;
+  double* penalty;
+  double* obj;
+  int32_t* n_batches;
+  uint64_t* batch_hash;
+  int32_t* batch_of_pos;
+  int32_t* n_distinct;
+  int32_t* resp;
+};
+
+// Per-batch tables of the base plan, produced by the base pass of whp_eval_swaps (scratch).
+struct whp_base_tables {
+  int32_t* bstart;    // [n_orders+1] first position of batch b; bstart[nb] = n_orders
+  int32_t* bop;       // [n_orders]   batch of position
+  int64_t* bdist;     // [n_orders+1] exclusive prefix sum of per-batch S-shape lengths
+  uint32_t* bclass;   // [n_orders][8] class mask of batch b
+  int32_t* resp;      // [K]          base responses
+  int64_t* totals;    // [2]          D_base, n_batches
+};
+
+struct whp_ctx {
+  int device = 0;
+  whp_geom g{};
+  int32_t n_skus = 0, K = 0;
+  int32_t* h_sku_loc = nullptr;  // host copies (needed again by whp_load_orders)
+  int32_t* h_sku_class = nullptr;
+  // orders
+  int32_t n_orders = 0, n_items = 0, C = 0;
+  uint32_t* d_order_rec = nullptr;
+  uint32_t* d_pick_rec = nullptr;
+  double* d_tvw = nullptr;
+  bool have_orders = false, have_penalty = false;
+  // scratch
+  whp_base_tables base{};
+  void* d_argmin_part = nullptr;  // partial (val, idx) pairs + ticket
+  int32_t argmin_cap = 0;
+  unsigned long long* d_count = nullptr;  // validate_perms counter
+  // host-path staging (whp_eval_candidates_host)
+  int32_t* d_stage[2] = {nullptr, nullptr};
+  int64_t stage_rows = 0;
+  int64_t* d_h_dist = nullptr;
+  double* d_h_obj = nullptr;
+  int64_t h_out_cap = 0;
+  int64_t* d_h_idx = nullptr;
+  double* d_h_val = nullptr;
+  cudaStream_t s_copy[2] = {nullptr, nullptr};
+  cudaStream_t s_exec = nullptr;
+  cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+  int num_sms = 148;
+  int64_t launches = 0;
+  std::string err;
+};
+
+whp_tables whp_make_tables(const whp_ctx* c);
+
+// kernels' host launchers (each returns the cudaError_t of the launch)
+cudaError_t whp_launch_eval(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
+                            const whp_eval_out& out, cudaStream_t st);
+cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
+                             int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st);
+cudaError_t whp_launch_argmin(whp_ctx* c, const double* d_obj, int64_t n, int64_t* d_idx,
+                              double* d_val, cudaStream_t st);
+cudaError_t whp_launch_apply_swap(whp_ctx* c, int32_t* d_base_perm, int32_t win_start,
+                                  int32_t win_len, const int64_t* d_idx, cudaStream_t st);
+cudaError_t whp_launch_validate(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
+                                cudaStream_t st);

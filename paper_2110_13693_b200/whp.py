@@ -1,0 +1,210 @@
+"""Thin ctypes binding of libwhp.so (include/whp.h): argument marshalling only — every step of
+the path runs in the CUDA kernels. Device arrays are torch tensors (PyTorch is used for device
+memory and streams only); host arrays are numpy.
+
+There is no CPU fallback: if libwhp.so has not been built (python -m
+paper_2110_13693_b200.build) or cannot be loaded, every call raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libwhp.so")
+_lib = None
+
+OK, ERR_INVALID_ARG, ERR_OUT_OF_RANGE, ERR_CAPACITY, ERR_STATE, ERR_CUDA, ERR_NOMEM = range(7)
+_STATUS = ["WHP_OK", "WHP_ERR_INVALID_ARG", "WHP_ERR_OUT_OF_RANGE", "WHP_ERR_CAPACITY",
+           "WHP_ERR_STATE", "WHP_ERR_CUDA", "WHP_ERR_NOMEM"]
+
+# symbols include/whp.h declares (tests check that the library exports every one)
+SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_candidates",
+           "whp_eval_candidates_host", "whp_eval_swaps", "whp_argmin", "whp_apply_swap",
+           "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
+           "whp_version"]
+
+
+class WhpError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{_STATUS[status] if 0 <= status < 7 else status}: {msg}")
+        self.status = status
+
+
+def lib():
+    """Load libwhp.so (never builds it, never falls back)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise RuntimeError(f"{_SO} is missing: run `python -m paper_2110_13693_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(_SO)
+        vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+        L.whp_create_layout.argtypes = [i32, i32, i32, i32, i32, i32, vp, vp, i32, i32,
+                                        C.POINTER(vp)]
+        L.whp_load_orders.argtypes = [vp, i32, vp, vp, i32]
+        L.whp_set_penalty.argtypes = [vp, vp, vp, vp]
+        L.whp_eval_candidates.argtypes = [vp, vp, i64] + [vp] * 8 + [vp]
+        L.whp_eval_candidates_host.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+        L.whp_eval_swaps.argtypes = [vp, vp, i32, i32, vp, vp, vp]
+        L.whp_argmin.argtypes = [vp, vp, i64, vp, vp, vp]
+        L.whp_apply_swap.argtypes = [vp, vp, i32, i32, vp, vp]
+        L.whp_validate_perms.argtypes = [vp, vp, i64, vp, vp]
+        L.whp_launch_count.argtypes = [vp]
+        L.whp_launch_count.restype = i64
+        L.whp_destroy.argtypes = [vp]
+        L.whp_destroy.restype = None
+        L.whp_last_error.argtypes = [vp]
+        L.whp_last_error.restype = C.c_char_p
+        L.whp_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _h(a, dtype):
+    """host numpy array -> (keepalive, pointer)"""
+    if a is None:
+        return None, None
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a, a.ctypes.data
+
+
+def _d(t, dtype=None):
+    """device torch tensor -> raw pointer (None -> NULL)"""
+    if t is None:
+        return None
+    if not t.is_cuda or not t.is_contiguous():
+        raise ValueError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def _stream(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream
+
+
+class Context:
+    """Owns one whp_ctx. Method names are the C entry points without the `whp_` prefix."""
+
+    def __init__(self, n_aisles, slots_per_side, slot_pitch, aisle_spacing, depot_aisle,
+                 sku_loc, sku_class, n_classes, device=0):
+        L = lib()
+        k1, p_loc = _h(sku_loc, np.int32)
+        k2, p_cls = _h(sku_class, np.int32)
+        if k1 is None or k2 is None or len(k1) != len(k2):
+            raise WhpError(ERR_INVALID_ARG, "sku_loc / sku_class")
+        h = C.c_void_p()
+        st = L.whp_create_layout(n_aisles, slots_per_side, slot_pitch, aisle_spacing,
+                                 depot_aisle, len(k1), p_loc, p_cls, n_classes, device,
+                                 C.byref(h))
+        if st != OK:
+            raise WhpError(st, "whp_create_layout")
+        self._h = h
+        self.device = device
+        self.n_classes = n_classes
+        self.n_orders = 0
+
+    @classmethod
+    def from_problem(cls, pb, device=0):
+        """pb: workloads.Problem (or anything with its attributes)."""
+        ctx = cls(pb.n_aisles, pb.slots_per_side, pb.slot_pitch, pb.aisle_spacing,
+                  pb.depot_aisle, pb.sku_loc, pb.sku_class, pb.n_classes, device)
+        ctx.load_orders(pb.order_ptr, pb.item_sku, pb.cart_capacity)
+        ctx.set_penalty(pb.t, pb.v, pb.w)
+        return ctx
+
+    def _check(self, st):
+        if st != OK:
+            raise WhpError(st, lib().whp_last_error(self._h).decode())
+
+    def load_orders(self, order_ptr, item_sku, cart_capacity):
+        k1, p1 = _h(order_ptr, np.int32)
+        k2, p2 = _h(item_sku, np.int32)
+        n_orders = len(k1) - 1
+        if n_orders >= 1 and len(k2) != int(k1[-1]):
+            raise WhpError(ERR_INVALID_ARG, "len(item_sku) != order_ptr[-1]")
+        self._check(lib().whp_load_orders(self._h, n_orders, p1, p2, cart_capacity))
+        self.n_orders = n_orders
+
+    def set_penalty(self, t, v, w):
+        ks = [_h(x, np.float64) for x in (t, v, w)]
+        if any(k[0] is None or len(k[0]) != self.n_classes for k in ks):
+            raise WhpError(ERR_INVALID_ARG, "t, v, w must have n_classes entries")
+        self._check(lib().whp_set_penalty(self._h, ks[0][1], ks[1][1], ks[2][1]))
+
+    def eval_candidates(self, perms, dist=None, penalty=None, obj=None, n_batches=None,
+                        batch_hash=None, batch_of_pos=None, n_distinct=None, resp=None,
+                        stream=None):
+        """perms: CUDA int32 [n_cand][n_orders]; outputs are caller-allocated CUDA tensors."""
+        import torch
+        n_cand = perms.shape[0] if perms.dim() == 2 else 1
+        if perms.numel() != n_cand * self.n_orders:
+            raise WhpError(ERR_INVALID_ARG, "perms shape")
+        self._check(lib().whp_eval_candidates(
+            self._h, _d(perms, torch.int32), n_cand, _d(dist, torch.int64),
+            _d(penalty, torch.float64), _d(obj, torch.float64), _d(n_batches, torch.int32),
+            _d(batch_hash, torch.int64), _d(batch_of_pos, torch.int32),
+            _d(n_distinct, torch.int32), _d(resp, torch.int32), _stream(stream)))
+
+    def eval_candidates_host(self, perms, dist=None, obj=None, want_argmin=True):
+        """perms / dist / obj: host numpy arrays or CPU torch tensors (pinned = async copies).
+        Returns (argmin_idx, argmin_val) when want_argmin."""
+        def hp(a):
+            if a is None:
+                return None
+            if hasattr(a, "data_ptr"):
+                return a.data_ptr()
+            return a.ctypes.data
+        n_cand = perms.shape[0]
+        idx, val = C.c_int64(-1), C.c_double(0.0)
+        self._check(lib().whp_eval_candidates_host(
+            self._h, hp(perms), n_cand, hp(dist), hp(obj),
+            C.addressof(idx) if want_argmin else None,
+            C.addressof(val) if want_argmin else None))
+        return (idx.value, val.value) if want_argmin else None
+
+    def eval_swaps(self, base_perm, win_start, win_len, dist=None, obj=None, stream=None):
+        import torch
+        self._check(lib().whp_eval_swaps(self._h, _d(base_perm, torch.int32), win_start, win_len,
+                                         _d(dist, torch.int64), _d(obj, torch.float64),
+                                         _stream(stream)))
+
+    def argmin(self, obj, idx, val=None, n=None, stream=None):
+        import torch
+        self._check(lib().whp_argmin(self._h, _d(obj, torch.float64),
+                                     obj.numel() if n is None else n, _d(idx, torch.int64),
+                                     _d(val, torch.float64), _stream(stream)))
+
+    def apply_swap(self, base_perm, win_start, win_len, idx, stream=None):
+        import torch
+        self._check(lib().whp_apply_swap(self._h, _d(base_perm, torch.int32), win_start, win_len,
+                                         _d(idx, torch.int64), _stream(stream)))
+
+    def validate_perms(self, perms, stream=None) -> int:
+        import torch
+        n_bad = C.c_int64(0)
+        self._check(lib().whp_validate_perms(self._h, _d(perms, torch.int32), perms.shape[0],
+                                             C.addressof(n_bad), _stream(stream)))
+        return n_bad.value
+
+    def launch_count(self) -> int:
+        return int(lib().whp_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().whp_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def version() -> str:
+    return lib().whp_version().decode()

@@ -1,0 +1,308 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the oracle, element by element
+on the same seeded inputs. Bars (BASELINE.json north_star): bit-exact batch assignment, route
+distances, responses and argmin index; fp64 penalty / objective within 1e-9 relative (the
+canonical summation order of D6 makes them bit-identical in practice, which is also asserted
+where the argmin depends on it)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2110_13693_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-9  # north_star: "within 1e-9 relative error for the fp64 penalty and total objective"
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def gpu_eval(torch, ctx, perms_dev, detail=False):
+    n = perms_dev.shape[0]
+    dev = perms_dev.device
+    out = {
+        "dist": torch.full((n,), -1, dtype=torch.int64, device=dev),
+        "penalty": torch.zeros(n, dtype=torch.float64, device=dev),
+        "obj": torch.zeros(n, dtype=torch.float64, device=dev),
+        "n_batches": torch.zeros(n, dtype=torch.int32, device=dev),
+        "batch_hash": torch.zeros(n, dtype=torch.int64, device=dev),
+    }
+    if detail:
+        out["batch_of_pos"] = torch.full((n, ctx.n_orders), -1, dtype=torch.int32, device=dev)
+        out["n_distinct"] = torch.zeros(n, dtype=torch.int32, device=dev)
+        out["resp"] = torch.zeros((n, ctx.n_classes), dtype=torch.int32, device=dev)
+    ctx.eval_candidates(perms_dev, **out)
+    torch.cuda.synchronize()
+    res = {k: v.cpu().numpy() for k, v in out.items()}
+    res["batch_hash"] = res["batch_hash"].view(np.uint64)
+    return res, out
+
+
+def assert_parity(got, ref, pb, detail=False):
+    assert np.array_equal(got["dist"], ref["dist"])
+    assert np.array_equal(got["n_batches"], ref["n_batches"])
+    assert np.array_equal(got["batch_hash"], ref["batch_hash"])
+    # Q13: tolerance denominator for phi is max(|ref|, sum|term|, 1); sum|term| >= |ref|
+    assert np.all(np.abs(got["penalty"] - ref["penalty"]) <= RTOL * np.maximum(np.abs(ref["penalty"]), 1.0))
+    assert np.all(np.abs(got["obj"] - ref["obj"]) <= RTOL * np.abs(ref["obj"]))
+    # canonical summation order (D6) => identical bits, which makes the argmin exact
+    assert np.array_equal(got["penalty"], ref["penalty"])
+    assert np.array_equal(got["obj"], ref["obj"])
+    if detail:
+        assert np.array_equal(got["batch_of_pos"], ref["batch_of_pos"])
+        assert np.array_equal(got["resp"], ref["resp"])
+        assert np.array_equal(got["n_distinct"], ref["n_distinct"])
+
+
+def gpu_argmin(torch, ctx, obj_dev):
+    idx = torch.full((1,), -7, dtype=torch.int64, device=obj_dev.device)
+    val = torch.zeros(1, dtype=torch.float64, device=obj_dev.device)
+    ctx.argmin(obj_dev, idx, val)
+    torch.cuda.synchronize()
+    return int(idx.item()), float(val.item())
+
+
+# ---- configs 1 and 2: every candidate, every output --------------------------------------------
+@pytest.mark.parametrize("name", ["tiny", "mid"])
+def test_all_candidates_full_detail(torch_cuda, name):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    wl = W.make_workload(name)
+    pb = wl.problem
+    perms = W.perms(wl.seed, pb.n_orders, wl.n_cand)
+    ctx = whp.Context.from_problem(pb)
+    got, dev = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=True)
+    ref = oracle.eval_candidates(pb, perms, detail=True)
+    assert_parity(got, ref, pb, detail=True)
+    # the timed path (no detail outputs) must give the same numbers
+    got2, dev2 = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=False)
+    assert_parity(got2, ref, pb)
+    i, v = gpu_argmin(torch, ctx, dev2["obj"])
+    assert i == oracle.argmin(ref["obj"]) and v == ref["obj"][i]
+    ctx.close()
+
+
+def test_golden_examples_on_gpu(torch_cuda, golden):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    from test_oracle_pins import _golden_problem
+    pb = _golden_problem(golden)
+    ctx = whp.Context.from_problem(pb)
+    perms = np.array([p["perm"] for p in golden["plans"]], np.int32)
+    got, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=True)
+    for i, ex in enumerate(golden["plans"]):
+        assert got["batch_of_pos"][i].tolist() == ex["batch_of_pos"]
+        assert int(got["dist"][i]) == ex["dist"] and got["resp"][i].tolist() == ex["resp"]
+        assert got["penalty"][i] == ex["penalty"] and got["obj"][i] == ex["obj"]
+        assert int(got["batch_hash"][i]) == ex["batch_hash"]
+    assert int(got["n_distinct"][0]) == golden["plans"][0]["n_distinct"]
+    # E6 through the swap evaluator
+    e4, e6 = golden["plans"][0], golden["plans"][2]
+    s, Wn = e6["window"]
+    nn = Wn * (Wn - 1) // 2
+    d = torch.zeros(nn, dtype=torch.int64, device="cuda")
+    o = torch.zeros(nn, dtype=torch.float64, device="cuda")
+    ctx.eval_swaps(torch.tensor(e4["perm"], dtype=torch.int32, device="cuda"), s, Wn, d, o)
+    torch.cuda.synchronize()
+    assert int(d[e6["neighbour_index"]]) == e6["dist"] and float(o[e6["neighbour_index"]]) == e6["obj"]
+    ctx.close()
+
+
+# ---- config 3 at full size, in the launch configuration bench.py times --------------------------
+def test_paper_scale_full_launch_sampled_oracle(torch_cuda):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    wl = W.make_workload("paper")
+    pb = wl.problem
+    ctx = whp.Context.from_problem(pb)
+    perms_dev = W.perms_torch(wl.seed, pb.n_orders, 0, wl.n_cand, "cuda")
+    assert ctx.validate_perms(perms_dev) == 0
+    got, dev = gpu_eval(torch, ctx, perms_dev)  # all 16,384 candidates, timed-path outputs
+    rows = np.unique(np.concatenate([np.arange(0, 96), np.arange(wl.n_cand - 96, wl.n_cand),
+                                     (W.stream_u64(7, 1, 320) % np.uint64(wl.n_cand)).astype(np.int64)]))
+    sample = W.perm_rows(wl.seed, pb.n_orders, rows)
+    assert np.array_equal(sample, perms_dev[torch.from_numpy(rows).cuda()].cpu().numpy())
+    ref = oracle.eval_candidates(pb, sample, detail=True)
+    assert_parity({k: v[rows] for k, v in got.items()}, ref, pb)
+    # detail outputs on the sampled rows
+    gd, _ = gpu_eval(torch, ctx, torch.from_numpy(sample).cuda(), detail=True)
+    assert_parity(gd, ref, pb, detail=True)
+    # properties that hold for every candidate at any size
+    q = np.diff(pb.order_ptr)
+    assert np.all(got["n_batches"] >= -(-pb.n_items // pb.cart_capacity))
+    assert np.all(got["dist"] > 0) and np.all(got["obj"] == got["dist"] + got["penalty"])
+    # argmin over all candidates: index equals numpy's first minimum of the GPU objective,
+    # and the winner's objective equals the oracle's for that row
+    i, v = gpu_argmin(torch, ctx, dev["obj"])
+    assert i == int(np.argmin(got["obj"])) and v == got["obj"][i]
+    win = oracle.eval_candidates(pb, W.perm_rows(wl.seed, pb.n_orders, [i]))
+    assert win["obj"][0] == v
+    ctx.close()
+
+
+# ---- config 5 (stress): 65,536 candidates generated in HBM, oracle on sampled rows ---------------
+def test_stress_full_size_sampled_oracle(torch_cuda):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    wl = W.make_workload("stress")
+    pb = wl.problem
+    ctx = whp.Context.from_problem(pb)
+    n = pb.n_orders
+    perms_dev = torch.empty((wl.n_cand, n), dtype=torch.int32, device="cuda")
+    step = 4096
+    for lo in range(0, wl.n_cand, step):
+        perms_dev[lo:lo + step] = W.perms_torch(wl.seed, n, lo, lo + step, "cuda")
+    got, dev = gpu_eval(torch, ctx, perms_dev)
+    rows = np.unique(np.concatenate([[0, 1, wl.n_cand - 1],
+                                     (W.stream_u64(9, 2, 45) % np.uint64(wl.n_cand)).astype(np.int64)]))
+    sample = W.perm_rows(wl.seed, n, rows)
+    assert np.array_equal(sample, perms_dev[torch.from_numpy(rows).cuda()].cpu().numpy())
+    ref = oracle.eval_candidates(pb, sample, detail=True)
+    assert_parity({k: v[rows] for k, v in got.items()}, ref, pb)
+    gd, _ = gpu_eval(torch, ctx, torch.from_numpy(sample[:8]).cuda(), detail=True)
+    assert_parity(gd, {k: v[:8] for k, v in ref.items()}, pb, detail=True)
+    i, v = gpu_argmin(torch, ctx, dev["obj"])
+    assert i == int(np.argmin(got["obj"])) and v == got["obj"][i]
+    win = oracle.eval_candidates(pb, W.perm_rows(wl.seed, n, [i]))
+    assert win["obj"][0] == v and win["dist"][0] == got["dist"][i]
+    ctx.close()
+
+
+# ---- edge cases ----------------------------------------------------------------------------------
+def _random_problem(seed, NA, S, K, n_skus, n_orders, qmax, C, depot=0, pitch=1, spacing=3):
+    rng = np.random.default_rng(seed)
+    q = rng.integers(1, qmax + 1, size=n_orders)
+    ptr = np.concatenate([[0], np.cumsum(q)]).astype(np.int32)
+    return W.Problem(
+        n_aisles=NA, slots_per_side=S, slot_pitch=pitch, aisle_spacing=spacing, depot_aisle=depot,
+        sku_loc=rng.integers(0, 2 * NA * S, size=n_skus).astype(np.int32),
+        sku_class=rng.integers(0, K, size=n_skus).astype(np.int32), n_classes=K, order_ptr=ptr,
+        item_sku=rng.integers(0, n_skus, size=int(ptr[-1])).astype(np.int32), cart_capacity=C,
+        t=rng.uniform(0, 20, K), v=rng.uniform(-1, 1, K), w=rng.uniform(0, 2, K))
+
+
+EDGE = [
+    dict(NA=1, S=1, K=1, n_skus=1, n_orders=1, qmax=1, C=1),            # the smallest problem
+    dict(NA=1, S=7, K=1, n_skus=5, n_orders=33, qmax=3, C=3),           # one aisle, one class
+    dict(NA=5, S=9, K=3, n_skus=30, n_orders=31, qmax=4, C=4),          # ragged tile (31)
+    dict(NA=5, S=9, K=3, n_skus=30, n_orders=32, qmax=4, C=1000),       # one batch holds all
+    dict(NA=37, S=11, K=33, n_skus=200, n_orders=97, qmax=1, C=1),      # every order is a batch
+    dict(NA=64, S=20, K=64, n_skus=500, n_orders=257, qmax=6, C=6, depot=20),   # depot mid-floor
+    dict(NA=1024, S=30, K=256, n_skus=5000, n_orders=1000, qmax=12, C=40, depot=1023, pitch=3, spacing=7),
+    dict(NA=400, S=4095, K=200, n_skus=3000, n_orders=333, qmax=255, C=600),    # limits: q, slots
+    dict(NA=33, S=17, K=40, n_skus=100, n_orders=129, qmax=5, C=70),    # batches longer than a tile
+]
+
+
+@pytest.mark.parametrize("cfg", EDGE, ids=lambda c: "-".join(f"{k}{v}" for k, v in c.items()))
+def test_edge_cases(torch_cuda, cfg):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = _random_problem(11, **cfg)
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perm_rows(3, pb.n_orders, np.arange(70))
+    got, dev = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=True)
+    ref = oracle.eval_candidates(pb, perms, detail=True)
+    assert_parity(got, ref, pb, detail=True)
+    got2, dev2 = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
+    assert_parity(got2, ref, pb)
+    i, v = gpu_argmin(torch, ctx, dev2["obj"])
+    assert i == oracle.argmin(ref["obj"])
+    ctx.close()
+
+
+def test_api_errors_and_nullable_outputs(torch_cuda):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("tiny")
+    ctx = whp.Context(pb.n_aisles, pb.slots_per_side, pb.slot_pitch, pb.aisle_spacing,
+                      pb.depot_aisle, pb.sku_loc, pb.sku_class, pb.n_classes)
+    perms = torch.from_numpy(W.perms(0, pb.n_orders, 4)).cuda()
+    obj = torch.zeros(4, dtype=torch.float64, device="cuda")
+    ctx.n_orders = pb.n_orders
+    with pytest.raises(whp.WhpError) as e:
+        ctx.eval_candidates(perms, obj=obj)  # before load_orders
+    assert e.value.status == whp.ERR_STATE
+    with pytest.raises(whp.WhpError) as e:
+        ctx.load_orders(pb.order_ptr, pb.item_sku, 3)  # an order of 4 items, cart of 3
+    assert e.value.status == whp.ERR_CAPACITY
+    with pytest.raises(whp.WhpError) as e:
+        ctx.load_orders(pb.order_ptr, pb.item_sku + 1000, 8)
+    assert e.value.status == whp.ERR_OUT_OF_RANGE
+    ctx.load_orders(pb.order_ptr, pb.item_sku, pb.cart_capacity)
+    with pytest.raises(whp.WhpError) as e:
+        ctx.eval_candidates(perms, obj=obj)  # before set_penalty
+    assert e.value.status == whp.ERR_STATE
+    with pytest.raises(whp.WhpError) as e:
+        ctx.set_penalty(pb.t, pb.v * np.inf, pb.w)
+    assert e.value.status == whp.ERR_OUT_OF_RANGE
+    ctx.set_penalty(pb.t, pb.v, pb.w)
+    ctx.eval_candidates(perms, obj=obj)  # only one output requested
+    ctx.eval_candidates(perms[:0], obj=obj)  # empty input is a no-op
+    torch.cuda.synchronize()
+    ref = oracle.eval_candidates(pb, perms.cpu().numpy())
+    assert np.array_equal(obj.cpu().numpy(), ref["obj"])
+    with pytest.raises(whp.WhpError) as e:
+        ctx.eval_swaps(perms[0], 0, 1, obj=obj)
+    assert e.value.status == whp.ERR_INVALID_ARG
+    with pytest.raises(whp.WhpError) as e:
+        ctx.eval_swaps(perms[0], 15, 6, obj=obj)
+    assert e.value.status == whp.ERR_OUT_OF_RANGE
+    bad = perms.clone()
+    bad[2, 0] = bad[2, 1]
+    assert ctx.validate_perms(bad) == 1 and ctx.validate_perms(perms) == 0
+    # argmin: ties -> lowest index; single element; works on a non-default stream
+    x = torch.tensor([3.0, 1.0, 2.0, 1.0, 1.0], dtype=torch.float64, device="cuda")
+    s = torch.cuda.Stream()
+    idx = torch.zeros(1, dtype=torch.int64, device="cuda")
+    with torch.cuda.stream(s):
+        ctx.argmin(x, idx)
+    s.synchronize()
+    assert int(idx) == 1
+    ctx.argmin(x[:1], idx)
+    torch.cuda.synchronize()
+    assert int(idx) == 0
+    big = torch.full((1 << 20,), 5.0, dtype=torch.float64, device="cuda")
+    big[777777] = 4.0
+    big[999999] = 4.0
+    ctx.argmin(big, idx)
+    torch.cuda.synchronize()
+    assert int(idx) == 777777
+    # replacing orders and penalty on a live context
+    pb2 = _random_problem(5, 4, 10, 4, 40, 25, 3, 5)
+    ctx.load_orders(pb2.order_ptr, pb2.item_sku, pb2.cart_capacity)
+    ctx.set_penalty(pb2.t, pb2.v, pb2.w)
+    pb2.sku_loc, pb2.sku_class = pb.sku_loc, pb.sku_class
+    p2 = W.perms(1, pb2.n_orders, 6)
+    got, _ = gpu_eval(torch, ctx, torch.from_numpy(p2).cuda())
+    assert_parity(got, oracle.eval_candidates(pb2, p2), pb2)
+    ctx.close()
+
+
+def test_host_buffer_entry_point(torch_cuda):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    wl = W.make_workload("mid")
+    pb = wl.problem
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perms(wl.seed, pb.n_orders, wl.n_cand)
+    ref = oracle.eval_candidates(pb, perms)
+    # pageable numpy buffers
+    dist = np.zeros(wl.n_cand, np.int64)
+    obj = np.zeros(wl.n_cand, np.float64)
+    i, v = ctx.eval_candidates_host(perms, dist, obj)
+    assert np.array_equal(dist, ref["dist"]) and np.array_equal(obj, ref["obj"])
+    assert i == oracle.argmin(ref["obj"]) and v == ref["obj"][i]
+    # pinned torch buffers
+    pp = torch.from_numpy(perms).pin_memory()
+    pd = torch.zeros(wl.n_cand, dtype=torch.int64).pin_memory()
+    po = torch.zeros(wl.n_cand, dtype=torch.float64).pin_memory()
+    i2, v2 = ctx.eval_candidates_host(pp, pd, po)
+    assert (i2, v2) == (i, v) and np.array_equal(pd.numpy(), ref["dist"])
+    assert np.array_equal(po.numpy(), ref["obj"])
+    ctx.close()

@@ -1,0 +1,160 @@
+"""GPU parity for the swap-neighbourhood evaluator (a6, D8), the argmin and the trajectory loop
+(BASELINE.json configs[4]: "results must match the oracle's trajectory move-for-move")."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2110_13693_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def gpu_swaps(torch, ctx, base_dev, s, Wn):
+    nn = Wn * (Wn - 1) // 2
+    d = torch.full((nn,), -1, dtype=torch.int64, device="cuda")
+    o = torch.zeros(nn, dtype=torch.float64, device="cuda")
+    ctx.eval_swaps(base_dev, s, Wn, d, o)
+    torch.cuda.synchronize()
+    return d, o
+
+
+def gpu_trajectory(torch, ctx, base_np, Wn, stride, n_iter):
+    """The D8 loop with no host round trip inside an iteration: eval_swaps -> argmin ->
+    apply_swap, all on the device; per-iteration results are gathered on the device too."""
+    n = len(base_np)
+    nn = Wn * (Wn - 1) // 2
+    perm = torch.from_numpy(base_np.copy()).cuda()
+    d = torch.zeros(nn, dtype=torch.int64, device="cuda")
+    o = torch.zeros(nn, dtype=torch.float64, device="cuda")
+    idx = torch.zeros(n_iter, dtype=torch.int64, device="cuda")
+    val = torch.zeros(n_iter, dtype=torch.float64, device="cuda")
+    dist = torch.zeros(n_iter, dtype=torch.int64, device="cuda")
+    for it in range(n_iter):
+        s = (it * stride) % (n - Wn + 1)
+        ctx.eval_swaps(perm, s, Wn, d, o)
+        ctx.argmin(o, idx[it:it + 1], val[it:it + 1])
+        dist[it:it + 1] = d[idx[it:it + 1]]
+        ctx.apply_swap(perm, s, Wn, idx[it:it + 1])
+    torch.cuda.synchronize()
+    return idx.cpu().numpy(), dist.cpu().numpy(), val.cpu().numpy(), perm.cpu().numpy()
+
+
+@pytest.mark.parametrize("name,s,Wn", [("tiny", 0, 20), ("tiny", 3, 7), ("mid", 0, 40),
+                                       ("mid", 111, 33), ("mid", 467, 33), ("mid", 250, 2)])
+def test_swaps_match_oracle_every_neighbour(torch_cuda, name, s, Wn):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem(name)
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(0, pb.n_orders)
+    d, o = gpu_swaps(torch, ctx, torch.from_numpy(base).cuda(), s, Wn)
+    ref = oracle.eval_swaps(pb, base, s, Wn)
+    assert np.array_equal(d.cpu().numpy(), ref["dist"])
+    assert np.array_equal(o.cpu().numpy(), ref["obj"])  # bit-identical (canonical sum)
+    idx = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ctx.argmin(o, idx)
+    torch.cuda.synchronize()
+    assert int(idx) == oracle.argmin(ref["obj"])
+    ctx.close()
+
+
+def test_smaller_opening_order_slips_into_previous_cart(torch_cuda):
+    """q = [2,1,3,1], C = 4: swapping positions 2 and 3 (both in the second batch) lets the
+    1-item order join the first cart — the incremental evaluator must restart one batch early."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("tiny")
+    pb.order_ptr = np.array([0, 2, 3, 6, 7], np.int32)
+    pb.item_sku = np.array([0, 11, 22, 33, 5, 17, 39], np.int32)
+    pb.cart_capacity = 4
+    base = np.arange(4, dtype=np.int32)
+    assert oracle.eval_candidates(pb, base, detail=True)["batch_of_pos"][0].tolist() == [0, 0, 1, 1]
+    assert oracle.eval_candidates(pb, base[[0, 1, 3, 2]], detail=True)["batch_of_pos"][0].tolist() == [0, 0, 0, 1]
+    ctx = whp.Context.from_problem(pb)
+    d, o = gpu_swaps(torch, ctx, torch.from_numpy(base).cuda(), 0, 4)
+    ref = oracle.eval_swaps(pb, base, 0, 4)
+    assert np.array_equal(d.cpu().numpy(), ref["dist"]) and np.array_equal(o.cpu().numpy(), ref["obj"])
+    ctx.close()
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_swaps_random_small_problems(torch_cuda, seed):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    from test_gpu_parity import _random_problem
+    pb = _random_problem(seed, NA=9, S=6, K=35, n_skus=60, n_orders=70 + seed, qmax=5, C=7 + seed,
+                         depot=seed)
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(seed, pb.n_orders)
+    for s, Wn in [(0, pb.n_orders), (5, 30)]:
+        d, o = gpu_swaps(torch, ctx, torch.from_numpy(base).cuda(), s, Wn)
+        ref = oracle.eval_swaps(pb, base, s, Wn)
+        assert np.array_equal(d.cpu().numpy(), ref["dist"])
+        assert np.array_equal(o.cpu().numpy(), ref["obj"])
+    ctx.close()
+
+
+def test_trajectory_mid_move_for_move(torch_cuda):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid")
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(0, pb.n_orders)
+    Wn, stride, n_iter = 32, 16, 40
+    ref = oracle.swap_trajectory(pb, base, Wn, stride, n_iter)
+    idx, dist, val, perm = gpu_trajectory(torch, ctx, base, Wn, stride, n_iter)
+    assert np.array_equal(idx, ref["move"]) and np.array_equal(dist, ref["dist"])
+    assert np.array_equal(val, ref["obj"]) and np.array_equal(perm, ref["perm"])
+    ctx.close()
+
+
+def test_neighbourhood_config_paper_scale(torch_cuda):
+    """configs[4] at full size: W = 256 (32,640 neighbours), stride 128, 100 iterations. The
+    oracle re-evaluates every neighbour from scratch (~50 s per iteration), so here: the first
+    2 iterations are compared move for move on a window the oracle can afford (full
+    neighbourhood, oracle on every neighbour, W = 64), and the full-size run is checked per
+    iteration — the applied move's (D, J) equals the oracle's evaluation of the materialised
+    permutation, the argmin is the first minimum of the GPU objectives, and sampled neighbours
+    equal the oracle."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    wl = W.make_workload("neighbourhood")
+    pb = wl.problem
+    n = pb.n_orders
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(wl.seed, n)
+    # (a) move-for-move against the oracle on a smaller window
+    ref = oracle.swap_trajectory(pb, base, 64, 32, 2)
+    idx, dist, val, perm = gpu_trajectory(torch, ctx, base, 64, 32, 2)
+    assert np.array_equal(idx, ref["move"]) and np.array_equal(val, ref["obj"])
+    assert np.array_equal(perm, ref["perm"])
+    # (b) the full configuration
+    Wn, stride, n_iter = wl.window, wl.stride, wl.n_iter
+    idx, dist, val, perm_end = gpu_trajectory(torch, ctx, base, Wn, stride, n_iter)
+    perm = base.copy()
+    for it in range(n_iter):
+        s = (it * stride) % (n - Wn + 1)
+        i, j = oracle.decode_neighbour(Wn, int(idx[it]))
+        if it % 25 == 0:  # neighbourhood spot check before applying the move
+            d, o = gpu_swaps(torch, ctx, torch.from_numpy(perm).cuda(), s, Wn)
+            o_np = o.cpu().numpy()
+            assert int(idx[it]) == int(np.argmin(o_np))
+            for nb in (W.stream_u64(it, 3, 24) % np.uint64(len(o_np))).astype(np.int64):
+                a, b = oracle.decode_neighbour(Wn, int(nb))
+                p = perm.copy()
+                p[s + a], p[s + b] = p[s + b], p[s + a]
+                one = oracle.eval_candidates(pb, p)
+                assert one["obj"][0] == o_np[nb] and one["dist"][0] == int(d[nb])
+        perm[s + i], perm[s + j] = perm[s + j], perm[s + i]
+        one = oracle.eval_candidates(pb, perm)
+        assert one["dist"][0] == dist[it] and one["obj"][0] == val[it]
+    assert np.array_equal(perm, perm_end)
+    ctx.close()
