@@ -36,11 +36,13 @@ template <class T>
 void dfree(T*& p) { if (p) { cudaFree(p); p = nullptr; } }
 
 void free_orders(whp_ctx* c) {
-  dfree(c->d_order_rec); dfree(c->d_pick_rec);
+  dfree(c->d_order_rec); dfree(c->d_pick_rec); dfree(c->d_pick_fast);
   dfree(c->base.bstart); dfree(c->base.bop); dfree(c->base.bdist); dfree(c->base.bclass);
   dfree(c->base.resp); dfree(c->base.totals);
   dfree(c->d_stage[0]); dfree(c->d_stage[1]);
   c->stage_rows = 0;
+  dfree(c->d_bpos); dfree(c->d_nb); dfree(c->d_dist_scratch); dfree(c->d_r_scratch);
+  c->fast_cap = 0; c->fast_pitch = 0;
   c->have_orders = false;
 }
 
@@ -99,10 +101,12 @@ whp_status whp_create_layout(int32_t n_aisles, int32_t slots_per_side, int32_t s
   if (cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess) { whp_destroy(c); return WHP_ERR_CUDA; }
   c->num_sms = prop.multiProcessorCount;
   c->argmin_cap = c->num_sms * 4;
+  c->smem_optin = (int)prop.sharedMemPerBlockOptin;
   cudaError_t e = cudaMalloc(&c->d_tvw, sizeof(double) * 3 * (size_t)n_classes);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_argmin_part, 16 * (size_t)c->argmin_cap + 16);
   if (e == cudaSuccess) e = cudaMemset(c->d_argmin_part, 0, 16 * (size_t)c->argmin_cap + 16);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_count, sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_task, 2 * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_h_idx, sizeof(int64_t));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_h_val, sizeof(double));
   for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
@@ -144,7 +148,7 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
     const int32_t loc = c->h_sku_loc[item_sku[i]];
     const uint32_t aisle = (uint32_t)(loc / (2 * S)), side = (uint32_t)((loc % (2 * S)) / S);
     const uint32_t slot1 = (uint32_t)(loc % S) + 1u;
-    prec[i] = (aisle << WHP_PICK_AISLE_SHIFT) | (slot1 << WHP_PICK_SLOT_SHIFT) |
+    prec[i] = WHP_PICK_PACK_AISLE(aisle) | (slot1 << WHP_PICK_SLOT_SHIFT) |
               (side << WHP_PICK_LOC_SHIFT) | (uint32_t)c->h_sku_class[item_sku[i]];
   }
   device_guard dg(c->device);
@@ -154,6 +158,7 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   const size_t no = (size_t)n_orders;
   WHP_CUDA(c, cudaMalloc(&c->d_order_rec, 4 * no));
   WHP_CUDA(c, cudaMalloc(&c->d_pick_rec, 4 * (size_t)n_items));
+  WHP_CUDA(c, cudaMalloc(&c->d_pick_fast, 4 * (size_t)n_items));
   WHP_CUDA(c, cudaMalloc(&c->base.bstart, 4 * (no + 1)));
   WHP_CUDA(c, cudaMalloc(&c->base.bop, 4 * no));
   WHP_CUDA(c, cudaMalloc(&c->base.bdist, 8 * (no + 1)));
@@ -162,6 +167,11 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   WHP_CUDA(c, cudaMalloc(&c->base.totals, 16));
   WHP_CUDA(c, cudaMemcpy(c->d_order_rec, orec.data(), 4 * no, cudaMemcpyHostToDevice));
   WHP_CUDA(c, cudaMemcpy(c->d_pick_rec, prec.data(), 4 * (size_t)n_items, cudaMemcpyHostToDevice));
+  for (int32_t o = 0; o < n_orders; ++o) {  // K2's copy: the side bit becomes the end-of-order flag
+    for (int32_t i = order_ptr[o]; i < order_ptr[o + 1]; ++i) prec[i] &= ~(1u << WHP_PICK_LOC_SHIFT);
+    prec[order_ptr[o + 1] - 1] |= 1u << WHP_PICK_LOC_SHIFT;
+  }
+  WHP_CUDA(c, cudaMemcpy(c->d_pick_fast, prec.data(), 4 * (size_t)n_items, cudaMemcpyHostToDevice));
   c->have_orders = true;
   return WHP_OK;
 }
@@ -330,7 +340,7 @@ void whp_destroy(whp_ctx* c) {
     device_guard dg(c->device);
     cudaDeviceSynchronize();
     free_orders(c);
-    dfree(c->d_tvw); dfree(c->d_argmin_part); dfree(c->d_count);
+    dfree(c->d_tvw); dfree(c->d_argmin_part); dfree(c->d_count); dfree(c->d_task);
     dfree(c->d_h_dist); dfree(c->d_h_obj); dfree(c->d_h_idx); dfree(c->d_h_val);
     for (int k = 0; k < 2; ++k) {
       if (c->s_copy[k]) cudaStreamDestroy(c->s_copy[k]);

@@ -1,6 +1,8 @@
 // whp_eval.cu — whp_eval_candidates: a1–a5 for explicit candidate plans.
 // General kernel: one warp per candidate over the general walker (whp_walk.cuh); supports
 // every output and any geometry within the limits.
+#include <cstdlib>
+
 #include "whp_walk.cuh"
 
 namespace {
@@ -53,6 +55,8 @@ cudaError_t whp_launch_eval(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
                             const whp_eval_out& out, cudaStream_t st) {
   const whp_tables T = whp_make_tables(c);
   const bool detail = out.batch_of_pos || out.n_distinct || out.resp;
+  if (!detail && whp_fast_eligible(c) && getenv("WHP_FORCE_GENERAL") == nullptr)
+    return whp_launch_eval_fast(c, d_perms, n_cand, out, st);
   int64_t blocks = (n_cand + kWarpsPerBlock - 1) / kWarpsPerBlock;
   const int64_t cap = (int64_t)c->num_sms * 64;
   if (blocks > cap) blocks = cap;

@@ -10,12 +10,15 @@
 
 // ---- packed device tables -----------------------------------------------------
 // order record, 32 bit:  item_off[31:8] | q[7:0]            (q = number of items, 1..255)
-// pick  record, 32 bit:  aisle[30:21] | slot1[20:9] | side[8] | class[7:0]
-//   slot1 = slot + 1 (depth = slot1 * slot_pitch). The field order makes an unsigned max over
-//   the records of a batch return (a_max, deepest slot in a_max) in its top 22 bits (D3).
+// pick  record, 32 bit:  a_hi[31:26] | 0 [25] | a_lo[24:21] | slot1[20:9] | side[8] | class[7:0]
+//   aisle = a_hi*16 + a_lo; slot1 = slot + 1 (depth = slot1 * slot_pitch). The field order makes
+//   an unsigned max over the records of a batch return (a_max, deepest slot in a_max) in its
+//   top 23 bits (D3). The zero spacer bit lets (rec >> 21) feed a 5-bit shift amount directly
+//   (bit index inside a 16-aisle word) and a_hi = rec >> 26 index the word, without masks.
 #define WHP_Q_BITS 8
 #define WHP_Q_MASK 0xffu
-#define WHP_PICK_AISLE_SHIFT 21
+#define WHP_PICK_PACK_AISLE(a) ((((uint32_t)(a) >> 4) << 26) | (((uint32_t)(a) & 15u) << 21))
+#define WHP_PICK_AISLE(rec) ((((rec) >> 26) << 4) | (((rec) >> 21) & 15u))
 #define WHP_PICK_SLOT_SHIFT 9
 #define WHP_PICK_SLOT_MASK 0xfffu
 #define WHP_PICK_LOC_SHIFT 8 /* rec >> 8 identifies the location (aisle, slot, side) */
@@ -73,6 +76,7 @@ struct whp_ctx {
   int32_t n_orders = 0, n_items = 0, C = 0;
   uint32_t* d_order_rec = nullptr;
   uint32_t* d_pick_rec = nullptr;
+  uint32_t* d_pick_fast = nullptr;  // pick records with bit 8 = "last pick of its order" (K2)
   double* d_tvw = nullptr;
   bool have_orders = false, have_penalty = false;
   // scratch
@@ -80,6 +84,15 @@ struct whp_ctx {
   void* d_argmin_part = nullptr;  // partial (val, idx) pairs + ticket
   int32_t argmin_cap = 0;
   unsigned long long* d_count = nullptr;  // validate_perms counter
+  // fast candidate path scratch (whp_fast.cu), grow-only
+  uint16_t* d_bpos = nullptr;        // [fast_cap][fast_pitch] batch start positions
+  int32_t* d_nb = nullptr;           // [fast_cap]
+  int64_t* d_dist_scratch = nullptr; // [fast_cap]
+  uint32_t* d_r_scratch = nullptr;   // [fast_cap][ceil(K/2)] packed 16-bit responses
+  unsigned long long* d_task = nullptr;  // [2] work-stealing counter, max batch load
+  int64_t fast_cap = 0;
+  int32_t fast_pitch = 0;
+  int smem_optin = 0;
   // host-path staging (whp_eval_candidates_host)
   int32_t* d_stage[2] = {nullptr, nullptr};
   int64_t stage_rows = 0;
@@ -101,6 +114,9 @@ whp_tables whp_make_tables(const whp_ctx* c);
 // kernels' host launchers (each returns the cudaError_t of the launch)
 cudaError_t whp_launch_eval(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
                             const whp_eval_out& out, cudaStream_t st);
+bool whp_fast_eligible(const whp_ctx* c);
+cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
+                                 const whp_eval_out& out, cudaStream_t st);
 cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                              int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st);
 cudaError_t whp_launch_argmin(whp_ctx* c, const double* d_obj, int64_t n, int64_t* d_idx,

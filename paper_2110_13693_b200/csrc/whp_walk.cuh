@@ -56,7 +56,7 @@ __device__ __forceinline__ void whp_close_batch(const whp_tables& T, whp_warp_sm
   const int m = __reduce_add_sync(WHP_FULL, __popc(aw));
   const int lo = aw ? lane * 32 + __ffs(aw) - 1 : 0x7fffffff;
   const int64_t a_min = __reduce_min_sync(WHP_FULL, lo);
-  const int64_t a_max = st.kmax >> WHP_PICK_AISLE_SHIFT;
+  const int64_t a_max = WHP_PICK_AISLE(st.kmax);
   const int64_t d_last =
       (int64_t)((st.kmax >> WHP_PICK_SLOT_SHIFT) & WHP_PICK_SLOT_MASK) * T.g.slot_pitch;
   const int64_t a0 = T.g.depot_aisle;
@@ -143,7 +143,7 @@ __device__ __forceinline__ int32_t whp_walk(const whp_tables& T, whp_warp_smem* 
         for (int32_t i = 0; i < q; ++i) {
           const uint32_t pr = __ldg(T.pick_rec + off + i);
           km = max(km, pr);
-          const uint32_t a = pr >> WHP_PICK_AISLE_SHIFT;
+          const uint32_t a = WHP_PICK_AISLE(pr);
           const uint32_t c = pr & WHP_PICK_CLASS_MASK;
           atomicOr(&sm->amask[a >> 5], 1u << (a & 31));
           atomicOr(&sm->cmask[c >> 5], 1u << (c & 31));

@@ -3,6 +3,8 @@ on the same seeded inputs. Bars (BASELINE.json north_star): bit-exact batch assi
 distances, responses and argmin index; fp64 penalty / objective within 1e-9 relative (the
 canonical summation order of D6 makes them bit-identical in practice, which is also asserted
 where the argmin depends on it)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -20,6 +22,14 @@ def torch_cuda():
     if not torch.cuda.is_available():
         pytest.skip("no CUDA device")
     return torch
+
+
+class force_general:
+    """Route non-detail calls through the general walker instead of the tuned K1/K2/K3 path."""
+    def __enter__(self):
+        os.environ["WHP_FORCE_GENERAL"] = "1"
+    def __exit__(self, *a):
+        os.environ.pop("WHP_FORCE_GENERAL", None)
 
 
 def gpu_eval(torch, ctx, perms_dev, detail=False):
@@ -82,6 +92,9 @@ def test_all_candidates_full_detail(torch_cuda, name):
     # the timed path (no detail outputs) must give the same numbers
     got2, dev2 = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=False)
     assert_parity(got2, ref, pb)
+    with force_general():
+        got3, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=False)
+    assert_parity(got3, ref, pb)
     i, v = gpu_argmin(torch, ctx, dev2["obj"])
     assert i == oracle.argmin(ref["obj"]) and v == ref["obj"][i]
     ctx.close()
@@ -196,6 +209,15 @@ EDGE = [
     dict(NA=1024, S=30, K=256, n_skus=5000, n_orders=1000, qmax=12, C=40, depot=1023, pitch=3, spacing=7),
     dict(NA=400, S=4095, K=200, n_skus=3000, n_orders=333, qmax=255, C=600),    # limits: q, slots
     dict(NA=33, S=17, K=40, n_skus=100, n_orders=129, qmax=5, C=70),    # batches longer than a tile
+    # multiples of 4 orders: these run the tuned K1/K2/K3 path
+    dict(NA=1, S=1, K=1, n_skus=1, n_orders=4, qmax=1, C=1),
+    dict(NA=5, S=9, K=3, n_skus=30, n_orders=32, qmax=4, C=4),
+    dict(NA=17, S=9, K=255, n_skus=300, n_orders=260, qmax=9, C=9, depot=5, pitch=2),
+    dict(NA=1024, S=30, K=256, n_skus=5000, n_orders=1000, qmax=12, C=40, depot=1023, pitch=3, spacing=7),
+    dict(NA=1024, S=30, K=256, n_skus=5000, n_orders=1000, qmax=12, C=40),
+    dict(NA=400, S=4095, K=200, n_skus=3000, n_orders=332, qmax=255, C=600),
+    dict(NA=40, S=50, K=20, n_skus=900, n_orders=2000, qmax=2, C=2),    # ~1,500 batches per plan
+    dict(NA=40, S=50, K=20, n_skus=900, n_orders=64, qmax=3, C=100000), # one batch, huge cart
 ]
 
 
@@ -211,6 +233,14 @@ def test_edge_cases(torch_cuda, cfg):
     assert_parity(got, ref, pb, detail=True)
     got2, dev2 = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
     assert_parity(got2, ref, pb)
+    with force_general():
+        got3, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
+    assert_parity(got3, ref, pb)
+    for seg in ("1", "2", "32"):  # segment counts of the tuned path (ignored when not legal)
+        os.environ["WHP_SEGMENTS"] = seg
+        got4, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
+        os.environ.pop("WHP_SEGMENTS")
+        assert_parity(got4, ref, pb)
     i, v = gpu_argmin(torch, ctx, dev2["obj"])
     assert i == oracle.argmin(ref["obj"])
     ctx.close()
