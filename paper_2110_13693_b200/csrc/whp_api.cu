@@ -36,13 +36,14 @@ template <class T>
 void dfree(T*& p) { if (p) { cudaFree(p); p = nullptr; } }
 
 void free_orders(whp_ctx* c) {
-  dfree(c->d_order_rec); dfree(c->d_pick_rec); dfree(c->d_pick_fast);
+  dfree(c->d_order_rec); dfree(c->d_pick_rec); dfree(c->d_pick_fast); dfree(c->d_order_fast);
   dfree(c->base.bstart); dfree(c->base.bop); dfree(c->base.bdist); dfree(c->base.bclass);
   dfree(c->base.resp); dfree(c->base.totals);
   dfree(c->d_stage[0]); dfree(c->d_stage[1]);
   c->stage_rows = 0;
-  dfree(c->d_bpos); dfree(c->d_nb); dfree(c->d_dist_scratch); dfree(c->d_r_scratch);
-  c->fast_cap = 0; c->fast_pitch = 0;
+  dfree(c->d_bmask); dfree(c->d_cstream); dfree(c->d_nb); dfree(c->d_dist_scratch);
+  dfree(c->d_planes);
+  c->fast_cap = 0; c->fast_pitch = 0; c->fast_plane_words = 0;
   c->have_orders = false;
 }
 
@@ -158,7 +159,6 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   const size_t no = (size_t)n_orders;
   WHP_CUDA(c, cudaMalloc(&c->d_order_rec, 4 * no));
   WHP_CUDA(c, cudaMalloc(&c->d_pick_rec, 4 * (size_t)n_items));
-  WHP_CUDA(c, cudaMalloc(&c->d_pick_fast, 4 * (size_t)n_items));
   WHP_CUDA(c, cudaMalloc(&c->base.bstart, 4 * (no + 1)));
   WHP_CUDA(c, cudaMalloc(&c->base.bop, 4 * no));
   WHP_CUDA(c, cudaMalloc(&c->base.bdist, 8 * (no + 1)));
@@ -167,11 +167,27 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   WHP_CUDA(c, cudaMalloc(&c->base.totals, 16));
   WHP_CUDA(c, cudaMemcpy(c->d_order_rec, orec.data(), 4 * no, cudaMemcpyHostToDevice));
   WHP_CUDA(c, cudaMemcpy(c->d_pick_rec, prec.data(), 4 * (size_t)n_items, cudaMemcpyHostToDevice));
-  for (int32_t o = 0; o < n_orders; ++o) {  // K2's copy: the side bit becomes the end-of-order flag
-    for (int32_t i = order_ptr[o]; i < order_ptr[o + 1]; ++i) prec[i] &= ~(1u << WHP_PICK_LOC_SHIFT);
-    prec[order_ptr[o + 1] - 1] |= 1u << WHP_PICK_LOC_SHIFT;
+  // tuned-path tables (layout in whp_internal.cuh)
+  std::vector<uint32_t> ofast((size_t)n_orders), pfast;
+  pfast.reserve((size_t)n_items + (size_t)n_orders);
+  bool fast_ok = true;
+  for (int32_t o = 0; o < n_orders; ++o) {
+    const size_t cur = pfast.size() / 2;
+    if (cur > 0xffff) fast_ok = false;
+    for (int32_t i = order_ptr[o]; i < order_ptr[o + 1]; ++i) {
+      uint32_t r = prec[i] & ~(1u << WHP_PICK_LOC_SHIFT);
+      if (i == order_ptr[o + 1] - 1) r |= 1u << WHP_PICK_LOC_SHIFT;
+      pfast.push_back(r);
+    }
+    if (pfast.size() & 1) pfast.push_back(0u);
+    ofast[o] = ((uint32_t)(cur & 0xffff) << WHP_Q_BITS) | (uint32_t)(order_ptr[o + 1] - order_ptr[o]);
   }
-  WHP_CUDA(c, cudaMemcpy(c->d_pick_fast, prec.data(), 4 * (size_t)n_items, cudaMemcpyHostToDevice));
+  c->n_items_pad = (int32_t)pfast.size();
+  c->fast_tables_ok = fast_ok;
+  WHP_CUDA(c, cudaMalloc(&c->d_pick_fast, 4 * pfast.size()));
+  WHP_CUDA(c, cudaMalloc(&c->d_order_fast, 4 * no));
+  WHP_CUDA(c, cudaMemcpy(c->d_pick_fast, pfast.data(), 4 * pfast.size(), cudaMemcpyHostToDevice));
+  WHP_CUDA(c, cudaMemcpy(c->d_order_fast, ofast.data(), 4 * no, cudaMemcpyHostToDevice));
   c->have_orders = true;
   return WHP_OK;
 }

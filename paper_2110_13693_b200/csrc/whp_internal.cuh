@@ -76,7 +76,12 @@ struct whp_ctx {
   int32_t n_orders = 0, n_items = 0, C = 0;
   uint32_t* d_order_rec = nullptr;
   uint32_t* d_pick_rec = nullptr;
-  uint32_t* d_pick_fast = nullptr;  // pick records with bit 8 = "last pick of its order" (K2)
+  // tuned-path tables: every order's picks start at an even index (one pad word after an odd
+  // order), bit 8 = "last pick of its order"; order_fast = (first_pick_index/2) << 8 | q
+  uint32_t* d_pick_fast = nullptr;
+  uint32_t* d_order_fast = nullptr;
+  int32_t n_items_pad = 0;
+  bool fast_tables_ok = false;
   double* d_tvw = nullptr;
   bool have_orders = false, have_penalty = false;
   // scratch
@@ -85,12 +90,13 @@ struct whp_ctx {
   int32_t argmin_cap = 0;
   unsigned long long* d_count = nullptr;  // validate_perms counter
   // fast candidate path scratch (whp_fast.cu), grow-only
-  uint16_t* d_bpos = nullptr;        // [fast_cap][fast_pitch] batch start positions
+  uint32_t* d_bmask = nullptr;       // [fast_cap][fast_pitch] bitmask of batch-start positions
+  uint16_t* d_cstream = nullptr;     // [fast_cap][cs_pitch] first-pick cursor of every position
   int32_t* d_nb = nullptr;           // [fast_cap]
   int64_t* d_dist_scratch = nullptr; // [fast_cap]
-  uint32_t* d_r_scratch = nullptr;   // [fast_cap][ceil(K/2)] packed 16-bit responses
-  unsigned long long* d_task = nullptr;  // [2] work-stealing counter, max batch load
-  int64_t fast_cap = 0;
+  uint32_t* d_planes = nullptr;      // [fast_cap][S][8 planes][KW] bit-sliced class counters
+  unsigned long long* d_task = nullptr;  // [2] work-stealing counter
+  int64_t fast_cap = 0, fast_plane_words = 0;
   int32_t fast_pitch = 0;
   int smem_optin = 0;
   // host-path staging (whp_eval_candidates_host)

@@ -95,6 +95,11 @@ def test_all_candidates_full_detail(torch_cuda, name):
     with force_general():
         got3, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=False)
     assert_parity(got3, ref, pb)
+    # responses alone come from the tuned path's vertical counters
+    resp = torch.full((wl.n_cand, pb.n_classes), -1, dtype=torch.int32, device="cuda")
+    ctx.eval_candidates(torch.from_numpy(perms).cuda(), resp=resp)
+    torch.cuda.synchronize()
+    assert np.array_equal(resp.cpu().numpy(), ref["resp"])
     i, v = gpu_argmin(torch, ctx, dev2["obj"])
     assert i == oracle.argmin(ref["obj"]) and v == ref["obj"][i]
     ctx.close()
