@@ -39,6 +39,10 @@ __device__ __forceinline__ int4 lds128(uint32_t a) {
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) {
   asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v));
 }
+// if (k < n) st.shared [a] = v — predicated, never a branch
+__device__ __forceinline__ void sts32_if_lt(uint32_t k, uint32_t n, uint32_t a, uint32_t v) {
+  asm volatile("{ .reg .pred pq; setp.lt.u32 pq, %0, %1; @pq st.shared.u32 [%2], %3; }" ::"r"(k), "r"(n), "r"(a), "r"(v));
+}
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
 }
@@ -66,63 +70,85 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
   uint32_t* sorec = reinterpret_cast<uint32_t*>(smem_raw + kRing * kBoundsThreads * 16);
   const uint32_t sorec0 = smem_u32(sorec);
   for (int i = threadIdx.x; i < n_orders; i += kBoundsThreads) sorec[i] = __ldg(order_fast + i);
-  const int64_t c_raw = (int64_t)blockIdx.x * kBoundsThreads + threadIdx.x;
-  const bool have = c_raw < n_cand;
-  const int64_t c = have ? c_raw : n_cand - 1;  // idle tail threads redo the last row, no writes
-  const int4* __restrict__ row = reinterpret_cast<const int4*>(perms + c * n_orders);
+  const int64_t c = (int64_t)blockIdx.x * kBoundsThreads + threadIdx.x;
+  const bool have = c < n_cand;
+  const int4* __restrict__ row = reinterpret_cast<const int4*>(perms + (have ? c : 0) * n_orders);
   const int n4 = n_orders >> 2;
+  if (have) {
 #pragma unroll 1
-  for (int k = 0; k < kRing; ++k) {
-    if (k < n4) cp_async16(ring0 + k * (kBoundsThreads * 16), row + k);
-    cp_async_commit();
+    for (int k = 0; k < kRing; ++k) {
+      if (k < n4) cp_async16(ring0 + k * (kBoundsThreads * 16), row + k);
+      cp_async_commit();
+    }
   }
   __syncthreads();  // sorec visible
+  if (!have) return;
   uint32_t* __restrict__ bm = bmask + c * bm_pitch;
   uint2* __restrict__ cs = reinterpret_cast<uint2*>(cstream + c * cs_pitch);
   const int nw = (n_orders + 31) >> 5;
   int load = 0;
   uint32_t nb = 0;
   int p4 = 0, slot = 0;
+  // 3-stage software pipeline, one chunk (4 positions) per stage: (A) order ids of chunk i+2
+  // leave the cp.async ring, (B) their order records are gathered for chunk i+1, (C) chunk i
+  // runs the next-fit recurrence — the only loop-carried dependency chain.
+  int4 ids = make_int4(0, 0, 0, 0);
+  uint32_t rb[4] = {0, 0, 0, 0}, rc[4] = {0, 0, 0, 0};
+  auto stage_a = [&](int chunk) {  // chunk may run past the row end: the slot is then stale
+    cp_async_wait<kRing - 1>();
+    const uint32_t slot_addr = ring0 + slot * (kBoundsThreads * 16);
+    const int4 v = lds128(slot_addr);
+    if (chunk + kRing < n4) cp_async16(slot_addr, row + chunk + kRing);
+    cp_async_commit();
+    slot = (slot + 1) & (kRing - 1);
+    return v;
+  };
+  auto stage_b = [&](const int4& v, uint32_t (&r)[4]) {
+    // ids past the row end are stale ring contents: clamp so the gather stays in the table
+    r[0] = lds32(sorec0 + 4 * min((uint32_t)v.x, (uint32_t)n_orders - 1));
+    r[1] = lds32(sorec0 + 4 * min((uint32_t)v.y, (uint32_t)n_orders - 1));
+    r[2] = lds32(sorec0 + 4 * min((uint32_t)v.z, (uint32_t)n_orders - 1));
+    r[3] = lds32(sorec0 + 4 * min((uint32_t)v.w, (uint32_t)n_orders - 1));
+  };
+  ids = stage_a(0);
+  stage_b(ids, rc);
+  ids = stage_a(1);
+  stage_b(ids, rb);
+  ids = stage_a(2);
 #pragma unroll 1
   for (int w = 0; w < nw; ++w) {
     uint32_t bits = (w == 0) ? 1u : 0u;  // batch 0 starts at position 0
 #pragma unroll
     for (int k = 0; k < 8; ++k, ++p4) {
       if (p4 < n4) {
-        cp_async_wait<kRing - 1>();
-        const uint32_t slot_addr = ring0 + slot * (kBoundsThreads * 16);
-        const int4 v = lds128(slot_addr);
-        const uint32_t r0 = lds32(sorec0 + 4 * v.x), r1 = lds32(sorec0 + 4 * v.y);
-        const uint32_t r2 = lds32(sorec0 + 4 * v.z), r3 = lds32(sorec0 + 4 * v.w);
-        if (p4 + kRing < n4) cp_async16(slot_addr, row + p4 + kRing);
-        cp_async_commit();
-        slot = (slot + 1) & (kRing - 1);
-        if (have)  // cursor stream: 4 x u16 = bits 8..23 of the order records
-          cs[p4] = make_uint2(__byte_perm(r0, r1, 0x6521), __byte_perm(r2, r3, 0x6521));
-        const uint32_t rr[4] = {r0, r1, r2, r3};
+        uint32_t rn[4];
+        stage_b(ids, rn);        // chunk p4 + 2
+        ids = stage_a(p4 + 3);
+        // cursor stream: 4 x u16 = bits 8..23 of the order records
+        cs[p4] = make_uint2(__byte_perm(rc[0], rc[1], 0x6521), __byte_perm(rc[2], rc[3], 0x6521));
 #pragma unroll
         for (int t = 0; t < 4; ++t) {
-          const int q = (int)(rr[t] & WHP_Q_MASK);
+          const int q = (int)(rc[t] & WHP_Q_MASK);
           const int load2 = load + q;
           const bool over = load2 > C;
           load = over ? q : load2;
           if (over) bits |= 1u << (4 * k + t);
+          rc[t] = rb[t];
+          rb[t] = rn[t];
         }
       }
     }
     nb += __popc(bits);
     if (w == (n_orders >> 5)) bits |= 1u << (n_orders & 31);  // end sentinel in a partial word
-    if (have) bm[w] = bits;
+    bm[w] = bits;
   }
-  if (!have) return;
   if ((n_orders & 31) == 0) bm[nw] = 1u;  // end sentinel in a word of its own
   nb_scratch[c] = (int32_t)nb;
   if (n_batches_out) n_batches_out[c] = (int32_t)nb;
 }
 
 // ------------------------------------------------------------------------------------------ K2
-constexpr int kIdRing = 4;   // 16-byte cursor chunks (8 cursors) in flight per lane
-constexpr int kPlanes = 8;   // vertical counter bit planes: up to 255 batches per segment
+constexpr int kMaxPlanes = 8;  // vertical counter bit planes: up to 255 batches per segment
 #define WHP_FAST_LAST 0x100u
 
 struct sets_params {
@@ -130,12 +156,13 @@ struct sets_params {
   int log2S;
   int aw_words;    // aisle words per lane  = ceil(NA/16)
   int ring_words;  // per-lane ring of first-pick cursors of the open batch = C + 2
+  int id_slots;    // 16-byte cursor-stream chunks resident per lane (power of two, covers a batch)
   int bm_pitch, cs_pitch;
   int n_items_pad;
   int64_t n_tasks;  // warp tasks = ceil(n_cand*S/32)
 };
 
-template <bool SMEM_TABLES, bool DEPOT0, int KW>
+template <bool SMEM_TABLES, bool DEPOT0, int KW, int kPlanes>
 __global__ void __launch_bounds__(512, 1)
 whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restrict__ pick_fast,
                 const uint16_t* __restrict__ cstream, const uint32_t* __restrict__ bmask,
@@ -154,7 +181,7 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
     __syncthreads();
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int priv_words = (CW + P.aw_words + P.ring_words + kIdRing * 4) * 32;
+  const int priv_words = (CW + P.aw_words + P.ring_words + P.id_slots * 4) * 32;
   // private words of this lane: word w at my_c[w*32] (bank = lane)
   uint32_t* my_c = priv + (size_t)warp * priv_words + lane;
   const uint32_t cbase = smem_u32(my_c);
@@ -214,23 +241,14 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
     uint32_t bw_next = __ldg(bm + min(wi + 1, P.bm_pitch - 1));
     int p = 32 * wi + __ffs(bw) - 1;  // first position of the segment
 
-    // ---- cursor stream of this lane through a private cp.async ring ([slot][lane] x 16 B)
+    // ---- cursor stream of this lane through a private cp.async ring ([slot][lane] x 16 B):
+    // chunk c (cursors of positions 8c..8c+7) lives in slot c mod kIdRing
     const uint4* __restrict__ cs = reinterpret_cast<const uint4*>(cstream + cand * P.cs_pitch);
-    int vi = p >> 3;  // next chunk to consume
-#pragma unroll
-    for (int k = 0; k < kIdRing; ++k) {
-      cp_async16(idring + ((vi + k) & (kIdRing - 1)) * 512, cs + min(vi + k, n8 - 1));
+    {
+      const int c0 = p >> 3;
+      for (int k = 0; k < P.id_slots; ++k)
+        cp_async16(idring + ((c0 + k) & (P.id_slots - 1)) * 512, cs + min(c0 + k, n8 - 1));
       cp_async_commit();
-    }
-    cp_async_wait<kIdRing - 1>();
-    int4 va = lds128(idring + (vi & (kIdRing - 1)) * 512);
-    cp_async16(idring + (vi & (kIdRing - 1)) * 512, cs + min(vi + kIdRing, n8 - 1));
-    cp_async_commit();
-    ++vi;
-    int vleft = 8 - (p & 7);
-    for (int k = p & 7; k > 0; --k) {
-      va.x = __funnelshift_r(va.x, va.y, 16); va.y = __funnelshift_r(va.y, va.z, 16);
-      va.z = __funnelshift_r(va.z, va.w, 16); va.w = (int)((uint32_t)va.w >> 16);
     }
 
     int64_t D = 0;
@@ -250,24 +268,36 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         p = pe;
       }
       const bool live = left > 0;
-      // ---- prefill the private ring with the first-pick cursor of every order of the batch
-      const int maxleft = __reduce_max_sync(WHP_FULL, left);
-      for (int k = 0; k < maxleft; ++k) {
-        if (k < left) {
-          const uint32_t cur16 = (uint32_t)va.x & 0xffffu;
-          va.x = __funnelshift_r(va.x, va.y, 16); va.y = __funnelshift_r(va.y, va.z, 16);
-          va.z = __funnelshift_r(va.z, va.w, 16); va.w = (int)((uint32_t)va.w >> 16);
-          if (--vleft == 0) {
-            const uint32_t slot = idring + (vi & (kIdRing - 1)) * 512;
-            cp_async_wait<kIdRing - 1>();
-            va = lds128(slot);
-            cp_async16(slot, cs + min(vi + kIdRing, n8 - 1));
-            cp_async_commit();
-            ++vi;
-            vleft = 8;
+      // ---- prefill the private ring with the first-pick cursor of every order of the batch,
+      // one 16-byte chunk (8 positions) of the cursor stream at a time
+      const int p0 = p - left;                       // first position of the batch
+      const int nc = live ? ((p - 1) >> 3) - (p0 >> 3) + 1 : 0;   // chunks the batch touches
+      const int nf = (p >> 3) - (p0 >> 3);           // chunks the batch finishes
+      const int ncmax = __reduce_max_sync(WHP_FULL, nc);
+      cp_async_wait<0>();  // issued a whole batch ago: normally complete already
+      for (int i = 0; i < ncmax; ++i) {
+        if (i < nc) {
+          const int c = (p0 >> 3) + i;
+          const int4 v = lds128(idring + (c & (P.id_slots - 1)) * 512);
+          const int kb = 8 * c - p0;               // ring index of the chunk's first cursor
+          const uint32_t rb = ring + kb * 128;
+          const uint32_t vv[4] = {(uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w};
+#pragma unroll
+          for (int e = 0; e < 8; ++e) {
+            const uint32_t c16 = (e & 1) ? (vv[e >> 1] >> 16) : (vv[e >> 1] & 0xffffu);
+            sts32_if_lt((uint32_t)(kb + e), (uint32_t)left, rb + e * 128,
+                        SMEM_TABLES ? pick_base + 8 * c16 : 2 * c16);
           }
-          sts32(ring + k * 128, SMEM_TABLES ? pick_base + 8 * cur16 : 2 * cur16);
         }
+      }
+      {  // refill the slots of the finished chunks; they land while the batch is processed
+        const int nfmax = __reduce_max_sync(WHP_FULL, nf);
+        for (int i = 0; i < nfmax; ++i)
+          if (i < nf) {
+            const int c = (p0 >> 3) + i;
+            cp_async16(idring + (c & (P.id_slots - 1)) * 512, cs + min(c + P.id_slots, n8 - 1));
+          }
+        cp_async_commit();
       }
       const uint32_t stamp_hi = (uint32_t)(j + 1) << 16;
       uint32_t kmax = 0, kmin = 0xffffffffu;
@@ -275,17 +305,17 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       uint32_t cur = lds32(ring);
       uint32_t n_cur = lds32(ring + 128);
       uint32_t rp = ring + 256;
+      const uint32_t rp_end = rp + 128 * left;  // the lane is done after `left` orders
       uint32_t rec = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
 #pragma unroll 1
       for (int t = 0; t < Cmax; ++t) {
-        if (left > 0) {
+        if (rp != rp_end) {
           // cursor of the next step's pick: next record, or the next order's first pick
           uint32_t nxt = cur + (SMEM_TABLES ? 4u : 1u);
           if (rec & WHP_FAST_LAST) {
             nxt = n_cur;
             n_cur = lds32(rp);
             rp += 128;
-            --left;
           }
           cur = nxt;
           const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
@@ -344,12 +374,34 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       dist_scratch[cand] = D;
       if (hash_out) hash_out[cand] = hash;
     }
-    if (have) {
-      uint32_t* __restrict__ po = planes_out + (cand * P.S + seg) * (kPlanes * KW);
+    // bit-sliced addition of the S lanes' vertical counters (one more plane per level)
+    {
+      uint32_t* __restrict__ po = planes_out + cand * ((kMaxPlanes + 5) * KW);
 #pragma unroll
-      for (int pp = 0; pp < kPlanes; ++pp)
+      for (int w = 0; w < KW; ++w) {
+        uint32_t a[kPlanes + 5];
 #pragma unroll
-        for (int w = 0; w < KW; ++w) po[pp * KW + w] = pl[pp][w];
+        for (int pp = 0; pp < kPlanes + 5; ++pp) a[pp] = pp < kPlanes ? pl[pp][w] : 0u;
+#pragma unroll
+        for (int lvl = 0; lvl < 5; ++lvl) {
+          if ((1 << lvl) < P.S) {
+            uint32_t carry = 0;
+#pragma unroll
+            for (int pp = 0; pp < kPlanes + lvl; ++pp) {
+              const uint32_t b = __shfl_xor_sync(WHP_FULL, a[pp], 1 << lvl);
+              const uint32_t sum = a[pp] ^ b ^ carry;
+              carry = (a[pp] & b) | (carry & (a[pp] ^ b));
+              a[pp] = sum;
+            }
+            a[kPlanes + lvl] = carry;
+          }
+        }
+        if (have && seg == 0) {
+#pragma unroll
+          for (int pp = 0; pp < kPlanes + 5; ++pp)
+            if (pp < kPlanes + P.log2S) po[pp * KW + w] = a[pp];
+        }
+      }
     }
     __syncwarp();
   }
@@ -360,20 +412,29 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
 // canonical 32-lane accumulation of D6.
 __global__ void __launch_bounds__(256)
 whp_finish_kernel(const whp_tables T, int64_t n_cand, const int64_t* __restrict__ dist_scratch,
-                  const uint32_t* __restrict__ planes, int S, int KW, int planes_used,
+                  const uint32_t* __restrict__ planes, int KW, int planes_used,
                   int64_t* __restrict__ dist, double* __restrict__ penalty,
                   double* __restrict__ obj, int32_t* __restrict__ resp) {
   const int lane = threadIdx.x & 31;
   const int64_t cand = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (cand >= n_cand) return;
-  const uint32_t* __restrict__ pc = planes + cand * S * (kPlanes * KW);
+  // the candidate's (kMaxPlanes+5) x KW counter words, one coalesced read, then warp broadcasts
+  const uint32_t* __restrict__ pc = planes + cand * ((kMaxPlanes + 5) * KW);
+  const int total = planes_used * KW;  // <= 13 * 8 = 104
+  uint32_t regs[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) regs[i] = (lane + 32 * i < total) ? __ldg(pc + lane + 32 * i) : 0u;
   double s = 0.0;
   const int kw_used = (T.K + 31) >> 5;
   for (int w = 0; w < kw_used; ++w) {
     int r = 0;
-    for (int seg = 0; seg < S; ++seg)
-      for (int pp = 0; pp < planes_used; ++pp)
-        r += (int)((__ldg(pc + (seg * kPlanes + pp) * KW + w) >> lane) & 1u) << pp;
+    for (int pp = 0; pp < planes_used; ++pp) {
+      const int idx = pp * KW + w;
+      const int hi = idx >> 5;
+      const uint32_t src = hi == 0 ? regs[0] : hi == 1 ? regs[1] : hi == 2 ? regs[2] : regs[3];
+      const uint32_t word = __shfl_sync(WHP_FULL, src, idx & 31);
+      r += (int)((word >> lane) & 1u) << pp;
+    }
     const int k = 32 * w + lane;
     if (k < T.K) {
       if (resp) resp[cand * T.K + k] = r;
@@ -417,12 +478,14 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   const int64_t nb_ub = nb_upper_bound(c);
   const int32_t bm_pitch = (int32_t)((((c->n_orders + 31) >> 5) + 2 + 3) & ~3);
   const int32_t cs_pitch = (int32_t)((c->n_orders + 7) & ~7);
-  const int KW = c->K <= 32 ? 1 : c->K <= 64 ? 2 : c->K <= 128 ? 4 : 8;
+  const int KW = c->K <= 32 ? 1 : c->K <= 64 ? 2 : c->K <= 128 ? 4 : c->K <= 224 ? 7 : 8;
   const int aw_words = (c->g.n_aisles + 15) / 16;
   const int ring_words = c->C + 2;
+  int id_slots = 4;  // a batch of C orders touches at most (C+14)/8 chunks
+  while (id_slots < (c->C + 14) / 8 + 1) id_slots <<= 1;
   // K2 shape
   const size_t table_bytes = 4 * (((size_t)c->n_items_pad + 31) & ~(size_t)31);
-  const size_t priv_per_warp = (size_t)(2 * KW + aw_words + ring_words + kIdRing * 4) * 128;
+  const size_t priv_per_warp = (size_t)(2 * KW + aw_words + ring_words + id_slots * 4) * 128;
   const size_t smem_max = (size_t)c->smem_optin - 1024;
   const bool smem_tables = table_bytes + 4 * priv_per_warp <= smem_max;
   const size_t avail = smem_max - (smem_tables ? table_bytes : 0);
@@ -438,10 +501,15 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
     int v = atoi(e);
     if (v >= 1 && v <= 32 && (v & (v - 1)) == 0 && (nb_ub + v - 1) / v <= 255) S = v;
   }
-  int planes_used = 1;
-  while ((1ll << planes_used) <= (nb_ub + S - 1) / S) ++planes_used;
+  int log2S = 0;
+  while ((1 << log2S) < S) ++log2S;
+  int seg_planes = 1;  // planes of one segment's counters; one more per combine level
+  while ((1ll << seg_planes) <= (nb_ub + S - 1) / S) ++seg_planes;
+  const bool depot0_pl = c->g.depot_aisle == 0;
+  const int kernel_planes = (depot0_pl && seg_planes <= 6) ? 6 : 8;  // the instantiation used
+  const int planes_used = kernel_planes + log2S;
   // scratch (grow-only; reallocated when the shape changes)
-  const int64_t plane_words = (int64_t)S * kPlanes * KW;
+  const int64_t plane_words = (int64_t)(kMaxPlanes + 5) * KW;
   if (c->fast_cap < n_cand || c->fast_pitch != bm_pitch || c->fast_plane_words < plane_words) {
     cudaError_t e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return e;
@@ -477,26 +545,32 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   {
     sets_params P;
     P.S = S; P.log2S = 0; while ((1 << P.log2S) < S) ++P.log2S;
-    P.aw_words = aw_words; P.ring_words = ring_words;
+    P.aw_words = aw_words; P.ring_words = ring_words; P.id_slots = id_slots;
     P.bm_pitch = bm_pitch; P.cs_pitch = cs_pitch; P.n_items_pad = c->n_items_pad;
     P.n_tasks = (n_cand * S + 31) / 32;
     int64_t blocks = (P.n_tasks + warps - 1) / warps;
     if (blocks > c->num_sms) blocks = c->num_sms;
     const size_t smem = (smem_tables ? table_bytes : 0) + priv_per_warp * warps;
     const bool depot0 = c->g.depot_aisle == 0;
-#define WHP_LAUNCH_SETS(ST, D0, KWV)                                                             \
+#define WHP_LAUNCH_SETS_PL(ST, D0, KWV, PLV)                                                     \
   do {                                                                                           \
-    cudaFuncSetAttribute(whp_sets_kernel<ST, D0, KWV>,                                           \
+    cudaFuncSetAttribute(whp_sets_kernel<ST, D0, KWV, PLV>,                                      \
                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);            \
-    whp_sets_kernel<ST, D0, KWV><<<(unsigned)blocks, warps * 32, smem, st>>>(                    \
+    whp_sets_kernel<ST, D0, KWV, PLV><<<(unsigned)blocks, warps * 32, smem, st>>>(               \
         T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, n_cand, c->d_dist_scratch,      \
         c->d_planes, out.batch_hash, c->d_task);                                                 \
+  } while (0)
+#define WHP_LAUNCH_SETS(ST, D0, KWV)                                                             \
+  do {                                                                                           \
+    if (D0 && seg_planes <= 6) WHP_LAUNCH_SETS_PL(ST, D0, KWV, 6);                               \
+    else WHP_LAUNCH_SETS_PL(ST, D0, KWV, 8);                                                     \
   } while (0)
 #define WHP_LAUNCH_SETS_KW(ST, D0)                                                               \
   do {                                                                                           \
     if (KW == 1) WHP_LAUNCH_SETS(ST, D0, 1);                                                     \
     else if (KW == 2) WHP_LAUNCH_SETS(ST, D0, 2);                                                \
     else if (KW == 4) WHP_LAUNCH_SETS(ST, D0, 4);                                                \
+    else if (KW == 7) WHP_LAUNCH_SETS(ST, D0, 7);                                                \
     else WHP_LAUNCH_SETS(ST, D0, 8);                                                             \
   } while (0)
     if (smem_tables && depot0) WHP_LAUNCH_SETS_KW(true, true);
@@ -505,6 +579,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
     else WHP_LAUNCH_SETS_KW(false, false);
 #undef WHP_LAUNCH_SETS_KW
 #undef WHP_LAUNCH_SETS
+#undef WHP_LAUNCH_SETS_PL
     c->launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -512,7 +587,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   // K3
   if (out.dist || out.penalty || out.obj || out.resp) {
     const unsigned blocks = (unsigned)((n_cand * 32 + 255) / 256);
-    whp_finish_kernel<<<blocks, 256, 0, st>>>(T, n_cand, c->d_dist_scratch, c->d_planes, S, KW,
+    whp_finish_kernel<<<blocks, 256, 0, st>>>(T, n_cand, c->d_dist_scratch, c->d_planes, KW,
                                               planes_used, out.dist, out.penalty, out.obj,
                                               out.resp);
     c->launches += 1;
