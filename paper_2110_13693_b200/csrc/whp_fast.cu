@@ -305,35 +305,40 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       uint32_t cur = lds32(ring);
       uint32_t n_cur = lds32(ring + 128);
       uint32_t rp = ring + 256;
-      const uint32_t rp_end = rp + 128 * left;  // the lane is done after `left` orders
+      const uint32_t rp_end = rp + 128 * max(left - 1, 0);  // left-1 moves to a next order
       uint32_t rec = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
-#pragma unroll 1
+      // Branch-free step: every lane runs Cmax steps. A lane that has finished its batch stays
+      // on the batch's final pick and re-inserts it (set inserts and max are idempotent); a
+      // lane without a batch walks to the end of order 0 and stays there — its sets are
+      // discarded at the close below.
+#pragma unroll 2
       for (int t = 0; t < Cmax; ++t) {
-        if (rp != rp_end) {
-          // cursor of the next step's pick: next record, or the next order's first pick
-          uint32_t nxt = cur + (SMEM_TABLES ? 4u : 1u);
-          if (rec & WHP_FAST_LAST) {
-            nxt = n_cur;
-            n_cur = lds32(rp);
-            rp += 128;
-          }
-          cur = nxt;
-          const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
-          // ---- this step's pick
-          kmax = max(kmax, rec);
-          if (!DEPOT0) kmin = min(kmin, rec);
-          const uint32_t aaddr = abase + ((rec >> 26) << 7);
-          const uint32_t abit = one_shl_wrap(rec >> 21);  // spacer bit: (rec >> 21) mod 32 = a_lo
-          const uint32_t x = max(lds32(aaddr), stamp_hi);  // an older stamp compares lower: empty
-          const uint32_t x2 = x | abit;
-          asm("{ .reg .pred pp; setp.ne.u32 pp, %1, %2; @pp add.s32 %0, %0, 1; }" : "+r"(m) : "r"(x2), "r"(x));
-          sts32(aaddr, x2);
-          const uint32_t caddr = cbase + ((rec & 0xf0u) << 3);
-          const uint32_t cbit = one_shl_wrap(rec & 15u);
-          const uint32_t y = max(lds32(caddr), stamp_hi);
-          sts32(caddr, y | cbit);
-          rec = rec_next;
+        // cursor of the next step's pick: next record, the next order's first pick, or stay
+        uint32_t nxt = cur + (SMEM_TABLES ? 4u : 1u);
+        const bool last = (rec & WHP_FAST_LAST) != 0;
+        const bool more = last && (rp != rp_end);
+        if (last) nxt = cur;
+        if (more) {
+          nxt = n_cur;
+          n_cur = lds32(rp);
+          rp += 128;
         }
+        cur = nxt;
+        const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
+        // ---- this step's pick
+        kmax = max(kmax, rec);
+        if (!DEPOT0) kmin = min(kmin, rec);
+        const uint32_t aaddr = abase + ((rec >> 26) << 7);
+        const uint32_t abit = one_shl_wrap(rec >> 21);  // spacer bit: (rec >> 21) mod 32 = a_lo
+        const uint32_t x = max(lds32(aaddr), stamp_hi);  // an older stamp compares lower: empty
+        const uint32_t x2 = x | abit;
+        asm("{ .reg .pred pp; setp.ne.u32 pp, %1, %2; @pp add.s32 %0, %0, 1; }" : "+r"(m) : "r"(x2), "r"(x));
+        sts32(aaddr, x2);
+        const uint32_t caddr = cbase + ((rec & 0xf0u) << 3);
+        const uint32_t cbit = one_shl_wrap(rec & 15u);
+        const uint32_t y = max(lds32(caddr), stamp_hi);
+        sts32(caddr, y | cbit);
+        rec = rec_next;
       }
       // ---- close the batch: D4, and the class set into the vertical counters (D5)
       if (live) {
@@ -351,10 +356,10 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       }
 #pragma unroll
       for (int w = 0; w < KW; ++w) {
-        // lanes without a batch j never wrote this stamp: max() leaves them an empty set
+        // lanes without a batch j ran the steps on a dummy pick: their set is discarded
         const uint32_t y0 = max(lds32(cbase + (2 * w) * 128), stamp_hi);
         const uint32_t y1 = max(lds32(cbase + (2 * w + 1) * 128), stamp_hi);
-        uint32_t carry = __byte_perm(y0, y1, 0x5410);  // 32 class bits of this batch
+        uint32_t carry = live ? __byte_perm(y0, y1, 0x5410) : 0u;  // 32 class bits of this batch
 #pragma unroll
         for (int pp = 0; pp < kPlanes; ++pp) {
           const uint32_t t2 = pl[pp][w] & carry;
