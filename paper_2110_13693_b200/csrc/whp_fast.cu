@@ -78,6 +78,7 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
 #pragma unroll 1
     for (int k = 0; k < kRing; ++k) {
       if (k < n4) cp_async16(ring0 + k * (kBoundsThreads * 16), row + k);
+      else asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(ring0 + k * (kBoundsThreads * 16)), "r"(0u));
       cp_async_commit();
     }
   }
@@ -86,7 +87,9 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
   uint32_t* __restrict__ bm = bmask + c * bm_pitch;
   uint2* __restrict__ cs = reinterpret_cast<uint2*>(cstream + c * cs_pitch);
   const int nw = (n_orders + 31) >> 5;
-  int load = 0;
+  // Next-fit recurrence on room = C - load, one dependent instruction per position:
+  //   room' = umin(room - q, C - q)   (room < q wraps room - q above C - q: a new batch opens)
+  uint32_t room = (uint32_t)C;
   uint32_t nb = 0;
   int p4 = 0, slot = 0;
   // 3-stage software pipeline, one chunk (4 positions) per stage: (A) order ids of chunk i+2
@@ -104,11 +107,10 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
     return v;
   };
   auto stage_b = [&](const int4& v, uint32_t (&r)[4]) {
-    // ids past the row end are stale ring contents: clamp so the gather stays in the table
-    r[0] = lds32(sorec0 + 4 * min((uint32_t)v.x, (uint32_t)n_orders - 1));
-    r[1] = lds32(sorec0 + 4 * min((uint32_t)v.y, (uint32_t)n_orders - 1));
-    r[2] = lds32(sorec0 + 4 * min((uint32_t)v.z, (uint32_t)n_orders - 1));
-    r[3] = lds32(sorec0 + 4 * min((uint32_t)v.w, (uint32_t)n_orders - 1));
+    // ids past the row end are stale ring contents (ids of earlier chunks, or the zero fill):
+    // always valid order ids, so the gather stays in the table
+    r[0] = lds32(sorec0 + 4 * v.x); r[1] = lds32(sorec0 + 4 * v.y);
+    r[2] = lds32(sorec0 + 4 * v.z); r[3] = lds32(sorec0 + 4 * v.w);
   };
   ids = stage_a(0);
   stage_b(ids, rc);
@@ -128,10 +130,9 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
         cs[p4] = make_uint2(__byte_perm(rc[0], rc[1], 0x6521), __byte_perm(rc[2], rc[3], 0x6521));
 #pragma unroll
         for (int t = 0; t < 4; ++t) {
-          const int q = (int)(rc[t] & WHP_Q_MASK);
-          const int load2 = load + q;
-          const bool over = load2 > C;
-          load = over ? q : load2;
+          const uint32_t q = rc[t] & WHP_Q_MASK;
+          const bool over = room < q;
+          room = min(room - q, (uint32_t)C - q);
           if (over) bits |= 1u << (4 * k + t);
           rc[t] = rb[t];
           rb[t] = rn[t];
