@@ -1,125 +1,382 @@
 // whp_swaps.cu — whp_eval_swaps (a6, D8): pairwise-swap neighbourhood of a base plan with
-// rescoring limited to the batches a swap can affect.
+// rescoring limited to the batches a swap can affect (DESIGN.md §6.3).
 //
-//   base pass   one walk of the base plan that tabulates, per batch b: first position
-//               bstart[b], exclusive prefix of S-shape lengths bdist[b], class mask bclass[b];
-//               plus batch_of_pos, base responses and totals.
-//   neighbours  one warp per swap (i,j): batches before the one holding position i are
-//               untouched (next-fit only looks forward) — except that when i opens its batch a
-//               smaller order may slip into the previous cart, so the rewalk then starts one
-//               batch earlier. The rewalk stops at the first new batch start P > j that is
-//               also a base batch start (from there on both plans are identical), or at the
-//               end. D and r are patched: minus the replaced base batches, plus the new ones.
+//   base pass   ONE block tabulates the base plan: item-count prefix pre[p], order record per
+//               position, next-fit boundaries (parallel "where does a batch opened at p end"
+//               + one pointer chase), then one warp per batch scores it with the picks of the
+//               batch flattened over the lanes. Tables: bstart[b], bop[p], prefix of batch
+//               lengths bdist[b], class mask bclass[b], class-count prefix rpre[b][k], totals.
+//   neighbours  one warp per swap (pi,pj). Next-fit only looks forward, so batches before the
+//               one holding pi are untouched — except that when pi opens its batch a smaller
+//               order may slip into the previous cart, so the rewalk then starts one batch
+//               earlier. Equal item counts leave every boundary in place: only the two batches
+//               holding pi and pj are rescored. Otherwise the rewalk re-batches from there and
+//               stops at the first new batch start P > pj that is also a base batch start
+//               (from there on both plans are identical), or at the end.
+//               D and r are patched: minus the replaced base batches (prefix differences),
+//               plus the new ones.
 #include "whp_walk.cuh"
 
 namespace {
 
-struct base_sink {
-  whp_base_tables B;
-  __device__ __forceinline__ void operator()(int32_t b, int32_t start_pos, int64_t dist,
-                                             const uint32_t* cmask) {
-    const int lane = whp_lane();
-    if (lane == 0) { B.bstart[b] = start_pos; B.bdist[b] = dist; }
-    if (lane < 8) B.bclass[(int64_t)b * 8 + lane] = cmask[lane];
+// The base plan with positions pi and pj exchanged (pi = pj = -1: the base plan itself), seen
+// through the base tables: pre = exclusive item-count prefix, orec = order record by position.
+// A window [lo, lo+cnt) of both tables may be staged in shared memory.
+struct swap_seq {
+  const int32_t* pre;      // global tables (plain loads: the base pass writes them itself)
+  const uint32_t* orec;
+  const int32_t* s_pre;    // shared-memory copy of pre[lo .. lo+n_pre)
+  const uint32_t* s_orec;  // shared-memory copy of orec[lo .. lo+n_orec)
+  int32_t lo;
+  uint32_t n_pre, n_orec;  // 0: nothing staged
+  int32_t pi, pj, delta;   // delta = q(pj) - q(pi)
+  __device__ __forceinline__ int32_t pre_base(int32_t p) const {
+    const uint32_t k = (uint32_t)(p - lo);
+    return k < n_pre ? s_pre[k] : pre[p];
+  }
+  __device__ __forceinline__ int32_t pre_at(int32_t p) const {
+    return pre_base(p) + ((p > pi && p <= pj) ? delta : 0);
+  }
+  __device__ __forceinline__ uint32_t orec_at(int32_t p) const {
+    const int32_t s = (p == pi) ? pj : ((p == pj) ? pi : p);
+    const uint32_t k = (uint32_t)(s - lo);
+    return k < n_orec ? s_orec[k] : orec[s];
   }
 };
 
-__global__ void __launch_bounds__(32)
-whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
-                      const whp_base_tables B) {
-  __shared__ whp_warp_smem sm;
-  const int lane = threadIdx.x;
-  sm.amask[lane] = 0;
-  if (lane < 8) sm.cmask[lane] = 0;
-  for (int k = lane; k < T.K; k += 32) sm.r[k] = 0;
-  __syncwarp();
-  whp_walk_state st;
-  whp_walk_init(st, 0);
-  auto perm_at = [base_perm](int32_t p) { return __ldg(base_perm + p); };
-  base_sink sink{B};
-  whp_walk<false, false>(T, &sm, st, perm_at, 0, T.n_orders, whp_no_stop(), sink, B.bop);
-  __syncwarp();
-  const int32_t nb = st.b + 1;
-  // exclusive prefix sum of the per-batch lengths, in place; bdist[nb] = D_base
-  int64_t carry = 0;
-  for (int32_t base = 0; base <= nb; base += 32) {
-    const int32_t b = base + lane;
-    const int64_t x = (b < nb) ? B.bdist[b] : 0;
-    int64_t incl = x;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-      const int64_t y = __shfl_up_sync(WHP_FULL, incl, d);
-      if (lane >= d) incl += y;
-    }
-    if (b <= nb) B.bdist[b] = carry + incl - x;
-    carry += __shfl_sync(WHP_FULL, incl, 31);
+struct warp_sets {
+  uint32_t amask[32];  // aisle occupancy of the batch being scored
+  uint32_t cmask[8];   // class occupancy
+};
+
+// End of the batch that opens at position p (D2): the largest e <= n with
+// pre(e) - pre(p) <= C. Every order has at least one item, so e - p <= C. Warp-collective.
+__device__ __forceinline__ int32_t batch_end(const swap_seq& q, int32_t p, int32_t n, int32_t C) {
+  const int lane = whp_lane();
+  const int32_t lim = q.pre_at(p) + C;
+  int32_t e = p;
+  for (;;) {
+    const int32_t cand = e + 1 + lane;
+    const bool ok = cand <= n && q.pre_at(cand) <= lim;
+    const uint32_t bal = __ballot_sync(WHP_FULL, ok);
+    const int cnt = (bal == WHP_FULL) ? 32 : __ffs(~bal) - 1;  // prefix is increasing
+    e += cnt;
+    if (cnt < 32) return e;
   }
-  for (int k = lane; k < T.K; k += 32) B.resp[k] = sm.r[k];
-  if (lane == 0) { B.bstart[nb] = T.n_orders; B.totals[0] = st.D; B.totals[1] = nb; }
 }
 
-struct swap_stop {
-  const int32_t* bop;
-  int32_t pj;
-  __device__ __forceinline__ bool operator()(int32_t P) const {
-    return P > pj && __ldg(bop + P) != __ldg(bop + P - 1);
+// D3 + D4 of the batch at positions [s, e): the picks of the batch are flattened over the
+// lanes (item t belongs to the last position whose prefix is <= t). Returns dist_b on every
+// lane; leaves the batch's class mask in sets->cmask (the caller consumes and clears it).
+__device__ __forceinline__ int64_t score_batch(const whp_tables& T, warp_sets* sets,
+                                               const swap_seq& q, int32_t s, int32_t e) {
+  const int lane = whp_lane();
+  const int32_t base0 = q.pre_at(s);
+  const int32_t load = q.pre_at(e) - base0;
+  uint32_t kmax = 0, kmin = 0xffffffffu;
+  for (int32_t t0 = 0; t0 < load; t0 += 32) {
+    const int32_t t = t0 + lane;
+    if (t < load) {
+      int32_t lo = s, hi = e - 1;
+      while (lo < hi) {
+        const int32_t mid = (lo + hi + 1) >> 1;
+        if (q.pre_at(mid) - base0 <= t) lo = mid; else hi = mid - 1;
+      }
+      const uint32_t orec = q.orec_at(lo);
+      const uint32_t pr = __ldg(T.pick_rec + (orec >> WHP_Q_BITS) + (t - (q.pre_at(lo) - base0)));
+      kmax = max(kmax, pr);
+      kmin = min(kmin, pr);
+      const uint32_t a = WHP_PICK_AISLE(pr);
+      const uint32_t c = pr & WHP_PICK_CLASS_MASK;
+      atomicOr(&sets->amask[a >> 5], 1u << (a & 31));
+      atomicOr(&sets->cmask[c >> 5], 1u << (c & 31));
+    }
   }
-};
+  kmax = __reduce_max_sync(WHP_FULL, kmax);
+  kmin = __reduce_min_sync(WHP_FULL, kmin);
+  __syncwarp();
+  const uint32_t aw = sets->amask[lane];
+  sets->amask[lane] = 0;
+  const int m = __reduce_add_sync(WHP_FULL, __popc(aw));
+  const int64_t a_max = WHP_PICK_AISLE(kmax), a_min = WHP_PICK_AISLE(kmin);
+  const int64_t d_last =
+      (int64_t)((kmax >> WHP_PICK_SLOT_SHIFT) & WHP_PICK_SLOT_MASK) * T.g.slot_pitch;
+  const int64_t a0 = T.g.depot_aisle;
+  const int64_t H = (int64_t)T.g.aisle_spacing *
+                    (llabs(a0 - a_min) + (a_max - a_min) + llabs(a_max - a0));
+  const int64_t Vt = (m & 1) ? (int64_t)(m - 1) * T.g.aisle_len + 2 * d_last
+                             : (int64_t)m * T.g.aisle_len;
+  return H + Vt;
+}
 
+// D6 with lane l owning classes l, l+32, ... (the canonical 32-lane accumulation)
+__device__ __forceinline__ double penalty_regs(const whp_tables& T, const int32_t (&r)[8]) {
+  const int lane = whp_lane();
+  double s = 0.0;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    const int k = 32 * w + lane;
+    if (k < T.K) {
+      const double c = __dsub_rn(__ldg(T.tvw + k), (double)r[w]);
+      const double u = __dmul_rn(__ldg(T.tvw + 2 * T.K + k), c);
+      const double term = __dadd_rn(__dmul_rn(__ldg(T.tvw + T.K + k), c), __dmul_rn(u, u));
+      s = __dadd_rn(s, term);
+    }
+  }
+#pragma unroll
+  for (int off = 16; off >= 1; off >>= 1) s = __dadd_rn(s, __shfl_xor_sync(WHP_FULL, s, off));
+  return s;
+}
+
+// ------------------------------------------------------------------------------ base pass
+constexpr int kBaseThreads = 1024;
+
+// block-wide exclusive scan of one value per thread; returns the exclusive prefix and, through
+// `total`, the block sum. `ws` is a 32-entry scratch.
+template <class V>
+__device__ __forceinline__ V block_excl_scan(V x, V* ws, V& total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  V incl = x;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const V y = __shfl_up_sync(WHP_FULL, incl, d);
+    if (lane >= d) incl += y;
+  }
+  __syncthreads();  // ws may still be read from a previous call
+  if (lane == 31) ws[warp] = incl;
+  __syncthreads();
+  if (warp == 0) {
+    const V v = ws[lane];
+    V wi = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const V y = __shfl_up_sync(WHP_FULL, wi, d);
+      if (lane >= d) wi += y;
+    }
+    ws[lane] = wi - v;
+    if (lane == 31) ws[32] = wi;
+  }
+  __syncthreads();
+  total = ws[32];
+  return ws[warp] + incl - x;
+}
+
+__global__ void __launch_bounds__(kBaseThreads)
+whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
+                      const whp_base_tables B, int smem_tables) {
+  extern __shared__ __align__(16) uint8_t dyn[];
+  __shared__ warp_sets sets_all[kBaseThreads / 32];
+  __shared__ int32_t s_resp[WHP_MAX_CLASSES];
+  __shared__ int64_t s_scan64[33];
+  __shared__ int32_t s_scan32[33];
+  __shared__ int32_t s_nb;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int32_t n = T.n_orders;
+  // item-count prefix and "next batch start" tables: shared memory when they fit
+  int32_t* pre = smem_tables ? reinterpret_cast<int32_t*>(dyn) : B.pre;
+  int32_t* nxt = smem_tables ? reinterpret_cast<int32_t*>(dyn) + (n + 1) : B.bop;
+  sets_all[warp].amask[lane] = 0;
+  if (lane < 8) sets_all[warp].cmask[lane] = 0;
+  for (int k = tid; k < WHP_MAX_CLASSES; k += kBaseThreads) s_resp[k] = 0;
+
+  // ---- A: order record of every position; exclusive prefix of the item counts
+  int32_t carry = 0;
+  for (int32_t p0 = 0; p0 < n; p0 += kBaseThreads) {
+    const int32_t p = p0 + tid;
+    uint32_t orec = 0;
+    if (p < n) { orec = __ldg(T.order_rec + __ldg(base_perm + p)); B.orec[p] = orec; }
+    const int32_t qv = (int32_t)(orec & WHP_Q_MASK);
+    int32_t tot;
+    const int32_t ex = block_excl_scan<int32_t>(qv, s_scan32, tot);
+    if (p < n) { pre[p] = carry + ex; if (smem_tables) B.pre[p] = carry + ex; }
+    carry += tot;
+  }
+  if (tid == 0) { pre[n] = carry; B.pre[n] = carry; }
+  __syncthreads();
+
+  // ---- B: nxt[p] = where the batch that opens at p ends (binary search in p+1 .. p+C)
+  for (int32_t p = tid; p < n; p += kBaseThreads) {
+    const int32_t lim = pre[p] + T.C;
+    int32_t lo = p + 1, hi = min(n, p + T.C);  // pre[lo] <= lim always (q <= C)
+    while (lo < hi) {
+      const int32_t mid = (lo + hi + 1) >> 1;
+      if (pre[mid] <= lim) lo = mid; else hi = mid - 1;
+    }
+    nxt[p] = lo;
+  }
+  __syncthreads();
+
+  // ---- C: one thread chases the boundaries
+  if (tid == 0) {
+    int32_t b = 0;
+    for (int32_t p = 0; p < n; p = nxt[p]) B.bstart[b++] = p;
+    B.bstart[b] = n;
+    s_nb = b;
+  }
+  __syncthreads();
+  const int32_t nb = s_nb;
+
+  // ---- D: one warp per batch
+  swap_seq q{B.pre, B.orec, pre, nullptr, 0, smem_tables ? (uint32_t)(n + 1) : 0u, 0u, -1, -1, 0};
+  warp_sets* sets = &sets_all[warp];
+  const int KW = (T.K + 31) >> 5;
+  for (int32_t b = warp; b < nb; b += kBaseThreads / 32) {
+    const int32_t s = B.bstart[b], e = B.bstart[b + 1];
+    const int64_t dist = score_batch(T, sets, q, s, e);
+    for (int32_t p = s + lane; p < e; p += 32) B.bop[p] = b;
+    if (lane == 0) B.bdist[b] = dist;
+    if (lane < 8) {
+      const uint32_t cm = sets->cmask[lane];
+      B.bclass[(int64_t)b * 8 + lane] = cm;
+      sets->cmask[lane] = 0;
+    }
+    __syncwarp();
+  }
+  __syncthreads();
+
+  // ---- E: exclusive prefix of the batch lengths (bdist[nb] = D_base), class-count prefix
+  int64_t carry64 = 0;
+  for (int32_t b0 = 0; b0 <= nb; b0 += kBaseThreads) {
+    const int32_t b = b0 + tid;
+    const int64_t x = (b < nb) ? B.bdist[b] : 0;
+    int64_t tot;
+    const int64_t ex = block_excl_scan<int64_t>(x, s_scan64, tot);
+    if (b <= nb) B.bdist[b] = carry64 + ex;
+    carry64 += tot;
+  }
+  for (int k = tid; k < T.K; k += kBaseThreads) {
+    int32_t acc = 0;
+    const int w = k >> 5, bit = k & 31;
+    B.rpre[k] = 0;
+    for (int32_t b = 0; b < nb; ++b) {
+      acc += (int32_t)((B.bclass[(int64_t)b * 8 + w] >> bit) & 1u);
+      B.rpre[(int64_t)(b + 1) * T.K + k] = acc;
+    }
+    B.resp[k] = acc;
+    s_resp[k] = acc;
+  }
+  __syncthreads();
+  if (warp == 0) {
+    int32_t r[8];
+#pragma unroll
+    for (int w = 0; w < 8; ++w) r[w] = (32 * w + lane < T.K) ? s_resp[32 * w + lane] : 0;
+    const double phi = penalty_regs(T, r);
+    if (lane == 0) {
+      B.totals[0] = carry64;
+      B.totals[1] = nb;
+      B.ftotals[0] = phi;
+      B.ftotals[1] = __dadd_rn((double)carry64, phi);
+    }
+  }
+  (void)KW;
+}
+
+// ------------------------------------------------------------------------------ neighbours
 constexpr int kSwapWarps = 8;
+constexpr int kStage = 1024;  // positions of pre / orec staged per block
 
 __global__ void __launch_bounds__(kSwapWarps * 32)
-whp_swaps_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
-                 const whp_base_tables B, int32_t win_start, int32_t W, int64_t n_nb,
-                 int64_t* __restrict__ d_dist, double* __restrict__ d_obj) {
-  __shared__ whp_warp_smem sm_all[kSwapWarps];
+whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start, int32_t W,
+                 int64_t n_nb, int64_t* __restrict__ d_dist, double* __restrict__ d_obj) {
+  __shared__ warp_sets sets_all[kSwapWarps];
+  __shared__ int32_t s_pre[kStage + 1];
+  __shared__ uint32_t s_orec[kStage];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  whp_warp_smem* sm = &sm_all[warp];
-  sm->amask[lane] = 0;
-  if (lane < 8) sm->cmask[lane] = 0;
+  warp_sets* sets = &sets_all[warp];
+  sets->amask[lane] = 0;
+  if (lane < 8) sets->cmask[lane] = 0;
+  const int32_t n = T.n_orders;
   const int32_t nb = (int32_t)B.totals[1];
-  const int KW = (T.K + 31) >> 5;
-  for (int64_t n = (int64_t)blockIdx.x * kSwapWarps + warp; n < n_nb;
-       n += (int64_t)gridDim.x * kSwapWarps) {
+  // stage the tables from the start of the batch before the window's first batch
+  int32_t lo;
+  {
+    const int32_t bw = __ldg(B.bop + win_start);
+    lo = __ldg(B.bstart + (bw > 0 ? bw - 1 : 0));
+  }
+  const int32_t cnt = min(kStage, n - lo);
+  for (int k = threadIdx.x; k <= cnt; k += blockDim.x) s_pre[k] = __ldg(B.pre + lo + k);
+  for (int k = threadIdx.x; k < cnt; k += blockDim.x) s_orec[k] = __ldg(B.orec + lo + k);
+  __syncthreads();
+  const int64_t D_base = B.totals[0];
+
+  for (int64_t nn = (int64_t)blockIdx.x * kSwapWarps + warp; nn < n_nb;
+       nn += (int64_t)gridDim.x * kSwapWarps) {
     // neighbour index -> (i', j'), row i' starts at i'(2W-i'-1)/2
     const double wm = 2.0 * W - 1.0;
-    int64_t i = (int64_t)floor((wm - sqrt(wm * wm - 8.0 * (double)n)) * 0.5);
+    int64_t i = (int64_t)floor((wm - sqrt(wm * wm - 8.0 * (double)nn)) * 0.5);
     i = max((int64_t)0, min(i, (int64_t)W - 2));
-    while (i > 0 && i * (2 * (int64_t)W - i - 1) / 2 > n) --i;
-    while ((i + 1) * (2 * (int64_t)W - i - 2) / 2 <= n) ++i;
-    const int64_t j = i + 1 + (n - i * (2 * (int64_t)W - i - 1) / 2);
+    while (i > 0 && i * (2 * (int64_t)W - i - 1) / 2 > nn) --i;
+    while ((i + 1) * (2 * (int64_t)W - i - 2) / 2 <= nn) ++i;
+    const int64_t j = i + 1 + (nn - i * (2 * (int64_t)W - i - 1) / 2);
     const int32_t pi = win_start + (int32_t)i, pj = win_start + (int32_t)j;
+    const int32_t bi = __ldg(B.bop + pi), bj = __ldg(B.bop + pj);
+    swap_seq q{B.pre, B.orec, s_pre, s_orec, lo, (uint32_t)(cnt + 1), (uint32_t)cnt, pi, pj, 0};
+    const int32_t qi = (int32_t)(q.orec_at(pj) & WHP_Q_MASK);  // orec_at swaps: this is q(pi)
+    const int32_t qj = (int32_t)(q.orec_at(pi) & WHP_Q_MASK);
+    q.delta = qj - qi;
+    // a smaller order arriving at the opening position of a cart may slip into the cart before
+    const bool slip = q.delta < 0 && bi > 0 && pi == __ldg(B.bstart + bi);
+    if (bi == bj && !slip) {  // both orders stay in the same cart: nothing changes
+      if (lane == 0) {
+        if (d_dist) d_dist[nn] = D_base;
+        if (d_obj) d_obj[nn] = B.ftotals[1];
+      }
+      continue;
+    }
 
-    int32_t b0 = __ldg(B.bop + pi);
-    int32_t p0 = __ldg(B.bstart + b0);
-    if (pi == p0 && b0 > 0) { b0 -= 1; p0 = __ldg(B.bstart + b0); }
-    for (int k = lane; k < T.K; k += 32) sm->r[k] = 0;
-    __syncwarp();
-    whp_walk_state st;
-    whp_walk_init(st, b0);
-    auto perm_at = [base_perm, pi, pj](int32_t p) {
-      return __ldg(base_perm + (p == pi ? pj : (p == pj ? pi : p)));
+    int64_t D = D_base;
+    int32_t r[8];
+#pragma unroll
+    for (int w = 0; w < 8; ++w) r[w] = 0;
+    auto add_classes = [&]() {  // new batch: + its classes, then clear the mask
+      __syncwarp();
+#pragma unroll
+      for (int w = 0; w < 8; ++w) r[w] += (int32_t)((sets->cmask[w] >> lane) & 1u);
+      __syncwarp();
+      if (lane < 8) sets->cmask[lane] = 0;
+      __syncwarp();
     };
-    const int32_t end = whp_walk<false, true>(T, sm, st, perm_at, p0, T.n_orders,
-                                              swap_stop{B.bop, pj}, whp_no_sink(), nullptr);
-    __syncwarp();
-    const int32_t b_end = (end >= T.n_orders) ? nb : __ldg(B.bop + end);
-    const int64_t D = B.totals[0] - (B.bdist[b_end] - B.bdist[b0]) + st.D;
-    // r = r_base - (classes of the replaced base batches) + (classes of the new batches)
-    for (int w = 0; w < KW; ++w) {
+    auto remove_base = [&](int32_t b_from, int32_t b_to) {  // base batches [b_from, b_to)
+      D -= B.bdist[b_to] - B.bdist[b_from];
+#pragma unroll
+      for (int w = 0; w < 8; ++w) {
+        const int k = 32 * w + lane;
+        if (k < T.K)
+          r[w] -= __ldg(B.rpre + (int64_t)b_to * T.K + k) - __ldg(B.rpre + (int64_t)b_from * T.K + k);
+      }
+    };
+    if (q.delta == 0) {
+      // boundaries stay: rescore the two carts that exchange an order
+      remove_base(bi, bi + 1);
+      remove_base(bj, bj + 1);
+      D += score_batch(T, sets, q, __ldg(B.bstart + bi), __ldg(B.bstart + bi + 1));
+      add_classes();
+      D += score_batch(T, sets, q, __ldg(B.bstart + bj), __ldg(B.bstart + bj + 1));
+      add_classes();
+    } else {
+      const int32_t b0 = slip ? bi - 1 : bi;
+      int32_t p = __ldg(B.bstart + b0);
+      int32_t b_end;
+      for (;;) {
+        const int32_t e = batch_end(q, p, n, T.C);
+        D += score_batch(T, sets, q, p, e);
+        add_classes();
+        p = e;
+        if (p >= n) { b_end = nb; break; }
+        if (p > pj && __ldg(B.bop + p) != __ldg(B.bop + p - 1)) { b_end = __ldg(B.bop + p); break; }
+      }
+      remove_base(b0, b_end);
+    }
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
       const int k = 32 * w + lane;
-      int32_t rk = (k < T.K) ? __ldg(B.resp + k) + sm->r[k] : 0;
-      for (int32_t b = b0; b < b_end; ++b)
-        rk -= (int32_t)((__ldg(B.bclass + (int64_t)b * 8 + w) >> lane) & 1u);
-      if (k < T.K) sm->r[k] = rk;
+      if (k < T.K) r[w] += __ldg(B.resp + k);
     }
-    __syncwarp();
-    const double phi = whp_penalty(T, sm->r);
+    const double phi = penalty_regs(T, r);
     if (lane == 0) {
-      if (d_dist) d_dist[n] = D;
-      if (d_obj) d_obj[n] = __dadd_rn((double)D, phi);
+      if (d_dist) d_dist[nn] = D;
+      if (d_obj) d_obj[nn] = __dadd_rn((double)D, phi);
     }
-    __syncwarp();
   }
 }
 
@@ -128,17 +385,22 @@ whp_swaps_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
 cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                              int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st) {
   const whp_tables T = whp_make_tables(c);
-  whp_swaps_base_kernel<<<1, 32, 0, st>>>(T, d_base_perm, c->base);
-  c->launches += 1;
-  cudaError_t e = cudaGetLastError();
+  const size_t need = 4 * (2 * (size_t)c->n_orders + 1);
+  const int smem_tables = need + 12 * 1024 <= (size_t)c->smem_optin ? 1 : 0;
+  cudaError_t e = cudaFuncSetAttribute(whp_swaps_base_kernel,
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       smem_tables ? (int)need : 0);
   if (e != cudaSuccess) return e;
+  whp_swaps_base_kernel<<<1, kBaseThreads, smem_tables ? need : 0, st>>>(T, d_base_perm, c->base,
+                                                                        smem_tables);
+  c->launches += 1;
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
   const int64_t n_nb = (int64_t)win_len * (win_len - 1) / 2;
   int64_t blocks = (n_nb + kSwapWarps - 1) / kSwapWarps;
-  const int64_t cap = (int64_t)c->num_sms * 64;
+  const int64_t cap = (int64_t)c->num_sms * 8;
   if (blocks > cap) blocks = cap;
-  whp_swaps_kernel<<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(T, d_base_perm, c->base,
-                                                                 win_start, win_len, n_nb,
-                                                                 d_dist, d_obj);
+  whp_swaps_kernel<<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(T, c->base, win_start, win_len,
+                                                                 n_nb, d_dist, d_obj);
   c->launches += 1;
   return cudaGetLastError();
 }
