@@ -68,6 +68,9 @@ struct whp_base_tables {
   int32_t* pre;       // [n_orders+1] exclusive prefix of the item counts along the plan
   uint32_t* orec;     // [n_orders]   order record of every position
   int32_t* rpre;      // [nb_max+1][K] class-visit counts of the batches before b
+  int32_t* nxt;       // [n_orders]   end of the batch that would open at position p
+  int64_t* dist_at;   // [n_orders]   S-shape length of that batch (region of the window only)
+  uint32_t* cls_at;   // [n_orders][8] its class mask
 };
 
 struct whp_ctx {

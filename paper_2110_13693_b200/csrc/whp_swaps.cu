@@ -174,7 +174,7 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
   const int32_t n = T.n_orders;
   // item-count prefix and "next batch start" tables: shared memory when they fit
   int32_t* pre = smem_tables ? reinterpret_cast<int32_t*>(dyn) : B.pre;
-  int32_t* nxt = smem_tables ? reinterpret_cast<int32_t*>(dyn) + (n + 1) : B.bop;
+  int32_t* nxt = smem_tables ? reinterpret_cast<int32_t*>(dyn) + (n + 1) : B.nxt;
   sets_all[warp].amask[lane] = 0;
   if (lane < 8) sets_all[warp].cmask[lane] = 0;
   for (int k = tid; k < WHP_MAX_CLASSES; k += kBaseThreads) s_resp[k] = 0;
@@ -203,6 +203,7 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
       if (pre[mid] <= lim) lo = mid; else hi = mid - 1;
     }
     nxt[p] = lo;
+    if (smem_tables) B.nxt[p] = lo;
   }
   __syncthreads();
 
@@ -244,16 +245,26 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
     if (b <= nb) B.bdist[b] = carry64 + ex;
     carry64 += tot;
   }
-  for (int k = tid; k < T.K; k += kBaseThreads) {
-    int32_t acc = 0;
-    const int w = k >> 5, bit = k & 31;
-    B.rpre[k] = 0;
-    for (int32_t b = 0; b < nb; ++b) {
-      acc += (int32_t)((B.bclass[(int64_t)b * 8 + w] >> bit) & 1u);
-      B.rpre[(int64_t)(b + 1) * T.K + k] = acc;
+  // rpre[b][k] = number of batches before b that visit class k: warp w owns class word w; for
+  // 32 batches at a time a ballot per class bit gives the visits as a mask over the batches
+  if (warp < KW) {
+    const int w = warp;
+    const uint32_t le_mask = WHP_FULL >> (31 - lane);
+    int32_t cnt = 0;  // lane j: visits of class 32w+j so far
+    if (32 * w + lane < T.K) B.rpre[32 * w + lane] = 0;
+    for (int32_t b0 = 0; b0 < nb; b0 += 32) {
+      const int32_t b = b0 + lane;
+      const uint32_t word = (b < nb) ? B.bclass[(int64_t)b * 8 + w] : 0u;
+#pragma unroll
+      for (int j = 0; j < 32; ++j) {
+        const uint32_t mask = __ballot_sync(WHP_FULL, (word >> j) & 1u);
+        const int32_t cj = __shfl_sync(WHP_FULL, cnt, j);
+        if (b < nb && 32 * w + j < T.K)
+          B.rpre[(int64_t)(b + 1) * T.K + 32 * w + j] = cj + __popc(mask & le_mask);
+        if (lane == j) cnt += __popc(mask);
+      }
     }
-    B.resp[k] = acc;
-    s_resp[k] = acc;
+    if (32 * w + lane < T.K) { B.resp[32 * w + lane] = cnt; s_resp[32 * w + lane] = cnt; }
   }
   __syncthreads();
   if (warp == 0) {
@@ -268,7 +279,29 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
       B.ftotals[1] = __dadd_rn((double)carry64, phi);
     }
   }
-  (void)KW;
+}
+
+// ------------------------------------------------------------------------------ region prep
+// For every position p of the region [rlo, rhi): the batch that WOULD open at p in the base
+// plan, [p, nxt[p]) — its S-shape length dist_at[p] and class mask cls_at[p]. A rescored plan
+// differs from the base plan only around the two swapped positions; every other new batch is
+// one of these (its end depends on its start alone), so a neighbour looks it up.
+constexpr int kPrepWarps = 8;
+
+__global__ void __launch_bounds__(kPrepWarps * 32)
+whp_swaps_prep_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, int32_t rhi) {
+  __shared__ warp_sets sets_all[kPrepWarps];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  warp_sets* sets = &sets_all[warp];
+  sets->amask[lane] = 0;
+  if (lane < 8) sets->cmask[lane] = 0;
+  __syncwarp();
+  const int32_t p = rlo + blockIdx.x * kPrepWarps + warp;
+  if (p >= rhi) return;
+  swap_seq q{B.pre, B.orec, nullptr, nullptr, 0, 0u, 0u, -1, -1, 0};
+  const int64_t dist = score_batch(T, sets, q, p, B.nxt[p]);
+  if (lane == 0) B.dist_at[p] = dist;
+  if (lane < 8) B.cls_at[(int64_t)p * 8 + lane] = sets->cmask[lane];
 }
 
 // ------------------------------------------------------------------------------ neighbours
@@ -277,7 +310,8 @@ constexpr int kStage = 1024;  // positions of pre / orec staged per block
 
 __global__ void __launch_bounds__(kSwapWarps * 32)
 whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start, int32_t W,
-                 int64_t n_nb, int64_t* __restrict__ d_dist, double* __restrict__ d_obj) {
+                 int32_t rlo, int32_t rhi, int64_t n_nb, int64_t* __restrict__ d_dist,
+                 double* __restrict__ d_obj) {
   __shared__ warp_sets sets_all[kSwapWarps];
   __shared__ int32_t s_pre[kStage + 1];
   __shared__ uint32_t s_orec[kStage];
@@ -358,9 +392,29 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
       int32_t p = __ldg(B.bstart + b0);
       int32_t b_end;
       for (;;) {
-        const int32_t e = batch_end(q, p, n, T.C);
-        D += score_batch(T, sets, q, p, e);
-        add_classes();
+        // A batch that holds neither swapped position and ends where the base criterion ends
+        // it is the tabulated batch of its start; the others are scored from their picks.
+        int32_t e;
+        bool table;
+        if (p > pj) {
+          e = __ldg(B.nxt + p);
+          table = true;
+        } else {
+          e = batch_end(q, p, n, T.C);
+          table = (p > pi || e <= pi) && e <= pj && __ldg(B.nxt + p) == e;
+        }
+        if (table && p >= rlo && p < rhi) {
+          D += __ldg(B.dist_at + p);
+          const uint4 c0 = __ldg(reinterpret_cast<const uint4*>(B.cls_at + (int64_t)p * 8));
+          const uint4 c1 = __ldg(reinterpret_cast<const uint4*>(B.cls_at + (int64_t)p * 8) + 1);
+          r[0] += (int32_t)((c0.x >> lane) & 1u); r[1] += (int32_t)((c0.y >> lane) & 1u);
+          r[2] += (int32_t)((c0.z >> lane) & 1u); r[3] += (int32_t)((c0.w >> lane) & 1u);
+          r[4] += (int32_t)((c1.x >> lane) & 1u); r[5] += (int32_t)((c1.y >> lane) & 1u);
+          r[6] += (int32_t)((c1.z >> lane) & 1u); r[7] += (int32_t)((c1.w >> lane) & 1u);
+        } else {
+          D += score_batch(T, sets, q, p, e);
+          add_classes();
+        }
         p = e;
         if (p >= n) { b_end = nb; break; }
         if (p > pj && __ldg(B.bop + p) != __ldg(B.bop + p - 1)) { b_end = __ldg(B.bop + p); break; }
@@ -395,12 +449,23 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
                                                                         smem_tables);
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  // region of tabulated hypothetical batches: from two cart lengths before the window (the
+  // rewalk may start one batch early) to a margin after it (until the boundaries resynchronise;
+  // beyond the margin a neighbour scores its batches from their picks)
+  const int64_t margin = 16ll * c->C > 512 ? 16ll * c->C : 512;
+  const int32_t rlo = (int32_t)((int64_t)win_start - 2ll * c->C > 0 ? (int64_t)win_start - 2ll * c->C : 0);
+  const int32_t rhi = (int32_t)((int64_t)win_start + win_len + margin < c->n_orders
+                                    ? (int64_t)win_start + win_len + margin : c->n_orders);
+  whp_swaps_prep_kernel<<<(unsigned)((rhi - rlo + kPrepWarps - 1) / kPrepWarps), kPrepWarps * 32,
+                          0, st>>>(T, c->base, rlo, rhi);
+  c->launches += 1;
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
   const int64_t n_nb = (int64_t)win_len * (win_len - 1) / 2;
   int64_t blocks = (n_nb + kSwapWarps - 1) / kSwapWarps;
   const int64_t cap = (int64_t)c->num_sms * 8;
   if (blocks > cap) blocks = cap;
   whp_swaps_kernel<<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(T, c->base, win_start, win_len,
-                                                                 n_nb, d_dist, d_obj);
+                                                                 rlo, rhi, n_nb, d_dist, d_obj);
   c->launches += 1;
   return cudaGetLastError();
 }
