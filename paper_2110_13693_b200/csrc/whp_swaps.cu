@@ -245,26 +245,24 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
     if (b <= nb) B.bdist[b] = carry64 + ex;
     carry64 += tot;
   }
-  // rpre[b][k] = number of batches before b that visit class k: warp w owns class word w; for
-  // 32 batches at a time a ballot per class bit gives the visits as a mask over the batches
+  // rpre[b][k] = number of batches before b that visit class k. Warp w owns class word w, its
+  // lane j class 32w+j: a running count over the batches, one coalesced row store per batch.
   if (warp < KW) {
     const int w = warp;
-    const uint32_t le_mask = WHP_FULL >> (31 - lane);
-    int32_t cnt = 0;  // lane j: visits of class 32w+j so far
-    if (32 * w + lane < T.K) B.rpre[32 * w + lane] = 0;
+    const bool mine = 32 * w + lane < T.K;
+    int32_t cnt = 0;
+    int32_t* __restrict__ row = B.rpre + 32 * w + lane;
+    if (mine) row[0] = 0;
     for (int32_t b0 = 0; b0 < nb; b0 += 32) {
       const int32_t b = b0 + lane;
       const uint32_t word = (b < nb) ? B.bclass[(int64_t)b * 8 + w] : 0u;
-#pragma unroll
-      for (int j = 0; j < 32; ++j) {
-        const uint32_t mask = __ballot_sync(WHP_FULL, (word >> j) & 1u);
-        const int32_t cj = __shfl_sync(WHP_FULL, cnt, j);
-        if (b < nb && 32 * w + j < T.K)
-          B.rpre[(int64_t)(b + 1) * T.K + 32 * w + j] = cj + __popc(mask & le_mask);
-        if (lane == j) cnt += __popc(mask);
+      const int nbb = min(32, nb - b0);
+      for (int bb = 0; bb < nbb; ++bb) {
+        cnt += (int32_t)((__shfl_sync(WHP_FULL, word, bb) >> lane) & 1u);
+        if (mine) row[(int64_t)(b0 + bb + 1) * T.K] = cnt;
       }
     }
-    if (32 * w + lane < T.K) { B.resp[32 * w + lane] = cnt; s_resp[32 * w + lane] = cnt; }
+    if (mine) { B.resp[32 * w + lane] = cnt; s_resp[32 * w + lane] = cnt; }
   }
   __syncthreads();
   if (warp == 0) {
