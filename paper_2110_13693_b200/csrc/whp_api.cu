@@ -44,7 +44,7 @@ void free_orders(whp_ctx* c) {
   dfree(c->d_stage[0]); dfree(c->d_stage[1]);
   c->stage_rows = 0;
   dfree(c->d_bmask); dfree(c->d_cstream); dfree(c->d_nb); dfree(c->d_dist_scratch);
-  dfree(c->d_planes);
+  dfree(c->d_planes); dfree(c->d_segstart);
   c->fast_cap = 0; c->fast_pitch = 0; c->fast_plane_words = 0;
   c->have_orders = false;
 }

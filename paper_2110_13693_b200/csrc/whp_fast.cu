@@ -55,97 +55,163 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
 }
 
 // ------------------------------------------------------------------------------------------ K1
-constexpr int kBoundsThreads = 64;
-constexpr int kRing = 32;  // 16-byte permutation chunks in flight per thread (cp.async ring)
+constexpr int kBoundsThreads = 64;   // candidates per block, one per thread
+constexpr int kChunkBytes = 256;     // bytes of a permutation row per bulk copy (64 positions)
+constexpr int kChunkStride = kChunkBytes + 16;  // per-thread buffer stride: 128-bit reads of a
+                                                // quarter warp fall into distinct banks
+constexpr int kStages = 3;
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// TMA bulk copy global -> shared, completion counted in bytes on the mbarrier
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// 4 x n4 positions of one row: order ids from the staged chunk, their records from the order
+// table in shared memory, the next-fit recurrence on room = C - load with one dependent
+// instruction per position:  room' = umin(room - q, C - q)  (room < q wraps room - q above
+// C - q: a new batch opens). Returns the batch-start bits; writes the 16-bit cursors.
+template <int N4>
+__device__ __forceinline__ uint32_t bounds_word(uint32_t buf, uint32_t sorec0, uint32_t C,
+                                                uint32_t& room, uint4* __restrict__ cs_out,
+                                                int n4_runtime, bool write) {
+  uint32_t bits = 0;
+  uint32_t cw[4];
+#pragma unroll
+  for (int g = 0; g < N4; ++g) {
+    if (N4 == 8 || g < n4_runtime) {
+      const int4 v = lds128(buf + 16 * g);
+      const uint32_t r0 = lds32(sorec0 + 4 * v.x), r1 = lds32(sorec0 + 4 * v.y);
+      const uint32_t r2 = lds32(sorec0 + 4 * v.z), r3 = lds32(sorec0 + 4 * v.w);
+      // cursor stream: 4 x u16 = bits 8..23 of the order records
+      cw[(2 * g) & 3] = __byte_perm(r0, r1, 0x6521);
+      cw[(2 * g + 1) & 3] = __byte_perm(r2, r3, 0x6521);
+      const uint32_t rr[4] = {r0, r1, r2, r3};
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        const uint32_t q = rr[t] & WHP_Q_MASK;
+        if (room < q) bits |= 1u << (4 * g + t);
+        room = min(room - q, C - q);
+      }
+      if ((g & 1) && write) cs_out[g >> 1] = make_uint4(cw[0], cw[1], cw[2], cw[3]);
+    }
+  }
+  if (N4 != 8 && (n4_runtime & 1) && write) {  // odd tail: the last 4 cursors, upper half unused
+    const int g = n4_runtime - 1;
+    cs_out[g >> 1] = make_uint4(cw[(2 * g) & 3], cw[(2 * g + 1) & 3], 0u, 0u);
+  }
+  return bits;
+}
 
 __global__ void __launch_bounds__(kBoundsThreads)
 whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int32_t C,
                   const int32_t* __restrict__ perms, int64_t n_cand,
                   uint32_t* __restrict__ bmask, int32_t bm_pitch, uint16_t* __restrict__ cstream,
                   int32_t cs_pitch, int32_t* __restrict__ nb_scratch,
-                  int32_t* __restrict__ n_batches_out) {
+                  int32_t* __restrict__ n_batches_out, int32_t* __restrict__ segstart,
+                  int32_t ss_pitch, int32_t S, int32_t log2S) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  // [ring: kRing slots x 64 threads x 16 B][order_fast: (cursor << 8 | q) per order]
-  const uint32_t ring0 = smem_u32(smem_raw) + threadIdx.x * 16;
-  uint32_t* sorec = reinterpret_cast<uint32_t*>(smem_raw + kRing * kBoundsThreads * 16);
-  const uint32_t sorec0 = smem_u32(sorec);
-  for (int i = threadIdx.x; i < n_orders; i += kBoundsThreads) sorec[i] = __ldg(order_fast + i);
-  const int64_t c = (int64_t)blockIdx.x * kBoundsThreads + threadIdx.x;
-  const bool have = c < n_cand;
-  const int4* __restrict__ row = reinterpret_cast<const int4*>(perms + (have ? c : 0) * n_orders);
-  const int n4 = n_orders >> 2;
-  if (have) {
-#pragma unroll 1
-    for (int k = 0; k < kRing; ++k) {
-      if (k < n4) cp_async16(ring0 + k * (kBoundsThreads * 16), row + k);
-      else asm volatile("st.shared.v4.u32 [%0], {%1,%1,%1,%1};" ::"r"(ring0 + k * (kBoundsThreads * 16)), "r"(0u));
-      cp_async_commit();
-    }
-  }
-  __syncthreads();  // sorec visible
-  if (!have) return;
-  uint32_t* __restrict__ bm = bmask + c * bm_pitch;
-  uint2* __restrict__ cs = reinterpret_cast<uint2*>(cstream + c * cs_pitch);
+  // [chunk buffers: kStages x 64 threads x kChunkStride][order table][stash of the boundary
+  //  words: nw x 64][mbarriers: kStages x 2 warps]
   const int nw = (n_orders + 31) >> 5;
-  // Next-fit recurrence on room = C - load, one dependent instruction per position:
-  //   room' = umin(room - q, C - q)   (room < q wraps room - q above C - q: a new batch opens)
+  const int tid = threadIdx.x, warp = tid >> 5;
+  uint8_t* sp = smem_raw + kStages * kBoundsThreads * kChunkStride;
+  uint32_t* sorec = reinterpret_cast<uint32_t*>(sp);
+  sp += 4 * (size_t)((n_orders + 3) & ~3);
+  uint32_t* stash = reinterpret_cast<uint32_t*>(sp);
+  sp += 4 * (size_t)nw * kBoundsThreads;
+  const uint32_t bars = smem_u32(sp);
+  const uint32_t buf0 = smem_u32(smem_raw) + tid * kChunkStride;
+  const uint32_t sorec0 = smem_u32(sorec);
+  for (int i = tid; i < n_orders; i += kBoundsThreads) sorec[i] = __ldg(order_fast + i);
+  if ((tid & 31) == 0)
+    for (int s = 0; s < kStages; ++s) mbar_init(bars + 8 * (s * 2 + warp), 32);
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  __syncthreads();
+  const int64_t c_raw = (int64_t)blockIdx.x * kBoundsThreads + tid;
+  const bool have = c_raw < n_cand;
+  const int64_t c = have ? c_raw : n_cand - 1;  // idle threads shadow the last plan, no writes
+  const uint8_t* __restrict__ row = reinterpret_cast<const uint8_t*>(perms + c * n_orders);
+  const int row_bytes = 4 * n_orders;
+  const int nchunks = (row_bytes + kChunkBytes - 1) / kChunkBytes;
+  for (int k = 0; k < kStages && k < nchunks; ++k) {
+    const uint32_t bytes = (uint32_t)min(kChunkBytes, row_bytes - k * kChunkBytes);
+    const uint32_t bar = bars + 8 * (k * 2 + warp);
+    mbar_expect_tx(bar, bytes);
+    bulk_g2s(buf0 + k * (kBoundsThreads * kChunkStride), row + (size_t)k * kChunkBytes, bytes, bar);
+  }
+  uint32_t* __restrict__ bm = bmask + c * bm_pitch;
+  uint4* __restrict__ cs = reinterpret_cast<uint4*>(cstream + c * cs_pitch);
   uint32_t room = (uint32_t)C;
   uint32_t nb = 0;
-  int p4 = 0, slot = 0;
-  // 3-stage software pipeline, one chunk (4 positions) per stage: (A) order ids of chunk i+2
-  // leave the cp.async ring, (B) their order records are gathered for chunk i+1, (C) chunk i
-  // runs the next-fit recurrence — the only loop-carried dependency chain.
-  int4 ids = make_int4(0, 0, 0, 0);
-  uint32_t rb[4] = {0, 0, 0, 0}, rc[4] = {0, 0, 0, 0};
-  auto stage_a = [&](int chunk) {  // chunk may run past the row end: the slot is then stale
-    cp_async_wait<kRing - 1>();
-    const uint32_t slot_addr = ring0 + slot * (kBoundsThreads * 16);
-    const int4 v = lds128(slot_addr);
-    if (chunk + kRing < n4) cp_async16(slot_addr, row + chunk + kRing);
-    cp_async_commit();
-    slot = (slot + 1) & (kRing - 1);
-    return v;
-  };
-  auto stage_b = [&](const int4& v, uint32_t (&r)[4]) {
-    // ids past the row end are stale ring contents (ids of earlier chunks, or the zero fill):
-    // always valid order ids, so the gather stays in the table
-    r[0] = lds32(sorec0 + 4 * v.x); r[1] = lds32(sorec0 + 4 * v.y);
-    r[2] = lds32(sorec0 + 4 * v.z); r[3] = lds32(sorec0 + 4 * v.w);
-  };
-  ids = stage_a(0);
-  stage_b(ids, rc);
-  ids = stage_a(1);
-  stage_b(ids, rb);
-  ids = stage_a(2);
+  int stage = 0;
+  uint32_t parity = 0;
 #pragma unroll 1
-  for (int w = 0; w < nw; ++w) {
-    uint32_t bits = (w == 0) ? 1u : 0u;  // batch 0 starts at position 0
+  for (int k = 0; k < nchunks; ++k) {
+    const uint32_t bar = bars + 8 * (stage * 2 + warp);
+    const uint32_t buf = buf0 + stage * (kBoundsThreads * kChunkStride);
+    mbar_wait(bar, parity);
+    const int npos = min(kChunkBytes / 4, n_orders - k * (kChunkBytes / 4));
 #pragma unroll
-    for (int k = 0; k < 8; ++k, ++p4) {
-      if (p4 < n4) {
-        uint32_t rn[4];
-        stage_b(ids, rn);        // chunk p4 + 2
-        ids = stage_a(p4 + 3);
-        // cursor stream: 4 x u16 = bits 8..23 of the order records
-        cs[p4] = make_uint2(__byte_perm(rc[0], rc[1], 0x6521), __byte_perm(rc[2], rc[3], 0x6521));
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          const uint32_t q = rc[t] & WHP_Q_MASK;
-          const bool over = room < q;
-          room = min(room - q, (uint32_t)C - q);
-          if (over) bits |= 1u << (4 * k + t);
-          rc[t] = rb[t];
-          rb[t] = rn[t];
-        }
+    for (int h = 0; h < 2; ++h) {
+      const int w = 2 * k + h;
+      const int left = npos - 32 * h;
+      if (left > 0) {
+        uint32_t bits;
+        if (left >= 32) bits = bounds_word<8>(buf + 128 * h, sorec0, (uint32_t)C, room, cs + 4 * w, 8, have);
+        else bits = bounds_word<7>(buf + 128 * h, sorec0, (uint32_t)C, room, cs + 4 * w, left >> 2, have);
+        if (w == 0) bits |= 1u;  // batch 0 starts at position 0
+        nb += __popc(bits);
+        stash[w * kBoundsThreads + tid] = bits;
+        if (w == (n_orders >> 5)) bits |= 1u << (n_orders & 31);  // end sentinel, partial word
+        if (have) bm[w] = bits;
       }
     }
-    nb += __popc(bits);
-    if (w == (n_orders >> 5)) bits |= 1u << (n_orders & 31);  // end sentinel in a partial word
-    bm[w] = bits;
+    if (k + kStages < nchunks) {  // refill this stage (its values have been consumed above)
+      const int kn = k + kStages;
+      const uint32_t bytes = (uint32_t)min(kChunkBytes, row_bytes - kn * kChunkBytes);
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      mbar_expect_tx(bar, bytes);
+      bulk_g2s(buf, row + (size_t)kn * kChunkBytes, bytes, bar);
+    }
+    if (++stage == kStages) { stage = 0; parity ^= 1u; }
   }
+  if (!have) return;
   if ((n_orders & 31) == 0) bm[nw] = 1u;  // end sentinel in a word of its own
   nb_scratch[c] = (int32_t)nb;
   if (n_batches_out) n_batches_out[c] = (int32_t)nb;
+  // first position of every segment: segment s starts with batch floor(s * nb / S)
+  int32_t* __restrict__ ss = segstart + c * ss_pitch;
+  int seg = 0, target = 0, acc = 0;
+  for (int w = 0; w < nw && seg < S; ++w) {
+    const uint32_t bits = stash[w * kBoundsThreads + tid];
+    const int pc = __popc(bits);
+    while (seg < S && target < acc + pc) {
+      uint32_t t = bits;
+      for (int r = target - acc; r > 0; --r) t &= t - 1;
+      ss[seg] = 32 * w + __ffs(t) - 1;
+      ++seg;
+      target = (int)(((int64_t)seg * nb) >> log2S);
+    }
+    acc += pc;
+  }
 }
 
 // ------------------------------------------------------------------------------------------ K2
@@ -155,24 +221,28 @@ constexpr int kMaxPlanes = 8;  // vertical counter bit planes: up to 255 batches
 struct sets_params {
   int S;           // segments per candidate (power of two <= 32)
   int log2S;
-  int aw_words;    // aisle words per lane  = ceil(NA/16)
-  int ring_words;  // per-lane ring of first-pick cursors of the open batch = C + 2
-  int id_slots;    // 16-byte cursor-stream chunks resident per lane (power of two, covers a batch)
-  int bm_pitch, cs_pitch;
+  int aw_words;    // 32-aisle occupancy words per lane = ceil(NA/32)
+  int ring_mask;   // bytes of the per-lane cursor ring - 1 (ring = 8 or 16 chunks of 16 B)
+  int bm_pitch, cs_pitch, ss_pitch;
   int n_items_pad;
+  int fits32;      // every per-batch length fits 31 bits
   int64_t n_tasks;  // warp tasks = ceil(n_cand*S/32)
 };
 
+__device__ __forceinline__ uint32_t lds16(uint32_t a) {
+  uint16_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a)); return v;
+}
+
 template <bool SMEM_TABLES, bool DEPOT0, int KW, int kPlanes>
-__global__ void __launch_bounds__(512, 1)
+__global__ void __launch_bounds__(kPlanes <= 6 ? 768 : 512, 1)
 whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restrict__ pick_fast,
                 const uint16_t* __restrict__ cstream, const uint32_t* __restrict__ bmask,
-                const int32_t* __restrict__ nb_scratch, int64_t n_cand,
-                int64_t* __restrict__ dist_scratch, uint32_t* __restrict__ planes_out,
-                uint64_t* __restrict__ hash_out, unsigned long long* __restrict__ task_counter) {
+                const int32_t* __restrict__ nb_scratch, const int32_t* __restrict__ segstart,
+                int64_t n_cand, int64_t* __restrict__ dist_scratch,
+                uint32_t* __restrict__ planes_out, uint64_t* __restrict__ hash_out,
+                unsigned long long* __restrict__ task_counter) {
   extern __shared__ __align__(16) uint32_t smem[];
   // layout: [pick table n_items_pad] (if staged) [per-warp private words]
-  constexpr int CW = 2 * KW;  // 16-bit stamped class words per lane
   uint32_t* priv = smem;
   uint32_t pick_base = 0;
   if (SMEM_TABLES) {
@@ -182,20 +252,22 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
     __syncthreads();
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int priv_words = (CW + P.aw_words + P.ring_words + P.id_slots * 4) * 32;
-  // private words of this lane: word w at my_c[w*32] (bank = lane)
-  uint32_t* my_c = priv + (size_t)warp * priv_words + lane;
-  const uint32_t cbase = smem_u32(my_c);
-  const uint32_t abase = cbase + CW * 128;
-  const uint32_t ring = abase + P.aw_words * 128;
-  const uint32_t idring = cbase - lane * 4 + (CW + P.aw_words + P.ring_words) * 128 + lane * 16;
-  for (int w = 0; w < P.ring_words; ++w) sts32(ring + w * 128, pick_base);
+  // private state of a lane: KW class words and aw_words aisle words laid out [word][lane]
+  // (bank = lane), then its cursor ring, lane-major with a stride of ring + 16 bytes
+  const int ring_stride = P.ring_mask + 1 + 16;
+  const int priv_bytes = (KW + P.aw_words) * 128 + 32 * ring_stride;
+  const uint32_t wbase = smem_u32(priv) + (uint32_t)warp * priv_bytes;
+  const uint32_t cbase = wbase + lane * 4;
+  const uint32_t abase = cbase + KW * 128;
+  const uint32_t ringbase = wbase + (KW + P.aw_words) * 128 + lane * ring_stride;
+  const int chunks = (P.ring_mask + 1) >> 4;
   const int Cmax = T.C;
   const int64_t A = T.g.aisle_len;
   const int64_t P2 = 2 * (int64_t)T.g.aisle_spacing;
   const int n8 = P.cs_pitch >> 3;  // 16-byte chunks per cursor-stream row
+  for (int w = 0; w < KW + P.aw_words; ++w) sts32(cbase + w * 128, 0u);
 
-  __shared__ unsigned long long s_task[16];
+  __shared__ unsigned long long s_task[32];
   for (;;) {
     // claim the next warp task (32 consecutive (candidate, segment) pairs)
     if (lane == 0) s_task[warp] = atomicAdd(task_counter, 1ull);
@@ -208,54 +280,43 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
     const int seg = (int)(unit & (P.S - 1));
     const bool have = cand_raw < n_cand;
     const int64_t cand = have ? cand_raw : n_cand - 1;
-    int b_lo = 0, b_hi = 0;
+    int b_lo = 0, nbseg = 0;
     if (have) {
       const int nb = __ldg(nb_scratch + cand);
       b_lo = (int)((int64_t)seg * nb >> P.log2S);
-      b_hi = (int)((int64_t)(seg + 1) * nb >> P.log2S);
+      nbseg = (int)((int64_t)(seg + 1) * nb >> P.log2S) - b_lo;
     }
-    const int nbseg = b_hi - b_lo;
     const int nbmax = __reduce_max_sync(WHP_FULL, nbseg);
-    // clear the private set words (stamp 0 is older than every live batch)
-    for (int w = 0; w < CW + P.aw_words; ++w) my_c[w * 32] = 0;
     uint32_t pl[kPlanes][KW];
 #pragma unroll
     for (int p = 0; p < kPlanes; ++p)
 #pragma unroll
       for (int w = 0; w < KW; ++w) pl[p][w] = 0;
 
-    // ---- locate the first batch of the segment in the boundary bitmask (select b_lo)
+    // ---- first batch of the segment: its start position comes from K1
     const uint32_t* __restrict__ bm = bmask + cand * P.bm_pitch;
-    int wi = 0;
-    uint32_t bw = __ldg(bm);
-    if (nbseg > 0) {
-      int acc = 0;
-      for (;;) {
-        const int pc = __popc(bw);
-        if (acc + pc > b_lo) break;
-        acc += pc;
-        ++wi;
-        bw = __ldg(bm + wi);
-      }
-      for (int r = b_lo - acc; r > 0; --r) bw &= bw - 1;  // drop the starts before mine
-    }
+    int p = __ldg(segstart + cand * P.ss_pitch + seg);
+    int wi = p >> 5;
+    uint32_t bw = __ldg(bm + wi) & (WHP_FULL << (p & 31));
     uint32_t bw_next = __ldg(bm + min(wi + 1, P.bm_pitch - 1));
-    int p = 32 * wi + __ffs(bw) - 1;  // first position of the segment
 
-    // ---- cursor stream of this lane through a private cp.async ring ([slot][lane] x 16 B):
-    // chunk c (cursors of positions 8c..8c+7) lives in slot c mod kIdRing
+    // ---- cursor stream of this lane through its private cp.async ring: chunk c (cursors of
+    // positions 8c..8c+7) lives at ring offset (16 c) mod ring
     const uint4* __restrict__ cs = reinterpret_cast<const uint4*>(cstream + cand * P.cs_pitch);
+    int lo_prev;  // first chunk that was resident when the newest refill group was issued
     {
       const int c0 = p >> 3;
-      for (int k = 0; k < P.id_slots; ++k)
-        cp_async16(idring + ((c0 + k) & (P.id_slots - 1)) * 512, cs + min(c0 + k, n8 - 1));
+      for (int k = 0; k < chunks; ++k)
+        cp_async16(ringbase + (((c0 + k) << 4) & P.ring_mask), cs + min(c0 + k, n8 - 1));
       cp_async_commit();
+      lo_prev = c0 - chunks;
     }
 
     int64_t D = 0;
     uint64_t hash = 0;
     for (int j = 0; j < nbmax; ++j) {
       int left = 0;  // orders of batch j
+      const int p0 = p;
       if (j < nbseg) {
         bw &= bw - 1;  // past my own start bit: the next set bit is the next batch (or the end)
         while (bw == 0) {
@@ -269,45 +330,22 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         p = pe;
       }
       const bool live = left > 0;
-      // ---- prefill the private ring with the first-pick cursor of every order of the batch,
-      // one 16-byte chunk (8 positions) of the cursor stream at a time
-      const int p0 = p - left;                       // first position of the batch
-      const int nc = live ? ((p - 1) >> 3) - (p0 >> 3) + 1 : 0;   // chunks the batch touches
-      const int nf = (p >> 3) - (p0 >> 3);           // chunks the batch finishes
-      const int ncmax = __reduce_max_sync(WHP_FULL, nc);
-      cp_async_wait<0>();  // issued a whole batch ago: normally complete already
-      for (int i = 0; i < ncmax; ++i) {
-        if (i < nc) {
-          const int c = (p0 >> 3) + i;
-          const int4 v = lds128(idring + (c & (P.id_slots - 1)) * 512);
-          const int kb = 8 * c - p0;               // ring index of the chunk's first cursor
-          const uint32_t rb = ring + kb * 128;
-          const uint32_t vv[4] = {(uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w};
-#pragma unroll
-          for (int e = 0; e < 8; ++e) {
-            const uint32_t c16 = (e & 1) ? (vv[e >> 1] >> 16) : (vv[e >> 1] & 0xffffu);
-            sts32_if_lt((uint32_t)(kb + e), (uint32_t)left, rb + e * 128,
-                        SMEM_TABLES ? pick_base + 8 * c16 : 2 * c16);
-          }
-        }
+      // the newest refill group brought chunks lo_prev+chunks ..; everything older has landed
+      // after wait<1>. The batch reads cursors of positions p0 .. p (one ahead).
+      if (live && (p >> 3) >= lo_prev + chunks) cp_async_wait<0>(); else cp_async_wait<1>();
+      uint32_t v = live ? 2u * (uint32_t)p0 : 0u;          // 2 x position of the next order
+      const uint32_t v_end = live ? 2u * (uint32_t)p : 0u;
+      uint32_t cur;
+      if (live) {
+        const uint32_t c16 = lds16(ringbase + (v & P.ring_mask));
+        cur = SMEM_TABLES ? pick_base + 8 * c16 : 2 * c16;
+        v += 2;
+      } else {
+        cur = SMEM_TABLES ? pick_base : 0u;
       }
-      {  // refill the slots of the finished chunks; they land while the batch is processed
-        const int nfmax = __reduce_max_sync(WHP_FULL, nf);
-        for (int i = 0; i < nfmax; ++i)
-          if (i < nf) {
-            const int c = (p0 >> 3) + i;
-            cp_async16(idring + (c & (P.id_slots - 1)) * 512, cs + min(c + P.id_slots, n8 - 1));
-          }
-        cp_async_commit();
-      }
-      const uint32_t stamp_hi = (uint32_t)(j + 1) << 16;
-      uint32_t kmax = 0, kmin = 0xffffffffu;
-      int m = 0;
-      uint32_t cur = lds32(ring);
-      uint32_t n_cur = lds32(ring + 128);
-      uint32_t rp = ring + 256;
-      const uint32_t rp_end = rp + 128 * max(left - 1, 0);  // left-1 moves to a next order
+      uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));
       uint32_t rec = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
+      uint32_t kmax = 0, kmin = 0xffffffffu;
       // Branch-free step: every lane runs Cmax steps. A lane that has finished its batch stays
       // on the batch's final pick and re-inserts it (set inserts and max are idempotent); a
       // lane without a batch walks to the end of order 0 and stays there — its sets are
@@ -317,12 +355,12 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         // cursor of the next step's pick: next record, the next order's first pick, or stay
         uint32_t nxt = cur + (SMEM_TABLES ? 4u : 1u);
         const bool last = (rec & WHP_FAST_LAST) != 0;
-        const bool more = last && (rp != rp_end);
+        const bool more = last && (v != v_end);
         if (last) nxt = cur;
         if (more) {
-          nxt = n_cur;
-          n_cur = lds32(rp);
-          rp += 128;
+          nxt = SMEM_TABLES ? pick_base + 8 * n_c16 : 2 * n_c16;
+          v += 2;
+          n_c16 = lds16(ringbase + (v & P.ring_mask));
         }
         cur = nxt;
         const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
@@ -330,37 +368,55 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         kmax = max(kmax, rec);
         if (!DEPOT0) kmin = min(kmin, rec);
         const uint32_t aaddr = abase + ((rec >> 26) << 7);
-        const uint32_t abit = one_shl_wrap(rec >> 21);  // spacer bit: (rec >> 21) mod 32 = a_lo
-        const uint32_t x = max(lds32(aaddr), stamp_hi);  // an older stamp compares lower: empty
-        const uint32_t x2 = x | abit;
-        asm("{ .reg .pred pp; setp.ne.u32 pp, %1, %2; @pp add.s32 %0, %0, 1; }" : "+r"(m) : "r"(x2), "r"(x));
-        sts32(aaddr, x2);
-        const uint32_t caddr = cbase + ((rec & 0xf0u) << 3);
-        const uint32_t cbit = one_shl_wrap(rec & 15u);
-        const uint32_t y = max(lds32(caddr), stamp_hi);
-        sts32(caddr, y | cbit);
+        sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 21));
+        const uint32_t caddr = cbase + ((rec & 0xe0u) << 2);
+        sts32(caddr, lds32(caddr) | one_shl_wrap(rec));
         rec = rec_next;
       }
-      // ---- close the batch: D4, and the class set into the vertical counters (D5)
-      if (live) {
-        const int64_t a_max = WHP_PICK_AISLE(kmax);
-        const int64_t d_last =
-            (int64_t)((kmax >> WHP_PICK_SLOT_SHIFT) & WHP_PICK_SLOT_MASK) * T.g.slot_pitch;
-        int64_t H;
-        if (DEPOT0) {
-          H = P2 * a_max;
-        } else {
-          const int64_t a_min = WHP_PICK_AISLE(kmin), a0 = T.g.depot_aisle;
-          H = (int64_t)T.g.aisle_spacing * (llabs(a0 - a_min) + (a_max - a_min) + llabs(a_max - a0));
-        }
-        D += H + ((m & 1) ? (int64_t)(m - 1) * A + 2 * d_last : (int64_t)m * A);
+      {  // refill the slots of the chunks this batch finished; waited for two batches later
+        const int nf = live ? (p >> 3) - (p0 >> 3) : 0;
+        const int nfmax = __reduce_max_sync(WHP_FULL, nf);
+        for (int i = 0; i < nfmax; ++i)
+          if (i < nf) {
+            const int c = (p0 >> 3) + i;
+            cp_async16(ringbase + ((c << 4) & P.ring_mask), cs + min(c + chunks, n8 - 1));
+          }
+        cp_async_commit();
+        if (live) lo_prev = p0 >> 3;
       }
+      // ---- close the batch: m = distinct aisles, D4; the sets are emptied for the next batch
+      int m = 0;
+#pragma unroll 4
+      for (int w = 0; w < P.aw_words; ++w) {
+        m += __popc(lds32(abase + w * 128));
+        sts32(abase + w * 128, 0u);
+      }
+      if (live) {
+        const uint32_t a_max = WHP_PICK_AISLE(kmax);
+        const uint32_t slot1 = (kmax >> WHP_PICK_SLOT_SHIFT) & WHP_PICK_SLOT_MASK;
+        if (DEPOT0 && P.fits32) {
+          const uint32_t d2 = 2u * slot1 * (uint32_t)T.g.slot_pitch;
+          D += (uint32_t)P2 * a_max + (uint32_t)m * (uint32_t)A + ((m & 1) ? d2 - (uint32_t)A : 0u);
+        } else {
+          const int64_t d_last = (int64_t)slot1 * T.g.slot_pitch;
+          int64_t H;
+          if (DEPOT0) {
+            H = P2 * (int64_t)a_max;
+          } else {
+            const int64_t a_min = WHP_PICK_AISLE(kmin), a0 = T.g.depot_aisle;
+            H = (int64_t)T.g.aisle_spacing *
+                (llabs(a0 - a_min) + ((int64_t)a_max - a_min) + llabs((int64_t)a_max - a0));
+          }
+          D += H + ((m & 1) ? (int64_t)(m - 1) * A + 2 * d_last : (int64_t)m * A);
+        }
+      }
+      // the batch's class set goes into the vertical counters (D5)
 #pragma unroll
       for (int w = 0; w < KW; ++w) {
         // lanes without a batch j ran the steps on a dummy pick: their set is discarded
-        const uint32_t y0 = max(lds32(cbase + (2 * w) * 128), stamp_hi);
-        const uint32_t y1 = max(lds32(cbase + (2 * w + 1) * 128), stamp_hi);
-        uint32_t carry = live ? __byte_perm(y0, y1, 0x5410) : 0u;  // 32 class bits of this batch
+        uint32_t carry = lds32(cbase + w * 128);
+        sts32(cbase + w * 128, 0u);
+        if (!live) carry = 0u;
 #pragma unroll
         for (int pp = 0; pp < kPlanes; ++pp) {
           const uint32_t t2 = pl[pp][w] & carry;
@@ -369,6 +425,7 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         }
       }
     }
+    cp_async_wait<0>();  // nothing of this task may still land in the ring
     // ---- combine the S segment lanes of each candidate (D, hash); write the counters
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1)
@@ -468,13 +525,18 @@ static int64_t nb_upper_bound(const whp_ctx* c) {
   return ub < c->n_orders ? ub : c->n_orders;
 }
 
+static size_t bounds_smem_bytes(const whp_ctx* c) {
+  const size_t nw = ((size_t)c->n_orders + 31) >> 5;
+  return (size_t)kStages * kBoundsThreads * kChunkStride + 4 * (((size_t)c->n_orders + 3) & ~(size_t)3) +
+         4 * nw * kBoundsThreads + 8 * kStages * 2;
+}
+
 bool whp_fast_eligible(const whp_ctx* c) {
   if (!c->fast_tables_ok) return false;                       // cursors must fit 16 bits
   if (c->n_orders % 4 != 0 || c->n_orders >= 65536) return false;
   if ((nb_upper_bound(c) + 31) / 32 > 255) return false;      // 8 counter planes, S <= 32
-  if (c->C > 64) return false;                                // per-lane cursor ring of C+2 words
-  if ((size_t)kRing * kBoundsThreads * 16 + 4 * (size_t)c->n_orders > (size_t)c->smem_optin - 1024)
-    return false;                                             // K1: order table in shared memory
+  if (c->C > 64) return false;                                // per-lane cursor ring of 16 chunks
+  if (bounds_smem_bytes(c) > (size_t)c->smem_optin - 1024) return false;  // K1 tables in smem
   return true;
 }
 
@@ -484,25 +546,22 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   const int64_t nb_ub = nb_upper_bound(c);
   const int32_t bm_pitch = (int32_t)((((c->n_orders + 31) >> 5) + 2 + 3) & ~3);
   const int32_t cs_pitch = (int32_t)((c->n_orders + 7) & ~7);
+  const int32_t ss_pitch = 32;
   const int KW = c->K <= 32 ? 1 : c->K <= 64 ? 2 : c->K <= 128 ? 4 : c->K <= 224 ? 7 : 8;
-  const int aw_words = (c->g.n_aisles + 15) / 16;
-  const int ring_words = c->C + 2;
-  int id_slots = 4;  // a batch of C orders touches at most (C+14)/8 chunks
-  while (id_slots < (c->C + 14) / 8 + 1) id_slots <<= 1;
+  const int aw_words = (c->g.n_aisles + 31) / 32;
+  // cursor ring: a batch of C orders touches at most (C+14)/8 chunks of 8 cursors, and the
+  // cursor one past its end is read too
+  const int ring_bytes = ((c->C + 14) / 8 + 1 <= 8) ? 128 : 256;
   // K2 shape
   const size_t table_bytes = 4 * (((size_t)c->n_items_pad + 31) & ~(size_t)31);
-  const size_t priv_per_warp = (size_t)(2 * KW + aw_words + ring_words + id_slots * 4) * 128;
+  const size_t priv_per_warp = (size_t)(KW + aw_words) * 128 + 32 * (size_t)(ring_bytes + 16);
   const size_t smem_max = (size_t)c->smem_optin - 1024;
   const bool smem_tables = table_bytes + 4 * priv_per_warp <= smem_max;
   const size_t avail = smem_max - (smem_tables ? table_bytes : 0);
-  int warps = (int)(avail / priv_per_warp);
-  if (warps > 16) warps = 16;
-  if (const char* e = getenv("WHP_WARPS")) { int v = atoi(e); if (v >= 1 && v <= warps) warps = v; }
-  if (warps < 1) return cudaErrorInvalidConfiguration;
-  const int64_t resident_warps = (int64_t)c->num_sms * warps;
-  // segments: few enough batches per segment for the counter planes, and ~4 tasks per warp
+  // segments: few enough batches per segment for the counter planes, and >= 4 tasks per warp
+  int warps_cap = 24;
   int S = 1;
-  while (S < 32 && ((nb_ub + S - 1) / S > 255 || n_cand * S < 4 * resident_warps * 32)) S <<= 1;
+  while (S < 32 && ((nb_ub + S - 1) / S > 255 || n_cand * S < 4ll * c->num_sms * warps_cap * 32)) S <<= 1;
   if (const char* e = getenv("WHP_SEGMENTS")) {
     int v = atoi(e);
     if (v >= 1 && v <= 32 && (v & (v - 1)) == 0 && (nb_ub + v - 1) / v <= 255) S = v;
@@ -511,18 +570,26 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   while ((1 << log2S) < S) ++log2S;
   int seg_planes = 1;  // planes of one segment's counters; one more per combine level
   while ((1ll << seg_planes) <= (nb_ub + S - 1) / S) ++seg_planes;
-  const bool depot0_pl = c->g.depot_aisle == 0;
-  const int kernel_planes = (depot0_pl && seg_planes <= 6) ? 6 : 8;  // the instantiation used
+  const int kernel_planes = seg_planes <= 4 ? 4 : seg_planes <= 6 ? 6 : 8;  // the instantiation
+  if (kernel_planes > 6) warps_cap = 16;  // __launch_bounds__ of the 8-plane instantiation
+  int warps = (int)(avail / priv_per_warp);
+  if (warps > warps_cap) warps = warps_cap;
+  if (const char* e = getenv("WHP_WARPS")) { int v = atoi(e); if (v >= 1 && v <= warps) warps = v; }
+  if (warps < 1) return cudaErrorInvalidConfiguration;
   const int planes_used = kernel_planes + log2S;
+  // every per-batch length below 2^31: the close can work in 32 bits
+  const int64_t worst = 2ll * c->g.aisle_spacing * c->g.n_aisles +
+                        ((int64_t)c->g.n_aisles + 2) * c->g.aisle_len;
+  const int fits32 = worst < (1ll << 31) ? 1 : 0;
   // scratch (grow-only; reallocated when the shape changes)
   const int64_t plane_words = (int64_t)(kMaxPlanes + 5) * KW;
   if (c->fast_cap < n_cand || c->fast_pitch != bm_pitch || c->fast_plane_words < plane_words) {
     cudaError_t e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return e;
     cudaFree(c->d_bmask); cudaFree(c->d_cstream); cudaFree(c->d_nb); cudaFree(c->d_dist_scratch);
-    cudaFree(c->d_planes);
+    cudaFree(c->d_planes); cudaFree(c->d_segstart);
     c->d_bmask = nullptr; c->d_cstream = nullptr; c->d_nb = nullptr; c->d_dist_scratch = nullptr;
-    c->d_planes = nullptr;
+    c->d_planes = nullptr; c->d_segstart = nullptr;
     const int64_t cap = n_cand > c->fast_cap ? n_cand : c->fast_cap;
     const int64_t pw = plane_words > c->fast_plane_words ? plane_words : c->fast_plane_words;
     c->fast_cap = 0;
@@ -531,6 +598,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
     if ((e = cudaMalloc(&c->d_nb, 4 * (size_t)cap)) != cudaSuccess) return e;
     if ((e = cudaMalloc(&c->d_dist_scratch, 8 * (size_t)cap)) != cudaSuccess) return e;
     if ((e = cudaMalloc(&c->d_planes, 4 * (size_t)cap * pw)) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&c->d_segstart, 4 * (size_t)cap * ss_pitch)) != cudaSuccess) return e;
     if ((e = cudaMemsetAsync(c->d_bmask, 0, 4 * (size_t)cap * bm_pitch, st)) != cudaSuccess) return e;
     c->fast_cap = cap; c->fast_pitch = bm_pitch; c->fast_plane_words = pw;
   }
@@ -538,21 +606,22 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   {
     cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
-    const size_t smem = (size_t)kRing * kBoundsThreads * 16 + 4 * (size_t)c->n_orders;
+    const size_t smem = bounds_smem_bytes(c);
     cudaFuncSetAttribute(whp_bounds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
     const unsigned blocks = (unsigned)((n_cand + kBoundsThreads - 1) / kBoundsThreads);
     whp_bounds_kernel<<<blocks, kBoundsThreads, smem, st>>>(
         c->d_order_fast, c->n_orders, c->C, d_perms, n_cand, c->d_bmask, bm_pitch, c->d_cstream,
-        cs_pitch, c->d_nb, out.n_batches);
+        cs_pitch, c->d_nb, out.n_batches, c->d_segstart, ss_pitch, S, log2S);
     c->launches += 1;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
   }
   // K2
   {
     sets_params P;
-    P.S = S; P.log2S = 0; while ((1 << P.log2S) < S) ++P.log2S;
-    P.aw_words = aw_words; P.ring_words = ring_words; P.id_slots = id_slots;
-    P.bm_pitch = bm_pitch; P.cs_pitch = cs_pitch; P.n_items_pad = c->n_items_pad;
+    P.S = S; P.log2S = log2S;
+    P.aw_words = aw_words; P.ring_mask = ring_bytes - 1;
+    P.bm_pitch = bm_pitch; P.cs_pitch = cs_pitch; P.ss_pitch = ss_pitch;
+    P.n_items_pad = c->n_items_pad; P.fits32 = fits32;
     P.n_tasks = (n_cand * S + 31) / 32;
     int64_t blocks = (P.n_tasks + warps - 1) / warps;
     if (blocks > c->num_sms) blocks = c->num_sms;
@@ -563,12 +632,13 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
     cudaFuncSetAttribute(whp_sets_kernel<ST, D0, KWV, PLV>,                                      \
                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);            \
     whp_sets_kernel<ST, D0, KWV, PLV><<<(unsigned)blocks, warps * 32, smem, st>>>(               \
-        T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, n_cand, c->d_dist_scratch,      \
-        c->d_planes, out.batch_hash, c->d_task);                                                 \
+        T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand,          \
+        c->d_dist_scratch, c->d_planes, out.batch_hash, c->d_task);                              \
   } while (0)
 #define WHP_LAUNCH_SETS(ST, D0, KWV)                                                             \
   do {                                                                                           \
-    if (D0 && seg_planes <= 6) WHP_LAUNCH_SETS_PL(ST, D0, KWV, 6);                               \
+    if (kernel_planes == 4) WHP_LAUNCH_SETS_PL(ST, D0, KWV, 4);                                  \
+    else if (kernel_planes == 6) WHP_LAUNCH_SETS_PL(ST, D0, KWV, 6);                             \
     else WHP_LAUNCH_SETS_PL(ST, D0, KWV, 8);                                                     \
   } while (0)
 #define WHP_LAUNCH_SETS_KW(ST, D0)                                                               \

@@ -10,15 +10,16 @@
 
 // ---- packed device tables -----------------------------------------------------
 // order record, 32 bit:  item_off[31:8] | q[7:0]            (q = number of items, 1..255)
-// pick  record, 32 bit:  a_hi[31:26] | 0 [25] | a_lo[24:21] | slot1[20:9] | side[8] | class[7:0]
-//   aisle = a_hi*16 + a_lo; slot1 = slot + 1 (depth = slot1 * slot_pitch). The field order makes
-//   an unsigned max over the records of a batch return (a_max, deepest slot in a_max) in its
-//   top 23 bits (D3). The zero spacer bit lets (rec >> 21) feed a 5-bit shift amount directly
-//   (bit index inside a 16-aisle word) and a_hi = rec >> 26 index the word, without masks.
+// pick  record, 32 bit:  0 [31] | aisle[30:21] | slot1[20:9] | side[8] | class[7:0]
+//   slot1 = slot + 1 (depth = slot1 * slot_pitch). The field order makes an unsigned max (min)
+//   over the records of a batch return (a_max, deepest slot in a_max) ((a_min, ..)) in its top
+//   bits (D3). rec >> 26 is the index of the 32-aisle occupancy word and (rec >> 21) mod 32 the
+//   bit inside it; (rec & 0xe0) >> 5 the 32-class word and rec mod 32 the bit — so a funnel
+//   shift that wraps its shift amount needs no mask.
 #define WHP_Q_BITS 8
 #define WHP_Q_MASK 0xffu
-#define WHP_PICK_PACK_AISLE(a) ((((uint32_t)(a) >> 4) << 26) | (((uint32_t)(a) & 15u) << 21))
-#define WHP_PICK_AISLE(rec) ((((rec) >> 26) << 4) | (((rec) >> 21) & 15u))
+#define WHP_PICK_PACK_AISLE(a) ((uint32_t)(a) << 21)
+#define WHP_PICK_AISLE(rec) ((rec) >> 21)
 #define WHP_PICK_SLOT_SHIFT 9
 #define WHP_PICK_SLOT_MASK 0xfffu
 #define WHP_PICK_LOC_SHIFT 8 /* rec >> 8 identifies the location (aisle, slot, side) */
@@ -100,6 +101,7 @@ struct whp_ctx {
   uint32_t* d_bmask = nullptr;       // [fast_cap][fast_pitch] bitmask of batch-start positions
   uint16_t* d_cstream = nullptr;     // [fast_cap][cs_pitch] first-pick cursor of every position
   int32_t* d_nb = nullptr;           // [fast_cap]
+  int32_t* d_segstart = nullptr;     // [fast_cap][32] first position of every segment
   int64_t* d_dist_scratch = nullptr; // [fast_cap]
   uint32_t* d_planes = nullptr;      // [fast_cap][S][8 planes][KW] bit-sliced class counters
   unsigned long long* d_task = nullptr;  // [2] work-stealing counter
