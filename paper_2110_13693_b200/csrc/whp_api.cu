@@ -188,8 +188,7 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
     const size_t cur = pfast.size() / 2;
     if (cur > 0xffff) fast_ok = false;
     for (int32_t i = order_ptr[o]; i < order_ptr[o + 1]; ++i) {
-      uint32_t r = prec[i] & ~(1u << WHP_PICK_LOC_SHIFT);
-      if (i == order_ptr[o + 1] - 1) r |= 1u << WHP_PICK_LOC_SHIFT;
+      const uint32_t r = WHP_FAST_PACK(prec[i], i == order_ptr[o + 1] - 1);
       pfast.push_back(r);
     }
     if (pfast.size() & 1) pfast.push_back(0u);

@@ -39,10 +39,6 @@ __device__ __forceinline__ int4 lds128(uint32_t a) {
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) {
   asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v));
 }
-// if (k < n) st.shared [a] = v — predicated, never a branch
-__device__ __forceinline__ void sts32_if_lt(uint32_t k, uint32_t n, uint32_t a, uint32_t v) {
-  asm volatile("{ .reg .pred pq; setp.lt.u32 pq, %0, %1; @pq st.shared.u32 [%2], %3; }" ::"r"(k), "r"(n), "r"(a), "r"(v));
-}
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
 }
@@ -216,12 +212,13 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
 
 // ------------------------------------------------------------------------------------------ K2
 constexpr int kMaxPlanes = 8;  // vertical counter bit planes: up to 255 batches per segment
-#define WHP_FAST_LAST 0x100u
 
 struct sets_params {
   int S;           // segments per candidate (power of two <= 32)
   int log2S;
   int aw_words;    // 32-aisle occupancy words per lane = ceil(NA/32)
+  int awp;         // aw_words rounded up to a power of two: a warp's aisle words are awp*128 B
+  int kwp;         // the same for the KW class words
   int ring_mask;   // bytes of the per-lane cursor ring - 1 (ring = 8 or 16 chunks of 16 B)
   int bm_pitch, cs_pitch, ss_pitch;
   int n_items_pad;
@@ -230,7 +227,7 @@ struct sets_params {
 };
 
 __device__ __forceinline__ uint32_t lds16(uint32_t a) {
-  uint16_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a)); return v;
+  uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v;
 }
 
 template <bool SMEM_TABLES, bool DEPOT0, int KW, int kPlanes>
@@ -252,20 +249,26 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
     __syncthreads();
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  // private state of a lane: KW class words and aw_words aisle words laid out [word][lane]
-  // (bank = lane), then its cursor ring, lane-major with a stride of ring + 16 bytes
+  const int nwarps = blockDim.x >> 5;
+  // private state of a lane: aw_words aisle words and KW class words laid out [word][lane]
+  // (bank = lane), a warp's words aligned to their (power-of-two) size so that a word's
+  // address is base | offset; then the lane's cursor ring, lane-major, stride ring + 16 bytes
   const int ring_stride = P.ring_mask + 1 + 16;
-  const int priv_bytes = (KW + P.aw_words) * 128 + 32 * ring_stride;
-  const uint32_t wbase = smem_u32(priv) + (uint32_t)warp * priv_bytes;
-  const uint32_t cbase = wbase + lane * 4;
-  const uint32_t abase = cbase + KW * 128;
-  const uint32_t ringbase = wbase + (KW + P.aw_words) * 128 + lane * ring_stride;
+  const uint32_t a_area = (smem_u32(priv) + P.awp * 128 - 1) & ~(uint32_t)(P.awp * 128 - 1);
+  const uint32_t c_area = a_area + nwarps * P.awp * 128;  // awp >= kwp: aligned as well
+  const uint32_t abase = a_area + warp * P.awp * 128 + lane * 4;
+  const uint32_t cbase = c_area + warp * P.kwp * 128 + lane * 4;
+  const uint32_t ringbase = c_area + nwarps * P.kwp * 128 + (warp * 32 + lane) * ring_stride;
+  const uint32_t amask = (uint32_t)(P.awp - 1) << 7;
+  uint32_t pb;  // pinned in a register (the shared-window conversion is otherwise re-derived)
+  asm volatile("mov.u32 %0, %1;" : "=r"(pb) : "r"(pick_base));
   const int chunks = (P.ring_mask + 1) >> 4;
   const int Cmax = T.C;
   const int64_t A = T.g.aisle_len;
   const int64_t P2 = 2 * (int64_t)T.g.aisle_spacing;
   const int n8 = P.cs_pitch >> 3;  // 16-byte chunks per cursor-stream row
-  for (int w = 0; w < KW + P.aw_words; ++w) sts32(cbase + w * 128, 0u);
+  for (int w = 0; w < P.aw_words; ++w) sts32(abase + w * 128, 0u);
+  for (int w = 0; w < KW; ++w) sts32(cbase + w * 128, 0u);
 
   __shared__ unsigned long long s_task[32];
   for (;;) {
@@ -338,10 +341,10 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       uint32_t cur;
       if (live) {
         const uint32_t c16 = lds16(ringbase + (v & P.ring_mask));
-        cur = SMEM_TABLES ? pick_base + 8 * c16 : 2 * c16;
+        cur = SMEM_TABLES ? pb + 8 * c16 : 2 * c16;
         v += 2;
       } else {
-        cur = SMEM_TABLES ? pick_base : 0u;
+        cur = SMEM_TABLES ? pb : 0u;
       }
       uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));
       uint32_t rec = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
@@ -352,24 +355,23 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       // discarded at the close below.
 #pragma unroll 2
       for (int t = 0; t < Cmax; ++t) {
-        // cursor of the next step's pick: next record, the next order's first pick, or stay
-        uint32_t nxt = cur + (SMEM_TABLES ? 4u : 1u);
-        const bool last = (rec & WHP_FAST_LAST) != 0;
+        // cursor of the next step's pick: next record, the next order's first pick, or stay —
+        // all by selects; the look-ahead cursor is (re)loaded every step
+        const uint32_t first_of_next = SMEM_TABLES ? pb + 8 * n_c16 : 2 * n_c16;
+        const bool last = (int32_t)(rec << 26) < 0;  // WHP_FAST_LAST (bit 5) into the sign bit
         const bool more = last && (v != v_end);
-        if (last) nxt = cur;
-        if (more) {
-          nxt = SMEM_TABLES ? pick_base + 8 * n_c16 : 2 * n_c16;
-          v += 2;
-          n_c16 = lds16(ringbase + (v & P.ring_mask));
-        }
+        uint32_t nxt = last ? cur : cur + (SMEM_TABLES ? 4u : 1u);
+        nxt = more ? first_of_next : nxt;
+        v = more ? v + 2 : v;
+        n_c16 = lds16(ringbase + (v & P.ring_mask));
         cur = nxt;
         const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
         // ---- this step's pick
         kmax = max(kmax, rec);
         if (!DEPOT0) kmin = min(kmin, rec);
-        const uint32_t aaddr = abase + ((rec >> 26) << 7);
-        sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 21));
-        const uint32_t caddr = cbase + ((rec & 0xe0u) << 2);
+        const uint32_t aaddr = abase | ((rec >> 20) & amask);
+        sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 22));
+        const uint32_t caddr = cbase | (rec & 0x380u);
         sts32(caddr, lds32(caddr) | one_shl_wrap(rec));
         rec = rec_next;
       }
@@ -392,8 +394,8 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         sts32(abase + w * 128, 0u);
       }
       if (live) {
-        const uint32_t a_max = WHP_PICK_AISLE(kmax);
-        const uint32_t slot1 = (kmax >> WHP_PICK_SLOT_SHIFT) & WHP_PICK_SLOT_MASK;
+        const uint32_t a_max = WHP_FAST_AISLE(kmax);
+        const uint32_t slot1 = WHP_FAST_SLOT1(kmax);
         if (DEPOT0 && P.fits32) {
           const uint32_t d2 = 2u * slot1 * (uint32_t)T.g.slot_pitch;
           D += (uint32_t)P2 * a_max + (uint32_t)m * (uint32_t)A + ((m & 1) ? d2 - (uint32_t)A : 0u);
@@ -403,7 +405,7 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
           if (DEPOT0) {
             H = P2 * (int64_t)a_max;
           } else {
-            const int64_t a_min = WHP_PICK_AISLE(kmin), a0 = T.g.depot_aisle;
+            const int64_t a_min = WHP_FAST_AISLE(kmin), a0 = T.g.depot_aisle;
             H = (int64_t)T.g.aisle_spacing *
                 (llabs(a0 - a_min) + ((int64_t)a_max - a_min) + llabs((int64_t)a_max - a0));
           }
@@ -554,8 +556,12 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   const int ring_bytes = ((c->C + 14) / 8 + 1 <= 8) ? 128 : 256;
   // K2 shape
   const size_t table_bytes = 4 * (((size_t)c->n_items_pad + 31) & ~(size_t)31);
-  const size_t priv_per_warp = (size_t)(KW + aw_words) * 128 + 32 * (size_t)(ring_bytes + 16);
-  const size_t smem_max = (size_t)c->smem_optin - 1024;
+  int awp = 1, kwp = 1;
+  while (awp < aw_words) awp <<= 1;
+  while (kwp < KW) kwp <<= 1;
+  if (awp < kwp) awp = kwp;
+  const size_t priv_per_warp = (size_t)(kwp + awp) * 128 + 32 * (size_t)(ring_bytes + 16);
+  const size_t smem_max = (size_t)c->smem_optin - 1024 - (size_t)awp * 128;  // alignment slack
   const bool smem_tables = table_bytes + 4 * priv_per_warp <= smem_max;
   const size_t avail = smem_max - (smem_tables ? table_bytes : 0);
   // segments: few enough batches per segment for the counter planes, and >= 4 tasks per warp
@@ -619,18 +625,18 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   {
     sets_params P;
     P.S = S; P.log2S = log2S;
-    P.aw_words = aw_words; P.ring_mask = ring_bytes - 1;
+    P.aw_words = aw_words; P.awp = awp; P.kwp = kwp; P.ring_mask = ring_bytes - 1;
     P.bm_pitch = bm_pitch; P.cs_pitch = cs_pitch; P.ss_pitch = ss_pitch;
     P.n_items_pad = c->n_items_pad; P.fits32 = fits32;
     P.n_tasks = (n_cand * S + 31) / 32;
     int64_t blocks = (P.n_tasks + warps - 1) / warps;
     if (blocks > c->num_sms) blocks = c->num_sms;
-    const size_t smem = (smem_tables ? table_bytes : 0) + priv_per_warp * warps;
+    const size_t smem = (smem_tables ? table_bytes : 0) + priv_per_warp * warps + (size_t)awp * 128;
     const bool depot0 = c->g.depot_aisle == 0;
 #define WHP_LAUNCH_SETS_PL(ST, D0, KWV, PLV)                                                     \
   do {                                                                                           \
     cudaFuncSetAttribute(whp_sets_kernel<ST, D0, KWV, PLV>,                                      \
-                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);            \
+                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(c->smem_optin - 1024)); \
     whp_sets_kernel<ST, D0, KWV, PLV><<<(unsigned)blocks, warps * 32, smem, st>>>(               \
         T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand,          \
         c->d_dist_scratch, c->d_planes, out.batch_hash, c->d_task);                              \

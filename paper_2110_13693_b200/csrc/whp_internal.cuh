@@ -25,6 +25,17 @@
 #define WHP_PICK_LOC_SHIFT 8 /* rec >> 8 identifies the location (aisle, slot, side) */
 #define WHP_PICK_CLASS_MASK 0xffu
 
+// pick record of the tuned candidate path (whp_fast.cu), built from the record above:
+//   aisle[31:22] | slot1[21:10] | class>>5 [9:7] | 0 [6] | last-pick-of-its-order [5] | class&31 [4:0]
+//   (rec >> 20) & (words-1)<<7 and rec & 0x380 are the byte offsets of the 32-aisle and the
+//   32-class occupancy words of a lane; (rec >> 22) mod 32 and rec mod 32 the bits inside them.
+#define WHP_FAST_LAST 0x20u
+#define WHP_FAST_PACK(rec, last)                                                              \
+  ((WHP_PICK_AISLE(rec) << 22) | ((((rec) >> WHP_PICK_SLOT_SHIFT) & WHP_PICK_SLOT_MASK) << 10) | \
+   ((((rec) & WHP_PICK_CLASS_MASK) >> 5) << 7) | ((last) ? WHP_FAST_LAST : 0u) | ((rec) & 31u))
+#define WHP_FAST_AISLE(rec) ((rec) >> 22)
+#define WHP_FAST_SLOT1(rec) (((rec) >> 10) & 0xfffu)
+
 #define WHP_MAX_AISLES 1024
 #define WHP_MAX_SLOTS 4095
 #define WHP_MAX_CLASSES 256
