@@ -51,8 +51,13 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
 }
 
 // ------------------------------------------------------------------------------------------ K1
-constexpr int kBoundsThreads = 64;   // candidates per block, one per thread
-constexpr int kChunkBytes = 256;     // bytes of a permutation row per bulk copy (64 positions)
+// Next-fit batching (D2) is a sequential recurrence along the plan: one thread per plan. The
+// rows arrive through per-thread TMA bulk copies (an mbarrier per warp and stage); the loop is
+// software-pipelined by hand — while the recurrence runs over the 32 positions of word w, the
+// order ids of word w+1 leave the staging buffer and their order records are gathered from
+// the table in shared memory — so that a lone warp per scheduler still issues every cycle.
+constexpr int kBoundsThreads = 32;   // plans per block, one per thread
+constexpr int kChunkBytes = 256;     // bytes of a plan row per bulk copy (64 positions)
 constexpr int kChunkStride = kChunkBytes + 16;  // per-thread buffer stride: 128-bit reads of a
                                                 // quarter warp fall into distinct banks
 constexpr int kStages = 3;
@@ -80,65 +85,69 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
-// 4 x n4 positions of one row: order ids from the staged chunk, their records from the order
-// table in shared memory, the next-fit recurrence on room = C - load with one dependent
-// instruction per position:  room' = umin(room - q, C - q)  (room < q wraps room - q above
-// C - q: a new batch opens). Returns the batch-start bits; writes the 16-bit cursors.
-template <int N4>
-__device__ __forceinline__ uint32_t bounds_word(uint32_t buf, uint32_t sorec0, uint32_t C,
-                                                uint32_t& room, uint4* __restrict__ cs_out,
-                                                int n4_runtime, bool write) {
-  uint32_t bits = 0;
-  uint32_t cw[4];
+// order records of the positions of a word (ids from the staged chunk, records from the order
+// table in shared memory). FULL: all 32 positions, straight-line code; otherwise only the first
+// n4 groups of four exist and the others get record 0 (q = 0: no effect on the recurrence).
+template <bool FULL>
+__device__ __forceinline__ void gather_word(uint32_t (&r)[32], uint32_t buf, uint32_t sorec0, int n4) {
 #pragma unroll
-  for (int g = 0; g < N4; ++g) {
-    if (N4 == 8 || g < n4_runtime) {
+  for (int g = 0; g < 8; ++g) {
+    if (FULL || g < n4) {
       const int4 v = lds128(buf + 16 * g);
-      const uint32_t r0 = lds32(sorec0 + 4 * v.x), r1 = lds32(sorec0 + 4 * v.y);
-      const uint32_t r2 = lds32(sorec0 + 4 * v.z), r3 = lds32(sorec0 + 4 * v.w);
-      // cursor stream: 4 x u16 = bits 8..23 of the order records
-      cw[(2 * g) & 3] = __byte_perm(r0, r1, 0x6521);
-      cw[(2 * g + 1) & 3] = __byte_perm(r2, r3, 0x6521);
-      const uint32_t rr[4] = {r0, r1, r2, r3};
-#pragma unroll
-      for (int t = 0; t < 4; ++t) {
-        const uint32_t q = rr[t] & WHP_Q_MASK;
-        if (room < q) bits |= 1u << (4 * g + t);
-        room = min(room - q, C - q);
-      }
-      if ((g & 1) && write) cs_out[g >> 1] = make_uint4(cw[0], cw[1], cw[2], cw[3]);
+      r[4 * g + 0] = lds32(sorec0 + 4 * v.x); r[4 * g + 1] = lds32(sorec0 + 4 * v.y);
+      r[4 * g + 2] = lds32(sorec0 + 4 * v.z); r[4 * g + 3] = lds32(sorec0 + 4 * v.w);
+    } else {
+      r[4 * g + 0] = 0u; r[4 * g + 1] = 0u; r[4 * g + 2] = 0u; r[4 * g + 3] = 0u;
     }
   }
-  if (N4 != 8 && (n4_runtime & 1) && write) {  // odd tail: the last 4 cursors, upper half unused
-    const int g = n4_runtime - 1;
-    cs_out[g >> 1] = make_uint4(cw[(2 * g) & 3], cw[(2 * g + 1) & 3], 0u, 0u);
+}
+
+// The next-fit recurrence over one word, on room = C - load:  d = room - q;  room' =
+// umin(d, C - q)  (room < q wraps d above C - q: a new batch opens, and d's sign bit says so —
+// a funnel shift collects the 32 sign bits, first position last). Writes the 16-bit cursors
+// (bits 8..23 of the order records) of the first n4 groups of four positions.
+template <bool FULL>
+__device__ __forceinline__ uint32_t recur_word(const uint32_t (&r)[32], uint32_t C, uint32_t& room,
+                                               uint4* __restrict__ cs_out, int n4, bool write) {
+  uint32_t rev = 0;
+#pragma unroll
+  for (int i = 0; i < 32; ++i) {
+    const uint32_t q = r[i] & WHP_Q_MASK;
+    const uint32_t d = room - q;
+    rev = __funnelshift_l(d, rev, 1);  // (rev << 1) | (d >> 31)
+    room = min(d, C - q);
   }
-  return bits;
+  if (write) {
+#pragma unroll
+    for (int g2 = 0; g2 < 4; ++g2)
+      if (FULL || 2 * g2 < n4)
+        cs_out[g2] = make_uint4(__byte_perm(r[8 * g2 + 0], r[8 * g2 + 1], 0x6521),
+                                __byte_perm(r[8 * g2 + 2], r[8 * g2 + 3], 0x6521),
+                                __byte_perm(r[8 * g2 + 4], r[8 * g2 + 5], 0x6521),
+                                __byte_perm(r[8 * g2 + 6], r[8 * g2 + 7], 0x6521));
+  }
+  return __brev(rev);
 }
 
 __global__ void __launch_bounds__(kBoundsThreads)
 whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int32_t C,
                   const int32_t* __restrict__ perms, int64_t n_cand,
                   uint32_t* __restrict__ bmask, int32_t bm_pitch, uint16_t* __restrict__ cstream,
-                  int32_t cs_pitch, int32_t* __restrict__ nb_scratch,
-                  int32_t* __restrict__ n_batches_out, int32_t* __restrict__ segstart,
-                  int32_t ss_pitch, int32_t S, int32_t log2S) {
+                  int32_t cs_pitch) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  // [chunk buffers: kStages x 64 threads x kChunkStride][order table][stash of the boundary
-  //  words: nw x 64][mbarriers: kStages x 2 warps]
+  // [chunk buffers: kStages x 32 threads x kChunkStride][order table][mbarriers: kStages]
   const int nw = (n_orders + 31) >> 5;
-  const int tid = threadIdx.x, warp = tid >> 5;
+  const int tid = threadIdx.x;
   uint8_t* sp = smem_raw + kStages * kBoundsThreads * kChunkStride;
   uint32_t* sorec = reinterpret_cast<uint32_t*>(sp);
   sp += 4 * (size_t)((n_orders + 3) & ~3);
-  uint32_t* stash = reinterpret_cast<uint32_t*>(sp);
-  sp += 4 * (size_t)nw * kBoundsThreads;
   const uint32_t bars = smem_u32(sp);
   const uint32_t buf0 = smem_u32(smem_raw) + tid * kChunkStride;
+  constexpr uint32_t kStageBytes = kBoundsThreads * kChunkStride;
   const uint32_t sorec0 = smem_u32(sorec);
   for (int i = tid; i < n_orders; i += kBoundsThreads) sorec[i] = __ldg(order_fast + i);
-  if ((tid & 31) == 0)
-    for (int s = 0; s < kStages; ++s) mbar_init(bars + 8 * (s * 2 + warp), 32);
+  if (tid == 0)
+    for (int s = 0; s < kStages; ++s) mbar_init(bars + 8 * s, kBoundsThreads);
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();
   const int64_t c_raw = (int64_t)blockIdx.x * kBoundsThreads + tid;
@@ -149,64 +158,116 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
   const int nchunks = (row_bytes + kChunkBytes - 1) / kChunkBytes;
   for (int k = 0; k < kStages && k < nchunks; ++k) {
     const uint32_t bytes = (uint32_t)min(kChunkBytes, row_bytes - k * kChunkBytes);
-    const uint32_t bar = bars + 8 * (k * 2 + warp);
-    mbar_expect_tx(bar, bytes);
-    bulk_g2s(buf0 + k * (kBoundsThreads * kChunkStride), row + (size_t)k * kChunkBytes, bytes, bar);
+    mbar_expect_tx(bars + 8 * k, bytes);
+    bulk_g2s(buf0 + k * kStageBytes, row + (size_t)k * kChunkBytes, bytes, bars + 8 * k);
   }
   uint32_t* __restrict__ bm = bmask + c * bm_pitch;
   uint4* __restrict__ cs = reinterpret_cast<uint4*>(cstream + c * cs_pitch);
   uint32_t room = (uint32_t)C;
-  uint32_t nb = 0;
+  // chunk k = words 2k, 2k+1 lives in stage k mod kStages, phase parity (k / kStages) & 1
   int stage = 0;
   uint32_t parity = 0;
+  uint32_t ra[32], rb[32];
+  mbar_wait(bars, 0);
+  const int n_full = n_orders >> 5;            // words with all 32 positions
+  const int KF = n_full > 0 ? (n_full - 1) >> 1 : 0;  // chunks whose two words and successor are full
+  if (n_full > 0) gather_word<true>(ra, buf0, sorec0, 8);
 #pragma unroll 1
-  for (int k = 0; k < nchunks; ++k) {
-    const uint32_t bar = bars + 8 * (stage * 2 + warp);
-    const uint32_t buf = buf0 + stage * (kBoundsThreads * kChunkStride);
-    mbar_wait(bar, parity);
-    const int npos = min(kChunkBytes / 4, n_orders - k * (kChunkBytes / 4));
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      const int w = 2 * k + h;
-      const int left = npos - 32 * h;
-      if (left > 0) {
-        uint32_t bits;
-        if (left >= 32) bits = bounds_word<8>(buf + 128 * h, sorec0, (uint32_t)C, room, cs + 4 * w, 8, have);
-        else bits = bounds_word<7>(buf + 128 * h, sorec0, (uint32_t)C, room, cs + 4 * w, left >> 2, have);
-        if (w == 0) bits |= 1u;  // batch 0 starts at position 0
-        nb += __popc(bits);
-        stash[w * kBoundsThreads + tid] = bits;
-        if (w == (n_orders >> 5)) bits |= 1u << (n_orders & 31);  // end sentinel, partial word
-        if (have) bm[w] = bits;
-      }
-    }
-    if (k + kStages < nchunks) {  // refill this stage (its values have been consumed above)
+  for (int k = 0; k < KF; ++k) {
+    const uint32_t buf = buf0 + stage * kStageBytes;
+    const uint32_t bar = bars + 8 * stage;
+    // word 2k runs its recurrence while word 2k+1 is gathered
+    gather_word<true>(rb, buf + 128, sorec0, 8);
+    uint32_t bits = recur_word<true>(ra, (uint32_t)C, room, cs + 8 * k, 8, have);
+    if (k == 0) bits |= 1u;  // batch 0 starts at position 0
+    if (have) bm[2 * k] = bits;
+    if (++stage == kStages) { stage = 0; parity ^= 1u; }
+    mbar_wait(bars + 8 * stage, parity);
+    // word 2k+1 runs its recurrence while word 2k+2 (first of the next chunk) is gathered
+    gather_word<true>(ra, buf0 + stage * kStageBytes, sorec0, 8);
+    bits = recur_word<true>(rb, (uint32_t)C, room, cs + 8 * k + 4, 8, have);
+    if (have) bm[2 * k + 1] = bits;
+    if (k + kStages < nchunks) {  // chunk k is consumed: refill its stage
       const int kn = k + kStages;
       const uint32_t bytes = (uint32_t)min(kChunkBytes, row_bytes - kn * kChunkBytes);
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       mbar_expect_tx(bar, bytes);
       bulk_g2s(buf, row + (size_t)kn * kChunkBytes, bytes, bar);
     }
-    if (++stage == kStages) { stage = 0; parity ^= 1u; }
   }
-  if (!have) return;
-  if ((n_orders & 31) == 0) bm[nw] = 1u;  // end sentinel in a word of its own
-  nb_scratch[c] = (int32_t)nb;
-  if (n_batches_out) n_batches_out[c] = (int32_t)nb;
-  // first position of every segment: segment s starts with batch floor(s * nb / S)
-  int32_t* __restrict__ ss = segstart + c * ss_pitch;
-  int seg = 0, target = 0, acc = 0;
-  for (int w = 0; w < nw && seg < S; ++w) {
-    const uint32_t bits = stash[w * kBoundsThreads + tid];
-    const int pc = __popc(bits);
-    while (seg < S && target < acc + pc) {
-      uint32_t t = bits;
-      for (int r = target - acc; r > 0; --r) t &= t - 1;
-      ss[seg] = 32 * w + __ffs(t) - 1;
-      ++seg;
-      target = (int)(((int64_t)seg * nb) >> log2S);
+  // the last (at most three) words, the final one possibly partial; word 2*KF is in ra if full
+#pragma unroll 1
+  for (int w = 2 * KF; w < nw; ++w) {
+    const int left = n_orders - 32 * w;
+    const int n4 = min(8, left >> 2);
+    if (w > 2 * KF || n_full == 0) {
+      if (w > 0 && (w & 1) == 0) {
+        if (++stage == kStages) { stage = 0; parity ^= 1u; }
+        mbar_wait(bars + 8 * stage, parity);
+      }
+      gather_word<false>(ra, buf0 + stage * kStageBytes + 128 * (w & 1), sorec0, n4);
     }
-    acc += pc;
+    uint32_t bits = recur_word<false>(ra, (uint32_t)C, room, cs + 4 * w, n4, have);
+    if (w == 0) bits |= 1u;
+    if (left < 32) bits |= 1u << left;    // end sentinel in a partial last word
+    if (have) bm[w] = bits;
+  }
+  if (have && (n_orders & 31) == 0) bm[nw] = 1u;  // end sentinel in a word of its own
+}
+
+// One warp per plan: number of batches, and the first position of every segment (segment s
+// starts with batch floor(s * nb / S)).
+__global__ void __launch_bounds__(256)
+whp_segments_kernel(const uint32_t* __restrict__ bmask, int32_t bm_pitch, int32_t n_orders,
+                    int64_t n_cand, int32_t S, int32_t log2S, int32_t* __restrict__ nb_scratch,
+                    int32_t* __restrict__ n_batches_out, int32_t* __restrict__ segstart,
+                    int32_t ss_pitch) {
+  const int lane = threadIdx.x & 31;
+  const int64_t c = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (c >= n_cand) return;
+  const int nw = (n_orders + 31) >> 5;
+  const uint32_t* __restrict__ bm = bmask + c * bm_pitch;
+  auto word_at = [&](int w) -> uint32_t {
+    if (w >= nw) return 0u;
+    uint32_t x = __ldg(bm + w);
+    if (w == (n_orders >> 5)) x &= (1u << (n_orders & 31)) - 1u;  // drop the end sentinel
+    return x;
+  };
+  int nb = 0;
+  for (int w0 = 0; w0 < nw; w0 += 32) nb += __reduce_add_sync(WHP_FULL, __popc(word_at(w0 + lane)));
+  if (lane == 0) {
+    nb_scratch[c] = nb;
+    if (n_batches_out) n_batches_out[c] = nb;
+  }
+  const int target = (int)(((int64_t)lane * nb) >> log2S);  // lane = segment
+  int base = 0, found = 0;
+  for (int w0 = 0; w0 < nw; w0 += 32) {
+    const uint32_t x = word_at(w0 + lane);
+    const int pc = __popc(x);
+    int incl = pc;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const int y = __shfl_up_sync(WHP_FULL, incl, d);
+      if (lane >= d) incl += y;
+    }
+    const int total = __shfl_sync(WHP_FULL, incl, 31);
+    // smallest j with base + incl_j > target
+    int lo = 0, hi = 31;
+#pragma unroll
+    for (int it = 0; it < 5; ++it) {
+      const int mid = (lo + hi) >> 1;
+      const int im = __shfl_sync(WHP_FULL, incl, mid);
+      if (base + im > target) hi = mid; else lo = mid + 1;
+    }
+    const uint32_t xj = __shfl_sync(WHP_FULL, x, lo);
+    const int ej = __shfl_sync(WHP_FULL, incl - pc, lo);
+    if (!found && lane < S && target >= base && target < base + total) {
+      uint32_t t = xj;
+      for (int r = target - base - ej; r > 0; --r) t &= t - 1;
+      segstart[c * ss_pitch + lane] = 32 * (w0 + lo) + __ffs(t) - 1;
+      found = 1;
+    }
+    base += total;
   }
 }
 
@@ -228,6 +289,12 @@ struct sets_params {
 
 __device__ __forceinline__ uint32_t lds16(uint32_t a) {
   uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v;
+}
+
+// if (p) v = ld.shared.u16 [a] — predicated, never a branch; idle lanes cost no bank cycle
+__device__ __forceinline__ void lds16_if(uint32_t& v, uint32_t a, bool p) {
+  asm volatile("{ .reg .pred pq; setp.ne.u32 pq, %2, 0; @pq ld.shared.u16 %0, [%1]; }"
+               : "+r"(v) : "r"(a), "r"((uint32_t)p));
 }
 
 template <bool SMEM_TABLES, bool DEPOT0, int KW, int kPlanes>
@@ -356,14 +423,14 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
 #pragma unroll 2
       for (int t = 0; t < Cmax; ++t) {
         // cursor of the next step's pick: next record, the next order's first pick, or stay —
-        // all by selects; the look-ahead cursor is (re)loaded every step
+        // all by selects and one predicated load
         const uint32_t first_of_next = SMEM_TABLES ? pb + 8 * n_c16 : 2 * n_c16;
         const bool last = (int32_t)(rec << 26) < 0;  // WHP_FAST_LAST (bit 5) into the sign bit
         const bool more = last && (v != v_end);
         uint32_t nxt = last ? cur : cur + (SMEM_TABLES ? 4u : 1u);
         nxt = more ? first_of_next : nxt;
         v = more ? v + 2 : v;
-        n_c16 = lds16(ringbase + (v & P.ring_mask));
+        lds16_if(n_c16, ringbase + (v & P.ring_mask), more);  // the look-ahead cursor
         cur = nxt;
         const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
         // ---- this step's pick
@@ -528,9 +595,8 @@ static int64_t nb_upper_bound(const whp_ctx* c) {
 }
 
 static size_t bounds_smem_bytes(const whp_ctx* c) {
-  const size_t nw = ((size_t)c->n_orders + 31) >> 5;
   return (size_t)kStages * kBoundsThreads * kChunkStride + 4 * (((size_t)c->n_orders + 3) & ~(size_t)3) +
-         4 * nw * kBoundsThreads + 8 * kStages * 2;
+         8 * kStages;
 }
 
 bool whp_fast_eligible(const whp_ctx* c) {
@@ -538,7 +604,7 @@ bool whp_fast_eligible(const whp_ctx* c) {
   if (c->n_orders % 4 != 0 || c->n_orders >= 65536) return false;
   if ((nb_upper_bound(c) + 31) / 32 > 255) return false;      // 8 counter planes, S <= 32
   if (c->C > 64) return false;                                // per-lane cursor ring of 16 chunks
-  if (bounds_smem_bytes(c) > (size_t)c->smem_optin - 1024) return false;  // K1 tables in smem
+  if (bounds_smem_bytes(c) > (size_t)c->smem_optin - 1024) return false;  // K1: order table in smem
   return true;
 }
 
@@ -613,11 +679,17 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
     cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     const size_t smem = bounds_smem_bytes(c);
-    cudaFuncSetAttribute(whp_bounds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+    cudaFuncSetAttribute(whp_bounds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         c->smem_optin - 1024);
     const unsigned blocks = (unsigned)((n_cand + kBoundsThreads - 1) / kBoundsThreads);
     whp_bounds_kernel<<<blocks, kBoundsThreads, smem, st>>>(
         c->d_order_fast, c->n_orders, c->C, d_perms, n_cand, c->d_bmask, bm_pitch, c->d_cstream,
-        cs_pitch, c->d_nb, out.n_batches, c->d_segstart, ss_pitch, S, log2S);
+        cs_pitch);
+    c->launches += 1;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    whp_segments_kernel<<<(unsigned)((n_cand * 32 + 255) / 256), 256, 0, st>>>(
+        c->d_bmask, bm_pitch, c->n_orders, n_cand, S, log2S, c->d_nb, out.n_batches,
+        c->d_segstart, ss_pitch);
     c->launches += 1;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
   }
