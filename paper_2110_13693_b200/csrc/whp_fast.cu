@@ -57,10 +57,10 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
 // order ids of word w+1 leave the staging buffer and their order records are gathered from
 // the table in shared memory — so that a lone warp per scheduler still issues every cycle.
 constexpr int kBoundsThreads = 32;   // plans per block, one per thread
-constexpr int kChunkBytes = 256;     // bytes of a plan row per bulk copy (64 positions)
+constexpr int kChunkBytes = 512;     // bytes of a plan row per bulk copy (128 positions)
 constexpr int kChunkStride = kChunkBytes + 16;  // per-thread buffer stride: 128-bit reads of a
                                                 // quarter warp fall into distinct banks
-constexpr int kStages = 3;
+constexpr int kStages = 2;
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
@@ -135,7 +135,7 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
                   uint32_t* __restrict__ bmask, int32_t bm_pitch, uint16_t* __restrict__ cstream,
                   int32_t cs_pitch) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  // [chunk buffers: kStages x 32 threads x kChunkStride][order table][mbarriers: kStages]
+  // [chunk buffers: kStages x 32 threads x kChunkStride][order table][mbarriers: kStages + 1]
   const int nw = (n_orders + 31) >> 5;
   const int tid = threadIdx.x;
   uint8_t* sp = smem_raw + kStages * kBoundsThreads * kChunkStride;
@@ -145,11 +145,18 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
   const uint32_t buf0 = smem_u32(smem_raw) + tid * kChunkStride;
   constexpr uint32_t kStageBytes = kBoundsThreads * kChunkStride;
   const uint32_t sorec0 = smem_u32(sorec);
-  for (int i = tid; i < n_orders; i += kBoundsThreads) sorec[i] = __ldg(order_fast + i);
-  if (tid == 0)
-    for (int s = 0; s < kStages; ++s) mbar_init(bars + 8 * s, kBoundsThreads);
+  constexpr int kWarps = kBoundsThreads / 32;
+  if (tid == 0) {
+    for (int s = 0; s < kStages * kWarps; ++s) mbar_init(bars + 8 * s, 32);
+    mbar_init(bars + 8 * kStages * kWarps, 1);
+  }
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();
+  if (tid == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
+    mbar_expect_tx(bars + 8 * kStages * kWarps, 4u * (uint32_t)n_orders);
+    bulk_g2s(sorec0, order_fast, 4u * (uint32_t)n_orders, bars + 8 * kStages * kWarps);
+  }
+  const uint32_t wbars = bars + 8 * kStages * (tid >> 5);  // this warp's stage barriers
   const int64_t c_raw = (int64_t)blockIdx.x * kBoundsThreads + tid;
   const bool have = c_raw < n_cand;
   const int64_t c = have ? c_raw : n_cand - 1;  // idle threads shadow the last plan, no writes
@@ -158,35 +165,43 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
   const int nchunks = (row_bytes + kChunkBytes - 1) / kChunkBytes;
   for (int k = 0; k < kStages && k < nchunks; ++k) {
     const uint32_t bytes = (uint32_t)min(kChunkBytes, row_bytes - k * kChunkBytes);
-    mbar_expect_tx(bars + 8 * k, bytes);
-    bulk_g2s(buf0 + k * kStageBytes, row + (size_t)k * kChunkBytes, bytes, bars + 8 * k);
+    mbar_expect_tx(wbars + 8 * k, bytes);
+    bulk_g2s(buf0 + k * kStageBytes, row + (size_t)k * kChunkBytes, bytes, wbars + 8 * k);
   }
   uint32_t* __restrict__ bm = bmask + c * bm_pitch;
   uint4* __restrict__ cs = reinterpret_cast<uint4*>(cstream + c * cs_pitch);
   uint32_t room = (uint32_t)C;
-  // chunk k = words 2k, 2k+1 lives in stage k mod kStages, phase parity (k / kStages) & 1
+  // chunk k lives in stage k mod kStages, phase parity (k / kStages) & 1
   int stage = 0;
   uint32_t parity = 0;
   uint32_t ra[32], rb[32];
-  mbar_wait(bars, 0);
+  mbar_wait(bars + 8 * kStages * kWarps, 0);
+  mbar_wait(wbars, 0);
+  constexpr int WPC = kChunkBytes / 128;       // words per chunk (even)
   const int n_full = n_orders >> 5;            // words with all 32 positions
-  const int KF = n_full > 0 ? (n_full - 1) >> 1 : 0;  // chunks whose two words and successor are full
+  // chunks whose words and whose successor's first word are all full: the straight-line path
+  const int KF = n_full > 0 ? (n_full - 1) / WPC : 0;
   if (n_full > 0) gather_word<true>(ra, buf0, sorec0, 8);
 #pragma unroll 1
   for (int k = 0; k < KF; ++k) {
     const uint32_t buf = buf0 + stage * kStageBytes;
-    const uint32_t bar = bars + 8 * stage;
-    // word 2k runs its recurrence while word 2k+1 is gathered
-    gather_word<true>(rb, buf + 128, sorec0, 8);
-    uint32_t bits = recur_word<true>(ra, (uint32_t)C, room, cs + 8 * k, 8, have);
-    if (k == 0) bits |= 1u;  // batch 0 starts at position 0
-    if (have) bm[2 * k] = bits;
-    if (++stage == kStages) { stage = 0; parity ^= 1u; }
-    mbar_wait(bars + 8 * stage, parity);
-    // word 2k+1 runs its recurrence while word 2k+2 (first of the next chunk) is gathered
-    gather_word<true>(ra, buf0 + stage * kStageBytes, sorec0, 8);
-    bits = recur_word<true>(rb, (uint32_t)C, room, cs + 8 * k + 4, 8, have);
-    if (have) bm[2 * k + 1] = bits;
+    const uint32_t bar = wbars + 8 * stage;
+#pragma unroll
+    for (int j = 0; j < WPC; ++j) {
+      // word k*WPC+j runs its recurrence while the next word is gathered
+      uint32_t (&cur)[32] = (j & 1) ? rb : ra;
+      uint32_t (&nxt)[32] = (j & 1) ? ra : rb;
+      if (j == WPC - 1) {  // the next word opens the next chunk
+        if (++stage == kStages) { stage = 0; parity ^= 1u; }
+        mbar_wait(wbars + 8 * stage, parity);
+        gather_word<true>(nxt, buf0 + stage * kStageBytes, sorec0, 8);
+      } else {
+        gather_word<true>(nxt, buf + 128 * (j + 1), sorec0, 8);
+      }
+      uint32_t bits = recur_word<true>(cur, (uint32_t)C, room, cs + 4 * (k * WPC + j), 8, have);
+      if (k == 0 && j == 0) bits |= 1u;  // batch 0 starts at position 0
+      if (have) bm[k * WPC + j] = bits;
+    }
     if (k + kStages < nchunks) {  // chunk k is consumed: refill its stage
       const int kn = k + kStages;
       const uint32_t bytes = (uint32_t)min(kChunkBytes, row_bytes - kn * kChunkBytes);
@@ -195,17 +210,18 @@ whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int
       bulk_g2s(buf, row + (size_t)kn * kChunkBytes, bytes, bar);
     }
   }
-  // the last (at most three) words, the final one possibly partial; word 2*KF is in ra if full
+  // the last (at most WPC + 1) words, the final one possibly partial; word KF*WPC is in ra
+  // if it is full
 #pragma unroll 1
-  for (int w = 2 * KF; w < nw; ++w) {
+  for (int w = KF * WPC; w < nw; ++w) {
     const int left = n_orders - 32 * w;
     const int n4 = min(8, left >> 2);
-    if (w > 2 * KF || n_full == 0) {
-      if (w > 0 && (w & 1) == 0) {
+    if (w > KF * WPC || n_full == 0) {
+      if (w > 0 && (w % WPC) == 0) {
         if (++stage == kStages) { stage = 0; parity ^= 1u; }
-        mbar_wait(bars + 8 * stage, parity);
+        mbar_wait(wbars + 8 * stage, parity);
       }
-      gather_word<false>(ra, buf0 + stage * kStageBytes + 128 * (w & 1), sorec0, n4);
+      gather_word<false>(ra, buf0 + stage * kStageBytes + 128 * (w % WPC), sorec0, n4);
     }
     uint32_t bits = recur_word<false>(ra, (uint32_t)C, room, cs + 4 * w, n4, have);
     if (w == 0) bits |= 1u;
@@ -596,7 +612,7 @@ static int64_t nb_upper_bound(const whp_ctx* c) {
 
 static size_t bounds_smem_bytes(const whp_ctx* c) {
   return (size_t)kStages * kBoundsThreads * kChunkStride + 4 * (((size_t)c->n_orders + 3) & ~(size_t)3) +
-         8 * kStages;
+         8 * (kStages * (kBoundsThreads / 32) + 1);
 }
 
 bool whp_fast_eligible(const whp_ctx* c) {
