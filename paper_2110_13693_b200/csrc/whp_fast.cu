@@ -18,6 +18,9 @@
 //                          bit-sliced ("vertical") counters held in registers (D5).
 //   K3 whp_finish_kernel   one warp per candidate: decodes the vertical counters into r_k,
 //                          canonical fp64 penalty (D6), J, outputs.
+#include <cuda.h>
+#include <cudaTypedefs.h>
+
 #include <cstdlib>
 
 #include "whp_walk.cuh"
@@ -51,16 +54,17 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
 }
 
 // ------------------------------------------------------------------------------------------ K1
-// Next-fit batching (D2) is a sequential recurrence along the plan: one thread per plan. The
-// rows arrive through per-thread TMA bulk copies (an mbarrier per warp and stage); the loop is
-// software-pipelined by hand — while the recurrence runs over the 32 positions of word w, the
-// order ids of word w+1 leave the staging buffer and their order records are gathered from
-// the table in shared memory — so that a lone warp per scheduler still issues every cycle.
+// Next-fit batching (D2) is a sequential recurrence along the plan: one thread per plan, one
+// warp per block. The plans of a warp are 32 consecutive rows of the permutation matrix, so one
+// 2-D TMA tile load (tensor map over perms, box = 32 rows x 32 positions, 128-byte swizzle)
+// brings one 32-position word of all 32 plans with a single instruction; 8 tiles are in flight
+// per warp (an mbarrier per stage). The swizzle makes the lane-per-row 128-bit reads
+// conflict-free. The loop is software-pipelined by hand — while the recurrence runs over word w,
+// the order ids of word w+1 leave the tile and their order records are gathered from the table
+// in shared memory — so that a lone warp per scheduler keeps issuing.
 constexpr int kBoundsThreads = 32;   // plans per block, one per thread
-constexpr int kChunkBytes = 512;     // bytes of a plan row per bulk copy (128 positions)
-constexpr int kChunkStride = kChunkBytes + 16;  // per-thread buffer stride: 128-bit reads of a
-                                                // quarter warp fall into distinct banks
-constexpr int kStages = 2;
+constexpr int kStages = 4;           // tiles (words) in flight, power of two
+constexpr int kTileBytes = 32 * 128; // 32 rows x 32 positions x 4 B
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
@@ -84,16 +88,31 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// TMA 2-D tile store shared -> global (bulk async-group completion)
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* tm, int32_t x, int32_t y, uint32_t src) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+               ::"l"(tm), "r"(x), "r"(y), "r"(src) : "memory");
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+// TMA 2-D tile load: box at (x = first position, y = first plan) of the tensor map
+__device__ __forceinline__ void tma_tile_2d(uint32_t dst, const CUtensorMap* tm, int32_t x, int32_t y,
+                                            uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+      ::"r"(dst), "l"(tm), "r"(x), "r"(y), "r"(bar) : "memory");
+}
 
 // order records of the positions of a word (ids from the staged chunk, records from the order
 // table in shared memory). FULL: all 32 positions, straight-line code; otherwise only the first
 // n4 groups of four exist and the others get record 0 (q = 0: no effect on the recurrence).
 template <bool FULL>
-__device__ __forceinline__ void gather_word(uint32_t (&r)[32], uint32_t buf, uint32_t sorec0, int n4) {
+__device__ __forceinline__ void gather_word(uint32_t (&r)[32], uint32_t row, uint32_t swz,
+                                            uint32_t sorec0, int n4) {
+  // row = address of this lane's 128-byte row of the tile; 16-byte chunk g lives at g ^ (lane & 7)
 #pragma unroll
   for (int g = 0; g < 8; ++g) {
     if (FULL || g < n4) {
-      const int4 v = lds128(buf + 16 * g);
+      const int4 v = lds128(row + ((16 * g) ^ swz));
       r[4 * g + 0] = lds32(sorec0 + 4 * v.x); r[4 * g + 1] = lds32(sorec0 + 4 * v.y);
       r[4 * g + 2] = lds32(sorec0 + 4 * v.z); r[4 * g + 3] = lds32(sorec0 + 4 * v.w);
     } else {
@@ -102,133 +121,141 @@ __device__ __forceinline__ void gather_word(uint32_t (&r)[32], uint32_t buf, uin
   }
 }
 
-// The next-fit recurrence over one word, on room = C - load:  d = room - q;  room' =
-// umin(d, C - q)  (room < q wraps d above C - q: a new batch opens, and d's sign bit says so —
-// a funnel shift collects the 32 sign bits, first position last). Writes the 16-bit cursors
-// (bits 8..23 of the order records) of the first n4 groups of four positions.
-template <bool FULL>
+// The next-fit recurrence over one word, on room = C - load:  room' = umin(room - q, C - q)
+// (room < q wraps room - q above C - q: a new batch opens) — ONE dependent instruction per
+// position (a fused add-min); everything else hangs off the chain: e = q - 1 - room is
+// non-negative exactly when a batch opens, and a funnel shift collects the 32 sign bits, first
+// position last. Writes the 16-bit cursors (bits 8..23 of the order records) of the first n4
+// groups of four positions.
+// TILE: the cursors go to this lane's 128-byte row of a shared-memory tile (two words per
+// row, 16-byte chunk c at c ^ (lane & 7)) that a TMA tile store writes out; otherwise straight
+// to global memory (tail words).
+template <bool FULL, bool TILE>
 __device__ __forceinline__ uint32_t recur_word(const uint32_t (&r)[32], uint32_t C, uint32_t& room,
-                                               uint4* __restrict__ cs_out, int n4, bool write) {
+                                               uint4* __restrict__ cs_out, uint32_t out_row,
+                                               uint32_t swz, int half, int n4, bool write) {
   uint32_t rev = 0;
 #pragma unroll
   for (int i = 0; i < 32; ++i) {
-    const uint32_t q = r[i] & WHP_Q_MASK;
-    const uint32_t d = room - q;
-    rev = __funnelshift_l(d, rev, 1);  // (rev << 1) | (d >> 31)
-    room = min(d, C - q);
+    uint32_t ri = r[i];
+    // the records were gathered one phase ago: keep the scheduler from pulling their first
+    // use up to the loads (it would stall on the shared-memory latency there)
+    asm volatile("" : "+r"(ri));
+    const uint32_t q = ri & WHP_Q_MASK;
+    const uint32_t e = q + ~room;      // sign bit clear <=> room < q
+    rev = __funnelshift_l(e, rev, 1);  // (rev << 1) | (e >> 31)
+    room = min(room + (0u - q), C - q);
   }
-  if (write) {
 #pragma unroll
-    for (int g2 = 0; g2 < 4; ++g2)
-      if (FULL || 2 * g2 < n4)
-        cs_out[g2] = make_uint4(__byte_perm(r[8 * g2 + 0], r[8 * g2 + 1], 0x6521),
-                                __byte_perm(r[8 * g2 + 2], r[8 * g2 + 3], 0x6521),
-                                __byte_perm(r[8 * g2 + 4], r[8 * g2 + 5], 0x6521),
-                                __byte_perm(r[8 * g2 + 6], r[8 * g2 + 7], 0x6521));
+  for (int g2 = 0; g2 < 4; ++g2) {
+    if (FULL || 2 * g2 < n4) {
+      const uint32_t c0 = __byte_perm(r[8 * g2 + 0], r[8 * g2 + 1], 0x6521);
+      const uint32_t c1 = __byte_perm(r[8 * g2 + 2], r[8 * g2 + 3], 0x6521);
+      const uint32_t c2 = __byte_perm(r[8 * g2 + 4], r[8 * g2 + 5], 0x6521);
+      const uint32_t c3 = __byte_perm(r[8 * g2 + 6], r[8 * g2 + 7], 0x6521);
+      if (TILE) {
+        asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(out_row + ((16 * (g2 + 4 * half)) ^ swz)),
+                     "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+      } else if (write) {
+        cs_out[g2] = make_uint4(c0, c1, c2, c3);
+      }
+    }
   }
-  return __brev(rev);
+  return ~__brev(rev);
 }
 
 __global__ void __launch_bounds__(kBoundsThreads)
-whp_bounds_kernel(const uint32_t* __restrict__ order_fast, int32_t n_orders, int32_t C,
-                  const int32_t* __restrict__ perms, int64_t n_cand,
-                  uint32_t* __restrict__ bmask, int32_t bm_pitch, uint16_t* __restrict__ cstream,
-                  int32_t cs_pitch) {
+whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_cs,
+                  const uint32_t* __restrict__ order_fast,
+                  int32_t n_orders, int32_t C, int64_t n_cand, uint32_t* __restrict__ bmask,
+                  int32_t bm_pitch, uint16_t* __restrict__ cstream, int32_t cs_pitch) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  // [chunk buffers: kStages x 32 threads x kChunkStride][order table][mbarriers: kStages + 1]
+  // [tiles: kStages x 4 KB, 1 KB aligned (swizzle)][cursor tiles: 2 x 4 KB][order table]
+  // [mbarriers: kStages + 1]
   const int nw = (n_orders + 31) >> 5;
-  const int tid = threadIdx.x;
-  uint8_t* sp = smem_raw + kStages * kBoundsThreads * kChunkStride;
-  uint32_t* sorec = reinterpret_cast<uint32_t*>(sp);
-  sp += 4 * (size_t)((n_orders + 3) & ~3);
-  const uint32_t bars = smem_u32(sp);
-  const uint32_t buf0 = smem_u32(smem_raw) + tid * kChunkStride;
-  constexpr uint32_t kStageBytes = kBoundsThreads * kChunkStride;
-  const uint32_t sorec0 = smem_u32(sorec);
-  constexpr int kWarps = kBoundsThreads / 32;
-  if (tid == 0) {
-    for (int s = 0; s < kStages * kWarps; ++s) mbar_init(bars + 8 * s, 32);
-    mbar_init(bars + 8 * kStages * kWarps, 1);
+  const int lane = threadIdx.x;
+  const uint32_t tiles = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t otiles = tiles + kStages * kTileBytes;  // 32 rows x 64 cursors, two of them
+  const uint32_t sorec0 = otiles + 2 * kTileBytes;
+  const uint32_t bars = sorec0 + 4u * (uint32_t)((n_orders + 3) & ~3);
+  if (lane == 0) {
+    for (int s = 0; s <= kStages; ++s) mbar_init(bars + 8 * s, 1);
   }
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  __syncthreads();
-  if (tid == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
-    mbar_expect_tx(bars + 8 * kStages * kWarps, 4u * (uint32_t)n_orders);
-    bulk_g2s(sorec0, order_fast, 4u * (uint32_t)n_orders, bars + 8 * kStages * kWarps);
+  __syncwarp();
+  const int64_t row0 = (int64_t)blockIdx.x * kBoundsThreads;  // first plan of this warp
+  auto issue = [&](int w) {  // one lane: tile of word w into stage w mod kStages
+    const uint32_t bar = bars + 8 * (w & (kStages - 1));
+    mbar_expect_tx(bar, kTileBytes);
+    tma_tile_2d(tiles + (w & (kStages - 1)) * kTileBytes, &tmap, 32 * w, (int32_t)row0, bar);
+  };
+  if (lane == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
+    mbar_expect_tx(bars + 8 * kStages, 4u * (uint32_t)n_orders);
+    bulk_g2s(sorec0, order_fast, 4u * (uint32_t)n_orders, bars + 8 * kStages);
+    for (int w = 0; w < kStages && w < nw; ++w) issue(w);
   }
-  const uint32_t wbars = bars + 8 * kStages * (tid >> 5);  // this warp's stage barriers
-  const int64_t c_raw = (int64_t)blockIdx.x * kBoundsThreads + tid;
-  const bool have = c_raw < n_cand;
-  const int64_t c = have ? c_raw : n_cand - 1;  // idle threads shadow the last plan, no writes
-  const uint8_t* __restrict__ row = reinterpret_cast<const uint8_t*>(perms + c * n_orders);
-  const int row_bytes = 4 * n_orders;
-  const int nchunks = (row_bytes + kChunkBytes - 1) / kChunkBytes;
-  for (int k = 0; k < kStages && k < nchunks; ++k) {
-    const uint32_t bytes = (uint32_t)min(kChunkBytes, row_bytes - k * kChunkBytes);
-    mbar_expect_tx(wbars + 8 * k, bytes);
-    bulk_g2s(buf0 + k * kStageBytes, row + (size_t)k * kChunkBytes, bytes, wbars + 8 * k);
-  }
-  uint32_t* __restrict__ bm = bmask + c * bm_pitch;
-  uint4* __restrict__ cs = reinterpret_cast<uint4*>(cstream + c * cs_pitch);
+  const int64_t c = row0 + lane;
+  const bool have = c < n_cand;  // rows past the end arrive zero-filled: order 0, never written
+  uint32_t* __restrict__ bm = bmask + (have ? c : 0) * bm_pitch;
+  uint4* __restrict__ cs = reinterpret_cast<uint4*>(cstream + (have ? c : 0) * cs_pitch);
+  const uint32_t rowoff = lane * 128, swz = (lane & 7) << 4;
+  auto tile_row = [&](int w) { return tiles + (w & (kStages - 1)) * kTileBytes + rowoff; };
+  auto wait_word = [&](int w) { mbar_wait(bars + 8 * (w & (kStages - 1)), (w / kStages) & 1); };
+  auto refill = [&](int w) {  // word w is consumed by every lane: its stage takes word w + kStages
+    // (the tile was only READ, and every value read has been used: no proxy fence is needed
+    // before the async proxy overwrites it)
+    __syncwarp();
+    if (lane == 0 && w + kStages < nw) issue(w + kStages);
+  };
   uint32_t room = (uint32_t)C;
-  // chunk k lives in stage k mod kStages, phase parity (k / kStages) & 1
-  int stage = 0;
-  uint32_t parity = 0;
   uint32_t ra[32], rb[32];
-  mbar_wait(bars + 8 * kStages * kWarps, 0);
-  mbar_wait(wbars, 0);
-  constexpr int WPC = kChunkBytes / 128;       // words per chunk (even)
+  mbar_wait(bars + 8 * kStages, 0);
+  wait_word(0);
   const int n_full = n_orders >> 5;            // words with all 32 positions
-  // chunks whose words and whose successor's first word are all full: the straight-line path
-  const int KF = n_full > 0 ? (n_full - 1) / WPC : 0;
-  if (n_full > 0) gather_word<true>(ra, buf0, sorec0, 8);
+  // pairs of words (2k, 2k+1) whose successor 2k+2 is full too: the straight-line path
+  const int KF = n_full > 0 ? (n_full - 1) >> 1 : 0;
+  if (n_full > 0) gather_word<true>(ra, tile_row(0), swz, sorec0, 8);
 #pragma unroll 1
   for (int k = 0; k < KF; ++k) {
-    const uint32_t buf = buf0 + stage * kStageBytes;
-    const uint32_t bar = wbars + 8 * stage;
-#pragma unroll
-    for (int j = 0; j < WPC; ++j) {
-      // word k*WPC+j runs its recurrence while the next word is gathered
-      uint32_t (&cur)[32] = (j & 1) ? rb : ra;
-      uint32_t (&nxt)[32] = (j & 1) ? ra : rb;
-      if (j == WPC - 1) {  // the next word opens the next chunk
-        if (++stage == kStages) { stage = 0; parity ^= 1u; }
-        mbar_wait(wbars + 8 * stage, parity);
-        gather_word<true>(nxt, buf0 + stage * kStageBytes, sorec0, 8);
-      } else {
-        gather_word<true>(nxt, buf + 128 * (j + 1), sorec0, 8);
-      }
-      uint32_t bits = recur_word<true>(cur, (uint32_t)C, room, cs + 4 * (k * WPC + j), 8, have);
-      if (k == 0 && j == 0) bits |= 1u;  // batch 0 starts at position 0
-      if (have) bm[k * WPC + j] = bits;
-    }
-    if (k + kStages < nchunks) {  // chunk k is consumed: refill its stage
-      const int kn = k + kStages;
-      const uint32_t bytes = (uint32_t)min(kChunkBytes, row_bytes - kn * kChunkBytes);
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_expect_tx(bar, bytes);
-      bulk_g2s(buf, row + (size_t)kn * kChunkBytes, bytes, bar);
-    }
+    const int w = 2 * k;
+    const uint32_t otile = otiles + (k & 1) * kTileBytes;
+    // the tile store issued two iterations ago must have read this cursor tile
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+    __syncwarp();
+    // word w runs its recurrence while word w+1 is gathered
+    wait_word(w + 1);
+    gather_word<true>(rb, tile_row(w + 1), swz, sorec0, 8);
+    uint32_t bits = recur_word<true, true>(ra, (uint32_t)C, room, nullptr, otile + rowoff, swz, 0, 8, have);
+    if (k == 0) bits |= 1u;  // batch 0 starts at position 0
+    const uint32_t bits_even = bits;
+    refill(w);
+    // word w+1 runs its recurrence while word w+2 is gathered
+    wait_word(w + 2);
+    gather_word<true>(ra, tile_row(w + 2), swz, sorec0, 8);
+    bits = recur_word<true, true>(rb, (uint32_t)C, room, nullptr, otile + rowoff, swz, 1, 8, have);
+    if (have) *reinterpret_cast<uint2*>(bm + w) = make_uint2(bits_even, bits);
+    refill(w + 1);
+    // the 64 cursors of words w, w+1 of all 32 plans: one tile store (rows past n_cand clipped)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncwarp();
+    if (lane == 0) tma_store_2d(&tmap_cs, 32 * w, (int32_t)row0, otile);
   }
-  // the last (at most WPC + 1) words, the final one possibly partial; word KF*WPC is in ra
-  // if it is full
+  // the last (at most three) words, the final one possibly partial; word 2*KF is in ra if full
 #pragma unroll 1
-  for (int w = KF * WPC; w < nw; ++w) {
+  for (int w = 2 * KF; w < nw; ++w) {
     const int left = n_orders - 32 * w;
     const int n4 = min(8, left >> 2);
-    if (w > KF * WPC || n_full == 0) {
-      if (w > 0 && (w % WPC) == 0) {
-        if (++stage == kStages) { stage = 0; parity ^= 1u; }
-        mbar_wait(wbars + 8 * stage, parity);
-      }
-      gather_word<false>(ra, buf0 + stage * kStageBytes + 128 * (w % WPC), sorec0, n4);
+    if (w > 2 * KF || n_full == 0) {
+      wait_word(w);
+      gather_word<false>(ra, tile_row(w), swz, sorec0, n4);
     }
-    uint32_t bits = recur_word<false>(ra, (uint32_t)C, room, cs + 4 * w, n4, have);
+    uint32_t bits = recur_word<false, false>(ra, (uint32_t)C, room, cs + 4 * w, 0u, 0u, 0, n4, have);
     if (w == 0) bits |= 1u;
     if (left < 32) bits |= 1u << left;    // end sentinel in a partial last word
     if (have) bm[w] = bits;
   }
   if (have && (n_orders & 31) == 0) bm[nw] = 1u;  // end sentinel in a word of its own
+  if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // tiles still being read
 }
 
 // One warp per plan: number of batches, and the first position of every segment (segment s
@@ -611,8 +638,21 @@ static int64_t nb_upper_bound(const whp_ctx* c) {
 }
 
 static size_t bounds_smem_bytes(const whp_ctx* c) {
-  return (size_t)kStages * kBoundsThreads * kChunkStride + 4 * (((size_t)c->n_orders + 3) & ~(size_t)3) +
-         8 * (kStages * (kBoundsThreads / 32) + 1);
+  return 1024 + (size_t)(kStages + 2) * kTileBytes + 4 * (((size_t)c->n_orders + 3) & ~(size_t)3) +
+         8 * (kStages + 1);
+}
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+static PFN_cuTensorMapEncodeTiled tensor_map_encoder() {
+  static PFN_cuTensorMapEncodeTiled fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (PFN_cuTensorMapEncodeTiled)p;
+  }
+  return fn;
 }
 
 bool whp_fast_eligible(const whp_ctx* c) {
@@ -695,11 +735,32 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
     cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     const size_t smem = bounds_smem_bytes(c);
+    // tensor map over this call's permutation matrix: [n_cand][n_orders] int32, box 32 x 32
+    PFN_cuTensorMapEncodeTiled encode = tensor_map_encoder();
+    if (!encode) return cudaErrorNotSupported;
+    CUtensorMap tmap;
+    const cuuint64_t gdim[2] = {(cuuint64_t)c->n_orders, (cuuint64_t)n_cand};
+    const cuuint64_t gstride[1] = {4ull * (cuuint64_t)c->n_orders};
+    const cuuint32_t box[2] = {32, 32};
+    const cuuint32_t estr[2] = {1, 1};
+    if (encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_INT32, 2, (void*)d_perms, gdim, gstride, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+    // tensor map over the cursor stream: [n_cand][cs_pitch] u16, box 32 rows x 64 cursors
+    CUtensorMap tmap_cs;
+    const cuuint64_t cdim[2] = {(cuuint64_t)cs_pitch, (cuuint64_t)n_cand};
+    const cuuint64_t cstride[1] = {2ull * (cuuint64_t)cs_pitch};
+    const cuuint32_t cbox[2] = {64, 32};
+    if (encode(&tmap_cs, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, (void*)c->d_cstream, cdim, cstride, cbox,
+               estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
     cudaFuncSetAttribute(whp_bounds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          c->smem_optin - 1024);
     const unsigned blocks = (unsigned)((n_cand + kBoundsThreads - 1) / kBoundsThreads);
     whp_bounds_kernel<<<blocks, kBoundsThreads, smem, st>>>(
-        c->d_order_fast, c->n_orders, c->C, d_perms, n_cand, c->d_bmask, bm_pitch, c->d_cstream,
+        tmap, tmap_cs, c->d_order_fast, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch, c->d_cstream,
         cs_pitch);
     c->launches += 1;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
