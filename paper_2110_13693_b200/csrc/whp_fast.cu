@@ -593,23 +593,16 @@ whp_finish_kernel(const whp_tables T, int64_t n_cand, const int64_t* __restrict_
   const int lane = threadIdx.x & 31;
   const int64_t cand = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (cand >= n_cand) return;
-  // the candidate's (kMaxPlanes+5) x KW counter words, one coalesced read, then warp broadcasts
+  // the candidate's counter words are read by broadcast loads (every lane needs its own bit of
+  // every word): plane pp of class word w holds bit pp of r_k for the 32 classes of that word
   const uint32_t* __restrict__ pc = planes + cand * ((kMaxPlanes + 5) * KW);
-  const int total = planes_used * KW;  // <= 13 * 8 = 104
-  uint32_t regs[4];
-#pragma unroll
-  for (int i = 0; i < 4; ++i) regs[i] = (lane + 32 * i < total) ? __ldg(pc + lane + 32 * i) : 0u;
   double s = 0.0;
   const int kw_used = (T.K + 31) >> 5;
   for (int w = 0; w < kw_used; ++w) {
     int r = 0;
-    for (int pp = 0; pp < planes_used; ++pp) {
-      const int idx = pp * KW + w;
-      const int hi = idx >> 5;
-      const uint32_t src = hi == 0 ? regs[0] : hi == 1 ? regs[1] : hi == 2 ? regs[2] : regs[3];
-      const uint32_t word = __shfl_sync(WHP_FULL, src, idx & 31);
-      r += (int)((word >> lane) & 1u) << pp;
-    }
+#pragma unroll 4
+    for (int pp = 0; pp < planes_used; ++pp)
+      r |= (int)((__ldg(pc + pp * KW + w) >> lane) & 1u) << pp;
     const int k = 32 * w + lane;
     if (k < T.K) {
       if (resp) resp[cand * T.K + k] = r;

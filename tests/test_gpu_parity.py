@@ -251,6 +251,23 @@ def test_edge_cases(torch_cuda, cfg):
     ctx.close()
 
 
+@pytest.mark.parametrize("n_orders", [8, 28, 36, 60, 64, 68, 96, 100, 128, 132, 192, 196])
+@pytest.mark.parametrize("n_cand", [1, 33])
+def test_tuned_path_word_and_warp_tails(torch_cuda, n_orders, n_cand):
+    """K1 streams 32 plans x 32 positions per tile: every combination of full / partial last
+    word, odd / even number of words and a partial last warp of plans must agree with the
+    oracle (the tuned path is taken: n_orders is a multiple of 4)."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = _random_problem(5, NA=70, S=12, K=70, n_skus=400, n_orders=n_orders, qmax=5, C=11, depot=3)
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perm_rows(7, pb.n_orders, np.arange(n_cand))
+    got, dev = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
+    ref = oracle.eval_candidates(pb, perms)
+    assert_parity(got, ref, pb)
+    ctx.close()
+
+
 def test_api_errors_and_nullable_outputs(torch_cuda):
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
