@@ -40,7 +40,8 @@ void free_orders(whp_ctx* c) {
   dfree(c->base.bstart); dfree(c->base.bop); dfree(c->base.bdist); dfree(c->base.bclass);
   dfree(c->base.resp); dfree(c->base.totals); dfree(c->base.ftotals); dfree(c->base.pre);
   dfree(c->base.orec); dfree(c->base.rpre); dfree(c->base.nxt); dfree(c->base.dist_at);
-  dfree(c->base.cls_at);
+  dfree(c->base.cls_at); dfree(c->base.dtail); dfree(c->base.bF); dfree(c->base.rtail);
+  c->rtail_rows = 0;
   dfree(c->d_stage[0]); dfree(c->d_stage[1]);
   c->stage_rows = 0;
   dfree(c->d_bmask); dfree(c->d_cstream); dfree(c->d_nb); dfree(c->d_dist_scratch);
@@ -173,6 +174,8 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   WHP_CUDA(c, cudaMalloc(&c->base.nxt, 4 * no));
   WHP_CUDA(c, cudaMalloc(&c->base.dist_at, 8 * no));
   WHP_CUDA(c, cudaMalloc(&c->base.cls_at, 32 * no));
+  WHP_CUDA(c, cudaMalloc(&c->base.dtail, 8 * no));
+  WHP_CUDA(c, cudaMalloc(&c->base.bF, 4 * no));
   {  // consecutive next-fit batches together hold more than C items: nb <= 2 n_items/(C+1) + 1
     int64_t nb_max = 2ll * n_items / ((int64_t)cart_capacity + 1) + 1;
     if (nb_max > n_orders) nb_max = n_orders;

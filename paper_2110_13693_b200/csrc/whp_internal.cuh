@@ -83,6 +83,9 @@ struct whp_base_tables {
   int32_t* nxt;       // [n_orders]   end of the batch that would open at position p
   int64_t* dist_at;   // [n_orders]   S-shape length of that batch (region of the window only)
   uint32_t* cls_at;   // [n_orders][8] its class mask
+  int64_t* dtail;     // [n_orders]   chain sums (whp_swaps_chain_kernel), region only
+  int32_t* bF;        // [n_orders]   base batch where the chain of p meets the base plan
+  int32_t* rtail;     // [region][K]  class visits along the chain
 };
 
 struct whp_ctx {
@@ -105,6 +108,7 @@ struct whp_ctx {
   bool have_orders = false, have_penalty = false;
   // scratch
   whp_base_tables base{};
+  int64_t rtail_rows = 0;
   void* d_argmin_part = nullptr;  // partial (val, idx) pairs + ticket
   int32_t argmin_cap = 0;
   unsigned long long* d_count = nullptr;  // validate_perms counter

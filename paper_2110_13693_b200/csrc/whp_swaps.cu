@@ -302,6 +302,65 @@ whp_swaps_prep_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
   if (lane < 8) B.cls_at[(int64_t)p * 8 + lane] = sets->cmask[lane];
 }
 
+// ------------------------------------------------------------------------------ chains
+// A plan re-batched from position p follows p -> nxt[p] -> nxt[nxt[p]] ... until a start
+// coincides with a base batch start F(p) (from there on it IS the base plan). That chain depends
+// on p alone, and two next-fit chains take long to meet (tens of batches), so it is summed once
+// per region position: dtail[p] = lengths of the chain's batches before F(p), rtail[p][k] = their
+// class visits, bF[p] = base batch that starts at F(p) (nb: the chain runs to the end of the plan;
+// -1: it leaves the region first). With T(p) = dtail[p] + (D_base - bdist[bF[p]]), any stretch
+// s -> t of one chain costs T(s) - T(t).
+constexpr int kChainWarps = 16;
+
+__global__ void __launch_bounds__(kChainWarps * 32)
+whp_swaps_chain_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, int32_t rhi) {
+  // the region's hop records in shared memory (a chain is a run of dependent look-ups):
+  // [cls_at: rows x 8][dist_at: rows (int64)][nxt: rows; negative: p is a base batch start]
+  extern __shared__ __align__(16) uint8_t chain_smem[];
+  const int32_t rows = rhi - rlo;
+  uint4* s_cls = reinterpret_cast<uint4*>(chain_smem);
+  int64_t* s_dist = reinterpret_cast<int64_t*>(chain_smem + 32 * (size_t)rows);
+  int32_t* s_nx = reinterpret_cast<int32_t*>(chain_smem + 40 * (size_t)rows);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int32_t n = T.n_orders;
+  for (int32_t k = threadIdx.x; k < rows; k += blockDim.x) {
+    const int32_t p = rlo + k;
+    const bool start = p == 0 || B.bop[p] != B.bop[p - 1];
+    s_nx[k] = start ? -1 : B.nxt[p];
+    s_dist[k] = B.dist_at[p];
+  }
+  for (int32_t k = threadIdx.x; k < 2 * rows; k += blockDim.x)
+    s_cls[k] = reinterpret_cast<const uint4*>(B.cls_at + (int64_t)rlo * 8)[k];
+  __syncthreads();
+  const int32_t p0 = rlo + blockIdx.x * kChainWarps + warp;
+  if (p0 >= rhi) return;
+  int64_t D = 0;
+  int32_t r[8];
+#pragma unroll
+  for (int w = 0; w < 8; ++w) r[w] = 0;
+  int32_t p = p0, bF;
+  for (;;) {
+    if (p >= n) { bF = (int32_t)B.totals[1]; break; }
+    if (p >= rhi) { bF = -1; break; }
+    const int32_t nx = s_nx[p - rlo];
+    if (nx < 0) { bF = B.bop[p]; break; }
+    D += s_dist[p - rlo];
+    const uint4 c0 = s_cls[2 * (p - rlo)];
+    const uint4 c1 = s_cls[2 * (p - rlo) + 1];
+    r[0] += (int32_t)((c0.x >> lane) & 1u); r[1] += (int32_t)((c0.y >> lane) & 1u);
+    r[2] += (int32_t)((c0.z >> lane) & 1u); r[3] += (int32_t)((c0.w >> lane) & 1u);
+    r[4] += (int32_t)((c1.x >> lane) & 1u); r[5] += (int32_t)((c1.y >> lane) & 1u);
+    r[6] += (int32_t)((c1.z >> lane) & 1u); r[7] += (int32_t)((c1.w >> lane) & 1u);
+    p = nx;
+  }
+  if (lane == 0) { B.dtail[p0] = D; B.bF[p0] = bF; }
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    const int k = 32 * w + lane;
+    if (k < T.K) B.rtail[(int64_t)(p0 - rlo) * T.K + k] = r[w];
+  }
+}
+
 // ------------------------------------------------------------------------------ neighbours
 constexpr int kSwapWarps = 8;
 constexpr int kStage = 1024;  // positions of pre / orec staged per block
@@ -313,6 +372,7 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   __shared__ warp_sets sets_all[kSwapWarps];
   __shared__ int32_t s_pre[kStage + 1];
   __shared__ uint32_t s_orec[kStage];
+  __shared__ int32_t s_nxt[kStage];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
@@ -328,8 +388,13 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   const int32_t cnt = min(kStage, n - lo);
   for (int k = threadIdx.x; k <= cnt; k += blockDim.x) s_pre[k] = __ldg(B.pre + lo + k);
   for (int k = threadIdx.x; k < cnt; k += blockDim.x) s_orec[k] = __ldg(B.orec + lo + k);
+  for (int k = threadIdx.x; k < cnt; k += blockDim.x) s_nxt[k] = __ldg(B.nxt + lo + k);
   __syncthreads();
   const int64_t D_base = B.totals[0];
+  auto nxt_at = [&](int32_t p) -> int32_t {
+    const uint32_t k = (uint32_t)(p - lo);
+    return k < (uint32_t)cnt ? s_nxt[k] : __ldg(B.nxt + p);
+  };
 
   for (int64_t nn = (int64_t)blockIdx.x * kSwapWarps + warp; nn < n_nb;
        nn += (int64_t)gridDim.x * kSwapWarps) {
@@ -390,8 +455,44 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
       int32_t p = __ldg(B.bstart + b0);
       int32_t b_end;
       for (;;) {
+        // (1) past pj the rest of the rewalk is the chain of p, summed once per position
+        if (p > pj && p >= rlo && p < rhi) {
+          const int32_t bf = __ldg(B.bF + p);
+          if (bf >= 0) {
+            D += __ldg(B.dtail + p);
+#pragma unroll
+            for (int w = 0; w < 8; ++w) {
+              const int k = 32 * w + lane;
+              if (k < T.K) r[w] += __ldg(B.rtail + (int64_t)(p - rlo) * T.K + k);
+            }
+            b_end = bf;
+            break;
+          }
+        }
+        // (2) between pi and pj the prefix is shifted uniformly: batches that end before pj
+        // are the chain of p as well — hop to its last node t before pj, add T(p) - T(t)
+        if (p > pi && p < pj && p >= rlo && pj < rhi) {
+          int32_t t = p;
+          for (int32_t nx = nxt_at(t); nx < pj; nx = nxt_at(t)) t = nx;
+          if (t != p) {
+            const int32_t bfp = __ldg(B.bF + p), bft = __ldg(B.bF + t);
+            if (bfp >= 0 && bft >= 0) {
+              D += (__ldg(B.dtail + p) - __ldg(B.dtail + t)) + (B.bdist[bft] - B.bdist[bfp]);
+#pragma unroll
+              for (int w = 0; w < 8; ++w) {
+                const int k = 32 * w + lane;
+                if (k < T.K) {
+                  r[w] += __ldg(B.rtail + (int64_t)(p - rlo) * T.K + k) -
+                          __ldg(B.rtail + (int64_t)(t - rlo) * T.K + k);
+                  if (bft != bfp)
+                    r[w] += __ldg(B.rpre + (int64_t)bft * T.K + k) - __ldg(B.rpre + (int64_t)bfp * T.K + k);
+                }
+              }
+              p = t;
+            }
+          }
+        }
         // A batch that holds neither swapped position and ends where the base criterion ends
-        // it is the tabulated batch of its start; the others are scored from their picks.
         int32_t e;
         bool table;
         if (p > pj) {
@@ -456,6 +557,24 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
                                     ? (int64_t)win_start + win_len + margin : c->n_orders);
   whp_swaps_prep_kernel<<<(unsigned)((rhi - rlo + kPrepWarps - 1) / kPrepWarps), kPrepWarps * 32,
                           0, st>>>(T, c->base, rlo, rhi);
+  c->launches += 1;
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  // chain sums of the region (rtail grows with the region)
+  const int64_t rows = rhi - rlo;
+  if (c->rtail_rows < rows) {
+    if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return e;
+    cudaFree(c->base.rtail);
+    c->base.rtail = nullptr;
+    c->rtail_rows = 0;
+    if ((e = cudaMalloc(&c->base.rtail, 4 * (size_t)rows * (size_t)c->K)) != cudaSuccess) return e;
+    c->rtail_rows = rows;
+  }
+  const size_t chain_smem = 44 * (size_t)rows;
+  if (chain_smem + 2048 > (size_t)c->smem_optin) return cudaErrorInvalidConfiguration;
+  if ((e = cudaFuncSetAttribute(whp_swaps_chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)chain_smem)) != cudaSuccess) return e;
+  whp_swaps_chain_kernel<<<(unsigned)((rows + kChainWarps - 1) / kChainWarps), kChainWarps * 32,
+                           chain_smem, st>>>(T, c->base, rlo, rhi);
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   const int64_t n_nb = (int64_t)win_len * (win_len - 1) / 2;
