@@ -63,7 +63,7 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
 // the order ids of word w+1 leave the tile and their order records are gathered from the table
 // in shared memory — so that a lone warp per scheduler keeps issuing.
 constexpr int kBoundsThreads = 32;   // plans per block, one per thread
-constexpr int kStages = 4;           // tiles (words) in flight, power of two
+constexpr int kStages = 7;           // tiles (words) in flight per warp
 constexpr int kTileBytes = 32 * 128; // 32 rows x 32 positions x 4 B
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -185,9 +185,9 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   __syncwarp();
   const int64_t row0 = (int64_t)blockIdx.x * kBoundsThreads;  // first plan of this warp
   auto issue = [&](int w) {  // one lane: tile of word w into stage w mod kStages
-    const uint32_t bar = bars + 8 * (w & (kStages - 1));
+    const uint32_t bar = bars + 8 * (w % kStages);
     mbar_expect_tx(bar, kTileBytes);
-    tma_tile_2d(tiles + (w & (kStages - 1)) * kTileBytes, &tmap, 32 * w, (int32_t)row0, bar);
+    tma_tile_2d(tiles + (w % kStages) * kTileBytes, &tmap, 32 * w, (int32_t)row0, bar);
   };
   if (lane == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
     mbar_expect_tx(bars + 8 * kStages, 4u * (uint32_t)n_orders);
@@ -199,8 +199,8 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   uint32_t* __restrict__ bm = bmask + (have ? c : 0) * bm_pitch;
   uint4* __restrict__ cs = reinterpret_cast<uint4*>(cstream + (have ? c : 0) * cs_pitch);
   const uint32_t rowoff = lane * 128, swz = (lane & 7) << 4;
-  auto tile_row = [&](int w) { return tiles + (w & (kStages - 1)) * kTileBytes + rowoff; };
-  auto wait_word = [&](int w) { mbar_wait(bars + 8 * (w & (kStages - 1)), (w / kStages) & 1); };
+  auto tile_row = [&](int w) { return tiles + (w % kStages) * kTileBytes + rowoff; };
+  auto wait_word = [&](int w) { mbar_wait(bars + 8 * (w % kStages), (w / kStages) & 1); };
   auto refill = [&](int w) {  // word w is consumed by every lane: its stage takes word w + kStages
     // (the tile was only READ, and every value read has been used: no proxy fence is needed
     // before the async proxy overwrites it)
