@@ -62,7 +62,7 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
 // conflict-free. The loop is software-pipelined by hand — while the recurrence runs over word w,
 // the order ids of word w+1 leave the tile and their order records are gathered from the table
 // in shared memory — so that a lone warp per scheduler keeps issuing.
-constexpr int kBoundsThreads = 32;   // plans per block, one per thread
+constexpr int kBoundsThreads = 32;   // plans per block, one per thread (a warp = 32 rows)
 constexpr int kStages = 7;           // tiles (words) in flight per warp
 constexpr int kTileBytes = 32 * 128; // 32 rows x 32 positions x 4 B
 
@@ -170,30 +170,34 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
                   int32_t n_orders, int32_t C, int64_t n_cand, uint32_t* __restrict__ bmask,
                   int32_t bm_pitch, uint16_t* __restrict__ cstream, int32_t cs_pitch) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  // [tiles: kStages x 4 KB, 1 KB aligned (swizzle)][cursor tiles: 2 x 4 KB][order table]
-  // [mbarriers: kStages + 1]
+  // per warp: [tiles: kStages x 4 KB, 1 KB aligned (swizzle)][cursor tiles: 2 x 4 KB]; then
+  // the order table shared by the block's warps and the mbarriers (kStages per warp + 1)
   const int nw = (n_orders + 31) >> 5;
-  const int lane = threadIdx.x;
-  const uint32_t tiles = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const int lane = threadIdx.x & 31, wq = threadIdx.x >> 5;
+  constexpr int kWarps = kBoundsThreads / 32;
+  const uint32_t area = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  const uint32_t tiles = area + wq * (kStages + 2) * kTileBytes;
   const uint32_t otiles = tiles + kStages * kTileBytes;  // 32 rows x 64 cursors, two of them
-  const uint32_t sorec0 = otiles + 2 * kTileBytes;
-  const uint32_t bars = sorec0 + 4u * (uint32_t)((n_orders + 3) & ~3);
-  if (lane == 0) {
-    for (int s = 0; s <= kStages; ++s) mbar_init(bars + 8 * s, 1);
+  const uint32_t sorec0 = area + kWarps * (kStages + 2) * kTileBytes;
+  const uint32_t bar_table = sorec0 + 4u * (uint32_t)((n_orders + 3) & ~3);
+  const uint32_t bars = bar_table + 8 + 8 * kStages * wq;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages * kWarps + 1; ++s) mbar_init(bar_table + 8 * s, 1);
   }
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  __syncwarp();
-  const int64_t row0 = (int64_t)blockIdx.x * kBoundsThreads;  // first plan of this warp
+  __syncthreads();
+  const int64_t row0 = ((int64_t)blockIdx.x * kWarps + wq) * 32;  // first plan of this warp
   auto issue = [&](int w) {  // one lane: tile of word w into stage w mod kStages
     const uint32_t bar = bars + 8 * (w % kStages);
     mbar_expect_tx(bar, kTileBytes);
     tma_tile_2d(tiles + (w % kStages) * kTileBytes, &tmap, 32 * w, (int32_t)row0, bar);
   };
-  if (lane == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
-    mbar_expect_tx(bars + 8 * kStages, 4u * (uint32_t)n_orders);
-    bulk_g2s(sorec0, order_fast, 4u * (uint32_t)n_orders, bars + 8 * kStages);
-    for (int w = 0; w < kStages && w < nw; ++w) issue(w);
+  if (threadIdx.x == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
+    mbar_expect_tx(bar_table, 4u * (uint32_t)n_orders);
+    bulk_g2s(sorec0, order_fast, 4u * (uint32_t)n_orders, bar_table);
   }
+  if (lane == 0)
+    for (int w = 0; w < kStages && w < nw; ++w) issue(w);
   const int64_t c = row0 + lane;
   const bool have = c < n_cand;  // rows past the end arrive zero-filled: order 0, never written
   uint32_t* __restrict__ bm = bmask + (have ? c : 0) * bm_pitch;
@@ -209,7 +213,7 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   };
   uint32_t room = (uint32_t)C;
   uint32_t ra[32], rb[32];
-  mbar_wait(bars + 8 * kStages, 0);
+  mbar_wait(bar_table, 0);
   wait_word(0);
   const int n_full = n_orders >> 5;            // words with all 32 positions
   // pairs of words (2k, 2k+1) whose successor 2k+2 is full too: the straight-line path
@@ -631,8 +635,8 @@ static int64_t nb_upper_bound(const whp_ctx* c) {
 }
 
 static size_t bounds_smem_bytes(const whp_ctx* c) {
-  return 1024 + (size_t)(kStages + 2) * kTileBytes + 4 * (((size_t)c->n_orders + 3) & ~(size_t)3) +
-         8 * (kStages + 1);
+  return 1024 + (size_t)(kBoundsThreads / 32) * (kStages + 2) * kTileBytes +
+         4 * (((size_t)c->n_orders + 3) & ~(size_t)3) + 8 * ((kBoundsThreads / 32) * kStages + 1);
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
