@@ -575,7 +575,14 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
             a[kPlanes + lvl] = carry;
           }
         }
-        if (have && seg == 0) {
+        if (P.S == 32) {
+          // the warp is one plan and every lane holds its counters: lane l decodes r_k of class
+          // 32w + l and K3 reads the counts directly
+          uint32_t r = 0;
+#pragma unroll
+          for (int pp = 0; pp < kPlanes + 5; ++pp) r |= ((a[pp] >> lane) & 1u) << pp;
+          if (have) reinterpret_cast<uint16_t*>(po)[32 * w + lane] = (uint16_t)r;
+        } else if (have && seg == 0) {
 #pragma unroll
           for (int pp = 0; pp < kPlanes + 5; ++pp)
             if (pp < kPlanes + P.log2S) po[pp * KW + w] = a[pp];
@@ -604,9 +611,13 @@ whp_finish_kernel(const whp_tables T, int64_t n_cand, const int64_t* __restrict_
   const int kw_used = (T.K + 31) >> 5;
   for (int w = 0; w < kw_used; ++w) {
     int r = 0;
+    if (planes_used == 0) {  // K2 already decoded the counters (S = 32)
+      r = (int)__ldg(reinterpret_cast<const uint16_t*>(pc) + 32 * w + lane);
+    } else {
 #pragma unroll 4
-    for (int pp = 0; pp < planes_used; ++pp)
-      r |= (int)((__ldg(pc + pp * KW + w) >> lane) & 1u) << pp;
+      for (int pp = 0; pp < planes_used; ++pp)
+        r |= (int)((__ldg(pc + pp * KW + w) >> lane) & 1u) << pp;
+    }
     const int k = 32 * w + lane;
     if (k < T.K) {
       if (resp) resp[cand * T.K + k] = r;
@@ -816,7 +827,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   if (out.dist || out.penalty || out.obj || out.resp) {
     const unsigned blocks = (unsigned)((n_cand * 32 + 255) / 256);
     whp_finish_kernel<<<blocks, 256, 0, st>>>(T, n_cand, c->d_dist_scratch, c->d_planes, KW,
-                                              planes_used, out.dist, out.penalty, out.obj,
+                                              S == 32 ? 0 : planes_used, out.dist, out.penalty, out.obj,
                                               out.resp);
     c->launches += 1;
     return cudaGetLastError();
