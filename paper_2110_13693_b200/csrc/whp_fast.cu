@@ -319,7 +319,9 @@ whp_segments_kernel(const uint32_t* __restrict__ bmask, int32_t bm_pitch, int32_
 }
 
 // ------------------------------------------------------------------------------------------ K2
-constexpr int kMaxPlanes = 8;  // vertical counter bit planes: up to 255 batches per segment
+// vertical counter bit planes: at most 8 per segment (up to 255 batches) + 5 combine levels
+constexpr int kPlaneRow = 16;  // words per class word in a plan's counter row: 13 planes, or
+                               // (S = 32) the 32 decoded 16-bit counts
 
 struct sets_params {
   int S;           // segments per candidate (power of two <= 32)
@@ -555,7 +557,7 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
     }
     // bit-sliced addition of the S lanes' vertical counters (one more plane per level)
     {
-      uint32_t* __restrict__ po = planes_out + cand * ((kMaxPlanes + 5) * KW);
+      uint32_t* __restrict__ po = planes_out + cand * (kPlaneRow * KW);
 #pragma unroll
       for (int w = 0; w < KW; ++w) {
         uint32_t a[kPlanes + 5];
@@ -606,7 +608,7 @@ whp_finish_kernel(const whp_tables T, int64_t n_cand, const int64_t* __restrict_
   if (cand >= n_cand) return;
   // the candidate's counter words are read by broadcast loads (every lane needs its own bit of
   // every word): plane pp of class word w holds bit pp of r_k for the 32 classes of that word
-  const uint32_t* __restrict__ pc = planes + cand * ((kMaxPlanes + 5) * KW);
+  const uint32_t* __restrict__ pc = planes + cand * (kPlaneRow * KW);
   double s = 0.0;
   const int kw_used = (T.K + 31) >> 5;
   for (int w = 0; w < kw_used; ++w) {
@@ -718,7 +720,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
                         ((int64_t)c->g.n_aisles + 2) * c->g.aisle_len;
   const int fits32 = worst < (1ll << 31) ? 1 : 0;
   // scratch (grow-only; reallocated when the shape changes)
-  const int64_t plane_words = (int64_t)(kMaxPlanes + 5) * KW;
+  const int64_t plane_words = (int64_t)kPlaneRow * KW;
   if (c->fast_cap < n_cand || c->fast_pitch != bm_pitch || c->fast_plane_words < plane_words) {
     cudaError_t e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) return e;
