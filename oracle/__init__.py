@@ -12,6 +12,8 @@ from .binding import (  # noqa: F401
     eval_candidate_batches,
     eval_candidates,
     eval_swaps,
+    nhatc_loop,
+    nhatc_update,
     optimal_route,
     penalty,
     swap_trajectory,

@@ -152,3 +152,30 @@ def swap_trajectory(pb, base_perm, W: int, stride: int, n_iter: int) -> dict:
     del keep
     out["perm"] = perm
     return out
+
+
+def nhatc_update(r, t, v, w, beta: float):
+    """Reading N1: v <- v + 2 w^2 (t - r), w <- beta w. Returns new (v, w)."""
+    r, t = _i32(r), _f64(t)
+    v, w = _f64(v).copy(), _f64(w).copy()
+    _load().orc_nhatc_update(C.c_int32(len(r)), _p(r), _p(t), _p(v), _p(w), C.c_double(beta))
+    return v, w
+
+
+def nhatc_loop(pb, perms, n_outer: int, beta: float) -> dict:
+    """NEXT-1: n_outer times {score every plan (D1-D6), take the argmin (D7), read its
+    responses r*, update the multipliers (N1)}. Returns the per-iteration winner, its D and J,
+    and the final v, w."""
+    import copy
+    pb = copy.copy(pb)
+    pb.v, pb.w = _f64(pb.v).copy(), _f64(pb.w).copy()
+    hist = {"idx": np.zeros(n_outer, np.int64), "dist": np.zeros(n_outer, np.int64),
+            "obj": np.zeros(n_outer, np.float64)}
+    for it in range(n_outer):
+        out = eval_candidates(pb, perms)
+        i = argmin(out["obj"])
+        one = eval_candidates(pb, _i32(perms)[i], detail=True)
+        hist["idx"][it], hist["dist"][it], hist["obj"][it] = i, out["dist"][i], out["obj"][i]
+        pb.v, pb.w = nhatc_update(one["resp"][0], pb.t, pb.v, pb.w, beta)
+    hist["v"], hist["w"] = pb.v, pb.w
+    return hist

@@ -293,3 +293,22 @@ int32_t orc_swap_trajectory(const orc_geom* g, const int32_t* sku_loc, const int
   free(dist); free(obj);
   return 0;
 }
+
+/* ---- NEXT-1: NHATC multiplier update (outer loop of the coordination) ------------------------
+ * PAPER.md:152-162 (§5): in NHATC "targets and responses are communicated" between neighbours
+ * and the subproblem minimises f + phi(c); the paper prints neither phi nor the update of its
+ * parameters and cites Tosserams et al. 2010 for the method. DESIGN.md reading
+ * N1: with phi = v.c + ||w o c||^2 (north_star) the method-of-multipliers step of that reference
+ * is  v_k <- v_k + 2 w_k^2 c_k,  w_k <- beta w_k,  c = t - r* (r* = responses of the plan the
+ * subproblem solve returned). Rounding order: u = w*w; g = u*c; v' = v + 2*g (2*g is exact);
+ * w' = beta*w. Parity unpinned BY THE PAPER; pinned to reading N1 by hand-worked values. */
+void orc_nhatc_update(int32_t K, const int32_t* r, const double* t, double* v, double* w,
+                      double beta) {
+  for (int32_t k = 0; k < K; ++k) {
+    double c = t[k] - (double)r[k];
+    double u = w[k] * w[k];
+    double g = u * c;
+    v[k] = v[k] + 2.0 * g;
+    w[k] = beta * w[k];
+  }
+}

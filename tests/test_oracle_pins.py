@@ -382,3 +382,47 @@ def test_argmin_first_minimum():
     for _ in range(50):
         x = rng.integers(0, 6, size=int(rng.integers(1, 40))).astype(float)
         assert oracle.argmin(x) == int(np.argmin(x))
+
+
+# ---- NEXT-1: NHATC multiplier update (reading N1) -------------------------------------------
+def test_nhatc_update_golden(golden):
+    g = golden["nhatc_update"]
+    v, w = oracle.nhatc_update(g["r"], g["t"], g["v"], g["w"], g["beta"])
+    assert v.tolist() == g["v_new"] and w.tolist() == g["w_new"]
+
+
+def test_nhatc_update_special_cases_and_exact_rational():
+    from fractions import Fraction
+    rng = np.random.default_rng(3)
+    K = 37
+    r = rng.integers(0, 50, K)
+    t, v, w = rng.uniform(0, 40, K), rng.uniform(-3, 3, K), rng.uniform(0, 2, K)
+    v0, w0 = oracle.nhatc_update(r, t, v, np.zeros(K), 3.0)
+    assert np.array_equal(v0, v) and not w0.any()                  # w = 0: multipliers stay
+    v1, w1 = oracle.nhatc_update(r, r.astype(np.float64), v, w, 1.0)
+    assert np.array_equal(v1, v) and np.array_equal(w1, w)         # consistent plan, beta = 1
+    v2, w2 = oracle.nhatc_update(r, t, v, w, 2.5)
+    assert np.array_equal(w2, 2.5 * w)
+    for k in range(K):                                             # v' = v + 2 w^2 (t - r), exactly
+        c = Fraction(float(t[k])) - int(r[k])
+        exact = Fraction(float(v[k])) + 2 * Fraction(float(w[k])) ** 2 * c
+        bound = 4 * 2.0 ** -53 * (abs(v[k]) + 2 * w[k] ** 2 * abs(float(c)))
+        assert abs(float(Fraction(float(v2[k])) - exact)) <= bound
+    # the multiplier term moves against the inconsistency: (v' - v).c = 2 sum (w c)^2 >= 0
+    c = t - r
+    assert np.dot(v2 - v, c) >= 0.0
+
+
+def test_nhatc_loop_is_eval_argmin_update():
+    pb = W.make_problem("tiny")
+    perms = W.perms(0, pb.n_orders, 16)
+    h = oracle.nhatc_loop(pb, perms, 3, 1.5)
+    import copy
+    q = copy.copy(pb)
+    for it in range(3):
+        out = oracle.eval_candidates(q, perms, detail=True)
+        i = int(np.argmin(out["obj"]))
+        assert h["idx"][it] == i and h["obj"][it] == out["obj"][i] and h["dist"][it] == out["dist"][i]
+        q.v, q.w = oracle.nhatc_update(out["resp"][i], q.t, q.v, q.w, 1.5)
+    assert np.array_equal(h["v"], q.v) and np.array_equal(h["w"], q.w)
+    assert np.array_equal(h["w"], pb.w * 1.5 * 1.5 * 1.5)
