@@ -116,6 +116,25 @@ whp_status whp_argmin(whp_ctx* ctx, const double* d_obj, int64_t n, int64_t* d_i
 whp_status whp_apply_swap(whp_ctx* ctx, int32_t* d_base_perm, int32_t win_start,
                           int32_t win_len, const int64_t* d_idx, void* cuda_stream);
 
+/* ---- NEXT-1: the NHATC outer loop (§5 Eq. 3; update rule = reading N1 of
+ * DESIGN.md, the method-of-multipliers step of the cited Tosserams et al. 2010) ------------- */
+
+/* v_k <- v_k + 2 w_k^2 c_k, w_k <- beta w_k with c = t - r*, r* = row *d_idx (DEVICE int64,
+ * NULL = row 0) of d_resp_rows (DEVICE int32 [rows][n_classes], e.g. the d_resp output of
+ * whp_eval_candidates). Updates the context's penalty parameters in place, on the stream. */
+whp_status whp_nhatc_update(whp_ctx* ctx, const int32_t* d_resp_rows, const int64_t* d_idx,
+                            double beta, void* cuda_stream);
+
+/* n_outer times { whp_eval_candidates on d_perms -> whp_argmin -> record (winner index, its D,
+ * its J) into the DEVICE histories [n_outer] (each nullable) -> whp_nhatc_update with the
+ * winner's responses }, all on the stream with no host round trip. */
+whp_status whp_nhatc_solve(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand, int32_t n_outer,
+                           double beta, int64_t* d_idx_hist, int64_t* d_dist_hist,
+                           double* d_obj_hist, void* cuda_stream);
+
+/* Current penalty parameters to HOST double[n_classes] each (nullable). Synchronises the stream. */
+whp_status whp_get_penalty(whp_ctx* ctx, double* t, double* v, double* w, void* cuda_stream);
+
 /* Debug helper: *h_n_bad (host) receives the number of rows of d_perms that are not a
  * permutation of 0..n_orders-1. Synchronises the stream. */
 whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,

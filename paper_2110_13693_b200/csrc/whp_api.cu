@@ -365,6 +365,63 @@ whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t 
   return WHP_OK;
 }
 
+whp_status whp_nhatc_update(whp_ctx* c, const int32_t* d_resp_rows, const int64_t* d_idx,
+                            double beta, void* cuda_stream) {
+  whp_status s = ready(c);
+  if (s != WHP_OK) return s;
+  if (!d_resp_rows) return fail(c, WHP_ERR_INVALID_ARG, "d_resp_rows is null");
+  if (!std::isfinite(beta) || beta <= 0.0) return fail(c, WHP_ERR_OUT_OF_RANGE, "beta must be finite and positive");
+  device_guard dg(c->device);
+  WHP_CUDA(c, whp_launch_nhatc_update(c, d_resp_rows, d_idx, beta, (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
+whp_status whp_nhatc_solve(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int32_t n_outer,
+                           double beta, int64_t* d_idx_hist, int64_t* d_dist_hist,
+                           double* d_obj_hist, void* cuda_stream) {
+  whp_status s = ready(c);
+  if (s != WHP_OK) return s;
+  if (!d_perms || n_cand < 1 || n_outer < 0) return fail(c, WHP_ERR_INVALID_ARG, "bad argument");
+  if (!std::isfinite(beta) || beta <= 0.0) return fail(c, WHP_ERR_OUT_OF_RANGE, "beta must be finite and positive");
+  device_guard dg(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (c->h_out_cap < n_cand) {
+    WHP_CUDA(c, cudaStreamSynchronize(st));
+    dfree(c->d_h_dist); dfree(c->d_h_obj);
+    WHP_CUDA(c, cudaMalloc(&c->d_h_dist, 8 * (size_t)n_cand));
+    WHP_CUDA(c, cudaMalloc(&c->d_h_obj, 8 * (size_t)n_cand));
+    c->h_out_cap = n_cand;
+  }
+  if (c->n_resp_cap < n_cand) {
+    WHP_CUDA(c, cudaStreamSynchronize(st));
+    dfree(c->d_n_resp);
+    WHP_CUDA(c, cudaMalloc(&c->d_n_resp, 4 * (size_t)n_cand * (size_t)c->K));
+    c->n_resp_cap = n_cand;
+  }
+  for (int32_t it = 0; it < n_outer; ++it) {
+    whp_eval_out out{c->d_h_dist, nullptr, c->d_h_obj, nullptr, nullptr, nullptr, nullptr, c->d_n_resp};
+    WHP_CUDA(c, whp_launch_eval(c, d_perms, n_cand, out, st));
+    WHP_CUDA(c, whp_launch_argmin(c, c->d_h_obj, n_cand, c->d_h_idx, c->d_h_val, st));
+    WHP_CUDA(c, whp_launch_nhatc_record(c, c->d_h_idx, c->d_h_dist, c->d_h_obj, it, d_idx_hist,
+                                        d_dist_hist, d_obj_hist, st));
+    WHP_CUDA(c, whp_launch_nhatc_update(c, c->d_n_resp, c->d_h_idx, beta, st));
+  }
+  return WHP_OK;
+}
+
+whp_status whp_get_penalty(whp_ctx* c, double* t, double* v, double* w, void* cuda_stream) {
+  whp_status s = ready(c);
+  if (s != WHP_OK) return s;
+  device_guard dg(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t bytes = sizeof(double) * (size_t)c->K;
+  if (t) WHP_CUDA(c, cudaMemcpyAsync(t, c->d_tvw, bytes, cudaMemcpyDeviceToHost, st));
+  if (v) WHP_CUDA(c, cudaMemcpyAsync(v, c->d_tvw + c->K, bytes, cudaMemcpyDeviceToHost, st));
+  if (w) WHP_CUDA(c, cudaMemcpyAsync(w, c->d_tvw + 2 * (size_t)c->K, bytes, cudaMemcpyDeviceToHost, st));
+  WHP_CUDA(c, cudaStreamSynchronize(st));
+  return WHP_OK;
+}
+
 void whp_destroy(whp_ctx* c) {
   if (!c) return;
   {
@@ -372,7 +429,7 @@ void whp_destroy(whp_ctx* c) {
     cudaDeviceSynchronize();
     free_orders(c);
     dfree(c->d_tvw); dfree(c->d_argmin_part); dfree(c->d_count); dfree(c->d_task);
-    dfree(c->d_h_dist); dfree(c->d_h_obj); dfree(c->d_h_idx); dfree(c->d_h_val);
+    dfree(c->d_h_dist); dfree(c->d_h_obj); dfree(c->d_h_idx); dfree(c->d_h_val); dfree(c->d_n_resp);
     for (int k = 0; k < 2; ++k) {
       if (c->s_copy[k]) cudaStreamDestroy(c->s_copy[k]);
       if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]);

@@ -130,6 +130,9 @@ struct whp_ctx {
   double* d_h_obj = nullptr;
   int64_t h_out_cap = 0;
   int64_t* d_h_idx = nullptr;
+  // NHATC outer loop scratch (whp_nhatc_solve), grow-only
+  int32_t* d_n_resp = nullptr;  // [n_cand][K]
+  int64_t n_resp_cap = 0;
   double* d_h_val = nullptr;
   cudaStream_t s_copy[2] = {nullptr, nullptr};
   cudaStream_t s_exec = nullptr;
@@ -153,5 +156,10 @@ cudaError_t whp_launch_argmin(whp_ctx* c, const double* d_obj, int64_t n, int64_
                               double* d_val, cudaStream_t st);
 cudaError_t whp_launch_apply_swap(whp_ctx* c, int32_t* d_base_perm, int32_t win_start,
                                   int32_t win_len, const int64_t* d_idx, cudaStream_t st);
+cudaError_t whp_launch_nhatc_update(whp_ctx* c, const int32_t* d_resp_rows, const int64_t* d_idx,
+                                    double beta, cudaStream_t st);
+cudaError_t whp_launch_nhatc_record(whp_ctx* c, const int64_t* d_idx, const int64_t* dist,
+                                    const double* obj, int32_t it, int64_t* idx_hist,
+                                    int64_t* dist_hist, double* obj_hist, cudaStream_t st);
 cudaError_t whp_launch_validate(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
                                 cudaStream_t st);

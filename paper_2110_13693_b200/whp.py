@@ -22,7 +22,7 @@ _STATUS = ["WHP_OK", "WHP_ERR_INVALID_ARG", "WHP_ERR_OUT_OF_RANGE", "WHP_ERR_CAP
 SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_candidates",
            "whp_eval_candidates_host", "whp_eval_swaps", "whp_argmin", "whp_apply_swap",
            "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
-           "whp_version"]
+           "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty"]
 
 
 class WhpError(RuntimeError):
@@ -50,6 +50,9 @@ def lib():
         L.whp_argmin.argtypes = [vp, vp, i64, vp, vp, vp]
         L.whp_apply_swap.argtypes = [vp, vp, i32, i32, vp, vp]
         L.whp_validate_perms.argtypes = [vp, vp, i64, vp, vp]
+        L.whp_nhatc_update.argtypes = [vp, vp, vp, C.c_double, vp]
+        L.whp_nhatc_solve.argtypes = [vp, vp, i64, i32, C.c_double, vp, vp, vp, vp]
+        L.whp_get_penalty.argtypes = [vp, vp, vp, vp, vp]
         L.whp_launch_count.argtypes = [vp]
         L.whp_launch_count.restype = i64
         L.whp_destroy.argtypes = [vp]
@@ -183,6 +186,28 @@ class Context:
         import torch
         self._check(lib().whp_apply_swap(self._h, _d(base_perm, torch.int32), win_start, win_len,
                                          _d(idx, torch.int64), _stream(stream)))
+
+    def nhatc_update(self, resp_rows, idx=None, beta=1.0, stream=None):
+        """NEXT-1 (reading N1): v <- v + 2 w^2 (t - r*), w <- beta w; r* = row idx[0] of resp_rows."""
+        import torch
+        self._check(lib().whp_nhatc_update(self._h, _d(resp_rows, torch.int32),
+                                           _d(idx, torch.int64), float(beta), _stream(stream)))
+
+    def nhatc_solve(self, perms, n_outer, beta, idx_hist=None, dist_hist=None, obj_hist=None,
+                    stream=None):
+        """n_outer x {eval_candidates -> argmin -> record -> nhatc_update}, all on the device."""
+        import torch
+        n_cand = perms.shape[0]
+        self._check(lib().whp_nhatc_solve(self._h, _d(perms, torch.int32), n_cand, int(n_outer),
+                                          float(beta), _d(idx_hist, torch.int64),
+                                          _d(dist_hist, torch.int64), _d(obj_hist, torch.float64),
+                                          _stream(stream)))
+
+    def get_penalty(self, stream=None):
+        t, v, w = (np.zeros(self.n_classes, np.float64) for _ in range(3))
+        self._check(lib().whp_get_penalty(self._h, t.ctypes.data, v.ctypes.data, w.ctypes.data,
+                                          _stream(stream)))
+        return t, v, w
 
     def validate_perms(self, perms, stream=None) -> int:
         import torch

@@ -158,3 +158,42 @@ def test_neighbourhood_config_paper_scale(torch_cuda):
         assert one["dist"][0] == dist[it] and one["obj"][0] == val[it]
     assert np.array_equal(perm, perm_end)
     ctx.close()
+
+
+# ---- NEXT-1: NHATC outer loop on the device ---------------------------------------------------
+@pytest.mark.parametrize("name,n_cand,n_outer,beta", [("tiny", 64, 6, 1.5), ("mid", 512, 5, 1.25)])
+def test_nhatc_solve_matches_oracle_loop(torch_cuda, name, n_cand, n_outer, beta):
+    """eval -> argmin -> update, n_outer times with no host round trip: winners, their D and J and
+    the final multipliers equal the oracle's loop bit for bit (rounding order fixed by reading N1)."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem(name)
+    perms = W.perms(0, pb.n_orders, n_cand)
+    ctx = whp.Context.from_problem(pb)
+    idx = torch.zeros(n_outer, dtype=torch.int64, device="cuda")
+    dist = torch.zeros(n_outer, dtype=torch.int64, device="cuda")
+    obj = torch.zeros(n_outer, dtype=torch.float64, device="cuda")
+    ctx.nhatc_solve(torch.from_numpy(perms).cuda(), n_outer, beta, idx, dist, obj)
+    torch.cuda.synchronize()
+    ref = oracle.nhatc_loop(pb, perms, n_outer, beta)
+    assert np.array_equal(idx.cpu().numpy(), ref["idx"])
+    assert np.array_equal(dist.cpu().numpy(), ref["dist"])
+    assert np.array_equal(obj.cpu().numpy(), ref["obj"])
+    t, v, w = ctx.get_penalty()
+    assert np.array_equal(t, pb.t) and np.array_equal(v, ref["v"]) and np.array_equal(w, ref["w"])
+    ctx.close()
+
+
+def test_nhatc_update_single_step(torch_cuda, ):
+    torch = torch_cuda
+    import json, os
+    from paper_2110_13693_b200 import whp
+    g = json.load(open(os.path.join(os.path.dirname(__file__), "golden", "worked_examples.json")))["nhatc_update"]
+    pb = W.make_problem("tiny")
+    ctx = whp.Context.from_problem(pb)
+    ctx.set_penalty(g["t"], g["v"], g["w"])
+    rows = torch.tensor([[9, 9, 9, 9], g["r"]], dtype=torch.int32, device="cuda")
+    ctx.nhatc_update(rows, torch.tensor([1], dtype=torch.int64, device="cuda"), g["beta"])
+    t, v, w = ctx.get_penalty()
+    assert v.tolist() == g["v_new"] and w.tolist() == g["w_new"] and t.tolist() == g["t"]
+    ctx.close()
