@@ -197,6 +197,19 @@ def run_ours(args):
     torch.cuda.synchronize()
     same = bool(np.array_equal(h_obj.numpy(), obj.cpu().numpy()) and e_idx == int(idx.item()))
 
+    # ---- NEXT-1: the NHATC outer loop around the solve, on the device (not part of the step) ---
+    n_outer = 5
+    idx_h = torch.zeros(n_outer, dtype=torch.int64, device=dev)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ctx.nhatc_solve(perms, 1, 1.25, idx_h)  # warm-up (allocates the response scratch)
+    torch.cuda.synchronize()
+    ev0.record()
+    ctx.nhatc_solve(perms, n_outer, 1.25, idx_h)
+    ev1.record()
+    torch.cuda.synchronize()
+    nhatc_ms = ev0.elapsed_time(ev1) / n_outer
+    ctx.set_penalty(pb.t, pb.v, pb.w)  # restore the multipliers
+
     # ---- roofline of the dominant kernel (candidate evaluation) -----------------------------
     bytes_pc = harness.algorithmic_bytes_per_candidate(n, pb.n_items)
     peaks = harness.measured_peaks(ROOT)
@@ -238,6 +251,9 @@ def run_ours(args):
         "config": config_dict(pb, n_cand, world, wl_nb),
         "neighbourhood": {"ms_per_iteration_eval_swaps": s_ms,
                           "neighbours_per_s": nn / (s_ms * 1e-3)},
+        "nhatc_outer_loop": {"ms_per_outer_iteration": nhatc_ms,
+                             "what": "eval 16,384 plans (with responses) -> argmin -> multiplier "
+                                     "update, device only"},
         "roofline": roofline,
         "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": "candidate plans/s",
