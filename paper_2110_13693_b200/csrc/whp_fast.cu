@@ -142,7 +142,7 @@ __device__ __forceinline__ uint32_t recur_word(const uint32_t (&r)[32], uint32_t
     // use up to the loads (it would stall on the shared-memory latency there)
     asm volatile("" : "+r"(ri));
     const uint32_t q = ri & WHP_Q_MASK;
-    const uint32_t e = q + ~room;      // sign bit clear <=> room < q
+    const uint32_t e = q - room - 1u;  // sign bit clear <=> room < q
     rev = __funnelshift_l(e, rev, 1);  // (rev << 1) | (e >> 31)
     room = min(room + (0u - q), C - q);
   }

@@ -268,6 +268,73 @@ def test_tuned_path_word_and_warp_tails(torch_cuda, n_orders, n_cand):
     ctx.close()
 
 
+@pytest.mark.parametrize("name,n_cand", [("tiny", 37), ("mid", 100)])
+def test_outputs_stay_inside_their_buffers(torch_cuda, name, n_cand):
+    """Every caller buffer sits between guard words; no kernel (tuned path, general path, swaps,
+    argmin) may touch a guard (compute-sanitizer is not available on the GPU pool)."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem(name)
+    ctx = whp.Context.from_problem(pb)
+    G = 64
+
+    def guarded(shape, dtype):
+        n = int(np.prod(shape))
+        buf = torch.full((n + 2 * G,), 0x5A, dtype=dtype, device="cuda")
+        return buf, buf[G:G + n].view(*shape)
+
+    perms_np = W.perms(1, pb.n_orders, n_cand)
+    pbuf, perms = guarded((n_cand, pb.n_orders), torch.int32)
+    perms.copy_(torch.from_numpy(perms_np))
+    bufs = {}
+    for key, shape, dt in (("dist", (n_cand,), torch.int64), ("penalty", (n_cand,), torch.float64),
+                           ("obj", (n_cand,), torch.float64), ("n_batches", (n_cand,), torch.int32),
+                           ("batch_hash", (n_cand,), torch.int64),
+                           ("resp", (n_cand, pb.n_classes), torch.int32),
+                           ("batch_of_pos", (n_cand, pb.n_orders), torch.int32),
+                           ("n_distinct", (n_cand,), torch.int32)):
+        bufs[key] = guarded(shape, dt)
+    tuned = {k: v[1] for k, v in bufs.items() if k not in ("batch_of_pos", "n_distinct")}
+    ctx.eval_candidates(perms, **tuned)
+    ctx.eval_candidates(perms, **{k: v[1] for k, v in bufs.items()})
+    Wn = min(12, pb.n_orders)
+    nn = Wn * (Wn - 1) // 2
+    sd, so = guarded((nn,), torch.int64), guarded((nn,), torch.float64)
+    ibuf, idx = guarded((1,), torch.int64)
+    base_buf, base = guarded((pb.n_orders,), torch.int32)
+    base.copy_(perms[0])
+    ctx.eval_swaps(base, 1, Wn, sd[1], so[1])
+    ctx.argmin(so[1], idx)
+    ctx.apply_swap(base, 1, Wn, idx)
+    torch.cuda.synchronize()
+    for name_, (buf, view) in list(bufs.items()) + [("sd", sd), ("so", so), ("idx", (ibuf, idx)),
+                                                     ("base", (base_buf, base)), ("perms", (pbuf, perms))]:
+        guard = torch.full((G,), 0x5A, dtype=buf.dtype, device="cuda")
+        assert torch.equal(buf[:G], guard) and torch.equal(buf[-G:], guard), name_
+    assert np.array_equal(perms.cpu().numpy(), perms_np)
+    ref = oracle.eval_candidates(pb, perms_np, detail=True)
+    assert np.array_equal(bufs["dist"][1].cpu().numpy(), ref["dist"])
+    assert np.array_equal(bufs["resp"][1].cpu().numpy(), ref["resp"])
+    ctx.close()
+
+
+def test_unaligned_permutation_buffer(torch_cuda):
+    """A permutation matrix that starts 4 bytes off a 16-byte boundary cannot be described by a
+    TMA tensor map: the call must still be right (it takes the general path)."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid")
+    ctx = whp.Context.from_problem(pb)
+    perms_np = W.perms(2, pb.n_orders, 50)
+    buf = torch.zeros(50 * pb.n_orders + 8, dtype=torch.int32, device="cuda")
+    perms = buf[1:1 + 50 * pb.n_orders].view(50, pb.n_orders)
+    assert perms.data_ptr() % 16 == 4
+    perms.copy_(torch.from_numpy(perms_np))
+    got, _ = gpu_eval(torch, ctx, perms)
+    assert_parity(got, oracle.eval_candidates(pb, perms_np), pb)
+    ctx.close()
+
+
 def test_api_errors_and_nullable_outputs(torch_cuda):
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
