@@ -11,10 +11,12 @@ from .binding import (  # noqa: F401
     decode_neighbour,
     eval_candidate_batches,
     eval_candidates,
+    eval_legsum,
     eval_swaps,
     nhatc_loop,
     nhatc_update,
     optimal_route,
     penalty,
     swap_trajectory,
+    tour_length,
 )

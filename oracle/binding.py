@@ -34,6 +34,7 @@ def _load():
         _lib.orc_optimal_route.restype = C.c_int64
         _lib.orc_penalty.restype = C.c_double
         _lib.orc_argmin.restype = C.c_int64
+        _lib.orc_tour_length.restype = C.c_int64
     return _lib
 
 
@@ -179,3 +180,24 @@ def nhatc_loop(pb, perms, n_outer: int, beta: float) -> dict:
         pb.v, pb.w = nhatc_update(one["resp"][0], pb.t, pb.v, pb.w, beta)
     hist["v"], hist["w"] = pb.v, pb.w
     return hist
+
+
+def tour_length(geom, locs) -> int:
+    """NEXT-2: depot -> locs in the given order -> depot under D0's walking metric."""
+    locs = _i32(locs)
+    return int(_load().orc_tour_length(C.byref(_geom(geom)), _p(locs), C.c_int32(len(locs))))
+
+
+def eval_legsum(pb, perms) -> np.ndarray:
+    """NEXT-2 (reading N2): summed leg lengths of every plan, carts by next-fit (D2)."""
+    perms = _i32(perms)
+    if perms.ndim == 1:
+        perms = perms[None, :]
+    n_cand = perms.shape[0]
+    out = np.zeros(n_cand, np.int64)
+    g = _geom(pb)
+    keep = (_i32(pb.sku_loc), _i32(pb.order_ptr), _i32(pb.item_sku))
+    _load().orc_eval_legsum(C.byref(g), _p(keep[0]), C.c_int32(pb.n_orders), _p(keep[1]),
+                            _p(keep[2]), C.c_int32(pb.cart_capacity), _p(perms),
+                            C.c_int64(n_cand), _p(out))
+    return out

@@ -312,3 +312,51 @@ void orc_nhatc_update(int32_t K, const int32_t* r, const double* t, double* v, d
     w[k] = beta * w[k];
   }
 }
+
+/* ---- NEXT-2: the paper-literal subproblem 2 — leg sums ---------------------------------------
+ * PAPER.md:125-129 (§5, Eq. 2): min sum d_i with d_i the shortest-path ("Dijkstra") length
+ * between consecutive picking positions a_i, b_i of a picking sequence. DESIGN.md reading N2:
+ * every cart of the plan (D2) leaves the depot, visits its picks in plan order (orders in
+ * sequence, items of an order in CSR order) and returns to the depot; a leg costs D0's walking
+ * metric (Dijkstra's closed form in this layout, see walk()). */
+
+/* one tour: depot -> locs[0] -> ... -> locs[n-1] -> depot */
+int64_t orc_tour_length(const orc_geom* g, const int32_t* locs, int32_t n) {
+  if (n <= 0) return 0;
+  int32_t a = g->depot_aisle;
+  int64_t y = 0, len = 0;
+  for (int32_t i = 0; i < n; i++) {
+    int32_t a2 = loc_aisle(g, locs[i]);
+    int64_t y2 = loc_depth(g, locs[i]);
+    len += walk(g, a, y, a2, y2);
+    a = a2; y = y2;
+  }
+  return len + walk(g, a, y, g->depot_aisle, 0);
+}
+
+/* leg sum of every plan: perms[n_cand][n_orders] -> len[n_cand] */
+int32_t orc_eval_legsum(const orc_geom* g, const int32_t* sku_loc, int32_t n_orders,
+                        const int32_t* order_ptr, const int32_t* item_sku, int32_t C,
+                        const int32_t* perms, int64_t n_cand, int64_t* len) {
+  int32_t n_items = order_ptr[n_orders];
+  int32_t* locs = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n_items > 0 ? n_items : 1));
+  for (int64_t c = 0; c < n_cand; c++) {
+    const int32_t* perm = perms + c * n_orders;
+    int64_t total = 0;
+    int32_t load = 0, n = 0;
+    for (int32_t pos = 0; pos < n_orders; pos++) {
+      int32_t o = perm[pos];
+      int32_t q = order_ptr[o + 1] - order_ptr[o];
+      if (load > 0 && load + q > C) { /* D2: the cart is full, it returns */
+        total += orc_tour_length(g, locs, n);
+        load = 0; n = 0;
+      }
+      for (int32_t it = order_ptr[o]; it < order_ptr[o + 1]; it++) locs[n++] = sku_loc[item_sku[it]];
+      load += q;
+    }
+    total += orc_tour_length(g, locs, n);
+    len[c] = total;
+  }
+  free(locs);
+  return 0;
+}

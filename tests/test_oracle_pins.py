@@ -426,3 +426,48 @@ def test_nhatc_loop_is_eval_argmin_update():
         q.v, q.w = oracle.nhatc_update(out["resp"][i], q.t, q.v, q.w, 1.5)
     assert np.array_equal(h["v"], q.v) and np.array_equal(h["w"], q.w)
     assert np.array_equal(h["w"], pb.w * 1.5 * 1.5 * 1.5)
+
+
+# ---- NEXT-2: leg sums (reading N2) ----------------------------------------------------------------
+def test_legsum_golden(golden):
+    geom = tuple(golden["geometry"][k] for k in
+                 ("n_aisles", "slots_per_side", "slot_pitch", "aisle_spacing", "depot_aisle"))
+    for tour in golden["legsum"]["tours"]:
+        assert oracle.tour_length(geom, tour["locs"]) == tour["len"] == sum(tour["legs"])
+    pb = _golden_problem(golden)
+    plan = next(p for p in golden["plans"] if p["id"] == golden["legsum"]["plan"])
+    assert oracle.eval_legsum(pb, np.array(plan["perm"]))[0] == golden["legsum"]["total"]
+
+
+def test_tour_closed_forms_and_optimal_route_is_the_best_ordering():
+    import itertools
+    geom = (5, 9, 2, 3, 1)  # aisles, slots/side, pitch, spacing, depot aisle
+    S2 = 2 * 9
+    # one pick: out and back = the single-aisle closed form of D4 (m = 1)
+    for loc in (0, 7, 25, 44, 89):
+        a, depth = loc // S2, (loc % 9 + 1) * 2
+        assert oracle.tour_length(geom, [loc]) == 2 * (abs(a - 1) * 3 + depth) == oracle.batch_distance(geom, [loc])
+    # a repeated location adds nothing; a tour and its reverse are equally long
+    assert oracle.tour_length(geom, [7, 7, 30]) == oracle.tour_length(geom, [7, 30])
+    rng = np.random.default_rng(4)
+    for _ in range(30):
+        locs = rng.integers(0, 5 * S2, size=rng.integers(1, 7)).tolist()
+        assert oracle.tour_length(geom, locs) == oracle.tour_length(geom, locs[::-1])
+        # the exhaustive optimum (P3's routine) is the minimum of the tour length over orderings
+        best = min(oracle.tour_length(geom, list(p)) for p in itertools.permutations(locs))
+        assert best == oracle.optimal_route(geom, locs) <= oracle.tour_length(geom, locs)
+
+
+def test_legsum_is_the_sum_of_cart_tours():
+    pb = W.make_problem("tiny")
+    perms = W.perms(0, pb.n_orders, 8)
+    got = oracle.eval_legsum(pb, perms)
+    ref = oracle.eval_candidates(pb, perms, detail=True)
+    for c in range(8):
+        total = 0
+        bop = ref["batch_of_pos"][c]
+        for b in range(ref["n_batches"][c]):
+            locs = [int(pb.sku_loc[s]) for pos in np.nonzero(bop == b)[0]
+                    for s in pb.item_sku[pb.order_ptr[perms[c, pos]]:pb.order_ptr[perms[c, pos] + 1]]]
+            total += oracle.tour_length(pb, locs)
+        assert got[c] == total
