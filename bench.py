@@ -210,6 +210,16 @@ def run_ours(args):
     nhatc_ms = ev0.elapsed_time(ev1) / n_outer
     ctx.set_penalty(pb.t, pb.v, pb.w)  # restore the multipliers
 
+    # ---- NEXT-2: leg sums of the same plans (not part of the step) -----------------------------
+    leg = torch.zeros(n_cand, dtype=torch.int64, device=dev)
+    ctx.eval_legsum(perms, leg)
+    torch.cuda.synchronize()
+    ev0.record()
+    ctx.eval_legsum(perms, leg)
+    ev1.record()
+    torch.cuda.synchronize()
+    legsum_ms = ev0.elapsed_time(ev1)
+
     # ---- roofline of the dominant kernel (candidate evaluation) -----------------------------
     bytes_pc = harness.algorithmic_bytes_per_candidate(n, pb.n_items)
     peaks = harness.measured_peaks(ROOT)
@@ -254,6 +264,8 @@ def run_ours(args):
         "nhatc_outer_loop": {"ms_per_outer_iteration": nhatc_ms,
                              "what": "eval 16,384 plans (with responses) -> argmin -> multiplier "
                                      "update, device only"},
+        "legsum": {"ms": legsum_ms, "plans_per_s": n_cand / (legsum_ms * 1e-3),
+                   "what": "whp_eval_legsum on the same 16,384 plans (paper-literal Eq. 2)"},
         "roofline": roofline,
         "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": "candidate plans/s",

@@ -135,6 +135,15 @@ whp_status whp_nhatc_solve(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,
 /* Current penalty parameters to HOST double[n_classes] each (nullable). Synchronises the stream. */
 whp_status whp_get_penalty(whp_ctx* ctx, double* t, double* v, double* w, void* cuda_stream);
 
+/* ---- NEXT-2: the paper-literal subproblem 2 (§5 Eq. 2: min sum d_i, d_i the
+ * shortest-path length between consecutive picking positions; reading N2 of DESIGN.md) ------ */
+
+/* d_len[c] (DEVICE int64 [n_cand]) = summed leg lengths of plan c: every cart (next-fit, D2)
+ * leaves the depot, visits its picks in plan order and returns; a leg costs D0's walking
+ * metric. d_perms DEVICE int32 [n_cand][n_orders]. Needs whp_load_orders only. */
+whp_status whp_eval_legsum(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
+                           void* cuda_stream);
+
 /* Debug helper: *h_n_bad (host) receives the number of rows of d_perms that are not a
  * permutation of 0..n_orders-1. Synchronises the stream. */
 whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,

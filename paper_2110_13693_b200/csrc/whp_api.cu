@@ -365,6 +365,19 @@ whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t 
   return WHP_OK;
 }
 
+whp_status whp_eval_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
+                           void* cuda_stream) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!c->have_orders) return fail(c, WHP_ERR_STATE, "whp_load_orders has not been called");
+  if (n_cand < 0) return fail(c, WHP_ERR_INVALID_ARG, "n_cand < 0");
+  if (n_cand == 0) return WHP_OK;
+  if (!d_perms || !d_len) return fail(c, WHP_ERR_INVALID_ARG, "null pointer");
+  device_guard dg(c->device);
+  WHP_CUDA(c, whp_launch_legsum(c, d_perms, n_cand, d_len, (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
 whp_status whp_nhatc_update(whp_ctx* c, const int32_t* d_resp_rows, const int64_t* d_idx,
                             double beta, void* cuda_stream) {
   whp_status s = ready(c);

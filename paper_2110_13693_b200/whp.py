@@ -22,7 +22,8 @@ _STATUS = ["WHP_OK", "WHP_ERR_INVALID_ARG", "WHP_ERR_OUT_OF_RANGE", "WHP_ERR_CAP
 SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_candidates",
            "whp_eval_candidates_host", "whp_eval_swaps", "whp_argmin", "whp_apply_swap",
            "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
-           "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty"]
+           "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
+           "whp_eval_legsum"]
 
 
 class WhpError(RuntimeError):
@@ -53,6 +54,7 @@ def lib():
         L.whp_nhatc_update.argtypes = [vp, vp, vp, C.c_double, vp]
         L.whp_nhatc_solve.argtypes = [vp, vp, i64, i32, C.c_double, vp, vp, vp, vp]
         L.whp_get_penalty.argtypes = [vp, vp, vp, vp, vp]
+        L.whp_eval_legsum.argtypes = [vp, vp, i64, vp, vp]
         L.whp_launch_count.argtypes = [vp]
         L.whp_launch_count.restype = i64
         L.whp_destroy.argtypes = [vp]
@@ -186,6 +188,13 @@ class Context:
         import torch
         self._check(lib().whp_apply_swap(self._h, _d(base_perm, torch.int32), win_start, win_len,
                                          _d(idx, torch.int64), _stream(stream)))
+
+    def eval_legsum(self, perms, length, stream=None):
+        """NEXT-2 (reading N2): summed leg lengths of every plan into `length` (CUDA int64)."""
+        import torch
+        n_cand = perms.shape[0] if perms.dim() == 2 else 1
+        self._check(lib().whp_eval_legsum(self._h, _d(perms, torch.int32), n_cand,
+                                          _d(length, torch.int64), _stream(stream)))
 
     def nhatc_update(self, resp_rows, idx=None, beta=1.0, stream=None):
         """NEXT-1 (reading N1): v <- v + 2 w^2 (t - r*), w <- beta w; r* = row idx[0] of resp_rows."""

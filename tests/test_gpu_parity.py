@@ -335,6 +335,34 @@ def test_unaligned_permutation_buffer(torch_cuda):
     ctx.close()
 
 
+@pytest.mark.parametrize("name,n_cand", [("tiny", 64), ("mid", 300)])
+def test_legsum_matches_oracle(torch_cuda, name, n_cand):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem(name)
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perms(0, pb.n_orders, n_cand)
+    out = torch.full((n_cand,), -1, dtype=torch.int64, device="cuda")
+    ctx.eval_legsum(torch.from_numpy(perms).cuda(), out)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), oracle.eval_legsum(pb, perms))
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg", EDGE[:9], ids=lambda c: "-".join(f"{k}{v}" for k, v in c.items()))
+def test_legsum_edge_cases(torch_cuda, cfg):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = _random_problem(13, **cfg)
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perm_rows(5, pb.n_orders, np.arange(40))
+    out = torch.full((40,), -1, dtype=torch.int64, device="cuda")
+    ctx.eval_legsum(torch.from_numpy(perms).cuda(), out)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), oracle.eval_legsum(pb, perms))
+    ctx.close()
+
+
 def test_api_errors_and_nullable_outputs(torch_cuda):
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
