@@ -674,13 +674,86 @@ bool whp_fast_eligible(const whp_ctx* c) {
   return true;
 }
 
+static int32_t fast_bm_pitch(const whp_ctx* c) { return (int32_t)((((c->n_orders + 31) >> 5) + 2 + 3) & ~3); }
+static int32_t fast_cs_pitch(const whp_ctx* c) { return (int32_t)((c->n_orders + 7) & ~7); }
+constexpr int32_t kSsPitch = 32;
+
+// scratch of the tuned paths (grow-only; reallocated when the shape changes)
+static cudaError_t ensure_fast_scratch(whp_ctx* c, int64_t n_cand, int64_t plane_words, cudaStream_t st) {
+  const int32_t bm_pitch = fast_bm_pitch(c), cs_pitch = fast_cs_pitch(c), ss_pitch = kSsPitch;
+  if (c->fast_cap < n_cand || c->fast_pitch != bm_pitch || c->fast_plane_words < plane_words) {
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return e;
+    cudaFree(c->d_bmask); cudaFree(c->d_cstream); cudaFree(c->d_nb); cudaFree(c->d_dist_scratch);
+    cudaFree(c->d_planes); cudaFree(c->d_segstart);
+    c->d_bmask = nullptr; c->d_cstream = nullptr; c->d_nb = nullptr; c->d_dist_scratch = nullptr;
+    c->d_planes = nullptr; c->d_segstart = nullptr;
+    const int64_t cap = n_cand > c->fast_cap ? n_cand : c->fast_cap;
+    const int64_t pw = plane_words > c->fast_plane_words ? plane_words : c->fast_plane_words;
+    c->fast_cap = 0;
+    if ((e = cudaMalloc(&c->d_bmask, 4 * (size_t)cap * bm_pitch)) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&c->d_cstream, 2 * (size_t)cap * cs_pitch + 64)) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&c->d_nb, 4 * (size_t)cap)) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&c->d_dist_scratch, 8 * (size_t)cap)) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&c->d_planes, 4 * (size_t)cap * pw)) != cudaSuccess) return e;
+    if ((e = cudaMalloc(&c->d_segstart, 4 * (size_t)cap * ss_pitch)) != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(c->d_bmask, 0, 4 * (size_t)cap * bm_pitch, st)) != cudaSuccess) return e;
+    c->fast_cap = cap; c->fast_pitch = bm_pitch; c->fast_plane_words = pw;
+  }
+  return cudaSuccess;
+}
+
+// K1 (batch boundaries, cursor stream) and the segment starts of every plan
+static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int S,
+                                              int log2S, int32_t* n_batches_out, cudaStream_t st) {
+  const int32_t bm_pitch = fast_bm_pitch(c), cs_pitch = fast_cs_pitch(c), ss_pitch = kSsPitch;
+  {
+    cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    const size_t smem = bounds_smem_bytes(c);
+    // tensor map over this call's permutation matrix: [n_cand][n_orders] int32, box 32 x 32
+    PFN_cuTensorMapEncodeTiled encode = tensor_map_encoder();
+    if (!encode) return cudaErrorNotSupported;
+    CUtensorMap tmap;
+    const cuuint64_t gdim[2] = {(cuuint64_t)c->n_orders, (cuuint64_t)n_cand};
+    const cuuint64_t gstride[1] = {4ull * (cuuint64_t)c->n_orders};
+    const cuuint32_t box[2] = {32, 32};
+    const cuuint32_t estr[2] = {1, 1};
+    if (encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_INT32, 2, (void*)d_perms, gdim, gstride, box, estr,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+    // tensor map over the cursor stream: [n_cand][cs_pitch] u16, box 32 rows x 64 cursors
+    CUtensorMap tmap_cs;
+    const cuuint64_t cdim[2] = {(cuuint64_t)cs_pitch, (cuuint64_t)n_cand};
+    const cuuint64_t cstride[1] = {2ull * (cuuint64_t)cs_pitch};
+    const cuuint32_t cbox[2] = {64, 32};
+    if (encode(&tmap_cs, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, (void*)c->d_cstream, cdim, cstride, cbox,
+               estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return cudaErrorInvalidValue;
+    cudaFuncSetAttribute(whp_bounds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         c->smem_optin - 1024);
+    const unsigned blocks = (unsigned)((n_cand + kBoundsThreads - 1) / kBoundsThreads);
+    whp_bounds_kernel<<<blocks, kBoundsThreads, smem, st>>>(
+        tmap, tmap_cs, c->d_order_fast, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch, c->d_cstream,
+        cs_pitch);
+    c->launches += 1;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+    whp_segments_kernel<<<(unsigned)((n_cand * 32 + 255) / 256), 256, 0, st>>>(
+        c->d_bmask, bm_pitch, c->n_orders, n_cand, S, log2S, c->d_nb, n_batches_out,
+        c->d_segstart, ss_pitch);
+    c->launches += 1;
+    if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  }
+  return cudaSuccess;
+}
+
 cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
                                  const whp_eval_out& out, cudaStream_t st) {
   const whp_tables T = whp_make_tables(c);
   const int64_t nb_ub = nb_upper_bound(c);
-  const int32_t bm_pitch = (int32_t)((((c->n_orders + 31) >> 5) + 2 + 3) & ~3);
-  const int32_t cs_pitch = (int32_t)((c->n_orders + 7) & ~7);
-  const int32_t ss_pitch = 32;
+  const int32_t bm_pitch = fast_bm_pitch(c), cs_pitch = fast_cs_pitch(c), ss_pitch = kSsPitch;
   const int KW = c->K <= 32 ? 1 : c->K <= 64 ? 2 : c->K <= 128 ? 4 : c->K <= 224 ? 7 : 8;
   const int aw_words = (c->g.n_aisles + 31) / 32;
   // cursor ring: a batch of C orders touches at most (C+14)/8 chunks of 8 cursors, and the
@@ -719,67 +792,10 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   const int64_t worst = 2ll * c->g.aisle_spacing * c->g.n_aisles +
                         ((int64_t)c->g.n_aisles + 2) * c->g.aisle_len;
   const int fits32 = worst < (1ll << 31) ? 1 : 0;
-  // scratch (grow-only; reallocated when the shape changes)
-  const int64_t plane_words = (int64_t)kPlaneRow * KW;
-  if (c->fast_cap < n_cand || c->fast_pitch != bm_pitch || c->fast_plane_words < plane_words) {
-    cudaError_t e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return e;
-    cudaFree(c->d_bmask); cudaFree(c->d_cstream); cudaFree(c->d_nb); cudaFree(c->d_dist_scratch);
-    cudaFree(c->d_planes); cudaFree(c->d_segstart);
-    c->d_bmask = nullptr; c->d_cstream = nullptr; c->d_nb = nullptr; c->d_dist_scratch = nullptr;
-    c->d_planes = nullptr; c->d_segstart = nullptr;
-    const int64_t cap = n_cand > c->fast_cap ? n_cand : c->fast_cap;
-    const int64_t pw = plane_words > c->fast_plane_words ? plane_words : c->fast_plane_words;
-    c->fast_cap = 0;
-    if ((e = cudaMalloc(&c->d_bmask, 4 * (size_t)cap * bm_pitch)) != cudaSuccess) return e;
-    if ((e = cudaMalloc(&c->d_cstream, 2 * (size_t)cap * cs_pitch + 64)) != cudaSuccess) return e;
-    if ((e = cudaMalloc(&c->d_nb, 4 * (size_t)cap)) != cudaSuccess) return e;
-    if ((e = cudaMalloc(&c->d_dist_scratch, 8 * (size_t)cap)) != cudaSuccess) return e;
-    if ((e = cudaMalloc(&c->d_planes, 4 * (size_t)cap * pw)) != cudaSuccess) return e;
-    if ((e = cudaMalloc(&c->d_segstart, 4 * (size_t)cap * ss_pitch)) != cudaSuccess) return e;
-    if ((e = cudaMemsetAsync(c->d_bmask, 0, 4 * (size_t)cap * bm_pitch, st)) != cudaSuccess) return e;
-    c->fast_cap = cap; c->fast_pitch = bm_pitch; c->fast_plane_words = pw;
-  }
-  // K1
-  {
-    cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
-    if (e != cudaSuccess) return e;
-    const size_t smem = bounds_smem_bytes(c);
-    // tensor map over this call's permutation matrix: [n_cand][n_orders] int32, box 32 x 32
-    PFN_cuTensorMapEncodeTiled encode = tensor_map_encoder();
-    if (!encode) return cudaErrorNotSupported;
-    CUtensorMap tmap;
-    const cuuint64_t gdim[2] = {(cuuint64_t)c->n_orders, (cuuint64_t)n_cand};
-    const cuuint64_t gstride[1] = {4ull * (cuuint64_t)c->n_orders};
-    const cuuint32_t box[2] = {32, 32};
-    const cuuint32_t estr[2] = {1, 1};
-    if (encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_INT32, 2, (void*)d_perms, gdim, gstride, box, estr,
-               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-      return cudaErrorInvalidValue;
-    // tensor map over the cursor stream: [n_cand][cs_pitch] u16, box 32 rows x 64 cursors
-    CUtensorMap tmap_cs;
-    const cuuint64_t cdim[2] = {(cuuint64_t)cs_pitch, (cuuint64_t)n_cand};
-    const cuuint64_t cstride[1] = {2ull * (cuuint64_t)cs_pitch};
-    const cuuint32_t cbox[2] = {64, 32};
-    if (encode(&tmap_cs, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, (void*)c->d_cstream, cdim, cstride, cbox,
-               estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-      return cudaErrorInvalidValue;
-    cudaFuncSetAttribute(whp_bounds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                         c->smem_optin - 1024);
-    const unsigned blocks = (unsigned)((n_cand + kBoundsThreads - 1) / kBoundsThreads);
-    whp_bounds_kernel<<<blocks, kBoundsThreads, smem, st>>>(
-        tmap, tmap_cs, c->d_order_fast, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch, c->d_cstream,
-        cs_pitch);
-    c->launches += 1;
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
-    whp_segments_kernel<<<(unsigned)((n_cand * 32 + 255) / 256), 256, 0, st>>>(
-        c->d_bmask, bm_pitch, c->n_orders, n_cand, S, log2S, c->d_nb, out.n_batches,
-        c->d_segstart, ss_pitch);
-    c->launches += 1;
-    if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  }
+  cudaError_t e0 = ensure_fast_scratch(c, n_cand, (int64_t)kPlaneRow * KW, st);
+  if (e0 != cudaSuccess) return e0;
+  if ((e0 = launch_bounds_and_segments(c, d_perms, n_cand, S, log2S, out.n_batches, st)) != cudaSuccess)
+    return e0;
   // K2
   {
     sets_params P;
