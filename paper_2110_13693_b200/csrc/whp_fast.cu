@@ -595,6 +595,165 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
   }
 }
 
+// ------------------------------------------------------------------------------------------ KL
+// NEXT-2 tuned: leg sums (reading N2) on the K1 outputs. Same decomposition as K2 — one lane per
+// (plan, segment), one pick per branch-free step — but a step only adds the leg from the previous
+// pick (D0's walking metric); there are no sets. A cart starts and ends at the depot; a lane
+// that has finished its cart stays on its last pick (a zero leg).
+template <bool SMEM_TABLES>
+__global__ void __launch_bounds__(1024, 1)
+whp_legs_kernel(const whp_tables T, const sets_params P, const uint32_t* __restrict__ pick_fast,
+                const uint16_t* __restrict__ cstream, const uint32_t* __restrict__ bmask,
+                const int32_t* __restrict__ nb_scratch, const int32_t* __restrict__ segstart,
+                int64_t n_cand, int64_t* __restrict__ len_out,
+                unsigned long long* __restrict__ task_counter) {
+  extern __shared__ __align__(16) uint32_t smem[];
+  uint32_t* priv = smem;
+  uint32_t pick_base = 0;
+  if (SMEM_TABLES) {
+    for (int i = threadIdx.x; i < P.n_items_pad; i += blockDim.x) smem[i] = __ldg(pick_fast + i);
+    pick_base = smem_u32(smem);
+    priv = smem + ((P.n_items_pad + 31) & ~31);
+    __syncthreads();
+  }
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int ring_stride = P.ring_mask + 1 + 16;
+  const uint32_t ringbase = smem_u32(priv) + (warp * 32 + lane) * ring_stride;
+  uint32_t pb;
+  asm volatile("mov.u32 %0, %1;" : "=r"(pb) : "r"(pick_base));
+  const int chunks = (P.ring_mask + 1) >> 4;
+  const int Cmax = T.C;
+  const int n8 = P.cs_pitch >> 3;
+  const int32_t a0 = T.g.depot_aisle;
+  const int64_t A2 = 2 * T.g.aisle_len, Psp = T.g.aisle_spacing, pitch = T.g.slot_pitch;
+
+  __shared__ unsigned long long s_task[32];
+  for (;;) {
+    if (lane == 0) s_task[warp] = atomicAdd(task_counter, 1ull);
+    __syncwarp();
+    const int64_t task = (int64_t)s_task[warp];
+    __syncwarp();
+    if (task >= P.n_tasks) break;
+    const int64_t unit = task * 32 + lane;
+    const int64_t cand_raw = unit >> P.log2S;
+    const int seg = (int)(unit & (P.S - 1));
+    const bool have = cand_raw < n_cand;
+    const int64_t cand = have ? cand_raw : n_cand - 1;
+    int nbseg = 0;
+    if (have) {
+      const int nb = __ldg(nb_scratch + cand);
+      const int b_lo = (int)((int64_t)seg * nb >> P.log2S);
+      nbseg = (int)((int64_t)(seg + 1) * nb >> P.log2S) - b_lo;
+    }
+    const int nbmax = __reduce_max_sync(WHP_FULL, nbseg);
+    const uint32_t* __restrict__ bm = bmask + cand * P.bm_pitch;
+    int p = __ldg(segstart + cand * P.ss_pitch + seg);
+    int wi = p >> 5;
+    uint32_t bw = __ldg(bm + wi) & (WHP_FULL << (p & 31));
+    uint32_t bw_next = __ldg(bm + min(wi + 1, P.bm_pitch - 1));
+    const uint4* __restrict__ cs = reinterpret_cast<const uint4*>(cstream + cand * P.cs_pitch);
+    int lo_prev;
+    {
+      const int c0 = p >> 3;
+      for (int k = 0; k < chunks; ++k)
+        cp_async16(ringbase + (((c0 + k) << 4) & P.ring_mask), cs + min(c0 + k, n8 - 1));
+      cp_async_commit();
+      lo_prev = c0 - chunks;
+    }
+    int64_t L = 0;
+    for (int j = 0; j < nbmax; ++j) {
+      int left = 0;
+      const int p0 = p;
+      if (j < nbseg) {
+        bw &= bw - 1;
+        while (bw == 0) {
+          ++wi;
+          bw = bw_next;
+          bw_next = __ldg(bm + min(wi + 1, P.bm_pitch - 1));
+        }
+        const int pe = 32 * wi + __ffs(bw) - 1;
+        left = pe - p;
+        p = pe;
+      }
+      const bool live = left > 0;
+      if (live && (p >> 3) >= lo_prev + chunks) cp_async_wait<0>(); else cp_async_wait<1>();
+      uint32_t v = live ? 2u * (uint32_t)p0 : 0u;
+      const uint32_t v_end = live ? 2u * (uint32_t)p : 0u;
+      uint32_t cur;
+      if (live) {
+        const uint32_t c16 = lds16(ringbase + (v & P.ring_mask));
+        cur = SMEM_TABLES ? pb + 8 * c16 : 2 * c16;
+        v += 2;
+      } else {
+        cur = SMEM_TABLES ? pb : 0u;
+      }
+      uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));
+      uint32_t rec = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
+      // the cart sets out from the depot
+      int32_t pa = a0;
+      int64_t py = 0, Lb = 0;
+      uint32_t Lb32 = 0;
+      int32_t py32 = 0;
+#pragma unroll 2
+      for (int t = 0; t < Cmax; ++t) {
+        const uint32_t first_of_next = SMEM_TABLES ? pb + 8 * n_c16 : 2 * n_c16;
+        const bool last = (int32_t)(rec << 26) < 0;
+        const bool more = last && (v != v_end);
+        uint32_t nxt = last ? cur : cur + (SMEM_TABLES ? 4u : 1u);
+        nxt = more ? first_of_next : nxt;
+        v = more ? v + 2 : v;
+        lds16_if(n_c16, ringbase + (v & P.ring_mask), more);
+        cur = nxt;
+        const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
+        // ---- the leg from the previous point to this pick
+        const int32_t a = (int32_t)WHP_FAST_AISLE(rec);
+        if (P.fits32) {
+          const int32_t y = (int32_t)WHP_FAST_SLOT1(rec) * (int32_t)pitch;
+          const int32_t da = abs(a - pa);
+          const int32_t front = y + py32, back = (int32_t)A2 - front;
+          const int32_t cross = da * (int32_t)Psp + min(front, back);
+          Lb32 += (uint32_t)(da == 0 ? abs(y - py32) : cross);
+          py32 = y;
+        } else {
+          const int64_t y = (int64_t)WHP_FAST_SLOT1(rec) * pitch;
+          const int64_t da = llabs((int64_t)a - pa);
+          const int64_t front = y + py, back = A2 - front;
+          Lb += da == 0 ? llabs(y - py) : da * Psp + (front < back ? front : back);
+          py = y;
+        }
+        pa = a;
+        rec = rec_next;
+      }
+      {
+        const int nf = live ? (p >> 3) - (p0 >> 3) : 0;
+        const int nfmax = __reduce_max_sync(WHP_FULL, nf);
+        for (int i = 0; i < nfmax; ++i)
+          if (i < nf) {
+            const int c = (p0 >> 3) + i;
+            cp_async16(ringbase + ((c << 4) & P.ring_mask), cs + min(c + chunks, n8 - 1));
+          }
+        cp_async_commit();
+        if (live) lo_prev = p0 >> 3;
+      }
+      if (live) {  // the way home, and the cart's total (a lane without a cart walked a dummy)
+        if (P.fits32) {
+          const int32_t da = abs(pa - a0);
+          L += (int64_t)Lb32 + (da == 0 ? py32 : da * (int32_t)Psp + py32);
+        } else {
+          const int64_t da = llabs((int64_t)pa - a0);
+          L += Lb + (da == 0 ? py : da * Psp + py);
+        }
+      }
+    }
+    cp_async_wait<0>();
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1)
+      if (o < P.S) L += __shfl_xor_sync(WHP_FULL, L, o);
+    if (have && seg == 0) len_out[cand] = L;
+    __syncwarp();
+  }
+}
+
 // ------------------------------------------------------------------------------------------ K3
 // one warp per candidate; lane l owns classes l, l+32, ... in ascending order — exactly the
 // canonical 32-lane accumulation of D6.
@@ -851,4 +1010,48 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
     return cudaGetLastError();
   }
   return cudaSuccess;
+}
+
+// NEXT-2 on the tuned infrastructure: K1 + segments, then the leg kernel
+cudaError_t whp_launch_legsum_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
+                                   cudaStream_t st) {
+  const whp_tables T = whp_make_tables(c);
+  const int64_t nb_ub = nb_upper_bound(c);
+  const int ring_bytes = ((c->C + 14) / 8 + 1 <= 8) ? 128 : 256;
+  const size_t table_bytes = 4 * (((size_t)c->n_items_pad + 31) & ~(size_t)31);
+  const size_t priv_per_warp = 32 * (size_t)(ring_bytes + 16);
+  const size_t smem_max = (size_t)c->smem_optin - 1024;
+  const bool smem_tables = table_bytes + 4 * priv_per_warp <= smem_max;
+  int warps = (int)((smem_max - (smem_tables ? table_bytes : 0)) / priv_per_warp);
+  if (warps > 32) warps = 32;
+  if (warps < 1) return cudaErrorInvalidConfiguration;
+  int S = 1;
+  while (S < 32 && n_cand * S < 4ll * c->num_sms * warps * 32) S <<= 1;
+  int log2S = 0;
+  while ((1 << log2S) < S) ++log2S;
+  (void)nb_ub;
+  // a cart's legs in 32 bits: at most C + 1 legs, each below spacing * aisles + 2 * aisle length
+  const int64_t worst = ((int64_t)c->C + 2) * ((int64_t)c->g.aisle_spacing * c->g.n_aisles + 2 * c->g.aisle_len);
+  cudaError_t e = ensure_fast_scratch(c, n_cand, 0, st);
+  if (e != cudaSuccess) return e;
+  if ((e = launch_bounds_and_segments(c, d_perms, n_cand, S, log2S, nullptr, st)) != cudaSuccess) return e;
+  sets_params P{};
+  P.S = S; P.log2S = log2S; P.ring_mask = ring_bytes - 1;
+  P.bm_pitch = fast_bm_pitch(c); P.cs_pitch = fast_cs_pitch(c); P.ss_pitch = kSsPitch;
+  P.n_items_pad = c->n_items_pad; P.fits32 = worst < (1ll << 31) ? 1 : 0;
+  P.n_tasks = (n_cand * S + 31) / 32;
+  int64_t blocks = (P.n_tasks + warps - 1) / warps;
+  if (blocks > c->num_sms) blocks = c->num_sms;
+  const size_t smem = (smem_tables ? table_bytes : 0) + priv_per_warp * warps;
+  if (smem_tables) {
+    cudaFuncSetAttribute(whp_legs_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+    whp_legs_kernel<true><<<(unsigned)blocks, warps * 32, smem, st>>>(
+        T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand, d_len, c->d_task);
+  } else {
+    cudaFuncSetAttribute(whp_legs_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+    whp_legs_kernel<false><<<(unsigned)blocks, warps * 32, smem, st>>>(
+        T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand, d_len, c->d_task);
+  }
+  c->launches += 1;
+  return cudaGetLastError();
 }

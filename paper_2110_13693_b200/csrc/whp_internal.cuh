@@ -161,6 +161,8 @@ cudaError_t whp_launch_nhatc_update(whp_ctx* c, const int32_t* d_resp_rows, cons
 cudaError_t whp_launch_nhatc_record(whp_ctx* c, const int64_t* d_idx, const int64_t* dist,
                                     const double* obj, int32_t it, int64_t* idx_hist,
                                     int64_t* dist_hist, double* obj_hist, cudaStream_t st);
+cudaError_t whp_launch_legsum_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
+                                   cudaStream_t st);
 cudaError_t whp_launch_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                               cudaStream_t st);
 cudaError_t whp_launch_validate(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,

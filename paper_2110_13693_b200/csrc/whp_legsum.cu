@@ -7,6 +7,8 @@
 // chase give the cart boundaries; a lane sums the legs inside its order and the leg that
 // enters it (from the previous order's last pick, or from the depot when it opens a cart, plus
 // the previous cart's way home); a shuffle reduction adds the lanes.
+#include <cstdlib>
+
 #include "whp_walk.cuh"
 
 namespace {
@@ -104,6 +106,9 @@ whp_legsum_kernel(const whp_tables T, const int32_t* __restrict__ perms, int64_t
 
 cudaError_t whp_launch_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                               cudaStream_t st) {
+  // shapes the tuned path covers (and a 16-byte aligned matrix for its TMA tensor map)
+  if (whp_fast_eligible(c) && ((uintptr_t)d_perms & 15u) == 0 && getenv("WHP_FORCE_GENERAL") == nullptr)
+    return whp_launch_legsum_fast(c, d_perms, n_cand, d_len, st);
   const whp_tables T = whp_make_tables(c);
   int64_t blocks = (n_cand + kLegWarps - 1) / kLegWarps;
   const int64_t cap = (int64_t)c->num_sms * 64;
