@@ -15,6 +15,8 @@
 //               (from there on both plans are identical), or at the end.
 //               D and r are patched: minus the replaced base batches (prefix differences),
 //               plus the new ones.
+#include <cstdlib>
+
 #include "whp_walk.cuh"
 
 namespace {
@@ -551,7 +553,8 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
   // region of tabulated hypothetical batches: from two cart lengths before the window (the
   // rewalk may start one batch early) to a margin after it (until the boundaries resynchronise;
   // beyond the margin a neighbour scores its batches from their picks)
-  const int64_t margin = 16ll * c->C > 512 ? 16ll * c->C : 512;
+  int64_t margin = 16ll * c->C > 512 ? 16ll * c->C : 512;
+  if (const char* m = getenv("WHP_SWAP_MARGIN")) { const int v = atoi(m); if (v >= 0) margin = v; }  // tests: force the fallbacks
   const int32_t rlo = (int32_t)((int64_t)win_start - 2ll * c->C > 0 ? (int64_t)win_start - 2ll * c->C : 0);
   const int32_t rhi = (int32_t)((int64_t)win_start + win_len + margin < c->n_orders
                                     ? (int64_t)win_start + win_len + margin : c->n_orders);

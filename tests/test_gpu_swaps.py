@@ -66,6 +66,43 @@ def test_swaps_match_oracle_every_neighbour(torch_cuda, name, s, Wn):
     ctx.close()
 
 
+def test_swaps_full_length_window(torch_cuda):
+    """NEXT-4 groundwork: the window may be the whole plan (all n(n-1)/2 swaps); positions beyond
+    the staged region take the global-memory path of the look-up tables."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid", n_orders=300)
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(3, pb.n_orders)
+    d, o = gpu_swaps(torch, ctx, torch.from_numpy(base).cuda(), 0, pb.n_orders)
+    ref = oracle.eval_swaps(pb, base, 0, pb.n_orders)
+    assert np.array_equal(d.cpu().numpy(), ref["dist"])
+    assert np.array_equal(o.cpu().numpy(), ref["obj"])
+    ctx.close()
+
+
+@pytest.mark.parametrize("margin", ["0", "7", "40"])
+def test_swaps_chains_that_leave_the_tabulated_region(torch_cuda, margin):
+    """The chain sums cover the window plus a margin; with a tiny margin most chains leave the
+    region before they meet the base plan and the neighbour kernel must fall back to scoring
+    batch by batch — with the same results."""
+    import os
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid")
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(1, pb.n_orders)
+    ref = oracle.eval_swaps(pb, base, 60, 36)
+    os.environ["WHP_SWAP_MARGIN"] = margin
+    try:
+        d, o = gpu_swaps(torch, ctx, torch.from_numpy(base).cuda(), 60, 36)
+    finally:
+        os.environ.pop("WHP_SWAP_MARGIN")
+    assert np.array_equal(d.cpu().numpy(), ref["dist"])
+    assert np.array_equal(o.cpu().numpy(), ref["obj"])
+    ctx.close()
+
+
 def test_smaller_opening_order_slips_into_previous_cart(torch_cuda):
     """q = [2,1,3,1], C = 4: swapping positions 2 and 3 (both in the second batch) lets the
     1-item order join the first cart — the incremental evaluator must restart one batch early."""
