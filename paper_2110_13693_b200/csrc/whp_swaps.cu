@@ -167,19 +167,13 @@ __global__ void __launch_bounds__(kBaseThreads)
 whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
                       const whp_base_tables B, int smem_tables) {
   extern __shared__ __align__(16) uint8_t dyn[];
-  __shared__ warp_sets sets_all[kBaseThreads / 32];
-  __shared__ int32_t s_resp[WHP_MAX_CLASSES];
-  __shared__ int64_t s_scan64[33];
   __shared__ int32_t s_scan32[33];
   __shared__ int32_t s_nb;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x;
   const int32_t n = T.n_orders;
   // item-count prefix and "next batch start" tables: shared memory when they fit
   int32_t* pre = smem_tables ? reinterpret_cast<int32_t*>(dyn) : B.pre;
   int32_t* nxt = smem_tables ? reinterpret_cast<int32_t*>(dyn) + (n + 1) : B.nxt;
-  sets_all[warp].amask[lane] = 0;
-  if (lane < 8) sets_all[warp].cmask[lane] = 0;
-  for (int k = tid; k < WHP_MAX_CLASSES; k += kBaseThreads) s_resp[k] = 0;
 
   // ---- A: order record of every position; exclusive prefix of the item counts
   int32_t carry = 0;
@@ -209,8 +203,45 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
   }
   __syncthreads();
 
-  // ---- C: one thread chases the boundaries
-  if (tid == 0) {
+  // ---- C: the base boundaries = the positions reachable from 0 along nxt
+  if (smem_tables == 2) {
+    // pointer doubling: after round k, J = nxt^(2^(k+1)) and the marked positions are those at
+    // fewer than 2^(k+1) hops from 0; then a block scan ranks the marks (bstart, bop)
+    int32_t* J0 = reinterpret_cast<int32_t*>(dyn) + (2 * n + 1);
+    int32_t* J1 = J0 + n;
+    int32_t* mark = J1 + n;
+    for (int32_t p = tid; p < n; p += kBaseThreads) { J0[p] = nxt[p]; mark[p] = p == 0; }
+    __syncthreads();
+    int32_t* J = J0;
+    int32_t* Jn = J1;
+    for (;;) {
+      const bool done = J[0] >= n;  // 2^k hops from 0 leave the plan: every start is marked
+      for (int32_t p = tid; p < n; p += kBaseThreads)
+        if (mark[p] == 1) { const int32_t t = J[p]; if (t < n && mark[t] == 0) mark[t] = 2; }
+      __syncthreads();
+      for (int32_t p = tid; p < n; p += kBaseThreads) {
+        if (mark[p] == 2) mark[p] = 1;
+        const int32_t t = J[p];
+        Jn[p] = t < n ? J[t] : n;
+      }
+      __syncthreads();
+      if (done) break;
+      int32_t* tmp = J; J = Jn; Jn = tmp;
+    }
+    int32_t carry_b = 0;
+    for (int32_t p0 = 0; p0 < n; p0 += kBaseThreads) {
+      const int32_t p = p0 + tid;
+      const int32_t mk = (p < n) ? mark[p] : 0;
+      int32_t tot;
+      const int32_t ex = block_excl_scan<int32_t>(mk, s_scan32, tot);
+      if (p < n) {
+        if (mk) B.bstart[carry_b + ex] = p;
+        B.bop[p] = carry_b + ex + mk - 1;
+      }
+      carry_b += tot;
+    }
+    if (tid == 0) { B.bstart[carry_b] = n; s_nb = carry_b; }
+  } else if (tid == 0) {  // one thread chases the boundaries
     int32_t b = 0;
     for (int32_t p = 0; p < n; p = nxt[p]) B.bstart[b++] = p;
     B.bstart[b] = n;
@@ -219,52 +250,73 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
   __syncthreads();
   const int32_t nb = s_nb;
 
-  // ---- D: one warp per batch
-  swap_seq q{B.pre, B.orec, pre, nullptr, 0, smem_tables ? (uint32_t)(n + 1) : 0u, 0u, -1, -1, 0};
-  warp_sets* sets = &sets_all[warp];
-  const int KW = (T.K + 31) >> 5;
-  for (int32_t b = warp; b < nb; b += kBaseThreads / 32) {
-    const int32_t s = B.bstart[b], e = B.bstart[b + 1];
-    const int64_t dist = score_batch(T, sets, q, s, e);
-    for (int32_t p = s + lane; p < e; p += 32) B.bop[p] = b;
-    if (lane == 0) B.bdist[b] = dist;
-    if (lane < 8) {
-      const uint32_t cm = sets->cmask[lane];
-      B.bclass[(int64_t)b * 8 + lane] = cm;
-      sets->cmask[lane] = 0;
-    }
-    __syncwarp();
-  }
-  __syncthreads();
+  if (tid == 0) B.totals[1] = nb;
+}
 
+// Second half of the base pass, after whp_swaps_prep_kernel has scored the base batches
+// (dist_at / cls_at at their start positions): prefix of the batch lengths, class-count prefix,
+// base D, phi, J. One block.
+__global__ void __launch_bounds__(kBaseThreads)
+whp_swaps_base2_kernel(const whp_tables T, const whp_base_tables B) {
+  __shared__ int32_t s_resp[WHP_MAX_CLASSES];
+  __shared__ int64_t s_scan64[33];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int32_t nb = (int32_t)B.totals[1];
+  const int KW = (T.K + 31) >> 5;
+  for (int k = tid; k < WHP_MAX_CLASSES; k += kBaseThreads) s_resp[k] = 0;
   // ---- E: exclusive prefix of the batch lengths (bdist[nb] = D_base), class-count prefix
   int64_t carry64 = 0;
   for (int32_t b0 = 0; b0 <= nb; b0 += kBaseThreads) {
     const int32_t b = b0 + tid;
-    const int64_t x = (b < nb) ? B.bdist[b] : 0;
+    const int64_t x = (b < nb) ? B.dist_at[B.bstart[b]] : 0;
     int64_t tot;
     const int64_t ex = block_excl_scan<int64_t>(x, s_scan64, tot);
     if (b <= nb) B.bdist[b] = carry64 + ex;
     carry64 += tot;
   }
-  // rpre[b][k] = number of batches before b that visit class k. Warp w owns class word w, its
-  // lane j class 32w+j: a running count over the batches, one coalesced row store per batch.
-  if (warp < KW) {
-    const int w = warp;
-    const bool mine = 32 * w + lane < T.K;
-    int32_t cnt = 0;
-    int32_t* __restrict__ row = B.rpre + 32 * w + lane;
-    if (mine) row[0] = 0;
-    for (int32_t b0 = 0; b0 < nb; b0 += 32) {
-      const int32_t b = b0 + lane;
-      const uint32_t word = (b < nb) ? B.bclass[(int64_t)b * 8 + w] : 0u;
-      const int nbb = min(32, nb - b0);
-      for (int bb = 0; bb < nbb; ++bb) {
-        cnt += (int32_t)((__shfl_sync(WHP_FULL, word, bb) >> lane) & 1u);
-        if (mine) row[(int64_t)(b0 + bb + 1) * T.K] = cnt;
-      }
+  // rpre[b][k] = number of batches before b that visit class k, in three steps over chunks of
+  // 32 batches: per (class word, chunk) the chunk's visit totals (32 ballots), a running sum of
+  // the totals over the chunks per class, then a running count inside every chunk with one
+  // coalesced row store per batch.
+  const int32_t nchunks = (nb + 31) >> 5;
+  for (int32_t task = warp; task < KW * nchunks; task += kBaseThreads / 32) {
+    const int w = task % KW, c = task / KW;
+    const int32_t b = 32 * c + lane;
+    const uint32_t word = (b < nb) ? B.cls_at[(int64_t)B.bstart[b] * 8 + w] : 0u;
+    int32_t tot = 0;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) {
+      const int32_t pc = __popc(__ballot_sync(WHP_FULL, (word >> j) & 1u));
+      if (lane == j) tot = pc;
     }
-    if (mine) { B.resp[32 * w + lane] = cnt; s_resp[32 * w + lane] = cnt; }
+    // parked in row 32c+1 (rewritten in the last step)
+    if (32 * w + lane < T.K) B.rpre[(int64_t)(32 * c + 1) * T.K + 32 * w + lane] = tot;
+  }
+  __syncthreads();
+  for (int k = tid; k < T.K; k += kBaseThreads) {
+    int32_t run = 0;
+    for (int32_t c = 0; c < nchunks; ++c) {
+      const int32_t t = B.rpre[(int64_t)(32 * c + 1) * T.K + k];
+      B.rpre[(int64_t)(32 * c) * T.K + k] = run;
+      run += t;
+    }
+    if (nchunks == 0) B.rpre[k] = 0;
+    B.resp[k] = run;
+    s_resp[k] = run;
+  }
+  __syncthreads();
+  for (int32_t task = warp; task < KW * nchunks; task += kBaseThreads / 32) {
+    const int w = task % KW, c = task / KW;
+    const int32_t b = 32 * c + lane;
+    const uint32_t word = (b < nb) ? B.cls_at[(int64_t)B.bstart[b] * 8 + w] : 0u;
+    const bool mine = 32 * w + lane < T.K;
+    int32_t* __restrict__ row = B.rpre + 32 * w + lane;
+    int32_t cnt = mine ? row[(int64_t)(32 * c) * T.K] : 0;
+    const int nbb = min(32, nb - 32 * c);
+    for (int bb = 0; bb < nbb; ++bb) {
+      cnt += (int32_t)((__shfl_sync(WHP_FULL, word, bb) >> lane) & 1u);
+      if (mine) row[(int64_t)(32 * c + bb + 1) * T.K] = cnt;
+    }
   }
   __syncthreads();
   if (warp == 0) {
@@ -274,7 +326,6 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
     const double phi = penalty_regs(T, r);
     if (lane == 0) {
       B.totals[0] = carry64;
-      B.totals[1] = nb;
       B.ftotals[0] = phi;
       B.ftotals[1] = __dadd_rn((double)carry64, phi);
     }
@@ -296,8 +347,17 @@ whp_swaps_prep_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
   sets->amask[lane] = 0;
   if (lane < 8) sets->cmask[lane] = 0;
   __syncwarp();
-  const int32_t p = rlo + blockIdx.x * kPrepWarps + warp;
-  if (p >= rhi) return;
+  // warps 0 .. rows-1: the region positions; the others: the base batches (their starts)
+  const int32_t g = blockIdx.x * kPrepWarps + warp;
+  int32_t p;
+  if (g < rhi - rlo) {
+    p = rlo + g;
+  } else {
+    const int32_t b = g - (rhi - rlo);
+    if (b >= (int32_t)B.totals[1]) return;
+    p = B.bstart[b];
+    if (p >= rlo && p < rhi) return;  // scored as a region position
+  }
   swap_seq q{B.pre, B.orec, nullptr, nullptr, 0, 0u, 0u, -1, -1, 0};
   const int64_t dist = score_batch(T, sets, q, p, B.nxt[p]);
   if (lane == 0) B.dist_at[p] = dist;
@@ -540,8 +600,14 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
 cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                              int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st) {
   const whp_tables T = whp_make_tables(c);
-  const size_t need = 4 * (2 * (size_t)c->n_orders + 1);
-  const int smem_tables = need + 12 * 1024 <= (size_t)c->smem_optin ? 1 : 0;
+  // shared-memory tables of the base pass: pre + nxt, and (mode 2) three more arrays for the
+  // pointer doubling that finds the base boundaries
+  size_t need = 4 * (5 * (size_t)c->n_orders + 1);
+  int smem_tables = 2;
+  if (need + 12 * 1024 > (size_t)c->smem_optin) {
+    need = 4 * (2 * (size_t)c->n_orders + 1);
+    smem_tables = need + 12 * 1024 <= (size_t)c->smem_optin ? 1 : 0;
+  }
   cudaError_t e = cudaFuncSetAttribute(whp_swaps_base_kernel,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        smem_tables ? (int)need : 0);
@@ -558,8 +624,14 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
   const int32_t rlo = (int32_t)((int64_t)win_start - 2ll * c->C > 0 ? (int64_t)win_start - 2ll * c->C : 0);
   const int32_t rhi = (int32_t)((int64_t)win_start + win_len + margin < c->n_orders
                                     ? (int64_t)win_start + win_len + margin : c->n_orders);
-  whp_swaps_prep_kernel<<<(unsigned)((rhi - rlo + kPrepWarps - 1) / kPrepWarps), kPrepWarps * 32,
-                          0, st>>>(T, c->base, rlo, rhi);
+  // hypothetical batches of the region and the base batches themselves
+  int64_t nb_max = 2ll * c->n_items / ((int64_t)c->C + 1) + 1;
+  if (nb_max > c->n_orders) nb_max = c->n_orders;
+  whp_swaps_prep_kernel<<<(unsigned)((rhi - rlo + nb_max + kPrepWarps - 1) / kPrepWarps),
+                          kPrepWarps * 32, 0, st>>>(T, c->base, rlo, rhi);
+  c->launches += 1;
+  if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  whp_swaps_base2_kernel<<<1, kBaseThreads, 0, st>>>(T, c->base);
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   // chain sums of the region (rtail grows with the region)
