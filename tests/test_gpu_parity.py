@@ -163,6 +163,36 @@ def test_paper_scale_full_launch_sampled_oracle(torch_cuda):
     ctx.close()
 
 
+def test_paper_scale_legsum_and_nhatc_sampled_oracle(torch_cuda):
+    """NEXT-1 / NEXT-2 at the size bench.py times: leg sums of all 16,384 plans checked on
+    sampled rows; two NHATC outer iterations over the first 2,048 plans against the oracle's loop."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    wl = W.make_workload("paper")
+    pb = wl.problem
+    ctx = whp.Context.from_problem(pb)
+    perms_dev = W.perms_torch(wl.seed, pb.n_orders, 0, wl.n_cand, "cuda")
+    leg = torch.full((wl.n_cand,), -1, dtype=torch.int64, device="cuda")
+    ctx.eval_legsum(perms_dev, leg)
+    torch.cuda.synchronize()
+    rows = np.unique(np.concatenate([np.arange(0, 40), np.arange(wl.n_cand - 40, wl.n_cand),
+                                     (W.stream_u64(8, 1, 120) % np.uint64(wl.n_cand)).astype(np.int64)]))
+    sample = W.perm_rows(wl.seed, pb.n_orders, rows)
+    assert np.array_equal(leg.cpu().numpy()[rows], oracle.eval_legsum(pb, sample))
+    assert int(leg.min()) > 0
+    n_sub, n_outer, beta = 2048, 2, 1.25
+    sub = W.perm_rows(wl.seed, pb.n_orders, np.arange(n_sub))
+    idx = torch.zeros(n_outer, dtype=torch.int64, device="cuda")
+    obj = torch.zeros(n_outer, dtype=torch.float64, device="cuda")
+    ctx.nhatc_solve(perms_dev[:n_sub], n_outer, beta, idx, None, obj)
+    torch.cuda.synchronize()
+    ref = oracle.nhatc_loop(pb, sub, n_outer, beta)
+    assert np.array_equal(idx.cpu().numpy(), ref["idx"]) and np.array_equal(obj.cpu().numpy(), ref["obj"])
+    t, v, w = ctx.get_penalty()
+    assert np.array_equal(v, ref["v"]) and np.array_equal(w, ref["w"])
+    ctx.close()
+
+
 # ---- config 5 (stress): 65,536 candidates generated in HBM, oracle on sampled rows ---------------
 def test_stress_full_size_sampled_oracle(torch_cuda):
     torch = torch_cuda
