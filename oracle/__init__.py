@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     eval_candidates,
     eval_legsum,
     eval_swaps,
+    kmeans_slotting,
     nhatc_loop,
     nhatc_update,
     optimal_route,

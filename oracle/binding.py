@@ -201,3 +201,20 @@ def eval_legsum(pb, perms) -> np.ndarray:
                             _p(keep[2]), C.c_int32(pb.cart_capacity), _p(perms),
                             C.c_int64(n_cand), _p(out))
     return out
+
+
+def kmeans_slotting(geom, n_skus: int, item_sku, k: int, Z: int, iters: int) -> dict:
+    """NEXT-3 (reading N3): K-means of the SKUs on their pick frequency, then cluster-contiguous
+    slotting. Returns sku_loc, sku_class, assign, centroids, freq."""
+    item_sku = _i32(item_sku)
+    out = {"sku_loc": np.zeros(n_skus, np.int32), "sku_class": np.zeros(n_skus, np.int32),
+           "assign": np.zeros(n_skus, np.int32), "centroids": np.zeros(k, np.float64),
+           "freq": np.zeros(n_skus, np.int64)}
+    g = _geom(geom)
+    st = _load().orc_kmeans_slotting(C.byref(g), C.c_int32(n_skus), _p(item_sku),
+                                     C.c_int32(len(item_sku)), C.c_int32(k), C.c_int32(Z),
+                                     C.c_int32(iters), _p(out["sku_loc"]), _p(out["sku_class"]),
+                                     _p(out["assign"]), _p(out["centroids"]), _p(out["freq"]))
+    if st != 0:
+        raise ValueError("kmeans_slotting: bad arguments")
+    return out

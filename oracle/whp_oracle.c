@@ -360,3 +360,81 @@ int32_t orc_eval_legsum(const orc_geom* g, const int32_t* sku_loc, int32_t n_ord
   free(locs);
   return 0;
 }
+
+/* ---- NEXT-3: subproblem 3, product placement by picking frequency with K-means ----------------
+ * PAPER.md:134 (§5): "organize the products' positions concerning how often the products are
+ * selected ... an unsupervised classification method can determine the optimal placement using,
+ * e.g. K-means clustering (Macqueen, 1967)". Nothing else is printed. DESIGN.md reading N3:
+ *   feature   f_s = number of items of the day's orders that pick SKU s (an integer);
+ *   init      c_j = lo + (j + 0.5) * ((hi - lo) / k), lo / hi = min / max f, j = 0..k-1 (fp64);
+ *   Lloyd     iters times: a_s = argmin_j |f_s - c_j| (ties: lowest j);
+ *             c_j = (sum of f_s over a_s = j) / (count) — exact integer sum, one fp64 division —
+ *             an empty cluster keeps its centroid; then one final assignment;
+ *   slotting  clusters ranked by centroid, largest first (ties: lowest j); SKUs ordered by
+ *             (cluster rank, SKU id); locations ordered by (|aisle - depot aisle|, aisle, slot,
+ *             side); the i-th SKU gets the i-th location; class = cluster * Z + slot * Z div S
+ *             (the category x zone classes of reading Q10). */
+typedef struct { int32_t key, sku; } orc_pair;
+static int cmp_pair(const void* a, const void* b) {
+  const orc_pair* x = (const orc_pair*)a; const orc_pair* y = (const orc_pair*)b;
+  if (x->key != y->key) return (x->key > y->key) - (x->key < y->key);
+  return (x->sku > y->sku) - (x->sku < y->sku);
+}
+int32_t orc_kmeans_slotting(const orc_geom* g, int32_t n_skus, const int32_t* item_sku,
+                            int32_t n_items, int32_t k, int32_t Z, int32_t iters,
+                            int32_t* sku_loc, int32_t* sku_class, int32_t* assign,
+                            double* centroids, int64_t* freq_out) {
+  int32_t S = g->slots_per_side, NA = g->n_aisles;
+  if ((int64_t)n_skus > 2ll * NA * S || k < 1 || Z < 1) return 1;
+  int64_t* f = (int64_t*)calloc((size_t)n_skus, sizeof(int64_t));
+  for (int32_t i = 0; i < n_items; i++) f[item_sku[i]] += 1;
+  int64_t lo = f[0], hi = f[0];
+  for (int32_t s = 1; s < n_skus; s++) { if (f[s] < lo) lo = f[s]; if (f[s] > hi) hi = f[s]; }
+  double step = (double)(hi - lo) / (double)k;
+  for (int32_t j = 0; j < k; j++) centroids[j] = (double)lo + ((double)j + 0.5) * step;
+  for (int32_t it = 0; it <= iters; it++) {
+    for (int32_t s = 0; s < n_skus; s++) { /* nearest centroid, ties to the lowest index */
+      int32_t best = 0;
+      double bd = (double)f[s] - centroids[0]; if (bd < 0) bd = -bd;
+      for (int32_t j = 1; j < k; j++) {
+        double d = (double)f[s] - centroids[j]; if (d < 0) d = -d;
+        if (d < bd) { bd = d; best = j; }
+      }
+      assign[s] = best;
+    }
+    if (it == iters) break;
+    for (int32_t j = 0; j < k; j++) {
+      int64_t sum = 0, cnt = 0;
+      for (int32_t s = 0; s < n_skus; s++) if (assign[s] == j) { sum += f[s]; cnt++; }
+      if (cnt > 0) centroids[j] = (double)sum / (double)cnt;
+    }
+  }
+  /* rank of every cluster: larger centroid first, ties to the lower index */
+  int32_t* rank = (int32_t*)malloc(sizeof(int32_t) * (size_t)k);
+  for (int32_t j = 0; j < k; j++) {
+    int32_t r = 0;
+    for (int32_t i = 0; i < k; i++)
+      if (centroids[i] > centroids[j] || (centroids[i] == centroids[j] && i < j)) r++;
+    rank[j] = r;
+  }
+  orc_pair* skus = (orc_pair*)malloc(sizeof(orc_pair) * (size_t)n_skus);
+  for (int32_t s = 0; s < n_skus; s++) { skus[s].key = rank[assign[s]]; skus[s].sku = s; }
+  qsort(skus, (size_t)n_skus, sizeof(orc_pair), cmp_pair);
+  /* aisles by (|a - a0|, a) */
+  orc_pair* aisles = (orc_pair*)malloc(sizeof(orc_pair) * (size_t)NA);
+  for (int32_t a = 0; a < NA; a++) {
+    int32_t d = a - g->depot_aisle; if (d < 0) d = -d;
+    aisles[a].key = d; aisles[a].sku = a;
+  }
+  qsort(aisles, (size_t)NA, sizeof(orc_pair), cmp_pair);
+  for (int32_t i = 0; i < n_skus; i++) {
+    int32_t a = aisles[i / (2 * S)].sku, rem = i % (2 * S);
+    int32_t slot = rem / 2, side = rem % 2;
+    int32_t s = skus[i].sku;
+    sku_loc[s] = a * 2 * S + side * S + slot;
+    sku_class[s] = assign[s] * Z + (int32_t)((int64_t)slot * Z / S);
+  }
+  if (freq_out) memcpy(freq_out, f, sizeof(int64_t) * (size_t)n_skus);
+  free(f); free(rank); free(skus); free(aisles);
+  return 0;
+}

@@ -471,3 +471,57 @@ def test_legsum_is_the_sum_of_cart_tours():
                     for s in pb.item_sku[pb.order_ptr[perms[c, pos]]:pb.order_ptr[perms[c, pos] + 1]]]
             total += oracle.tour_length(pb, locs)
         assert got[c] == total
+
+
+# ---- NEXT-3: K-means slotting (reading N3) ---------------------------------------------------------
+def test_kmeans_hand_worked():
+    """Frequencies [5,1,1,6,1,5], k=2: lo=1, hi=6, step 2.5: c = [2.25, 4.75]; SKUs 0,3,5 -> cluster 1
+    (|5-4.75| = .25, |6-4.75| = 1.25), SKUs 1,2,4 -> cluster 0; centroids 1 and 16/3 (stable).
+    Cluster 1 ranks first: order 0,3,5,1,2,4 over the locations of aisle 0 (S=2, depot aisle 0):
+    i -> slot i div 2, side i mod 2 -> loc = side*2 + slot: 0,2,1,3; then aisle 1: 4,6."""
+    items = [0] * 5 + [1] + [2] + [3] * 6 + [4] + [5] * 5
+    out = oracle.kmeans_slotting((3, 2, 1, 3, 0), 6, items, 2, 1, 3)
+    assert out["freq"].tolist() == [5, 1, 1, 6, 1, 5]
+    assert out["assign"].tolist() == [1, 0, 0, 1, 0, 1]
+    assert out["centroids"].tolist() == [1.0, 16.0 / 3.0]
+    assert out["sku_loc"].tolist() == [0, 3, 4, 2, 6, 1]
+    assert out["sku_class"].tolist() == [1, 0, 0, 1, 0, 1]
+
+
+def test_kmeans_invariants():
+    from fractions import Fraction
+    pb = W.make_problem("mid")
+    k, Z = 10, 2
+    prev_sse = None
+    for iters in range(0, 6):
+        out = oracle.kmeans_slotting(pb, pb.n_skus, pb.item_sku, k, Z, iters)
+        f, a, c = out["freq"], out["assign"], out["centroids"]
+        assert f.sum() == pb.n_items and np.array_equal(f, np.bincount(pb.item_sku, minlength=pb.n_skus))
+        # nearest centroid, ties to the lowest index
+        d = np.abs(f[:, None].astype(np.float64) - c[None, :])
+        assert np.array_equal(a, np.argmin(d, axis=1))
+        # Lloyd's iterations never increase the within-cluster sum of squares
+        sse = float(((f - c[a]) ** 2).sum())
+        assert prev_sse is None or sse <= prev_sse * (1 + 1e-12)
+        prev_sse = sse
+    # slotting: injective, clusters contiguous in the location order, frequent clusters first
+    loc = out["sku_loc"]
+    assert len(set(loc.tolist())) == pb.n_skus
+    S2 = 2 * pb.slots_per_side
+    order_index = (loc // S2) * S2 + (loc % pb.slots_per_side) * 2 + (loc % S2) // pb.slots_per_side
+    by_pos = np.argsort(order_index)
+    cl = a[by_pos]
+    change = np.nonzero(np.diff(cl))[0]
+    assert len(change) == len(np.unique(a)) - 1                   # every cluster is one run
+    cents = c[cl[np.concatenate([[0], change + 1])]]
+    assert np.all(np.diff(cents) <= 0)                             # largest centroid first
+    zone = (loc % pb.slots_per_side) * Z // pb.slots_per_side
+    assert np.array_equal(out["sku_class"], a * Z + zone)
+    # with iters >= 1 a centroid of a non-empty cluster is the exact mean of its members at the
+    # last update: check on the converged state (assignment stable between iters 5 and 6)
+    out6 = oracle.kmeans_slotting(pb, pb.n_skus, pb.item_sku, k, Z, 60)
+    out7 = oracle.kmeans_slotting(pb, pb.n_skus, pb.item_sku, k, Z, 61)
+    assert np.array_equal(out6["assign"], out7["assign"])
+    for j in np.unique(out7["assign"]):
+        m = out7["freq"][out7["assign"] == j]
+        assert Fraction(float(out7["centroids"][j])) == Fraction(float(int(m.sum()) / len(m)))
