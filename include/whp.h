@@ -144,6 +144,23 @@ whp_status whp_get_penalty(whp_ctx* ctx, double* t, double* v, double* w, void* 
 whp_status whp_eval_legsum(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                            void* cuda_stream);
 
+/* ---- NEXT-3: subproblem 3 (§5: product placement by picking frequency, "e.g.
+ * K-means clustering"; reading N3 of DESIGN.md) ------------------------------------------- */
+
+/* K-means (k clusters, `iters` Lloyd iterations + a final assignment) of the n_skus SKUs on
+ * their pick frequency in item_sku (host int32 [n_items]), then cluster-contiguous slotting:
+ * clusters by centroid (largest first), SKUs by (cluster rank, id), locations by
+ * (|aisle - depot_aisle|, aisle, slot, side). Outputs, host: sku_loc, sku_class int32 [n_skus]
+ * (class = cluster * n_zones + slot * n_zones / slots_per_side) — the inputs of
+ * whp_create_layout with n_classes = k * n_zones; assign int32 [n_skus] and centroids
+ * double [k] are nullable. Needs no context; runs on cuda_device and synchronises.
+ * Limits: k <= 1024, k * n_zones <= 256, n_skus <= 2 * n_aisles * slots_per_side. */
+whp_status whp_kmeans_slotting(int32_t n_aisles, int32_t slots_per_side, int32_t depot_aisle,
+                               int32_t n_skus, const int32_t* item_sku, int32_t n_items,
+                               int32_t k, int32_t n_zones, int32_t iters, int32_t cuda_device,
+                               int32_t* sku_loc, int32_t* sku_class, int32_t* assign,
+                               double* centroids);
+
 /* Debug helper: *h_n_bad (host) receives the number of rows of d_perms that are not a
  * permutation of 0..n_orders-1. Synchronises the stream. */
 whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,

@@ -23,7 +23,7 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_eval_candidates_host", "whp_eval_swaps", "whp_argmin", "whp_apply_swap",
            "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
-           "whp_eval_legsum"]
+           "whp_eval_legsum", "whp_kmeans_slotting"]
 
 
 class WhpError(RuntimeError):
@@ -55,6 +55,7 @@ def lib():
         L.whp_nhatc_solve.argtypes = [vp, vp, i64, i32, C.c_double, vp, vp, vp, vp]
         L.whp_get_penalty.argtypes = [vp, vp, vp, vp, vp]
         L.whp_eval_legsum.argtypes = [vp, vp, i64, vp, vp]
+        L.whp_kmeans_slotting.argtypes = [i32, i32, i32, i32, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp]
         L.whp_launch_count.argtypes = [vp]
         L.whp_launch_count.restype = i64
         L.whp_destroy.argtypes = [vp]
@@ -238,6 +239,22 @@ class Context:
             self.close()
         except Exception:
             pass
+
+
+def kmeans_slotting(n_aisles, slots_per_side, depot_aisle, n_skus, item_sku, k, n_zones, iters,
+                    device=0) -> dict:
+    """NEXT-3 (reading N3): K-means of the SKUs on their pick frequency + cluster-contiguous
+    slotting, on the GPU. Returns sku_loc, sku_class (inputs of Context(...)), assign, centroids."""
+    k1, p1 = _h(item_sku, np.int32)
+    out = {"sku_loc": np.zeros(n_skus, np.int32), "sku_class": np.zeros(n_skus, np.int32),
+           "assign": np.zeros(n_skus, np.int32), "centroids": np.zeros(k, np.float64)}
+    st = lib().whp_kmeans_slotting(n_aisles, slots_per_side, depot_aisle, n_skus, p1, len(k1), k,
+                                   n_zones, iters, device, out["sku_loc"].ctypes.data,
+                                   out["sku_class"].ctypes.data, out["assign"].ctypes.data,
+                                   out["centroids"].ctypes.data)
+    if st != OK:
+        raise WhpError(st, "whp_kmeans_slotting")
+    return out
 
 
 def version() -> str:

@@ -399,6 +399,45 @@ def test_legsum_edge_cases(torch_cuda, cfg):
     ctx.close()
 
 
+@pytest.mark.parametrize("name,k,Z,iters", [("tiny", 4, 1, 5), ("mid", 10, 2, 8), ("paper", 50, 4, 12),
+                                            ("mid", 7, 3, 0)])
+def test_kmeans_slotting_matches_oracle(torch_cuda, name, k, Z, iters):
+    """NEXT-3 (reading N3): frequencies, assignment, centroids and the slotting are bit-identical
+    to the oracle (integer sums, one fp64 division per centroid); the layout it produces feeds
+    whp_create_layout and the evaluator agrees with the oracle on it."""
+    torch = torch_cuda
+    import copy
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem(name)
+    got = whp.kmeans_slotting(pb.n_aisles, pb.slots_per_side, pb.depot_aisle, pb.n_skus,
+                              pb.item_sku, k, Z, iters)
+    ref = oracle.kmeans_slotting(pb, pb.n_skus, pb.item_sku, k, Z, iters)
+    for key in ("assign", "centroids", "sku_loc", "sku_class"):
+        assert np.array_equal(got[key], ref[key]), key
+    pb2 = copy.copy(pb)
+    pb2.sku_loc, pb2.sku_class, pb2.n_classes = got["sku_loc"], got["sku_class"], k * Z
+    rng = np.random.default_rng(0)
+    pb2.t, pb2.v, pb2.w = rng.uniform(0, 9, k * Z), rng.uniform(0, 1, k * Z), rng.uniform(0, 1, k * Z)
+    ctx = whp.Context.from_problem(pb2)
+    perms = W.perms(0, pb.n_orders, 24)
+    g, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
+    assert_parity(g, oracle.eval_candidates(pb2, perms), pb2)
+    ctx.close()
+
+
+def test_kmeans_slotting_hand_worked_and_errors(torch_cuda):
+    from paper_2110_13693_b200 import whp
+    items = [0] * 5 + [1] + [2] + [3] * 6 + [4] + [5] * 5
+    out = whp.kmeans_slotting(3, 2, 0, 6, items, 2, 1, 3)
+    assert out["assign"].tolist() == [1, 0, 0, 1, 0, 1]
+    assert out["centroids"].tolist() == [1.0, 16.0 / 3.0]
+    assert out["sku_loc"].tolist() == [0, 3, 4, 2, 6, 1]
+    with pytest.raises(whp.WhpError):
+        whp.kmeans_slotting(1, 2, 0, 6, items, 2, 1, 3)       # 6 SKUs, 4 locations
+    with pytest.raises(whp.WhpError):
+        whp.kmeans_slotting(3, 2, 0, 6, items + [6], 2, 1, 3)  # SKU id out of range
+
+
 def test_api_errors_and_nullable_outputs(torch_cuda):
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
