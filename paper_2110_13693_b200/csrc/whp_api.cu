@@ -45,7 +45,8 @@ void free_orders(whp_ctx* c) {
   dfree(c->d_stage[0]); dfree(c->d_stage[1]);
   c->stage_rows = 0;
   dfree(c->d_bmask); dfree(c->d_cstream); dfree(c->d_nb); dfree(c->d_dist_scratch);
-  dfree(c->d_planes); dfree(c->d_segstart);
+  dfree(c->d_planes); dfree(c->d_segstart); dfree(c->d_perm_pad);
+  c->perm_pad_bytes = 0;
   c->fast_cap = 0; c->fast_pitch = 0; c->fast_plane_words = 0;
   c->have_orders = false;
 }
@@ -200,9 +201,10 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   c->n_items_pad = (int32_t)pfast.size();
   c->fast_tables_ok = fast_ok;
   WHP_CUDA(c, cudaMalloc(&c->d_pick_fast, 4 * pfast.size()));
-  WHP_CUDA(c, cudaMalloc(&c->d_order_fast, 4 * no));
+  ofast.resize((no + 3) & ~(size_t)3, 0u);  // padded to a multiple of 16 bytes (bulk copy)
+  WHP_CUDA(c, cudaMalloc(&c->d_order_fast, 4 * ofast.size()));
   WHP_CUDA(c, cudaMemcpy(c->d_pick_fast, pfast.data(), 4 * pfast.size(), cudaMemcpyHostToDevice));
-  WHP_CUDA(c, cudaMemcpy(c->d_order_fast, ofast.data(), 4 * no, cudaMemcpyHostToDevice));
+  WHP_CUDA(c, cudaMemcpy(c->d_order_fast, ofast.data(), 4 * ofast.size(), cudaMemcpyHostToDevice));
   c->have_orders = true;
   return WHP_OK;
 }

@@ -55,9 +55,7 @@ cudaError_t whp_launch_eval(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
                             const whp_eval_out& out, cudaStream_t st) {
   const whp_tables T = whp_make_tables(c);
   const bool detail = out.batch_of_pos || out.n_distinct;  // only the general walker has these
-  // (the tuned path reads the permutations through a TMA tensor map: 16-byte aligned base)
-  if (!detail && whp_fast_eligible(c) && ((uintptr_t)d_perms & 15u) == 0 &&
-      getenv("WHP_FORCE_GENERAL") == nullptr)
+  if (!detail && whp_fast_eligible(c) && getenv("WHP_FORCE_GENERAL") == nullptr)
     return whp_launch_eval_fast(c, d_perms, n_cand, out, st);
   int64_t blocks = (n_cand + kWarpsPerBlock - 1) / kWarpsPerBlock;
   const int64_t cap = (int64_t)c->num_sms * 64;

@@ -107,7 +107,7 @@ __device__ __forceinline__ void tma_tile_2d(uint32_t dst, const CUtensorMap* tm,
 // n4 groups of four exist and the others get record 0 (q = 0: no effect on the recurrence).
 template <bool FULL>
 __device__ __forceinline__ void gather_word(uint32_t (&r)[32], uint32_t row, uint32_t swz,
-                                            uint32_t sorec0, int n4) {
+                                            uint32_t sorec0, int n4, int left = 32) {
   // row = address of this lane's 128-byte row of the tile; 16-byte chunk g lives at g ^ (lane & 7)
 #pragma unroll
   for (int g = 0; g < 8; ++g) {
@@ -118,6 +118,11 @@ __device__ __forceinline__ void gather_word(uint32_t (&r)[32], uint32_t row, uin
     } else {
       r[4 * g + 0] = 0u; r[4 * g + 1] = 0u; r[4 * g + 2] = 0u; r[4 * g + 3] = 0u;
     }
+  }
+  if (!FULL) {  // a plan whose length is no multiple of 4: the tile is zero-filled past its end
+#pragma unroll
+    for (int i = 0; i < 32; ++i)
+      if (i >= left) r[i] = 0u;
   }
 }
 
@@ -193,8 +198,9 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     tma_tile_2d(tiles + (w % kStages) * kTileBytes, &tmap, 32 * w, (int32_t)row0, bar);
   };
   if (threadIdx.x == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
-    mbar_expect_tx(bar_table, 4u * (uint32_t)n_orders);
-    bulk_g2s(sorec0, order_fast, 4u * (uint32_t)n_orders, bar_table);
+    const uint32_t table_bytes = 4u * (uint32_t)((n_orders + 3) & ~3);  // the table is padded
+    mbar_expect_tx(bar_table, table_bytes);
+    bulk_g2s(sorec0, order_fast, table_bytes, bar_table);
   }
   if (lane == 0)
     for (int w = 0; w < kStages && w < nw; ++w) issue(w);
@@ -248,10 +254,10 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
 #pragma unroll 1
   for (int w = 2 * KF; w < nw; ++w) {
     const int left = n_orders - 32 * w;
-    const int n4 = min(8, left >> 2);
+    const int n4 = min(8, (left + 3) >> 2);
     if (w > 2 * KF || n_full == 0) {
       wait_word(w);
-      gather_word<false>(ra, tile_row(w), swz, sorec0, n4);
+      gather_word<false>(ra, tile_row(w), swz, sorec0, n4, left);
     }
     uint32_t bits = recur_word<false, false>(ra, (uint32_t)C, room, cs + 4 * w, 0u, 0u, 0, n4, have);
     if (w == 0) bits |= 1u;
@@ -826,7 +832,7 @@ static PFN_cuTensorMapEncodeTiled tensor_map_encoder() {
 
 bool whp_fast_eligible(const whp_ctx* c) {
   if (!c->fast_tables_ok) return false;                       // cursors must fit 16 bits
-  if (c->n_orders % 4 != 0 || c->n_orders >= 65536) return false;
+  if (c->n_orders >= 65536) return false;
   if ((nb_upper_bound(c) + 31) / 32 > 255) return false;      // 8 counter planes, S <= 32
   if (c->C > 64) return false;                                // per-lane cursor ring of 16 chunks
   if (bounds_smem_bytes(c) > (size_t)c->smem_optin - 1024) return false;  // K1: order table in smem
@@ -873,9 +879,28 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms
     // tensor map over this call's permutation matrix: [n_cand][n_orders] int32, box 32 x 32
     PFN_cuTensorMapEncodeTiled encode = tensor_map_encoder();
     if (!encode) return cudaErrorNotSupported;
+    // TMA needs a 16-byte aligned matrix with a row pitch that is a multiple of 16 bytes:
+    // otherwise the plans are first copied into a padded scratch matrix
+    size_t pitch_bytes = 4 * (size_t)c->n_orders;
+    if ((c->n_orders & 3) != 0 || ((uintptr_t)d_perms & 15u) != 0) {
+      pitch_bytes = 4 * (((size_t)c->n_orders + 3) & ~(size_t)3);
+      if (c->perm_pad_bytes < pitch_bytes * (size_t)n_cand) {
+        if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return e;
+        cudaFree(c->d_perm_pad);
+        c->d_perm_pad = nullptr;
+        c->perm_pad_bytes = 0;
+        if ((e = cudaMalloc(&c->d_perm_pad, pitch_bytes * (size_t)n_cand)) != cudaSuccess) return e;
+        c->perm_pad_bytes = pitch_bytes * (size_t)n_cand;
+      }
+      if ((e = cudaMemcpy2DAsync(c->d_perm_pad, pitch_bytes, d_perms, 4 * (size_t)c->n_orders,
+                                 4 * (size_t)c->n_orders, (size_t)n_cand, cudaMemcpyDeviceToDevice,
+                                 st)) != cudaSuccess)
+        return e;
+      d_perms = c->d_perm_pad;
+    }
     CUtensorMap tmap;
     const cuuint64_t gdim[2] = {(cuuint64_t)c->n_orders, (cuuint64_t)n_cand};
-    const cuuint64_t gstride[1] = {4ull * (cuuint64_t)c->n_orders};
+    const cuuint64_t gstride[1] = {(cuuint64_t)pitch_bytes};
     const cuuint32_t box[2] = {32, 32};
     const cuuint32_t estr[2] = {1, 1};
     if (encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_INT32, 2, (void*)d_perms, gdim, gstride, box, estr,

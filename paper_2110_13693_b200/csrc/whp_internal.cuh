@@ -117,6 +117,8 @@ struct whp_ctx {
   uint16_t* d_cstream = nullptr;     // [fast_cap][cs_pitch] first-pick cursor of every position
   int32_t* d_nb = nullptr;           // [fast_cap]
   int32_t* d_segstart = nullptr;     // [fast_cap][32] first position of every segment
+  int32_t* d_perm_pad = nullptr;     // padded copy of the plans (n_orders % 4 != 0 or unaligned)
+  size_t perm_pad_bytes = 0;
   int64_t* d_dist_scratch = nullptr; // [fast_cap]
   uint32_t* d_planes = nullptr;      // [fast_cap][S][8 planes][KW] bit-sliced class counters
   unsigned long long* d_task = nullptr;  // [2] work-stealing counter

@@ -106,8 +106,7 @@ whp_legsum_kernel(const whp_tables T, const int32_t* __restrict__ perms, int64_t
 
 cudaError_t whp_launch_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                               cudaStream_t st) {
-  // shapes the tuned path covers (and a 16-byte aligned matrix for its TMA tensor map)
-  if (whp_fast_eligible(c) && ((uintptr_t)d_perms & 15u) == 0 && getenv("WHP_FORCE_GENERAL") == nullptr)
+  if (whp_fast_eligible(c) && getenv("WHP_FORCE_GENERAL") == nullptr)  // shapes the tuned path covers
     return whp_launch_legsum_fast(c, d_perms, n_cand, d_len, st);
   const whp_tables T = whp_make_tables(c);
   int64_t blocks = (n_cand + kLegWarps - 1) / kLegWarps;

@@ -281,12 +281,13 @@ def test_edge_cases(torch_cuda, cfg):
     ctx.close()
 
 
-@pytest.mark.parametrize("n_orders", [8, 28, 36, 60, 64, 68, 96, 100, 128, 132, 192, 196])
+@pytest.mark.parametrize("n_orders", [5, 8, 28, 31, 33, 36, 60, 63, 64, 65, 68, 96, 97, 100, 128, 130,
+                                      132, 192, 195, 196])
 @pytest.mark.parametrize("n_cand", [1, 33])
 def test_tuned_path_word_and_warp_tails(torch_cuda, n_orders, n_cand):
     """K1 streams 32 plans x 32 positions per tile: every combination of full / partial last
     word, odd / even number of words and a partial last warp of plans must agree with the
-    oracle (the tuned path is taken: n_orders is a multiple of 4)."""
+    oracle (plan lengths that are no multiple of 4 go through a padded copy)."""
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
     pb = _random_problem(5, NA=70, S=12, K=70, n_skus=400, n_orders=n_orders, qmax=5, C=11, depot=3)
@@ -350,7 +351,7 @@ def test_outputs_stay_inside_their_buffers(torch_cuda, name, n_cand):
 
 def test_unaligned_permutation_buffer(torch_cuda):
     """A permutation matrix that starts 4 bytes off a 16-byte boundary cannot be described by a
-    TMA tensor map: the call must still be right (it takes the general path)."""
+    TMA tensor map: the call must still be right (the plans go through an aligned copy)."""
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
     pb = W.make_problem("mid")
