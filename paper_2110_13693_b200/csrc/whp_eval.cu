@@ -54,13 +54,13 @@ whp_eval_general_kernel(const whp_tables T, const int32_t* __restrict__ perms, i
 cudaError_t whp_launch_eval(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
                             const whp_eval_out& out, cudaStream_t st) {
   const whp_tables T = whp_make_tables(c);
-  const bool detail = out.batch_of_pos || out.n_distinct;  // only the general walker has these
+  const bool detail = out.n_distinct != nullptr;  // only the general walker counts distinct locations
   if (!detail && whp_fast_eligible(c) && getenv("WHP_FORCE_GENERAL") == nullptr)
     return whp_launch_eval_fast(c, d_perms, n_cand, out, st);
   int64_t blocks = (n_cand + kWarpsPerBlock - 1) / kWarpsPerBlock;
   const int64_t cap = (int64_t)c->num_sms * 64;
   if (blocks > cap) blocks = cap;
-  if (detail || out.resp)
+  if (detail || out.resp || out.batch_of_pos)
     whp_eval_general_kernel<true><<<(unsigned)blocks, kWarpsPerBlock * 32, 0, st>>>(
         T, d_perms, n_cand, out);
   else

@@ -324,6 +324,27 @@ whp_segments_kernel(const uint32_t* __restrict__ bmask, int32_t bm_pitch, int32_
   }
 }
 
+// batch_of_pos (D2, optional output) from the boundary mask: one warp per plan, a running batch
+// count over the words, lane i of word w writes position 32w + i (coalesced).
+__global__ void __launch_bounds__(256)
+whp_bop_kernel(const uint32_t* __restrict__ bmask, int32_t bm_pitch, int32_t n_orders,
+               int64_t n_cand, int32_t* __restrict__ batch_of_pos) {
+  const int lane = threadIdx.x & 31;
+  const int64_t c = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  if (c >= n_cand) return;
+  const int nw = (n_orders + 31) >> 5;
+  const uint32_t* __restrict__ bm = bmask + c * bm_pitch;
+  int32_t* __restrict__ row = batch_of_pos + c * n_orders;
+  int32_t before = 0;  // batches that start before the current word
+  for (int w = 0; w < nw; ++w) {
+    uint32_t x = __ldg(bm + w);
+    if (w == (n_orders >> 5)) x &= (1u << (n_orders & 31)) - 1u;  // drop the end sentinel
+    const int32_t p = 32 * w + lane;
+    if (p < n_orders) row[p] = before + __popc(x & (WHP_FULL >> (31 - lane))) - 1;
+    before += __popc(x);
+  }
+}
+
 // ------------------------------------------------------------------------------------------ K2
 // vertical counter bit planes: at most 8 per segment (up to 255 batches) + 5 combine levels
 constexpr int kPlaneRow = 16;  // words per class word in a plan's counter row: 13 planes, or
@@ -1021,6 +1042,13 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
 #undef WHP_LAUNCH_SETS_KW
 #undef WHP_LAUNCH_SETS
 #undef WHP_LAUNCH_SETS_PL
+    c->launches += 1;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+  }
+  if (out.batch_of_pos) {
+    whp_bop_kernel<<<(unsigned)((n_cand * 32 + 255) / 256), 256, 0, st>>>(
+        c->d_bmask, bm_pitch, c->n_orders, n_cand, out.batch_of_pos);
     c->launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

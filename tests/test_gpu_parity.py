@@ -294,8 +294,15 @@ def test_tuned_path_word_and_warp_tails(torch_cuda, n_orders, n_cand):
     ctx = whp.Context.from_problem(pb)
     perms = W.perm_rows(7, pb.n_orders, np.arange(n_cand))
     got, dev = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
-    ref = oracle.eval_candidates(pb, perms)
+    ref = oracle.eval_candidates(pb, perms, detail=True)
     assert_parity(got, ref, pb)
+    # batch_of_pos alone stays on the tuned path (derived from K1's boundary mask)
+    bop = torch.full((n_cand, pb.n_orders), -1, dtype=torch.int32, device="cuda")
+    d2 = torch.zeros(n_cand, dtype=torch.int64, device="cuda")
+    ctx.eval_candidates(torch.from_numpy(perms).cuda(), dist=d2, batch_of_pos=bop)
+    torch.cuda.synchronize()
+    assert np.array_equal(bop.cpu().numpy(), ref["batch_of_pos"])
+    assert np.array_equal(d2.cpu().numpy(), ref["dist"])
     ctx.close()
 
 
