@@ -1,23 +1,26 @@
-// whp_fast.cu — the tuned candidate path (timed outputs and r_k): three kernels with no
-// cross-lane operation inside the inner loops.
+// whp_fast.cu — the tuned candidate path: kernels with no cross-lane operation
+// inside their inner loops.
 //
-//   K1 whp_bounds_kernel   one THREAD per candidate runs the next-fit recurrence (D2) over its
-//                          permutation row (streamed through a cp.async ring) and writes (i) a
-//                          bitmask of batch-start positions, (ii) the batch count, (iii) the
-//                          "cursor stream": for every position the 16-bit index of the order's
-//                          first pick record, so K2 needs neither the permutation nor the order
-//                          table.
-//   K2 whp_sets_kernel     one LANE per (candidate, segment): a candidate's batches are cut into
-//                          S equal runs; a lane walks the picks of its run, one pick per step.
-//                          Its occupancy sets are PRIVATE shared-memory words laid out
-//                          [word][lane] (bank = lane: never a bank conflict); a word holds 16
-//                          set bits plus a 16-bit batch stamp, so an unsigned max() with
-//                          (stamp << 16) empties a stale word and nothing is ever cleared.
-//                          Per batch: S-shape length (D4) from the running distinct-aisle count
-//                          and the max pick record; the batch's class set is added into
-//                          bit-sliced ("vertical") counters held in registers (D5).
-//   K3 whp_finish_kernel   one warp per candidate: decodes the vertical counters into r_k,
-//                          canonical fp64 penalty (D6), J, outputs.
+//   K1 whp_bounds_kernel    one THREAD per plan runs the next-fit recurrence (D2) over its row of
+//                           the permutation matrix, which arrives as 2-D TMA tiles (32 plans x 32
+//                           positions, 128-byte swizzle, mbarrier pipeline). It writes (i) a
+//                           bitmask of batch-start positions and (ii) the "cursor stream": for
+//                           every position the 16-bit index of the order's first pick record, so
+//                           K2 needs neither the permutation nor the order table (out through
+//                           swizzled shared-memory tiles and TMA tile stores).
+//      whp_segments_kernel  one warp per plan: batch count, first position of every segment.
+//      whp_bop_kernel       optional batch_of_pos from the bitmask.
+//   K2 whp_sets_kernel      one LANE per (plan, segment): a plan's batches are cut into S equal
+//                           runs; a lane walks the picks of its run, one pick per branch-free
+//                           step. Its occupancy sets are PRIVATE 32-bit shared-memory words laid
+//                           out [word][lane] (bank = lane: never a bank conflict), addressed as
+//                           base | offset. At the batch close: m = sum of popc, the words are
+//                           cleared, S-shape length (D4) from m and the max pick record; the
+//                           batch's class set is added into bit-sliced ("vertical") counters
+//                           held in registers (D5). With S = 32 it also decodes r_k.
+//   KL whp_legs_kernel      NEXT-2: K2's decomposition without the sets — a step adds the leg
+//                           from the previous pick (D0's walking metric).
+//   K3 whp_finish_kernel    one warp per plan: r_k, canonical fp64 penalty (D6), J, outputs.
 #include <cuda.h>
 #include <cudaTypedefs.h>
 
@@ -57,7 +60,7 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
 // Next-fit batching (D2) is a sequential recurrence along the plan: one thread per plan, one
 // warp per block. The plans of a warp are 32 consecutive rows of the permutation matrix, so one
 // 2-D TMA tile load (tensor map over perms, box = 32 rows x 32 positions, 128-byte swizzle)
-// brings one 32-position word of all 32 plans with a single instruction; 8 tiles are in flight
+// brings one 32-position word of all 32 plans with a single instruction; kStages tiles are in flight
 // per warp (an mbarrier per stage). The swizzle makes the lane-per-row 128-bit reads
 // conflict-free. The loop is software-pipelined by hand — while the recurrence runs over word w,
 // the order ids of word w+1 leave the tile and their order records are gathered from the table

@@ -73,7 +73,6 @@ struct whp_base_tables {
   int32_t* bstart;    // [n_orders+1] first position of batch b; bstart[nb] = n_orders
   int32_t* bop;       // [n_orders]   batch of position
   int64_t* bdist;     // [n_orders+1] exclusive prefix sum of per-batch S-shape lengths
-  uint32_t* bclass;   // [n_orders][8] class mask of batch b
   int32_t* resp;      // [K]          base responses
   int64_t* totals;    // [2]          D_base, n_batches
   double* ftotals;    // [2]          phi_base, J_base

@@ -1,20 +1,25 @@
 // whp_swaps.cu — whp_eval_swaps (a6, D8): pairwise-swap neighbourhood of a base plan with
 // rescoring limited to the batches a swap can affect.
 //
-//   base pass   ONE block tabulates the base plan: item-count prefix pre[p], order record per
-//               position, next-fit boundaries (parallel "where does a batch opened at p end"
-//               + one pointer chase), then one warp per batch scores it with the picks of the
-//               batch flattened over the lanes. Tables: bstart[b], bop[p], prefix of batch
-//               lengths bdist[b], class mask bclass[b], class-count prefix rpre[b][k], totals.
+//   base pass   whp_swaps_base_kernel (one block): item-count prefix pre[p], order record per
+//               position, nxt[p] = end of the batch that would open at p, and the base batch
+//               starts (pointer doubling along nxt + a block scan: bstart[b], bop[p]).
+//               whp_swaps_prep_kernel (multi-block): the hypothetical batch [p, nxt[p]) of every
+//               position of the window region and of every base batch start, one warp per batch
+//               with its picks flattened over the lanes (dist_at[p], cls_at[p]).
+//               whp_swaps_base2_kernel (one block): prefix of the base batch lengths bdist[b],
+//               class-count prefix rpre[b][k], base D, phi, J.
+//               whp_swaps_chain_kernel: per region position the sums along its chain
+//               p -> nxt[p] -> ... up to where it meets the base plan (dtail, rtail, bF).
 //   neighbours  one warp per swap (pi,pj). Next-fit only looks forward, so batches before the
 //               one holding pi are untouched — except that when pi opens its batch a smaller
 //               order may slip into the previous cart, so the rewalk then starts one batch
 //               earlier. Equal item counts leave every boundary in place: only the two batches
-//               holding pi and pj are rescored. Otherwise the rewalk re-batches from there and
-//               stops at the first new batch start P > pj that is also a base batch start
-//               (from there on both plans are identical), or at the end.
-//               D and r are patched: minus the replaced base batches (prefix differences),
-//               plus the new ones.
+//               holding pi and pj are rescored. Otherwise the plan is re-batched from there;
+//               only the batches holding a swapped position are scored from their picks, the
+//               stretch between pi and pj is a difference of two chain sums and everything
+//               after pj one chain look-up. D and r are patched: minus the replaced base
+//               batches (prefix differences), plus the new ones.
 #include <cstdlib>
 
 #include "whp_walk.cuh"
