@@ -12,6 +12,7 @@ from .binding import (  # noqa: F401
     eval_candidate_batches,
     eval_candidates,
     eval_legsum,
+    eval_moves,
     eval_swaps,
     kmeans_slotting,
     nhatc_loop,

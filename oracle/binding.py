@@ -218,3 +218,15 @@ def kmeans_slotting(geom, n_skus: int, item_sku, k: int, Z: int, iters: int) -> 
     if st != 0:
         raise ValueError("kmeans_slotting: bad arguments")
     return out
+
+
+def eval_moves(pb, base_perm, win_start: int, win_len: int) -> dict:
+    """NEXT-4 (reading N4): every insertion move (i' -> j') inside the window, W(W-1) of them."""
+    base_perm = _i32(base_perm)
+    nn = win_len * (win_len - 1)
+    out = {"dist": np.zeros(nn, np.int64), "obj": np.zeros(nn, np.float64)}
+    args, keep = _common(pb)
+    _load().orc_eval_moves(*args, _p(base_perm), C.c_int32(win_start), C.c_int32(win_len),
+                           _p(out["dist"]), _p(out["obj"]))
+    del keep
+    return out

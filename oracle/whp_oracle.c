@@ -438,3 +438,33 @@ int32_t orc_kmeans_slotting(const orc_geom* g, int32_t n_skus, const int32_t* it
   free(f); free(rank); free(skus); free(aisles);
   return 0;
 }
+
+/* ---- NEXT-4: insertion (or-opt, one order) neighbourhood ---------------------------------------
+ * BASELINE.json configs[4] scores pairwise swaps; SURVEY.md §8(f) NEXT-4 names "insertion /
+ * or-opt moves" as the second workload on the same evaluator. DESIGN.md reading N4: inside the
+ * window [s, s+W) the move (i', j'), i' != j', takes the order at position s+i' out and puts it
+ * back so that it stands at position s+j' (the orders in between shift by one). Neighbour index
+ * n = i' (W-1) + (j' < i' ? j' : j'-1). Value = D2-D6 of the new sequence, re-evaluated from
+ * scratch here. */
+int32_t orc_eval_moves(const orc_geom* g, const int32_t* sku_loc, const int32_t* sku_class,
+                       int32_t K, int32_t n_orders, const int32_t* order_ptr,
+                       const int32_t* item_sku, int32_t C, const double* t, const double* v,
+                       const double* w, const int32_t* base_perm, int32_t win_start,
+                       int32_t win_len, int64_t* dist, double* obj) {
+  int32_t* p = (int32_t*)malloc(sizeof(int32_t) * (size_t)n_orders);
+  int64_t n = 0;
+  for (int32_t i = 0; i < win_len; i++)
+    for (int32_t j = 0; j < win_len; j++) {
+      if (j == i) continue;
+      memcpy(p, base_perm, sizeof(int32_t) * (size_t)n_orders);
+      int32_t from = win_start + i, to = win_start + j, moved = p[from];
+      if (from < to) for (int32_t q = from; q < to; q++) p[q] = p[q + 1];
+      else for (int32_t q = from; q > to; q--) p[q] = p[q - 1];
+      p[to] = moved;
+      orc_eval_candidate(g, sku_loc, sku_class, K, n_orders, order_ptr, item_sku, C, t, v, w, p,
+                         dist ? dist + n : 0, 0, obj ? obj + n : 0, 0, 0, 0, 0, 0, 0);
+      n++;
+    }
+  free(p);
+  return 0;
+}

@@ -525,3 +525,32 @@ def test_kmeans_invariants():
     for j in np.unique(out7["assign"]):
         m = out7["freq"][out7["assign"] == j]
         assert Fraction(float(out7["centroids"][j])) == Fraction(float(int(m.sum()) / len(m)))
+
+
+# ---- NEXT-4: insertion moves (reading N4) ------------------------------------------------------------
+def test_moves_equal_materialised_sequences_and_adjacent_moves_are_swaps(golden):
+    pb = W.make_problem("tiny")
+    base = W.base_perm(2, pb.n_orders)
+    s, Wn = 3, 9
+    mv = oracle.eval_moves(pb, base, s, Wn)
+    sw = oracle.eval_swaps(pb, base, s, Wn)
+    n = 0
+    for i in range(Wn):
+        for j in range(Wn):
+            if i == j:
+                continue
+            seq = np.delete(base, s + i)                      # built with numpy, not by the oracle
+            seq = np.insert(seq, s + j, base[s + i])
+            one = oracle.eval_candidates(pb, seq.astype(np.int32))
+            assert mv["dist"][n] == one["dist"][0] and mv["obj"][n] == one["obj"][0]
+            assert n == i * (Wn - 1) + (j if j < i else j - 1)
+            if abs(i - j) == 1:                               # an adjacent move is a swap
+                a, b = min(i, j), max(i, j)
+                k = a * (2 * Wn - a - 1) // 2 + (b - a - 1)
+                assert mv["dist"][n] == sw["dist"][k] and mv["obj"][n] == sw["obj"][k]
+            n += 1
+    # E4 -> E6 of the hand-worked examples: moving position 1 to position 2 is the swap (1, 2)
+    gp = _golden_problem(golden)
+    e6 = next(p for p in golden["plans"] if p["id"] == "E6")
+    m = oracle.eval_moves(gp, np.arange(6, dtype=np.int32), 0, 6)
+    assert m["dist"][1 * 5 + 1] == e6["dist"] and m["obj"][1 * 5 + 1] == e6["obj"]
