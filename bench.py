@@ -220,6 +220,17 @@ def run_ours(args):
     torch.cuda.synchronize()
     legsum_ms = ev0.elapsed_time(ev1)
 
+    # ---- NEXT-4: insertion-move neighbourhood of the trajectory plan (not part of the step) ---
+    mW = 128
+    mobj = torch.zeros(mW * (mW - 1), dtype=torch.float64, device=dev)
+    ctx.eval_moves(base, 0, mW, None, mobj)
+    torch.cuda.synchronize()
+    ev0.record()
+    ctx.eval_moves(base, 0, mW, None, mobj)
+    ev1.record()
+    torch.cuda.synchronize()
+    moves_ms = ev0.elapsed_time(ev1)
+
     # ---- roofline of the dominant kernel (candidate evaluation) -----------------------------
     bytes_pc = harness.algorithmic_bytes_per_candidate(n, pb.n_items)
     peaks = harness.measured_peaks(ROOT)
@@ -264,6 +275,9 @@ def run_ours(args):
         "nhatc_outer_loop": {"ms_per_outer_iteration": nhatc_ms,
                              "what": "eval 16,384 plans (with responses) -> argmin -> multiplier "
                                      "update, device only"},
+        "moves": {"ms": moves_ms, "neighbours": mW * (mW - 1),
+                  "neighbours_per_s": mW * (mW - 1) / (moves_ms * 1e-3),
+                  "what": "whp_eval_moves, all insertion moves of a 128-wide window"},
         "legsum": {"ms": legsum_ms, "plans_per_s": n_cand / (legsum_ms * 1e-3),
                    "what": "whp_eval_legsum on the same 16,384 plans (paper-literal Eq. 2)"},
         "roofline": roofline,

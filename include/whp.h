@@ -161,6 +161,21 @@ whp_status whp_kmeans_slotting(int32_t n_aisles, int32_t slots_per_side, int32_t
                                int32_t* sku_loc, int32_t* sku_class, int32_t* assign,
                                double* centroids);
 
+/* ---- NEXT-4: insertion (or-opt, one order) neighbourhood on the incremental evaluator
+ * (reading N4 of DESIGN.md) ------------------------------------------------ */
+
+/* All W(W-1) moves inside [win_start, win_start+win_len) of d_base_perm (DEVICE int32
+ * [n_orders]): move (i', j'), i' != j', takes the order at position win_start+i' out and puts it
+ * back at position win_start+j'; neighbour n = i'(W-1) + (j' < i' ? j' : j'-1); value = D2-D6
+ * of the new sequence. d_dist int64 / d_obj double DEVICE [W(W-1)], nullable. */
+whp_status whp_eval_moves(whp_ctx* ctx, const int32_t* d_base_perm, int32_t win_start,
+                          int32_t win_len, int64_t* d_dist, double* d_obj, void* cuda_stream);
+
+/* Applies move *d_idx (DEVICE int64, as written by whp_argmin over a whp_eval_moves result of
+ * the same window) to d_base_perm in place, on the device. */
+whp_status whp_apply_move(whp_ctx* ctx, int32_t* d_base_perm, int32_t win_start, int32_t win_len,
+                          const int64_t* d_idx, void* cuda_stream);
+
 /* Debug helper: *h_n_bad (host) receives the number of rows of d_perms that are not a
  * permutation of 0..n_orders-1. Synchronises the stream. */
 whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,

@@ -366,6 +366,35 @@ whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t 
   return WHP_OK;
 }
 
+whp_status whp_eval_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
+                          int32_t win_len, int64_t* d_dist, double* d_obj, void* cuda_stream) {
+  whp_status s = ready(c);
+  if (s != WHP_OK) return s;
+  if (!d_base_perm) return fail(c, WHP_ERR_INVALID_ARG, "d_base_perm is null");
+  if (win_len < 2) return fail(c, WHP_ERR_INVALID_ARG, "window shorter than 2");
+  if (win_start < 0 || (int64_t)win_start + win_len > c->n_orders)
+    return fail(c, WHP_ERR_OUT_OF_RANGE, "window outside the plan");
+  device_guard dg(c->device);
+  WHP_CUDA(c, whp_launch_moves(c, d_base_perm, win_start, win_len, d_dist, d_obj,
+                               (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
+whp_status whp_apply_move(whp_ctx* c, int32_t* d_base_perm, int32_t win_start, int32_t win_len,
+                          const int64_t* d_idx, void* cuda_stream) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!c->have_orders) return fail(c, WHP_ERR_STATE, "whp_load_orders has not been called");
+  if (!d_base_perm || !d_idx) return fail(c, WHP_ERR_INVALID_ARG, "null pointer");
+  if (win_len < 2) return fail(c, WHP_ERR_INVALID_ARG, "window shorter than 2");
+  if (win_start < 0 || (int64_t)win_start + win_len > c->n_orders)
+    return fail(c, WHP_ERR_OUT_OF_RANGE, "window outside the plan");
+  device_guard dg(c->device);
+  WHP_CUDA(c, whp_launch_apply_move(c, d_base_perm, win_start, win_len, d_idx,
+                                    (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
 whp_status whp_eval_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                            void* cuda_stream) {
   if (!c) return WHP_ERR_INVALID_ARG;

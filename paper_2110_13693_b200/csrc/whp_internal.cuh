@@ -153,6 +153,10 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
                                  const whp_eval_out& out, cudaStream_t st);
 cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                              int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st);
+cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
+                             int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st);
+cudaError_t whp_launch_apply_move(whp_ctx* c, int32_t* d_base_perm, int32_t win_start,
+                                  int32_t win_len, const int64_t* d_idx, cudaStream_t st);
 cudaError_t whp_launch_argmin(whp_ctx* c, const double* d_obj, int64_t n, int64_t* d_idx,
                               double* d_val, cudaStream_t st);
 cudaError_t whp_launch_apply_swap(whp_ctx* c, int32_t* d_base_perm, int32_t win_start,

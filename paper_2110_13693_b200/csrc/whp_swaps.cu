@@ -51,6 +51,36 @@ struct swap_seq {
   }
 };
 
+// NEXT-4 (reading N4): the base plan with the order at position pi taken out and put back at
+// position pj; the orders in between shift by one. qi = item count of the moved order.
+struct move_seq {
+  const int32_t* pre;
+  const uint32_t* orec;
+  const int32_t* s_pre;
+  const uint32_t* s_orec;
+  int32_t lo;
+  uint32_t n_pre, n_orec;
+  int32_t pi, pj, qi;
+  __device__ __forceinline__ int32_t pre_base(int32_t p) const {
+    const uint32_t k = (uint32_t)(p - lo);
+    return k < n_pre ? s_pre[k] : pre[p];
+  }
+  __device__ __forceinline__ int32_t pre_at(int32_t p) const {
+    if (pi < pj) return (p > pi && p <= pj) ? pre_base(p + 1) - qi : pre_base(p);
+    return (p > pj && p <= pi) ? pre_base(p - 1) + qi : pre_base(p);
+  }
+  __device__ __forceinline__ int32_t base_of(int32_t p) const {  // base position of new position p
+    if (p == pj) return pi;
+    if (pi < pj) return (p >= pi && p < pj) ? p + 1 : p;
+    return (p > pj && p <= pi) ? p - 1 : p;
+  }
+  __device__ __forceinline__ uint32_t orec_at(int32_t p) const {
+    const int32_t s = base_of(p);
+    const uint32_t k = (uint32_t)(s - lo);
+    return k < n_orec ? s_orec[k] : orec[s];
+  }
+};
+
 struct warp_sets {
   uint32_t amask[32];  // aisle occupancy of the batch being scored
   uint32_t cmask[8];   // class occupancy
@@ -58,7 +88,8 @@ struct warp_sets {
 
 // End of the batch that opens at position p (D2): the largest e <= n with
 // pre(e) - pre(p) <= C. Every order has at least one item, so e - p <= C. Warp-collective.
-__device__ __forceinline__ int32_t batch_end(const swap_seq& q, int32_t p, int32_t n, int32_t C) {
+template <class Seq>
+__device__ __forceinline__ int32_t batch_end(const Seq& q, int32_t p, int32_t n, int32_t C) {
   const int lane = whp_lane();
   const int32_t lim = q.pre_at(p) + C;
   int32_t e = p;
@@ -75,8 +106,9 @@ __device__ __forceinline__ int32_t batch_end(const swap_seq& q, int32_t p, int32
 // D3 + D4 of the batch at positions [s, e): the picks of the batch are flattened over the
 // lanes (item t belongs to the last position whose prefix is <= t). Returns dist_b on every
 // lane; leaves the batch's class mask in sets->cmask (the caller consumes and clears it).
+template <class Seq>
 __device__ __forceinline__ int64_t score_batch(const whp_tables& T, warp_sets* sets,
-                                               const swap_seq& q, int32_t s, int32_t e) {
+                                               const Seq& q, int32_t s, int32_t e) {
   const int lane = whp_lane();
   const int32_t base0 = q.pre_at(s);
   const int32_t load = q.pre_at(e) - base0;
@@ -600,11 +632,133 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   }
 }
 
+// ------------------------------------------------------------------------------ NEXT-4: moves
+// Insertion neighbourhood (reading N4): one warp per move (i' -> j'). The plan is re-batched
+// from the cart of the first changed position m = min(pi, pj) (one cart earlier when m opens
+// its cart: a different order there may slip back) until, after M = max(pi, pj), a new boundary
+// coincides with a base boundary. The orders between pi and pj only shift by one position, so a
+// new batch that lies between them and ends where the base criterion ends it is the tabulated
+// batch of its (shifted) base start; after M the rest is one chain look-up, as for swaps.
+__global__ void __launch_bounds__(kSwapWarps * 32)
+whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start, int32_t W,
+                 int32_t rlo, int32_t rhi, int64_t n_nb, int64_t* __restrict__ d_dist,
+                 double* __restrict__ d_obj) {
+  __shared__ warp_sets sets_all[kSwapWarps];
+  __shared__ int32_t s_pre[kStage + 1];
+  __shared__ uint32_t s_orec[kStage];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  warp_sets* sets = &sets_all[warp];
+  sets->amask[lane] = 0;
+  if (lane < 8) sets->cmask[lane] = 0;
+  const int32_t n = T.n_orders;
+  const int32_t nb = (int32_t)B.totals[1];
+  int32_t lo;
+  {
+    const int32_t bw = __ldg(B.bop + win_start);
+    lo = __ldg(B.bstart + (bw > 0 ? bw - 1 : 0));
+  }
+  const int32_t cnt = min(kStage, n - lo);
+  for (int k = threadIdx.x; k <= cnt; k += blockDim.x) s_pre[k] = __ldg(B.pre + lo + k);
+  for (int k = threadIdx.x; k < cnt; k += blockDim.x) s_orec[k] = __ldg(B.orec + lo + k);
+  __syncthreads();
+  const int64_t D_base = B.totals[0];
+  for (int64_t nn = (int64_t)blockIdx.x * kSwapWarps + warp; nn < n_nb;
+       nn += (int64_t)gridDim.x * kSwapWarps) {
+    const int32_t i = (int32_t)(nn / (W - 1));
+    const int32_t jr = (int32_t)(nn - (int64_t)i * (W - 1));
+    const int32_t j = jr < i ? jr : jr + 1;
+    const int32_t pi = win_start + i, pj = win_start + j;
+    const int32_t m = min(pi, pj), M = max(pi, pj);
+    move_seq q{B.pre, B.orec, s_pre, s_orec, lo, (uint32_t)(cnt + 1), (uint32_t)cnt, pi, pj, 0};
+    q.qi = q.pre_base(pi + 1) - q.pre_base(pi);
+    int32_t b0 = __ldg(B.bop + m);
+    if (b0 > 0 && m == __ldg(B.bstart + b0)) b0 -= 1;  // a different order opens the cart: may slip
+    int32_t p = __ldg(B.bstart + b0);
+    int64_t D = D_base;
+    int32_t r[8];
+#pragma unroll
+    for (int w = 0; w < 8; ++w) r[w] = 0;
+    int32_t b_end;
+    for (;;) {
+      if (p > M && p >= rlo && p < rhi) {  // the rest is the chain of p
+        const int32_t bf = __ldg(B.bF + p);
+        if (bf >= 0) {
+          D += __ldg(B.dtail + p);
+#pragma unroll
+          for (int w = 0; w < 8; ++w) {
+            const int k = 32 * w + lane;
+            if (k < T.K) r[w] += __ldg(B.rtail + (int64_t)(p - rlo) * T.K + k);
+          }
+          b_end = bf;
+          break;
+        }
+      }
+      const int32_t e = batch_end(q, p, n, T.C);
+      // base start of the batch if it is a run of base orders in base order: before m, after
+      // M, or between pi and pj without the re-inserted order (positions shifted by one)
+      int32_t bp = -1;
+      if (e <= m || p > M) bp = p;
+      else if (pi < pj && p >= pi && e <= pj) bp = p + 1;
+      else if (pj < pi && p > pj && e <= pi + 1) bp = p - 1;
+      if (bp >= rlo && bp < rhi && __ldg(B.nxt + bp) == bp + (e - p)) {
+        D += __ldg(B.dist_at + bp);
+        const uint4 c0 = __ldg(reinterpret_cast<const uint4*>(B.cls_at + (int64_t)bp * 8));
+        const uint4 c1 = __ldg(reinterpret_cast<const uint4*>(B.cls_at + (int64_t)bp * 8) + 1);
+        r[0] += (int32_t)((c0.x >> lane) & 1u); r[1] += (int32_t)((c0.y >> lane) & 1u);
+        r[2] += (int32_t)((c0.z >> lane) & 1u); r[3] += (int32_t)((c0.w >> lane) & 1u);
+        r[4] += (int32_t)((c1.x >> lane) & 1u); r[5] += (int32_t)((c1.y >> lane) & 1u);
+        r[6] += (int32_t)((c1.z >> lane) & 1u); r[7] += (int32_t)((c1.w >> lane) & 1u);
+      } else {
+        D += score_batch(T, sets, q, p, e);
+        __syncwarp();
+#pragma unroll
+        for (int w = 0; w < 8; ++w) r[w] += (int32_t)((sets->cmask[w] >> lane) & 1u);
+        __syncwarp();
+        if (lane < 8) sets->cmask[lane] = 0;
+        __syncwarp();
+      }
+      p = e;
+      if (p >= n) { b_end = nb; break; }
+      if (p > M && __ldg(B.bop + p) != __ldg(B.bop + p - 1)) { b_end = __ldg(B.bop + p); break; }
+    }
+    D -= B.bdist[b_end] - B.bdist[b0];
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+      const int k = 32 * w + lane;
+      if (k < T.K)
+        r[w] += __ldg(B.resp + k) - (__ldg(B.rpre + (int64_t)b_end * T.K + k) -
+                                     __ldg(B.rpre + (int64_t)b0 * T.K + k));
+    }
+    const double phi = penalty_regs(T, r);
+    if (lane == 0) {
+      if (d_dist) d_dist[nn] = D;
+      if (d_obj) d_obj[nn] = __dadd_rn((double)D, phi);
+    }
+  }
+}
+
+// apply move *d_idx (as written by whp_argmin over a whp_eval_moves result) to the plan
+__global__ void whp_apply_move_kernel(int32_t* __restrict__ base_perm, int32_t win_start, int32_t W,
+                                      const int64_t* __restrict__ d_idx) {
+  const int64_t nn = *d_idx;
+  if (nn < 0 || nn >= (int64_t)W * (W - 1)) return;
+  const int32_t i = (int32_t)(nn / (W - 1));
+  const int32_t jr = (int32_t)(nn - (int64_t)i * (W - 1));
+  const int32_t j = jr < i ? jr : jr + 1;
+  const int32_t from = win_start + i, to = win_start + j;
+  const int32_t moved = base_perm[from];
+  if (from < to) for (int32_t q = from; q < to; ++q) base_perm[q] = base_perm[q + 1];
+  else for (int32_t q = from; q > to; --q) base_perm[q] = base_perm[q - 1];
+  base_perm[to] = moved;
+}
+
 }  // namespace
 
-cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
-                             int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st) {
-  const whp_tables T = whp_make_tables(c);
+// base pass + region tables + chain sums of one window (shared by the swap and the move
+// neighbourhoods)
+static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const int32_t* d_base_perm,
+                                        int32_t win_start, int32_t win_len, int32_t* rlo_out,
+                                        int32_t* rhi_out, cudaStream_t st) {
   // shared-memory tables of the base pass: pre + nxt, and (mode 2) three more arrays for the
   // pointer doubling that finds the base boundaries
   size_t need = 4 * (5 * (size_t)c->n_orders + 1);
@@ -657,12 +811,46 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
                            chain_smem, st>>>(T, c->base, rlo, rhi);
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
+  *rlo_out = rlo;
+  *rhi_out = rhi;
+  return cudaSuccess;
+}
+
+cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
+                             int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st) {
+  const whp_tables T = whp_make_tables(c);
+  int32_t rlo, rhi;
+  cudaError_t e = launch_window_tables(c, T, d_base_perm, win_start, win_len, &rlo, &rhi, st);
+  if (e != cudaSuccess) return e;
   const int64_t n_nb = (int64_t)win_len * (win_len - 1) / 2;
   int64_t blocks = (n_nb + kSwapWarps - 1) / kSwapWarps;
   const int64_t cap = (int64_t)c->num_sms * 8;
   if (blocks > cap) blocks = cap;
   whp_swaps_kernel<<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(T, c->base, win_start, win_len,
                                                                  rlo, rhi, n_nb, d_dist, d_obj);
+  c->launches += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
+                             int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st) {
+  const whp_tables T = whp_make_tables(c);
+  int32_t rlo, rhi;
+  cudaError_t e = launch_window_tables(c, T, d_base_perm, win_start, win_len, &rlo, &rhi, st);
+  if (e != cudaSuccess) return e;
+  const int64_t n_nb = (int64_t)win_len * (win_len - 1);
+  int64_t blocks = (n_nb + kSwapWarps - 1) / kSwapWarps;
+  const int64_t cap = (int64_t)c->num_sms * 8;
+  if (blocks > cap) blocks = cap;
+  whp_moves_kernel<<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(T, c->base, win_start, win_len,
+                                                                 rlo, rhi, n_nb, d_dist, d_obj);
+  c->launches += 1;
+  return cudaGetLastError();
+}
+
+cudaError_t whp_launch_apply_move(whp_ctx* c, int32_t* d_base_perm, int32_t win_start,
+                                  int32_t win_len, const int64_t* d_idx, cudaStream_t st) {
+  whp_apply_move_kernel<<<1, 1, 0, st>>>(d_base_perm, win_start, win_len, d_idx);
   c->launches += 1;
   return cudaGetLastError();
 }

@@ -23,7 +23,7 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_eval_candidates_host", "whp_eval_swaps", "whp_argmin", "whp_apply_swap",
            "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
-           "whp_eval_legsum", "whp_kmeans_slotting"]
+           "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move"]
 
 
 class WhpError(RuntimeError):
@@ -56,6 +56,8 @@ def lib():
         L.whp_get_penalty.argtypes = [vp, vp, vp, vp, vp]
         L.whp_eval_legsum.argtypes = [vp, vp, i64, vp, vp]
         L.whp_kmeans_slotting.argtypes = [i32, i32, i32, i32, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp]
+        L.whp_eval_moves.argtypes = [vp, vp, i32, i32, vp, vp, vp]
+        L.whp_apply_move.argtypes = [vp, vp, i32, i32, vp, vp]
         L.whp_launch_count.argtypes = [vp]
         L.whp_launch_count.restype = i64
         L.whp_destroy.argtypes = [vp]
@@ -188,6 +190,18 @@ class Context:
     def apply_swap(self, base_perm, win_start, win_len, idx, stream=None):
         import torch
         self._check(lib().whp_apply_swap(self._h, _d(base_perm, torch.int32), win_start, win_len,
+                                         _d(idx, torch.int64), _stream(stream)))
+
+    def eval_moves(self, base_perm, win_start, win_len, dist=None, obj=None, stream=None):
+        """NEXT-4 (reading N4): all W(W-1) insertion moves inside the window."""
+        import torch
+        self._check(lib().whp_eval_moves(self._h, _d(base_perm, torch.int32), win_start, win_len,
+                                         _d(dist, torch.int64), _d(obj, torch.float64),
+                                         _stream(stream)))
+
+    def apply_move(self, base_perm, win_start, win_len, idx, stream=None):
+        import torch
+        self._check(lib().whp_apply_move(self._h, _d(base_perm, torch.int32), win_start, win_len,
                                          _d(idx, torch.int64), _stream(stream)))
 
     def eval_legsum(self, perms, length, stream=None):

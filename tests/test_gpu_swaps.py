@@ -234,3 +234,104 @@ def test_nhatc_update_single_step(torch_cuda, ):
     t, v, w = ctx.get_penalty()
     assert v.tolist() == g["v_new"] and w.tolist() == g["w_new"] and t.tolist() == g["t"]
     ctx.close()
+
+
+# ---- NEXT-4: insertion moves ----------------------------------------------------------------------
+def gpu_moves(torch, ctx, base_dev, s, Wn):
+    nn = Wn * (Wn - 1)
+    d = torch.full((nn,), -1, dtype=torch.int64, device="cuda")
+    o = torch.zeros(nn, dtype=torch.float64, device="cuda")
+    ctx.eval_moves(base_dev, s, Wn, d, o)
+    torch.cuda.synchronize()
+    return d, o
+
+
+@pytest.mark.parametrize("name,s,Wn", [("tiny", 0, 20), ("tiny", 3, 7), ("mid", 0, 30),
+                                       ("mid", 111, 25), ("mid", 470, 30), ("mid", 250, 2)])
+def test_moves_match_oracle_every_neighbour(torch_cuda, name, s, Wn):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem(name)
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(0, pb.n_orders)
+    d, o = gpu_moves(torch, ctx, torch.from_numpy(base).cuda(), s, Wn)
+    ref = oracle.eval_moves(pb, base, s, Wn)
+    assert np.array_equal(d.cpu().numpy(), ref["dist"])
+    assert np.array_equal(o.cpu().numpy(), ref["obj"])
+    ctx.close()
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_moves_random_small_problems_and_trajectory(torch_cuda, seed):
+    """Small random problems (many slips and resynchronisations), then a short descent:
+    eval_moves -> argmin -> apply_move on the device against the same loop with the oracle."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    rng = np.random.default_rng(seed)
+    n = 48
+    q = rng.integers(1, 5, size=n)
+    ptr = np.concatenate([[0], np.cumsum(q)]).astype(np.int32)
+    pb = W.Problem(n_aisles=9, slots_per_side=6, slot_pitch=1, aisle_spacing=2, depot_aisle=seed,
+                   sku_loc=rng.integers(0, 108, size=30).astype(np.int32),
+                   sku_class=rng.integers(0, 5, size=30).astype(np.int32), n_classes=5,
+                   order_ptr=ptr, item_sku=rng.integers(0, 30, size=int(ptr[-1])).astype(np.int32),
+                   cart_capacity=6, t=rng.uniform(0, 9, 5), v=rng.uniform(0, 1, 5), w=rng.uniform(0, 1, 5))
+    ctx = whp.Context.from_problem(pb)
+    perm = W.base_perm(seed, n).copy()
+    dev = torch.from_numpy(perm).cuda()
+    idx = torch.zeros(1, dtype=torch.int64, device="cuda")
+    for it in range(4):
+        s0, Wn = (it * 7) % (n - 16 + 1), 16
+        d, o = gpu_moves(torch, ctx, dev, s0, Wn)
+        ref = oracle.eval_moves(pb, perm, s0, Wn)
+        assert np.array_equal(d.cpu().numpy(), ref["dist"]) and np.array_equal(o.cpu().numpy(), ref["obj"])
+        ctx.argmin(o, idx)
+        ctx.apply_move(dev, s0, Wn, idx)
+        torch.cuda.synchronize()
+        k = oracle.argmin(ref["obj"])
+        assert int(idx) == k
+        i, jr = divmod(k, Wn - 1)
+        j = jr if jr < i else jr + 1
+        moved = perm[s0 + i]
+        perm = np.insert(np.delete(perm, s0 + i), s0 + j, moved).astype(np.int32)
+        assert np.array_equal(dev.cpu().numpy(), perm)
+    ctx.close()
+
+
+@pytest.mark.parametrize("margin", ["0", "9"])
+def test_moves_chains_that_leave_the_tabulated_region(torch_cuda, margin):
+    import os
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid")
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(4, pb.n_orders)
+    ref = oracle.eval_moves(pb, base, 200, 24)
+    os.environ["WHP_SWAP_MARGIN"] = margin
+    try:
+        d, o = gpu_moves(torch, ctx, torch.from_numpy(base).cuda(), 200, 24)
+    finally:
+        os.environ.pop("WHP_SWAP_MARGIN")
+    assert np.array_equal(d.cpu().numpy(), ref["dist"]) and np.array_equal(o.cpu().numpy(), ref["obj"])
+    ctx.close()
+
+
+def test_moves_paper_scale_sampled(torch_cuda):
+    """All 65,280 moves of a 256-wide window at paper scale; the oracle re-evaluates sampled ones."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    wl = W.make_workload("paper")
+    pb = wl.problem
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(wl.seed, pb.n_orders)
+    s0, Wn = 1280, 256
+    d, o = gpu_moves(torch, ctx, torch.from_numpy(base).cuda(), s0, Wn)
+    d, o = d.cpu().numpy(), o.cpu().numpy()
+    rows = np.unique((W.stream_u64(5, 3, 150) % np.uint64(Wn * (Wn - 1))).astype(np.int64))
+    for k in rows:
+        i, jr = divmod(int(k), Wn - 1)
+        j = jr if jr < i else jr + 1
+        seq = np.insert(np.delete(base, s0 + i), s0 + j, base[s0 + i]).astype(np.int32)
+        one = oracle.eval_candidates(pb, seq)
+        assert d[k] == one["dist"][0] and o[k] == one["obj"][0]
+    ctx.close()
