@@ -231,6 +231,10 @@ def run_ours(args):
     torch.cuda.synchronize()
     moves_ms = ev0.elapsed_time(ev1)
 
+    # ---- measured L2 read bandwidth (not in MEASURED_PEAKS.json): 200 read-only
+    # sweeps of a 32 MB buffer that stays resident in the 126 MB L2, one launch
+    l2_gbs = ctx.probe_l2_read(32 << 20, 200)
+
     # ---- roofline of the dominant kernel (candidate evaluation) -----------------------------
     bytes_pc = harness.algorithmic_bytes_per_candidate(n, pb.n_items)
     peaks = harness.measured_peaks(ROOT)
@@ -243,6 +247,7 @@ def run_ours(args):
         "kernel_share_of_step": k_ms_max / ms_per_step,
         "frac_packed_bytes": bytes_pc["packed"] * n_cand / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"],
         "frac_hbm_compulsory": bytes_pc["hbm_compulsory"] * n_cand / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"],
+        "l2_read_gbs_measured": l2_gbs, "frac_of_l2_read_peak": achieved / l2_gbs,
     }
 
     if rank != 0:

@@ -181,6 +181,11 @@ whp_status whp_apply_move(whp_ctx* ctx, int32_t* d_base_perm, int32_t win_start,
 whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,
                               int64_t* h_n_bad, void* cuda_stream);
 
+/* Measurement helper (bench.py): *h_ms (host) = time of `reps` read-only sweeps (16-byte loads
+ * that bypass L1) of a `bytes`-sized buffer, which stays L2-resident when bytes is well below the
+ * L2 size. Allocates and frees its own buffer; synchronises. */
+whp_status whp_probe_l2_read(whp_ctx* ctx, int64_t bytes, int32_t reps, float* h_ms);
+
 /* Kernel launches issued by this ctx since creation (bench.py's gpu_launches claim). */
 int64_t whp_launch_count(const whp_ctx* ctx);
 

@@ -465,6 +465,16 @@ whp_status whp_get_penalty(whp_ctx* c, double* t, double* v, double* w, void* cu
   return WHP_OK;
 }
 
+whp_status whp_probe_l2_read(whp_ctx* c, int64_t bytes, int32_t reps, float* h_ms) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  if (!h_ms || bytes < 16 || reps < 1) return fail(c, WHP_ERR_INVALID_ARG, "bad argument");
+  device_guard dg(c->device);
+  WHP_CUDA(c, cudaDeviceSynchronize());
+  WHP_CUDA(c, whp_launch_l2_probe(c, bytes & ~(int64_t)15, reps, h_ms));
+  return WHP_OK;
+}
+
 void whp_destroy(whp_ctx* c) {
   if (!c) return;
   {

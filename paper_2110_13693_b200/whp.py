@@ -23,7 +23,8 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_eval_candidates_host", "whp_eval_swaps", "whp_argmin", "whp_apply_swap",
            "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
-           "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move"]
+           "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move",
+           "whp_probe_l2_read"]
 
 
 class WhpError(RuntimeError):
@@ -58,6 +59,7 @@ def lib():
         L.whp_kmeans_slotting.argtypes = [i32, i32, i32, i32, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp]
         L.whp_eval_moves.argtypes = [vp, vp, i32, i32, vp, vp, vp]
         L.whp_apply_move.argtypes = [vp, vp, i32, i32, vp, vp]
+        L.whp_probe_l2_read.argtypes = [vp, i64, i32, vp]
         L.whp_launch_count.argtypes = [vp]
         L.whp_launch_count.restype = i64
         L.whp_destroy.argtypes = [vp]
@@ -239,6 +241,12 @@ class Context:
         self._check(lib().whp_validate_perms(self._h, _d(perms, torch.int32), perms.shape[0],
                                              C.addressof(n_bad), _stream(stream)))
         return n_bad.value
+
+    def probe_l2_read(self, nbytes=32 << 20, reps=200) -> float:
+        """Measured L2 read bandwidth in GB/s (read-only sweeps of an L2-resident buffer)."""
+        ms = C.c_float(0.0)
+        self._check(lib().whp_probe_l2_read(self._h, nbytes, reps, C.byref(ms)))
+        return nbytes * reps / (ms.value * 1e-3) / 1e9
 
     def launch_count(self) -> int:
         return int(lib().whp_launch_count(self._h))

@@ -20,7 +20,7 @@ def so_path():
 def _declared_symbols():
     text = open(os.path.join(ROOT, "include", "whp.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(whp_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(whp_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_symbols_are_exported(so_path):
