@@ -289,6 +289,50 @@ whp_segments_kernel(const uint32_t* __restrict__ bmask, int32_t bm_pitch, int32_
     if (w == (n_orders >> 5)) x &= (1u << (n_orders & 31)) - 1u;  // drop the end sentinel
     return x;
   };
+  if (nw <= 128) {
+    // up to four 32-word chunks: one pass over the mask, everything kept in registers
+    uint32_t x[4];
+    int incl[4], tot[4];
+    int nb = 0;
+#pragma unroll
+    for (int ch = 0; ch < 4; ++ch) {
+      x[ch] = word_at(32 * ch + lane);
+      int v = __popc(x[ch]);
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int y = __shfl_up_sync(WHP_FULL, v, d);
+        if (lane >= d) v += y;
+      }
+      incl[ch] = v;
+      tot[ch] = __shfl_sync(WHP_FULL, v, 31);
+      nb += tot[ch];
+    }
+    if (lane == 0) {
+      nb_scratch[c] = nb;
+      if (n_batches_out) n_batches_out[c] = nb;
+    }
+    const int target = (int)(((int64_t)lane * nb) >> log2S);  // lane = segment
+    int base = 0;
+#pragma unroll
+    for (int ch = 0; ch < 4; ++ch) {
+      int lo = 0, hi = 31;  // smallest j with base + incl_j > target
+#pragma unroll
+      for (int it = 0; it < 5; ++it) {
+        const int mid = (lo + hi) >> 1;
+        const int im = __shfl_sync(WHP_FULL, incl[ch], mid);
+        if (base + im > target) hi = mid; else lo = mid + 1;
+      }
+      const uint32_t xj = __shfl_sync(WHP_FULL, x[ch], lo);
+      const int ej = __shfl_sync(WHP_FULL, incl[ch] - __popc(x[ch]), lo);
+      if (lane < S && target >= base && target < base + tot[ch]) {
+        uint32_t t = xj;
+        for (int r = target - base - ej; r > 0; --r) t &= t - 1;
+        segstart[c * ss_pitch + lane] = 32 * (32 * ch + lo) + __ffs(t) - 1;
+      }
+      base += tot[ch];
+    }
+    return;
+  }
   int nb = 0;
   for (int w0 = 0; w0 < nw; w0 += 32) nb += __reduce_add_sync(WHP_FULL, __popc(word_at(w0 + lane)));
   if (lane == 0) {
