@@ -18,6 +18,9 @@
  *   - eval / argmin / apply calls are asynchronous on `cuda_stream` (a cudaStream_t passed
  *     as void*; NULL = the legacy default stream). Argument errors are detected
  *     synchronously before anything is launched.
+ *   - A context owns scratch that its kernels share: calls on one context must not overlap in
+ *     time on different streams (serialise them, or use one context per stream). Contexts are
+ *     not thread-safe; different contexts are independent.
  *   - All arrays are dense, row-major, native-endian.
  *   - A row of d_perms that is not a permutation of 0..n_orders-1 is a precondition
  *     violation (entries outside [0,n_orders) would read out of bounds); use
@@ -25,6 +28,8 @@
  *
  * Limits (WHP_ERR_OUT_OF_RANGE beyond them): n_aisles <= 1024, slots_per_side <= 4095,
  *   n_classes <= 256, n_orders < 2^24, total items < 2^24, cart_capacity < 2^20.
+ *   The tuned kernels additionally need n_orders < 65536, cart_capacity <= 64 and pick cursors
+ *   that fit 16 bits; other shapes run the general (slower) kernels with the same results.
  */
 #ifndef WHP_H
 #define WHP_H
