@@ -28,8 +28,9 @@
  *
  * Limits (WHP_ERR_OUT_OF_RANGE beyond them): n_aisles <= 1024, slots_per_side <= 4095,
  *   n_classes <= 256, n_orders < 2^24, total items < 2^24, cart_capacity < 2^20.
- *   The tuned kernels additionally need n_orders < 65536, cart_capacity <= 64 and pick cursors
- *   that fit 16 bits; other shapes run the general (slower) kernels with the same results.
+ *   The tuned kernels additionally need n_orders < 65536, cart_capacity <= 106 and pick cursors
+ *   that fit 16 bits; other shapes run the general (slower) kernels with
+ *   the same results.
  */
 #ifndef WHP_H
 #define WHP_H

@@ -902,7 +902,7 @@ bool whp_fast_eligible(const whp_ctx* c) {
   if (!c->fast_tables_ok) return false;                       // cursors must fit 16 bits
   if (c->n_orders >= 65536) return false;
   if ((nb_upper_bound(c) + 31) / 32 > 255) return false;      // 8 counter planes, S <= 32
-  if (c->C > 64) return false;                                // per-lane cursor ring of 16 chunks
+  if ((c->C + 14) / 8 + 1 > 16) return false;                // per-lane cursor ring of 16 chunks (C <= 106)
   if (bounds_smem_bytes(c) > (size_t)c->smem_optin - 1024) return false;  // K1: order table in smem
   return true;
 }

@@ -253,6 +253,9 @@ EDGE = [
     dict(NA=400, S=4095, K=200, n_skus=3000, n_orders=332, qmax=255, C=600),
     dict(NA=40, S=50, K=20, n_skus=900, n_orders=2000, qmax=2, C=2),    # ~1,500 batches per plan
     dict(NA=40, S=50, K=20, n_skus=900, n_orders=64, qmax=3, C=100000), # one batch, huge cart
+    dict(NA=60, S=30, K=90, n_skus=700, n_orders=400, qmax=7, C=106),   # largest cart of the tuned path
+    dict(NA=60, S=30, K=90, n_skus=700, n_orders=403, qmax=7, C=65),    # 16-chunk cursor ring
+    dict(NA=60, S=30, K=90, n_skus=700, n_orders=401, qmax=7, C=107),   # one item more: general path
 ]
 
 
