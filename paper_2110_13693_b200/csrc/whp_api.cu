@@ -38,7 +38,7 @@ void dfree(T*& p) { if (p) { cudaFree(p); p = nullptr; } }
 void free_orders(whp_ctx* c) {
   dfree(c->d_order_rec); dfree(c->d_pick_rec); dfree(c->d_pick_fast); dfree(c->d_order_fast);
   dfree(c->base.bstart); dfree(c->base.bop); dfree(c->base.bdist);
-  dfree(c->base.resp); dfree(c->base.totals); dfree(c->base.ftotals); dfree(c->base.pre);
+  dfree(c->base.resp); dfree(c->base.totals); dfree(c->base.pre);
   dfree(c->base.orec); dfree(c->base.rpre); dfree(c->base.nxt); dfree(c->base.dist_at);
   dfree(c->base.cls_at); dfree(c->base.dtail); dfree(c->base.bF); dfree(c->base.rtail);
   c->rtail_rows = 0;
@@ -168,7 +168,6 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   WHP_CUDA(c, cudaMalloc(&c->base.bdist, 8 * (no + 1)));
   WHP_CUDA(c, cudaMalloc(&c->base.resp, 4 * (size_t)c->K));
   WHP_CUDA(c, cudaMalloc(&c->base.totals, 16));
-  WHP_CUDA(c, cudaMalloc(&c->base.ftotals, 16));
   WHP_CUDA(c, cudaMalloc(&c->base.pre, 4 * (no + 1)));
   WHP_CUDA(c, cudaMalloc(&c->base.orec, 4 * no));
   WHP_CUDA(c, cudaMalloc(&c->base.nxt, 4 * no));

@@ -75,7 +75,6 @@ struct whp_base_tables {
   int64_t* bdist;     // [n_orders+1] exclusive prefix sum of per-batch S-shape lengths
   int32_t* resp;      // [K]          base responses
   int64_t* totals;    // [2]          D_base, n_batches
-  double* ftotals;    // [2]          phi_base, J_base
   int32_t* pre;       // [n_orders+1] exclusive prefix of the item counts along the plan
   uint32_t* orec;     // [n_orders]   order record of every position
   int32_t* rpre;      // [nb_max+1][K] class-visit counts of the batches before b

@@ -212,16 +212,26 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
   int32_t* pre = smem_tables ? reinterpret_cast<int32_t*>(dyn) : B.pre;
   int32_t* nxt = smem_tables ? reinterpret_cast<int32_t*>(dyn) + (n + 1) : B.nxt;
 
-  // ---- A: order record of every position; exclusive prefix of the item counts
+  // ---- A: order record of every position; exclusive prefix of the item counts (four
+  // consecutive positions per thread: the dependent global loads of a round overlap)
   int32_t carry = 0;
-  for (int32_t p0 = 0; p0 < n; p0 += kBaseThreads) {
-    const int32_t p = p0 + tid;
-    uint32_t orec = 0;
-    if (p < n) { orec = __ldg(T.order_rec + __ldg(base_perm + p)); B.orec[p] = orec; }
-    const int32_t qv = (int32_t)(orec & WHP_Q_MASK);
+  for (int32_t p0 = 0; p0 < n; p0 += 4 * kBaseThreads) {
+    const int32_t pb = p0 + 4 * tid;
+    uint32_t orec[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) orec[k] = (pb + k < n) ? __ldg(T.order_rec + __ldg(base_perm + pb + k)) : 0u;
+    int32_t qs[4], sum = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { qs[k] = sum; sum += (int32_t)(orec[k] & WHP_Q_MASK); }
     int32_t tot;
-    const int32_t ex = block_excl_scan<int32_t>(qv, s_scan32, tot);
-    if (p < n) { pre[p] = carry + ex; if (smem_tables) B.pre[p] = carry + ex; }
+    const int32_t ex = block_excl_scan<int32_t>(sum, s_scan32, tot);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (pb + k < n) {
+        B.orec[pb + k] = orec[k];
+        pre[pb + k] = carry + ex + qs[k];
+        if (smem_tables) B.pre[pb + k] = carry + ex + qs[k];
+      }
     carry += tot;
   }
   if (tid == 0) { pre[n] = carry; B.pre[n] = carry; }
@@ -266,15 +276,24 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
       int32_t* tmp = J; J = Jn; Jn = tmp;
     }
     int32_t carry_b = 0;
-    for (int32_t p0 = 0; p0 < n; p0 += kBaseThreads) {
-      const int32_t p = p0 + tid;
-      const int32_t mk = (p < n) ? mark[p] : 0;
-      int32_t tot;
-      const int32_t ex = block_excl_scan<int32_t>(mk, s_scan32, tot);
-      if (p < n) {
-        if (mk) B.bstart[carry_b + ex] = p;
-        B.bop[p] = carry_b + ex + mk - 1;
+    for (int32_t p0 = 0; p0 < n; p0 += 4 * kBaseThreads) {  // four positions per thread
+      const int32_t pb = p0 + 4 * tid;
+      int32_t mk[4], before[4], sum = 0;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        mk[k] = (pb + k < n) ? mark[pb + k] : 0;
+        before[k] = sum;
+        sum += mk[k];
       }
+      int32_t tot;
+      const int32_t ex = block_excl_scan<int32_t>(sum, s_scan32, tot);
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (pb + k < n) {
+          const int32_t rank = carry_b + ex + before[k];
+          if (mk[k]) B.bstart[rank] = pb + k;
+          B.bop[pb + k] = rank + mk[k] - 1;
+        }
       carry_b += tot;
     }
     if (tid == 0) { B.bstart[carry_b] = n; s_nb = carry_b; }
@@ -291,33 +310,35 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
 }
 
 // Second half of the base pass, after whp_swaps_prep_kernel has scored the base batches
-// (dist_at / cls_at at their start positions): prefix of the batch lengths, class-count prefix,
-// base D, phi, J. One block.
+// (dist_at / cls_at at their start positions). Block w < KW: the class-count prefix rpre[b][k] of
+// the 32 classes of word w, in three steps over chunks of 32 batches — the chunk's visit totals
+// (32 ballots, one warp per chunk), a running sum of the totals over the chunks per class, then
+// a running count inside every chunk with one coalesced row store per batch. Block KW: the
+// prefix of the batch lengths (bdist[nb] = D_base).
 __global__ void __launch_bounds__(kBaseThreads)
 whp_swaps_base2_kernel(const whp_tables T, const whp_base_tables B) {
-  __shared__ int32_t s_resp[WHP_MAX_CLASSES];
   __shared__ int64_t s_scan64[33];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int32_t nb = (int32_t)B.totals[1];
   const int KW = (T.K + 31) >> 5;
-  for (int k = tid; k < WHP_MAX_CLASSES; k += kBaseThreads) s_resp[k] = 0;
-  // ---- E: exclusive prefix of the batch lengths (bdist[nb] = D_base), class-count prefix
-  int64_t carry64 = 0;
-  for (int32_t b0 = 0; b0 <= nb; b0 += kBaseThreads) {
-    const int32_t b = b0 + tid;
-    const int64_t x = (b < nb) ? B.dist_at[B.bstart[b]] : 0;
-    int64_t tot;
-    const int64_t ex = block_excl_scan<int64_t>(x, s_scan64, tot);
-    if (b <= nb) B.bdist[b] = carry64 + ex;
-    carry64 += tot;
+  if ((int)blockIdx.x == KW) {
+    int64_t carry64 = 0;
+    for (int32_t b0 = 0; b0 <= nb; b0 += kBaseThreads) {
+      const int32_t b = b0 + tid;
+      const int64_t x = (b < nb) ? B.dist_at[B.bstart[b]] : 0;
+      int64_t tot;
+      const int64_t ex = block_excl_scan<int64_t>(x, s_scan64, tot);
+      if (b <= nb) B.bdist[b] = carry64 + ex;
+      carry64 += tot;
+    }
+    if (tid == 0) B.totals[0] = carry64;
+    return;
   }
-  // rpre[b][k] = number of batches before b that visit class k, in three steps over chunks of
-  // 32 batches: per (class word, chunk) the chunk's visit totals (32 ballots), a running sum of
-  // the totals over the chunks per class, then a running count inside every chunk with one
-  // coalesced row store per batch.
+  const int w = blockIdx.x;
+  const bool mine = 32 * w + lane < T.K;
   const int32_t nchunks = (nb + 31) >> 5;
-  for (int32_t task = warp; task < KW * nchunks; task += kBaseThreads / 32) {
-    const int w = task % KW, c = task / KW;
+  int32_t* __restrict__ row = B.rpre + 32 * w + lane;
+  for (int32_t c = warp; c < nchunks; c += kBaseThreads / 32) {
     const int32_t b = 32 * c + lane;
     const uint32_t word = (b < nb) ? B.cls_at[(int64_t)B.bstart[b] * 8 + w] : 0u;
     int32_t tot = 0;
@@ -326,45 +347,28 @@ whp_swaps_base2_kernel(const whp_tables T, const whp_base_tables B) {
       const int32_t pc = __popc(__ballot_sync(WHP_FULL, (word >> j) & 1u));
       if (lane == j) tot = pc;
     }
-    // parked in row 32c+1 (rewritten in the last step)
-    if (32 * w + lane < T.K) B.rpre[(int64_t)(32 * c + 1) * T.K + 32 * w + lane] = tot;
+    if (mine) row[(int64_t)(32 * c + 1) * T.K] = tot;  // parked in row 32c+1 (rewritten below)
   }
   __syncthreads();
-  for (int k = tid; k < T.K; k += kBaseThreads) {
+  if (warp == 0 && mine) {
     int32_t run = 0;
     for (int32_t c = 0; c < nchunks; ++c) {
-      const int32_t t = B.rpre[(int64_t)(32 * c + 1) * T.K + k];
-      B.rpre[(int64_t)(32 * c) * T.K + k] = run;
+      const int32_t t = row[(int64_t)(32 * c + 1) * T.K];
+      row[(int64_t)(32 * c) * T.K] = run;
       run += t;
     }
-    if (nchunks == 0) B.rpre[k] = 0;
-    B.resp[k] = run;
-    s_resp[k] = run;
+    if (nchunks == 0) row[0] = 0;
+    B.resp[32 * w + lane] = run;
   }
   __syncthreads();
-  for (int32_t task = warp; task < KW * nchunks; task += kBaseThreads / 32) {
-    const int w = task % KW, c = task / KW;
+  for (int32_t c = warp; c < nchunks; c += kBaseThreads / 32) {
     const int32_t b = 32 * c + lane;
     const uint32_t word = (b < nb) ? B.cls_at[(int64_t)B.bstart[b] * 8 + w] : 0u;
-    const bool mine = 32 * w + lane < T.K;
-    int32_t* __restrict__ row = B.rpre + 32 * w + lane;
     int32_t cnt = mine ? row[(int64_t)(32 * c) * T.K] : 0;
     const int nbb = min(32, nb - 32 * c);
     for (int bb = 0; bb < nbb; ++bb) {
       cnt += (int32_t)((__shfl_sync(WHP_FULL, word, bb) >> lane) & 1u);
       if (mine) row[(int64_t)(32 * c + bb + 1) * T.K] = cnt;
-    }
-  }
-  __syncthreads();
-  if (warp == 0) {
-    int32_t r[8];
-#pragma unroll
-    for (int w = 0; w < 8; ++w) r[w] = (32 * w + lane < T.K) ? s_resp[32 * w + lane] : 0;
-    const double phi = penalty_regs(T, r);
-    if (lane == 0) {
-      B.totals[0] = carry64;
-      B.ftotals[0] = phi;
-      B.ftotals[1] = __dadd_rn((double)carry64, phi);
     }
   }
 }
@@ -513,9 +517,13 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
     // a smaller order arriving at the opening position of a cart may slip into the cart before
     const bool slip = q.delta < 0 && bi > 0 && pi == __ldg(B.bstart + bi);
     if (bi == bj && !slip) {  // both orders stay in the same cart: nothing changes
+      int32_t rb[8];
+#pragma unroll
+      for (int w = 0; w < 8; ++w) rb[w] = (32 * w + lane < T.K) ? __ldg(B.resp + 32 * w + lane) : 0;
+      const double phi_base = penalty_regs(T, rb);
       if (lane == 0) {
         if (d_dist) d_dist[nn] = D_base;
-        if (d_obj) d_obj[nn] = B.ftotals[1];
+        if (d_obj) d_obj[nn] = __dadd_rn((double)D_base, phi_base);
       }
       continue;
     }
@@ -790,7 +798,7 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
                           kPrepWarps * 32, 0, st>>>(T, c->base, rlo, rhi);
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  whp_swaps_base2_kernel<<<1, kBaseThreads, 0, st>>>(T, c->base);
+  whp_swaps_base2_kernel<<<(unsigned)((c->K + 31) / 32 + 1), kBaseThreads, 0, st>>>(T, c->base);
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   // chain sums of the region (rtail grows with the region)
