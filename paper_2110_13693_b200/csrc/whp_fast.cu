@@ -421,7 +421,7 @@ __device__ __forceinline__ void lds16_if(uint32_t& v, uint32_t a, bool p) {
 }
 
 template <bool SMEM_TABLES, bool DEPOT0, int KW, int kPlanes>
-__global__ void __launch_bounds__(kPlanes <= 6 ? 768 : 512, 1)
+__global__ void __launch_bounds__(KW * kPlanes <= 42 ? 768 : 512, 1)  // counter registers: KW x planes
 whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restrict__ pick_fast,
                 const uint16_t* __restrict__ cstream, const uint32_t* __restrict__ bmask,
                 const int32_t* __restrict__ nb_scratch, const int32_t* __restrict__ segstart,
@@ -1034,7 +1034,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   int seg_planes = 1;  // planes of one segment's counters; one more per combine level
   while ((1ll << seg_planes) <= (nb_ub + S - 1) / S) ++seg_planes;
   const int kernel_planes = seg_planes <= 4 ? 4 : seg_planes <= 6 ? 6 : 8;  // the instantiation
-  if (kernel_planes > 6) warps_cap = 16;  // __launch_bounds__ of the 8-plane instantiation
+  if (KW * kernel_planes > 42) warps_cap = 16;  // __launch_bounds__ of the register-heavy instantiations
   int warps = (int)(avail / priv_per_warp);
   if (warps > warps_cap) warps = warps_cap;
   if (const char* e = getenv("WHP_WARPS")) { int v = atoi(e); if (v >= 1 && v <= warps) warps = v; }
