@@ -65,7 +65,6 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
 // conflict-free. The loop is software-pipelined by hand — while the recurrence runs over word w,
 // the order ids of word w+1 leave the tile and their order records are gathered from the table
 // in shared memory — so that a lone warp per scheduler keeps issuing.
-constexpr int kBoundsThreads = 32;   // plans per block, one per thread (a warp = 32 rows)
 constexpr int kStages = 7;           // tiles (words) in flight per warp
 constexpr int kTileBytes = 32 * 128; // 32 rows x 32 positions x 4 B
 
@@ -172,7 +171,8 @@ __device__ __forceinline__ uint32_t recur_word(const uint32_t (&r)[32], uint32_t
   return ~__brev(rev);
 }
 
-__global__ void __launch_bounds__(kBoundsThreads)
+template <int kWarps>  // warps per block: they share the order table (a warp = 32 plans)
+__global__ void __launch_bounds__(32 * kWarps)
 whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_cs,
                   const uint32_t* __restrict__ order_fast,
                   int32_t n_orders, int32_t C, int64_t n_cand, uint32_t* __restrict__ bmask,
@@ -182,7 +182,6 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   // the order table shared by the block's warps and the mbarriers (kStages per warp + 1)
   const int nw = (n_orders + 31) >> 5;
   const int lane = threadIdx.x & 31, wq = threadIdx.x >> 5;
-  constexpr int kWarps = kBoundsThreads / 32;
   const uint32_t area = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t tiles = area + wq * (kStages + 2) * kTileBytes;
   const uint32_t otiles = tiles + kStages * kTileBytes;  // 32 rows x 64 cursors, two of them
@@ -880,9 +879,19 @@ static int64_t nb_upper_bound(const whp_ctx* c) {
   return ub < c->n_orders ? ub : c->n_orders;
 }
 
-static size_t bounds_smem_bytes(const whp_ctx* c) {
-  return 1024 + (size_t)(kBoundsThreads / 32) * (kStages + 2) * kTileBytes +
-         4 * (((size_t)c->n_orders + 3) & ~(size_t)3) + 8 * ((kBoundsThreads / 32) * kStages + 1);
+static size_t bounds_smem_bytes(const whp_ctx* c, int warps = 1) {
+  return 1024 + (size_t)warps * (kStages + 2) * kTileBytes +
+         4 * (((size_t)c->n_orders + 3) & ~(size_t)3) + 8 * ((size_t)warps * kStages + 1);
+}
+// K1 wants four resident warps per SM (one per scheduler): blocks of one warp when four of
+// them fit, else two or four warps that share one copy of the order table
+static int bounds_warps(const whp_ctx* c) {
+  const size_t cap = (size_t)c->smem_optin;
+  if (4 * (bounds_smem_bytes(c, 1) + 1024) <= cap) return 1;
+  if (2 * (bounds_smem_bytes(c, 2) + 1024) <= cap) return 2;
+  if (bounds_smem_bytes(c, 4) + 1024 <= cap) return 4;
+  if (bounds_smem_bytes(c, 2) + 1024 <= cap) return 2;
+  return 1;
 }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
@@ -943,7 +952,8 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms
   {
     cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
-    const size_t smem = bounds_smem_bytes(c);
+    const int kw1 = bounds_warps(c);
+    const size_t smem = bounds_smem_bytes(c, kw1);
     // tensor map over this call's permutation matrix: [n_cand][n_orders] int32, box 32 x 32
     PFN_cuTensorMapEncodeTiled encode = tensor_map_encoder();
     if (!encode) return cudaErrorNotSupported;
@@ -984,12 +994,19 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms
                estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
-    cudaFuncSetAttribute(whp_bounds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                         c->smem_optin - 1024);
-    const unsigned blocks = (unsigned)((n_cand + kBoundsThreads - 1) / kBoundsThreads);
-    whp_bounds_kernel<<<blocks, kBoundsThreads, smem, st>>>(
-        tmap, tmap_cs, c->d_order_fast, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch, c->d_cstream,
-        cs_pitch);
+    const unsigned blocks = (unsigned)((n_cand + 32 * kw1 - 1) / (32 * kw1));
+#define WHP_LAUNCH_BOUNDS(KW1)                                                                  \
+  do {                                                                                          \
+    cudaFuncSetAttribute(whp_bounds_kernel<KW1>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                         c->smem_optin - 1024);                                                 \
+    whp_bounds_kernel<KW1><<<blocks, 32 * KW1, smem, st>>>(                                     \
+        tmap, tmap_cs, c->d_order_fast, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch,        \
+        c->d_cstream, cs_pitch);                                                                \
+  } while (0)
+    if (kw1 == 1) WHP_LAUNCH_BOUNDS(1);
+    else if (kw1 == 2) WHP_LAUNCH_BOUNDS(2);
+    else WHP_LAUNCH_BOUNDS(4);
+#undef WHP_LAUNCH_BOUNDS
     c->launches += 1;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
     whp_segments_kernel<<<(unsigned)((n_cand * 32 + 255) / 256), 256, 0, st>>>(
