@@ -17,8 +17,14 @@
  * Pin status: D0/D4 pinned by closed forms + brute-force optimal route (P1–P4, E1–E3);
  * D2 by batching invariants (P5) and E4–E6; D5/D6 by E4–E6, K=1 closed form and a long-double
  * cross-sum (P6, P8); D7 by P9; D8 by E6 and by equality with materialised permutations (P7).
+ * NEXT rows (each section below cites its passage and reading): NHATC update N1 pinned by a
+ * hand-worked step, special cases and exact rationals; leg sums N2 by hand-worked tours, the
+ * one-pick closed form and min-over-orderings = exhaustive optimum; K-means slotting N3 by a
+ * hand-worked example and nearest-centroid / SSE / exact-mean / contiguity invariants;
+ * insertion moves N4 against independently materialised sequences, swaps and E6.
  * "Parity unpinned" BY THE PAPER (it prints no formula for them): the choice of r_k (Q9), the
- * geometry constants (Q2–Q3) — they are pinned only to DESIGN.md's readings and hand-worked
+ * geometry constants (Q2–Q3), the update rule N1, the tour convention N2, the K-means details
+ * N3 and the move definition N4 — they are pinned only to DESIGN.md's readings and hand-worked
  * examples.
  */
 #include <stdint.h>
