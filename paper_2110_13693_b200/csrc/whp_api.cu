@@ -6,6 +6,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <algorithm>
 #include <vector>
 
 #include "whp_internal.cuh"
@@ -160,6 +161,20 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   WHP_CUDA(c, cudaDeviceSynchronize());  // nothing may still be reading the old tables
   free_orders(c);
   c->n_orders = n_orders; c->n_items = n_items; c->C = cart_capacity;
+  {
+    // Upper bound on the batch count of any plan. A cart b closes because the first order f of
+    // cart b+1 does not fit: load_b >= C + 1 - q_f. The nb-1 openers are distinct orders, so
+    // (nb-1)(C+1) - (sum of the nb-1 largest counts) <= n_items - 1; the left side grows with nb.
+    std::vector<int32_t> qs((size_t)n_orders);
+    for (int32_t o = 0; o < n_orders; ++o) qs[o] = order_ptr[o + 1] - order_ptr[o];
+    std::sort(qs.begin(), qs.end(), [](int32_t a, int32_t b) { return a > b; });
+    int64_t m = 0, top = 0;
+    while (m < n_orders && (m + 1) * ((int64_t)cart_capacity + 1) - (top + qs[(size_t)m]) <= (int64_t)n_items - 1) {
+      top += qs[(size_t)m];
+      ++m;
+    }
+    c->nb_ub = 1 + m < n_orders ? 1 + m : n_orders;
+  }
   const size_t no = (size_t)n_orders;
   WHP_CUDA(c, cudaMalloc(&c->d_order_rec, 4 * no));
   WHP_CUDA(c, cudaMalloc(&c->d_pick_rec, 4 * (size_t)n_items));

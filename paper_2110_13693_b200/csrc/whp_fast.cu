@@ -873,11 +873,8 @@ whp_finish_kernel(const whp_tables T, int64_t n_cand, const int64_t* __restrict_
 
 }  // namespace
 
-// nb <= 2*n_items/(C+1) + 1: consecutive next-fit batches together hold more than C items
-static int64_t nb_upper_bound(const whp_ctx* c) {
-  int64_t ub = 2ll * c->n_items / ((int64_t)c->C + 1) + 1;
-  return ub < c->n_orders ? ub : c->n_orders;
-}
+// upper bound on the number of batches of any plan (derived in whp_load_orders)
+static int64_t nb_upper_bound(const whp_ctx* c) { return c->nb_ub; }
 
 static size_t bounds_smem_bytes(const whp_ctx* c, int warps = 1) {
   return 1024 + (size_t)warps * (kStages + 2) * kTileBytes +

@@ -94,6 +94,7 @@ struct whp_ctx {
   int32_t* h_sku_class = nullptr;
   // orders
   int32_t n_orders = 0, n_items = 0, C = 0;
+  int64_t nb_ub = 0;  // upper bound on the number of batches of ANY plan (whp_load_orders)
   uint32_t* d_order_rec = nullptr;
   uint32_t* d_pick_rec = nullptr;
   // tuned-path tables: every order's picks start at an even index (one pad word after an odd

@@ -449,6 +449,50 @@ def test_kmeans_slotting_hand_worked_and_errors(torch_cuda):
         whp.kmeans_slotting(3, 2, 0, 6, items + [6], 2, 1, 3)  # SKU id out of range
 
 
+def _adversarial_perm(pb):
+    """A plan with (nearly) as many carts as possible: every cart is filled with small orders just
+    far enough that the next, large order does not fit — the situation the static bound on the
+    batch count (and with it the number of counter planes of K2) has to cover."""
+    q = np.diff(pb.order_ptr)
+    C = pb.cart_capacity
+    big = list(np.argsort(-q, kind="stable"))          # large orders open the carts
+    small = list(np.argsort(q, kind="stable"))         # small orders fill them
+    used = np.zeros(len(q), bool)
+    perm, load, bi, si = [], 0, 0, 0
+    while len(perm) < len(q):
+        while bi < len(big) and used[big[bi]]:
+            bi += 1
+        while si < len(small) and used[small[si]]:
+            si += 1
+        if bi >= len(big):
+            break
+        b = big[bi]
+        if load + q[b] > C or si >= len(small) or small[si] == b:
+            perm.append(b); used[b] = True                # opens a new cart (or nothing else left)
+            load = q[b] if load + q[b] > C else load + q[b]
+        else:
+            s_ = small[si]
+            perm.append(s_); used[s_] = True
+            load = q[s_] if load + q[s_] > C else load + q[s_]
+    return np.array(perm, dtype=np.int32)
+
+
+@pytest.mark.parametrize("name", ["mid", "paper"])
+def test_many_cart_plans_stay_within_the_counter_planes(torch_cuda, name):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem(name)
+    adv = _adversarial_perm(pb)
+    assert sorted(adv.tolist()) == list(range(pb.n_orders))
+    perms = np.stack([adv, adv[::-1].copy(), W.perm_rows(0, pb.n_orders, [0])[0]] * 11).astype(np.int32)
+    ctx = whp.Context.from_problem(pb)
+    got, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=False)
+    ref = oracle.eval_candidates(pb, perms)
+    assert ref["n_batches"][0] > 1.1 * ref["n_batches"][2]        # really more carts than a random plan
+    assert_parity(got, ref, pb)
+    ctx.close()
+
+
 def test_api_errors_and_nullable_outputs(torch_cuda):
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
