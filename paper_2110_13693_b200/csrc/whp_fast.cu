@@ -426,7 +426,8 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
                 const int32_t* __restrict__ nb_scratch, const int32_t* __restrict__ segstart,
                 int64_t n_cand, int64_t* __restrict__ dist_scratch,
                 uint32_t* __restrict__ planes_out, uint64_t* __restrict__ hash_out,
-                unsigned long long* __restrict__ task_counter) {
+                unsigned long long* __restrict__ task_counter, int64_t* __restrict__ o_dist,
+                double* __restrict__ o_pen, double* __restrict__ o_obj, int32_t* __restrict__ o_resp) {
   extern __shared__ __align__(16) uint32_t smem[];
   // layout: [pick table n_items_pad] (if staged) [per-warp private words]
   uint32_t* priv = smem;
@@ -624,10 +625,12 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         D += __shfl_xor_sync(WHP_FULL, D, o);
         hash += __shfl_xor_sync(WHP_FULL, hash, o);
       }
+    const bool fused = P.S == 32;  // the warp is one plan: it finishes D6 itself (no K3)
     if (have && seg == 0) {
-      dist_scratch[cand] = D;
+      if (!fused) dist_scratch[cand] = D;
       if (hash_out) hash_out[cand] = hash;
     }
+    double phi = 0.0;
     // bit-sliced addition of the S lanes' vertical counters (one more plane per level)
     {
       uint32_t* __restrict__ po = planes_out + cand * (kPlaneRow * KW);
@@ -650,18 +653,33 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
             a[kPlanes + lvl] = carry;
           }
         }
-        if (P.S == 32) {
-          // the warp is one plan and every lane holds its counters: lane l decodes r_k of class
-          // 32w + l and K3 reads the counts directly
+        if (fused) {
+          // every lane holds the plan's counters: lane l decodes r_k of class 32w + l and adds
+          // its term — ascending w, lane = k mod 32: the canonical accumulation of D6
           uint32_t r = 0;
 #pragma unroll
           for (int pp = 0; pp < kPlanes + 5; ++pp) r |= ((a[pp] >> lane) & 1u) << pp;
-          if (have) reinterpret_cast<uint16_t*>(po)[32 * w + lane] = (uint16_t)r;
+          const int k = 32 * w + lane;
+          if (k < T.K) {
+            if (o_resp && have) o_resp[cand * T.K + k] = (int32_t)r;
+            const double c = __dsub_rn(__ldg(T.tvw + k), (double)r);
+            const double u = __dmul_rn(__ldg(T.tvw + 2 * T.K + k), c);
+            phi = __dadd_rn(phi, __dadd_rn(__dmul_rn(__ldg(T.tvw + T.K + k), c), __dmul_rn(u, u)));
+          }
         } else if (have && seg == 0) {
 #pragma unroll
           for (int pp = 0; pp < kPlanes + 5; ++pp)
             if (pp < kPlanes + P.log2S) po[pp * KW + w] = a[pp];
         }
+      }
+    }
+    if (fused) {
+#pragma unroll
+      for (int off = 16; off >= 1; off >>= 1) phi = __dadd_rn(phi, __shfl_xor_sync(WHP_FULL, phi, off));
+      if (have && lane == 0) {
+        if (o_dist) o_dist[cand] = D;
+        if (o_pen) o_pen[cand] = phi;
+        if (o_obj) o_obj[cand] = __dadd_rn((double)D, phi);
       }
     }
     __syncwarp();
@@ -1080,7 +1098,8 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(c->smem_optin - 1024)); \
     whp_sets_kernel<ST, D0, KWV, PLV><<<(unsigned)blocks, warps * 32, smem, st>>>(               \
         T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand,          \
-        c->d_dist_scratch, c->d_planes, out.batch_hash, c->d_task);                              \
+        c->d_dist_scratch, c->d_planes, out.batch_hash, c->d_task, out.dist, out.penalty,      \
+        out.obj, out.resp);                                                                      \
   } while (0)
 #define WHP_LAUNCH_SETS(ST, D0, KWV)                                                             \
   do {                                                                                           \
@@ -1115,7 +1134,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
     if (e != cudaSuccess) return e;
   }
   // K3
-  if (out.dist || out.penalty || out.obj || out.resp) {
+  if (S != 32 && (out.dist || out.penalty || out.obj || out.resp)) {  // S = 32: K2 finished D6 itself
     const unsigned blocks = (unsigned)((n_cand * 32 + 255) / 256);
     whp_finish_kernel<<<blocks, 256, 0, st>>>(T, n_cand, c->d_dist_scratch, c->d_planes, KW,
                                               S == 32 ? 0 : planes_used, out.dist, out.penalty, out.obj,
