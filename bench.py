@@ -33,7 +33,7 @@ CPU_SAMPLE = 8192   # candidates the oracle is timed on for cpu_baseline (~12 s 
 REF_SAMPLE = 512    # candidates per step of --impl reference
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the candidate kernel, from the
 # ncu --set full capture recorded in profiles/ (None until measured for the current kernel)
-NCU_TRAFFIC_BYTES = 531.4e6  # K1 366.6 + segments 8.4 + K2 150.3 + K3 6.1 MB (profiles/r1_v6_tuned_path.md)
+NCU_TRAFFIC_BYTES = 521.3e6  # K1 367.2 + segments 8.4 + K2 145.7 MB (profiles/r1_v11_tuned_path.md)
 
 
 def config_dict(pb, n_cand, world, wl_nb):
@@ -240,7 +240,7 @@ def run_ours(args):
     peaks = harness.measured_peaks(ROOT)
     achieved = bytes_pc["survey"] * n_cand / (k_ms_max * 1e-3) / 1e9
     roofline = {
-        "bound": "hbm", "kernel": "whp_eval_candidates (bounds + segments + sets + finish kernels)", "achieved": achieved,
+        "bound": "hbm", "kernel": "whp_eval_candidates (bounds + segments + sets kernels)", "achieved": achieved,
         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
         "traffic": NCU_TRAFFIC_BYTES, "peak_source": peaks["source"] + ", burst copy figure",
         "bytes_per_candidate": bytes_pc["survey"], "kernel_ms": k_ms_max,
