@@ -192,6 +192,12 @@ whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_ca
  * L2 size. Allocates and frees its own buffer; synchronises. */
 whp_status whp_probe_l2_read(whp_ctx* ctx, int64_t bytes, int32_t reps, float* h_ms);
 
+/* Upper bound on the number of carts of ANY plan over the loaded orders (0 before
+ * whp_load_orders): the first orders of carts 1..nb-1 are distinct and each did not fit, so
+ * (nb-1)(C+1) - (sum of the nb-1 largest item counts) <= n_items - 1. The tuned kernels size
+ * their per-segment counters with it. */
+int64_t whp_max_batches(const whp_ctx* ctx);
+
 /* Kernel launches issued by this ctx since creation (bench.py's gpu_launches claim). */
 int64_t whp_launch_count(const whp_ctx* ctx);
 

@@ -70,6 +70,8 @@ const char* whp_last_error(const whp_ctx* c) { return c ? c->err.c_str() : "null
 
 int64_t whp_launch_count(const whp_ctx* c) { return c ? c->launches : 0; }
 
+int64_t whp_max_batches(const whp_ctx* c) { return (c && c->have_orders) ? c->nb_ub : 0; }
+
 whp_status whp_create_layout(int32_t n_aisles, int32_t slots_per_side, int32_t slot_pitch,
                              int32_t aisle_spacing, int32_t depot_aisle, int32_t n_skus,
                              const int32_t* sku_loc, const int32_t* sku_class, int32_t n_classes,

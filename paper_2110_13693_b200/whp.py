@@ -24,7 +24,7 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
            "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move",
-           "whp_probe_l2_read"]
+           "whp_probe_l2_read", "whp_max_batches"]
 
 
 class WhpError(RuntimeError):
@@ -60,6 +60,8 @@ def lib():
         L.whp_eval_moves.argtypes = [vp, vp, i32, i32, vp, vp, vp]
         L.whp_apply_move.argtypes = [vp, vp, i32, i32, vp, vp]
         L.whp_probe_l2_read.argtypes = [vp, i64, i32, vp]
+        L.whp_max_batches.argtypes = [vp]
+        L.whp_max_batches.restype = i64
         L.whp_launch_count.argtypes = [vp]
         L.whp_launch_count.restype = i64
         L.whp_destroy.argtypes = [vp]
@@ -247,6 +249,9 @@ class Context:
         ms = C.c_float(0.0)
         self._check(lib().whp_probe_l2_read(self._h, nbytes, reps, C.byref(ms)))
         return nbytes * reps / (ms.value * 1e-3) / 1e9
+
+    def max_batches(self) -> int:
+        return int(lib().whp_max_batches(self._h))
 
     def launch_count(self) -> int:
         return int(lib().whp_launch_count(self._h))

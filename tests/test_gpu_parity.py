@@ -493,6 +493,37 @@ def test_many_cart_plans_stay_within_the_counter_planes(torch_cuda, name):
     ctx.close()
 
 
+def test_batch_count_bound_holds_for_every_permutation(torch_cuda):
+    """whp_max_batches sizes K2's counters: it must bound the cart count of EVERY plan. Checked
+    exhaustively (all 5,040 orders of 7 orders, several random problems) and on the adversarial
+    plans of the named workloads; it is also reasonably tight."""
+    import itertools
+    from paper_2110_13693_b200 import whp
+    rng = np.random.default_rng(9)
+    for trial in range(6):
+        C = int(rng.integers(3, 9))
+        q = rng.integers(1, min(C, 5) + 1, size=7)
+        ptr = np.concatenate([[0], np.cumsum(q)]).astype(np.int32)
+        pb = W.Problem(n_aisles=3, slots_per_side=4, slot_pitch=1, aisle_spacing=2, depot_aisle=0,
+                       sku_loc=np.arange(10, dtype=np.int32), sku_class=np.zeros(10, np.int32),
+                       n_classes=1, order_ptr=ptr,
+                       item_sku=rng.integers(0, 10, size=int(ptr[-1])).astype(np.int32),
+                       cart_capacity=C, t=np.zeros(1), v=np.zeros(1), w=np.zeros(1))
+        ctx = whp.Context.from_problem(pb)
+        bound = ctx.max_batches()
+        perms = np.array(list(itertools.permutations(range(7))), dtype=np.int32)
+        nb = oracle.eval_candidates(pb, perms)["n_batches"]
+        assert nb.max() <= bound <= nb.max() + 1, (q, C, nb.max(), bound)
+        ctx.close()
+    for name in ("mid", "paper", "stress"):
+        pb = W.make_problem(name)
+        ctx = whp.Context.from_problem(pb)
+        adv = _adversarial_perm(pb)
+        nb = oracle.eval_candidates(pb, adv)["n_batches"][0]
+        assert nb <= ctx.max_batches() <= 1.12 * nb
+        ctx.close()
+
+
 def test_api_errors_and_nullable_outputs(torch_cuda):
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
