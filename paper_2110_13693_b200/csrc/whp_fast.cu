@@ -413,6 +413,32 @@ __device__ __forceinline__ uint32_t lds16(uint32_t a) {
   uint32_t v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a)); return v;
 }
 
+// One step's cursor transition for pick tables in shared memory, written in PTX so that the bit
+// test lands in a predicate and every update is a single predicated instruction:
+//   last = rec & LAST;  more = last && v != v_end;
+//   cur  = more ? pb + 8 * n_c16 : (last ? cur : cur + 4);
+//   if (more) { v += 2;  n_c16 = ld.shared.u16 [ringbase + (v & ring_mask)]; }
+__device__ __forceinline__ void step_cursor(uint32_t rec, uint32_t& cur, uint32_t& v, uint32_t v_end,
+                                            uint32_t& n_c16, uint32_t pb, uint32_t ringbase,
+                                            uint32_t ring_mask) {
+  asm volatile(
+      "{\n"
+      ".reg .pred pl, pm;\n"
+      ".reg .b32 t;\n"
+      "and.b32 t, %3, 0x20;\n"
+      "setp.ne.u32 pl, t, 0;\n"
+      "setp.ne.and.u32 pm, %1, %4, pl;\n"
+      "@!pl add.u32 %0, %0, 4;\n"
+      "@pm mad.lo.u32 %0, %2, 8, %5;\n"
+      "@pm add.u32 %1, %1, 2;\n"
+      "and.b32 t, %1, %7;\n"
+      "add.u32 t, t, %6;\n"
+      "@pm ld.shared.u16 %2, [t];\n"
+      "}\n"
+      : "+r"(cur), "+r"(v), "+r"(n_c16)
+      : "r"(rec), "r"(v_end), "r"(pb), "r"(ringbase), "r"(ring_mask));
+}
+
 // if (p) v = ld.shared.u16 [a] — predicated, never a branch; idle lanes cost no bank cycle
 __device__ __forceinline__ void lds16_if(uint32_t& v, uint32_t a, bool p) {
   asm volatile("{ .reg .pred pq; setp.ne.u32 pq, %2, 0; @pq ld.shared.u16 %0, [%1]; }"
@@ -547,14 +573,18 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       for (int t = 0; t < Cmax; ++t) {
         // cursor of the next step's pick: next record, the next order's first pick, or stay —
         // all by selects and one predicated load
-        const uint32_t first_of_next = SMEM_TABLES ? pb + 8 * n_c16 : 2 * n_c16;
-        const bool last = (int32_t)(rec << 26) < 0;  // WHP_FAST_LAST (bit 5) into the sign bit
-        const bool more = last && (v != v_end);
-        uint32_t nxt = last ? cur : cur + (SMEM_TABLES ? 4u : 1u);
-        nxt = more ? first_of_next : nxt;
-        v = more ? v + 2 : v;
-        lds16_if(n_c16, ringbase + (v & P.ring_mask), more);  // the look-ahead cursor
-        cur = nxt;
+        if (SMEM_TABLES) {
+          step_cursor(rec, cur, v, v_end, n_c16, pb, ringbase, (uint32_t)P.ring_mask);
+        } else {
+          const uint32_t first_of_next = 2 * n_c16;
+          const bool last = (int32_t)(rec << 26) < 0;  // WHP_FAST_LAST (bit 5) into the sign bit
+          const bool more = last && (v != v_end);
+          uint32_t nxt = last ? cur : cur + 1u;
+          nxt = more ? first_of_next : nxt;
+          v = more ? v + 2 : v;
+          lds16_if(n_c16, ringbase + (v & P.ring_mask), more);  // the look-ahead cursor
+          cur = nxt;
+        }
         const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
         // ---- this step's pick
         kmax = max(kmax, rec);
