@@ -21,6 +21,13 @@
  *   - A context owns scratch that its kernels share: calls on one context must not overlap in
  *     time on different streams (serialise them, or use one context per stream). Contexts are
  *     not thread-safe; different contexts are independent.
+ *   - CUDA graphs: scratch grows on the first call that needs more of it (that call allocates
+ *     and synchronises the stream). Once every call of a loop has run once at its sizes, the
+ *     calls that take a `cuda_stream` neither allocate nor synchronise and may be captured
+ *     (cudaStreamBeginCapture ... EndCapture) and replayed; scalar arguments such as win_start
+ *     are baked into the captured launches. Calls that hand a value back to the host
+ *     (the *_host entry points, whp_validate_perms, whp_get_penalty, whp_probe_l2_read)
+ *     synchronise and cannot be captured.
  *   - All arrays are dense, row-major, native-endian.
  *   - A row of d_perms that is not a permutation of 0..n_orders-1 is a precondition
  *     violation (entries outside [0,n_orders) would read out of bounds); use

@@ -153,6 +153,64 @@ def test_trajectory_mid_move_for_move(torch_cuda):
     ctx.close()
 
 
+def test_trajectory_replayed_from_a_cuda_graph(torch_cuda):
+    """After one eager pass (which sizes the context's scratch) every call of the loop is
+    asynchronous and allocation-free, so the whole trajectory — and a candidate evaluation with
+    its argmin — can be captured in a CUDA graph. A replay must reproduce the oracle's trajectory
+    move for move, twice."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid")
+    ctx = whp.Context.from_problem(pb)
+    n = pb.n_orders
+    base_np = W.base_perm(0, n)
+    Wn, stride, n_iter = 32, 16, 24
+    ref = oracle.swap_trajectory(pb, base_np, Wn, stride, n_iter)
+    perms_np = W.perm_rows(5, n, np.arange(300))
+    ref_c = oracle.eval_candidates(pb, perms_np)
+    nn = Wn * (Wn - 1) // 2
+    base0 = torch.from_numpy(base_np.copy()).cuda()
+    perm = base0.clone()
+    perms = torch.from_numpy(perms_np).cuda()
+    d = torch.zeros(nn, dtype=torch.int64, device="cuda")
+    o = torch.zeros(nn, dtype=torch.float64, device="cuda")
+    idx = torch.zeros(n_iter, dtype=torch.int64, device="cuda")
+    val = torch.zeros(n_iter, dtype=torch.float64, device="cuda")
+    cd = torch.zeros(300, dtype=torch.int64, device="cuda")
+    co = torch.zeros(300, dtype=torch.float64, device="cuda")
+    ci = torch.zeros(1, dtype=torch.int64, device="cuda")
+
+    def loop():
+        ctx.eval_candidates(perms, dist=cd, obj=co)
+        ctx.argmin(co, ci)
+        for it in range(n_iter):
+            s = (it * stride) % (n - Wn + 1)
+            ctx.eval_swaps(perm, s, Wn, d, o)
+            ctx.argmin(o, idx[it:it + 1], val[it:it + 1])
+            ctx.apply_swap(perm, s, Wn, idx[it:it + 1])
+
+    loop()  # eager: sizes the scratch
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    perm.copy_(base0)
+    torch.cuda.synchronize()
+    with torch.cuda.graph(g, stream=torch.cuda.Stream()):
+        loop()
+    for _ in range(2):
+        perm.copy_(base0)
+        idx.zero_(), val.zero_(), cd.zero_(), co.zero_(), ci.fill_(-1)
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(idx.cpu().numpy(), ref["move"])
+        assert np.array_equal(val.cpu().numpy(), ref["obj"])
+        assert np.array_equal(perm.cpu().numpy(), ref["perm"])
+        assert np.array_equal(cd.cpu().numpy(), ref_c["dist"])
+        assert np.array_equal(co.cpu().numpy(), ref_c["obj"])
+        assert int(ci.item()) == oracle.argmin(ref_c["obj"])
+    del g
+    ctx.close()
+
+
 def test_neighbourhood_config_paper_scale(torch_cuda):
     """configs[4] at full size: W = 256 (32,640 neighbours), stride 128, 100 iterations. The
     oracle re-evaluates every neighbour from scratch (~50 s per iteration), so here: the first
