@@ -149,7 +149,7 @@ def run_ours(args):
         it_counter[0] += 1
 
     def timed_run():
-        sampler = harness.ClockSampler(local_rank, 50).start().wait_first() if rank == 0 else None
+        sampler = harness.ClockSampler(local_rank, args.clock_period_ms).start().wait_first() if rank == 0 else None
         if sampler:
             sampler.mark()  # warm-up and timed steps are both "under load"
         for _ in range(args.warmup):
@@ -312,6 +312,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--clock-period-ms", type=int, default=50,
+                    help="nvidia-smi sampling period during the timed region")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)  # timing rule: at least 3 warm-up steps
     if args.impl == "reference":

@@ -305,6 +305,9 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
   }
   __syncthreads();
   const int32_t nb = s_nb;
+  if (smem_tables != 2)  // the chase left bstart only: batch of every position
+    for (int32_t b = tid; b < nb; b += kBaseThreads)
+      for (int32_t p = B.bstart[b]; p < B.bstart[b + 1]; ++p) B.bop[p] = b;
 
   if (tid == 0) B.totals[1] = nb;
 }
@@ -415,27 +418,33 @@ whp_swaps_prep_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
 // s -> t of one chain costs T(s) - T(t).
 constexpr int kChainWarps = 16;
 
+// STAGED: the hop records of the region sit in shared memory (a chain only moves forward, so a
+// block stages the rows from its own first position on); otherwise (a region too long for
+// shared memory) they are read from global memory.
+template <bool STAGED>
 __global__ void __launch_bounds__(kChainWarps * 32)
 whp_swaps_chain_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, int32_t rhi) {
-  // the region's hop records in shared memory (a chain is a run of dependent look-ups):
   // [cls_at: rows x 8][dist_at: rows (int64)][nxt: rows; negative: p is a base batch start]
   extern __shared__ __align__(16) uint8_t chain_smem[];
-  const int32_t rows = rhi - rlo;
+  const int32_t r0 = rlo + blockIdx.x * kChainWarps;  // first position of this block
+  const int32_t rows = STAGED ? rhi - r0 : 0;
   uint4* s_cls = reinterpret_cast<uint4*>(chain_smem);
   int64_t* s_dist = reinterpret_cast<int64_t*>(chain_smem + 32 * (size_t)rows);
   int32_t* s_nx = reinterpret_cast<int32_t*>(chain_smem + 40 * (size_t)rows);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int32_t n = T.n_orders;
-  for (int32_t k = threadIdx.x; k < rows; k += blockDim.x) {
-    const int32_t p = rlo + k;
-    const bool start = p == 0 || B.bop[p] != B.bop[p - 1];
-    s_nx[k] = start ? -1 : B.nxt[p];
-    s_dist[k] = B.dist_at[p];
+  if (STAGED) {
+    for (int32_t k = threadIdx.x; k < rows; k += blockDim.x) {
+      const int32_t p = r0 + k;
+      const bool start = p == 0 || B.bop[p] != B.bop[p - 1];
+      s_nx[k] = start ? -1 : B.nxt[p];
+      s_dist[k] = B.dist_at[p];
+    }
+    for (int32_t k = threadIdx.x; k < 2 * rows; k += blockDim.x)
+      s_cls[k] = reinterpret_cast<const uint4*>(B.cls_at + (int64_t)r0 * 8)[k];
+    __syncthreads();
   }
-  for (int32_t k = threadIdx.x; k < 2 * rows; k += blockDim.x)
-    s_cls[k] = reinterpret_cast<const uint4*>(B.cls_at + (int64_t)rlo * 8)[k];
-  __syncthreads();
-  const int32_t p0 = rlo + blockIdx.x * kChainWarps + warp;
+  const int32_t p0 = r0 + warp;
   if (p0 >= rhi) return;
   int64_t D = 0;
   int32_t r[8];
@@ -445,11 +454,21 @@ whp_swaps_chain_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo,
   for (;;) {
     if (p >= n) { bF = (int32_t)B.totals[1]; break; }
     if (p >= rhi) { bF = -1; break; }
-    const int32_t nx = s_nx[p - rlo];
-    if (nx < 0) { bF = B.bop[p]; break; }
-    D += s_dist[p - rlo];
-    const uint4 c0 = s_cls[2 * (p - rlo)];
-    const uint4 c1 = s_cls[2 * (p - rlo) + 1];
+    int32_t nx;
+    uint4 c0, c1;
+    if (STAGED) {
+      nx = s_nx[p - r0];
+      if (nx < 0) { bF = B.bop[p]; break; }
+      D += s_dist[p - r0];
+      c0 = s_cls[2 * (p - r0)];
+      c1 = s_cls[2 * (p - r0) + 1];
+    } else {
+      if (p == 0 || B.bop[p] != B.bop[p - 1]) { bF = B.bop[p]; break; }
+      nx = B.nxt[p];
+      D += B.dist_at[p];
+      c0 = reinterpret_cast<const uint4*>(B.cls_at + (int64_t)p * 8)[0];
+      c1 = reinterpret_cast<const uint4*>(B.cls_at + (int64_t)p * 8)[1];
+    }
     r[0] += (int32_t)((c0.x >> lane) & 1u); r[1] += (int32_t)((c0.y >> lane) & 1u);
     r[2] += (int32_t)((c0.z >> lane) & 1u); r[3] += (int32_t)((c0.w >> lane) & 1u);
     r[4] += (int32_t)((c1.x >> lane) & 1u); r[5] += (int32_t)((c1.y >> lane) & 1u);
@@ -786,7 +805,10 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
   // region of tabulated hypothetical batches: from two cart lengths before the window (the
   // rewalk may start one batch early) to a margin after it (until the boundaries resynchronise;
   // beyond the margin a neighbour scores its batches from their picks)
-  int64_t margin = 16ll * c->C > 512 ? 16ll * c->C : 512;
+  // (two next-fit chains need a median of ~150 positions to meet at paper scale, but the tail is
+  // long: with 512 positions one window in five still had chains that left the region, and every
+  // neighbour that lands on such a chain then scores tens of batches from their picks)
+  int64_t margin = 64ll * c->C > 2048 ? 64ll * c->C : 2048;
   if (const char* m = getenv("WHP_SWAP_MARGIN")) { const int v = atoi(m); if (v >= 0) margin = v; }  // tests: force the fallbacks
   const int32_t rlo = (int32_t)((int64_t)win_start - 2ll * c->C > 0 ? (int64_t)win_start - 2ll * c->C : 0);
   const int32_t rhi = (int32_t)((int64_t)win_start + win_len + margin < c->n_orders
@@ -812,11 +834,16 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
     c->rtail_rows = rows;
   }
   const size_t chain_smem = 44 * (size_t)rows;
-  if (chain_smem + 2048 > (size_t)c->smem_optin) return cudaErrorInvalidConfiguration;
-  if ((e = cudaFuncSetAttribute(whp_swaps_chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)chain_smem)) != cudaSuccess) return e;
-  whp_swaps_chain_kernel<<<(unsigned)((rows + kChainWarps - 1) / kChainWarps), kChainWarps * 32,
-                           chain_smem, st>>>(T, c->base, rlo, rhi);
+  const unsigned chain_blocks = (unsigned)((rows + kChainWarps - 1) / kChainWarps);
+  if (chain_smem + 2048 <= (size_t)c->smem_optin) {
+    if ((e = cudaFuncSetAttribute(whp_swaps_chain_kernel<true>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  (int)chain_smem)) != cudaSuccess) return e;
+    whp_swaps_chain_kernel<true><<<chain_blocks, kChainWarps * 32, chain_smem, st>>>(T, c->base,
+                                                                                      rlo, rhi);
+  } else {
+    whp_swaps_chain_kernel<false><<<chain_blocks, kChainWarps * 32, 0, st>>>(T, c->base, rlo, rhi);
+  }
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   *rlo_out = rlo;

@@ -103,6 +103,40 @@ def test_swaps_chains_that_leave_the_tabulated_region(torch_cuda, margin):
     ctx.close()
 
 
+@pytest.mark.parametrize("n_orders,s,Wn,margin", [(20000, 9000, 28, None), (20000, 9000, 28, "8000"),
+                                                  (30000, 21000, 12, None), (30000, 29988, 12, "9000")])
+def test_swaps_on_long_plans(torch_cuda, n_orders, s, Wn, margin):
+    """Stress-size plans. 20,000 orders: the base pass keeps only two of its five tables in shared
+    memory and one thread chases the batch boundaries; 30,000 orders: no table fits. With a region
+    of 8,000+ positions the hop records (44 bytes a position) do not fit shared memory either, so
+    the chain kernel reads them from global memory. Swaps and insertion moves of a small window
+    against the oracle."""
+    import os
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("stress", n_orders=n_orders)
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(2, pb.n_orders)
+    ref = oracle.eval_swaps(pb, base, s, Wn)
+    ref_m = oracle.eval_moves(pb, base, s, 10)
+    if margin is not None:
+        os.environ["WHP_SWAP_MARGIN"] = margin
+    try:
+        bd = torch.from_numpy(base).cuda()
+        d, o = gpu_swaps(torch, ctx, bd, s, Wn)
+        md = torch.zeros(90, dtype=torch.int64, device="cuda")
+        mo = torch.zeros(90, dtype=torch.float64, device="cuda")
+        ctx.eval_moves(bd, s, 10, md, mo)
+        torch.cuda.synchronize()
+    finally:
+        os.environ.pop("WHP_SWAP_MARGIN", None)
+    assert np.array_equal(d.cpu().numpy(), ref["dist"])
+    assert np.array_equal(o.cpu().numpy(), ref["obj"])
+    assert np.array_equal(md.cpu().numpy(), ref_m["dist"])
+    assert np.array_equal(mo.cpu().numpy(), ref_m["obj"])
+    ctx.close()
+
+
 def test_smaller_opening_order_slips_into_previous_cart(torch_cuda):
     """q = [2,1,3,1], C = 4: swapping positions 2 and 3 (both in the second batch) lets the
     1-item order join the first cart — the incremental evaluator must restart one batch early."""
