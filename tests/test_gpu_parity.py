@@ -218,6 +218,46 @@ def test_stress_full_size_sampled_oracle(torch_cuda):
     assert i == int(np.argmin(got["obj"])) and v == got["obj"][i]
     win = oracle.eval_candidates(pb, W.perm_rows(wl.seed, n, [i]))
     assert win["obj"][0] == v and win["dist"][0] == got["dist"][i]
+    # NEXT-2 at this size: the pick table (265 KB) does not fit shared memory, so the leg-sum
+    # kernel gathers it through L2 like the set kernel does
+    head = W.perm_rows(wl.seed, n, np.arange(40))
+    leg = torch.full((40,), -1, dtype=torch.int64, device="cuda")
+    ctx.eval_legsum(perms_dev[:40], leg)
+    torch.cuda.synchronize()
+    assert np.array_equal(leg.cpu().numpy(), oracle.eval_legsum(pb, head))
+    # NEXT-1 at this size (K = 32: one class word), 3 outer iterations over 256 plans
+    hist = oracle.nhatc_loop(pb, W.perm_rows(wl.seed, n, np.arange(256)), 3, 1.5)
+    idx_h = torch.zeros(3, dtype=torch.int64, device="cuda")
+    ctx.nhatc_solve(perms_dev[:256], 3, 1.5, idx_h)
+    t2, v2, w2 = ctx.get_penalty()
+    assert np.array_equal(idx_h.cpu().numpy(), hist["idx"])
+    assert np.array_equal(v2, hist["v"]) and np.array_equal(w2, hist["w"])
+    ctx.close()
+
+
+def test_more_orders_than_the_tuned_path_indexes(torch_cuda):
+    """66,000 orders: positions no longer fit the 16-bit cursors, so evaluation, leg sums and the
+    neighbourhood all take their general kernels (and the swap base pass runs without
+    shared-memory tables)."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = _random_problem(4, NA=50, S=40, K=70, n_skus=3000, n_orders=66000, qmax=4, C=9)
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perm_rows(8, pb.n_orders, np.arange(6))
+    got, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=True)
+    ref = oracle.eval_candidates(pb, perms, detail=True)
+    assert_parity(got, ref, pb, detail=True)
+    leg = torch.zeros(6, dtype=torch.int64, device="cuda")
+    ctx.eval_legsum(torch.from_numpy(perms).cuda(), leg)
+    torch.cuda.synchronize()
+    assert np.array_equal(leg.cpu().numpy(), oracle.eval_legsum(pb, perms))
+    s, Wn = 40000, 9
+    d = torch.zeros(Wn * (Wn - 1) // 2, dtype=torch.int64, device="cuda")
+    o = torch.zeros(Wn * (Wn - 1) // 2, dtype=torch.float64, device="cuda")
+    ctx.eval_swaps(torch.from_numpy(perms[0]).cuda(), s, Wn, d, o)
+    torch.cuda.synchronize()
+    rs = oracle.eval_swaps(pb, perms[0], s, Wn)
+    assert np.array_equal(d.cpu().numpy(), rs["dist"]) and np.array_equal(o.cpu().numpy(), rs["obj"])
     ctx.close()
 
 
