@@ -81,6 +81,49 @@ def test_swaps_full_length_window(torch_cuda):
     ctx.close()
 
 
+@pytest.mark.parametrize("kind", ["swaps", "moves"])
+def test_window_longer_than_the_staged_tables(torch_cuda, kind):
+    """The neighbour kernels stage 1,024 positions of the prefix / order tables in shared memory;
+    a 1,300-wide window reaches past them (global-memory path of the accessors). All 844,350
+    swaps (1,688,700 moves) are computed; a sample of them — biased to the far end — is checked
+    against the oracle on the materialised plans."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid", n_orders=1300)
+    ctx = whp.Context.from_problem(pb)
+    n = pb.n_orders
+    base = W.base_perm(4, n)
+    bd = torch.from_numpy(base).cuda()
+    rng = np.random.default_rng(12)
+    i = np.concatenate([rng.integers(0, n, 1500), rng.integers(0, 200, 700), rng.integers(1000, n, 800)])
+    j = np.concatenate([rng.integers(0, n, 1500), rng.integers(1030, n, 700), rng.integers(1000, n, 800)])
+    keep = i != j
+    i, j = i[keep], j[keep]
+    plans = np.repeat(base[None, :], len(i), axis=0)
+    if kind == "swaps":
+        i, j = np.minimum(i, j), np.maximum(i, j)
+        nn = n * (n - 1) // 2
+        idx = i * (2 * n - i - 1) // 2 + (j - i - 1)
+        plans[np.arange(len(i)), i], plans[np.arange(len(i)), j] = base[j], base[i]
+        d = torch.zeros(nn, dtype=torch.int64, device="cuda")
+        o = torch.zeros(nn, dtype=torch.float64, device="cuda")
+        ctx.eval_swaps(bd, 0, n, d, o)
+    else:
+        nn = n * (n - 1)
+        idx = i * (n - 1) + np.where(j < i, j, j - 1)
+        for r, (a, b) in enumerate(zip(i, j)):
+            plans[r] = np.insert(np.delete(base, a), b, base[a])
+        d = torch.zeros(nn, dtype=torch.int64, device="cuda")
+        o = torch.zeros(nn, dtype=torch.float64, device="cuda")
+        ctx.eval_moves(bd, 0, n, d, o)
+    torch.cuda.synchronize()
+    ref = oracle.eval_candidates(pb, plans)
+    sel = torch.from_numpy(idx).cuda()
+    assert np.array_equal(d[sel].cpu().numpy(), ref["dist"])
+    assert np.array_equal(o[sel].cpu().numpy(), ref["obj"])
+    ctx.close()
+
+
 @pytest.mark.parametrize("margin", ["0", "7", "40"])
 def test_swaps_chains_that_leave_the_tabulated_region(torch_cuda, margin):
     """The chain sums cover the window plus a margin; with a tiny margin most chains leave the
