@@ -285,8 +285,10 @@ def run_ours(args):
         "neighbourhood": {"ms_per_iteration_eval_swaps": s_ms,
                           "neighbours_per_s": nn / (s_ms * 1e-3)},
         "nhatc_outer_loop": {"ms_per_outer_iteration": nhatc_ms,
-                             "what": "eval 16,384 plans (with responses) -> argmin -> multiplier "
-                                     "update, device only"},
+                             "n_outer": n_outer,
+                             "what": "whp_nhatc_solve: 16,384 plans walked once (D, r), then per "
+                                     "outer iteration penalty -> argmin -> multiplier update, "
+                                     "device only; mean over the call"},
         "moves": {"ms": moves_ms, "neighbours": mW * (mW - 1),
                   "neighbours_per_s": mW * (mW - 1) / (moves_ms * 1e-3),
                   "what": "whp_eval_moves, all insertion moves of a 128-wide window"},

@@ -140,7 +140,9 @@ whp_status whp_nhatc_update(whp_ctx* ctx, const int32_t* d_resp_rows, const int6
 
 /* n_outer times { whp_eval_candidates on d_perms -> whp_argmin -> record (winner index, its D,
  * its J) into the DEVICE histories [n_outer] (each nullable) -> whp_nhatc_update with the
- * winner's responses }, all on the stream with no host round trip. */
+ * winner's responses }, all on the stream with no host round trip. The results are those of
+ * that loop bit for bit; since D and r of a plan do not depend on (t, v, w), the plans are
+ * walked once and the later iterations redo only the penalty (D6) on the stored responses. */
 whp_status whp_nhatc_solve(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand, int32_t n_outer,
                            double beta, int64_t* d_idx_hist, int64_t* d_dist_hist,
                            double* d_obj_hist, void* cuda_stream);

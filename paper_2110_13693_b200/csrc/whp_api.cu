@@ -458,8 +458,12 @@ whp_status whp_nhatc_solve(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, i
     c->n_resp_cap = n_cand;
   }
   for (int32_t it = 0; it < n_outer; ++it) {
-    whp_eval_out out{c->d_h_dist, nullptr, c->d_h_obj, nullptr, nullptr, nullptr, nullptr, c->d_n_resp};
-    WHP_CUDA(c, whp_launch_eval(c, d_perms, n_cand, out, st));
+    if (it == 0) {  // D and r of the plans: once per call, they do not depend on (t, v, w)
+      whp_eval_out out{c->d_h_dist, nullptr, c->d_h_obj, nullptr, nullptr, nullptr, nullptr, c->d_n_resp};
+      WHP_CUDA(c, whp_launch_eval(c, d_perms, n_cand, out, st));
+    } else {        // new multipliers: D6 again on the stored responses
+      WHP_CUDA(c, whp_launch_nhatc_rescore(c, c->d_n_resp, c->d_h_dist, n_cand, c->d_h_obj, st));
+    }
     WHP_CUDA(c, whp_launch_argmin(c, c->d_h_obj, n_cand, c->d_h_idx, c->d_h_val, st));
     WHP_CUDA(c, whp_launch_nhatc_record(c, c->d_h_idx, c->d_h_dist, c->d_h_obj, it, d_idx_hist,
                                         d_dist_hist, d_obj_hist, st));

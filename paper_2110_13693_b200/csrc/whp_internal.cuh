@@ -163,6 +163,8 @@ cudaError_t whp_launch_apply_swap(whp_ctx* c, int32_t* d_base_perm, int32_t win_
                                   int32_t win_len, const int64_t* d_idx, cudaStream_t st);
 cudaError_t whp_launch_nhatc_update(whp_ctx* c, const int32_t* d_resp_rows, const int64_t* d_idx,
                                     double beta, cudaStream_t st);
+cudaError_t whp_launch_nhatc_rescore(whp_ctx* c, const int32_t* d_resp_rows, const int64_t* d_dist,
+                                     int64_t n_cand, double* d_obj, cudaStream_t st);
 cudaError_t whp_launch_nhatc_record(whp_ctx* c, const int64_t* d_idx, const int64_t* dist,
                                     const double* obj, int32_t it, int64_t* idx_hist,
                                     int64_t* dist_hist, double* obj_hist, cudaStream_t st);
