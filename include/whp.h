@@ -26,7 +26,8 @@
  *     calls that take a `cuda_stream` neither allocate nor synchronise and may be captured
  *     (cudaStreamBeginCapture ... EndCapture) and replayed; scalar arguments such as win_start
  *     are baked into the captured launches. Calls that hand a value back to the host
- *     (the *_host entry points, whp_validate_perms, whp_get_penalty, whp_probe_l2_read)
+ *     (the *_host entry points, whp_validate_perms, whp_get_penalty, whp_get_swap_stats,
+ *     whp_probe_l2_read)
  *     synchronise and cannot be captured.
  *   - All arrays are dense, row-major, native-endian.
  *   - A row of d_perms that is not a permutation of 0..n_orders-1 is a precondition
@@ -195,6 +196,15 @@ whp_status whp_apply_move(whp_ctx* ctx, int32_t* d_base_perm, int32_t win_start,
  * permutation of 0..n_orders-1. Synchronises the stream. */
 whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,
                               int64_t* h_n_bad, void* cuda_stream);
+
+/* Measurement helper ("actually-rescored picks"): with enable != 0 every later
+ * whp_eval_swaps / whp_eval_moves call also counts the batches it scored from their picks and
+ * the picks in them (everything else in a neighbour's value is table look-ups); off by default.
+ * whp_get_swap_stats copies the counts of the latest such call to the host (each nullable) and
+ * synchronises the stream. */
+whp_status whp_set_swap_stats(whp_ctx* ctx, int32_t enable);
+whp_status whp_get_swap_stats(whp_ctx* ctx, int64_t* h_batches, int64_t* h_picks,
+                              void* cuda_stream);
 
 /* Measurement helper (bench.py): *h_ms (host) = time of `reps` read-only sweeps (16-byte loads
  * that bypass L1) of a `bytes`-sized buffer, which stays L2-resident when bytes is well below the

@@ -115,6 +115,8 @@ whp_status whp_create_layout(int32_t n_aisles, int32_t slots_per_side, int32_t s
   if (e == cudaSuccess) e = cudaMemset(c->d_argmin_part, 0, 16 * (size_t)c->argmin_cap + 16);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_count, sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_task, 2 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_swap_stats, 2 * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMemset(c->d_swap_stats, 0, 2 * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_h_idx, sizeof(int64_t));
   if (e == cudaSuccess) e = cudaMalloc(&c->d_h_val, sizeof(double));
   for (int k = 0; k < 2 && e == cudaSuccess; ++k) {
@@ -485,6 +487,26 @@ whp_status whp_get_penalty(whp_ctx* c, double* t, double* v, double* w, void* cu
   return WHP_OK;
 }
 
+whp_status whp_set_swap_stats(whp_ctx* c, int32_t enable) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  c->swap_stats = enable != 0;
+  return WHP_OK;
+}
+
+whp_status whp_get_swap_stats(whp_ctx* c, int64_t* h_batches, int64_t* h_picks, void* cuda_stream) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  device_guard dg(c->device);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  unsigned long long h[2] = {0, 0};
+  WHP_CUDA(c, cudaMemcpyAsync(h, c->d_swap_stats, sizeof(h), cudaMemcpyDeviceToHost, st));
+  WHP_CUDA(c, cudaStreamSynchronize(st));
+  if (h_batches) *h_batches = (int64_t)h[0];
+  if (h_picks) *h_picks = (int64_t)h[1];
+  return WHP_OK;
+}
+
 whp_status whp_probe_l2_read(whp_ctx* c, int64_t bytes, int32_t reps, float* h_ms) {
   if (!c) return WHP_ERR_INVALID_ARG;
   c->err.clear();
@@ -501,7 +523,7 @@ void whp_destroy(whp_ctx* c) {
     device_guard dg(c->device);
     cudaDeviceSynchronize();
     free_orders(c);
-    dfree(c->d_tvw); dfree(c->d_argmin_part); dfree(c->d_count); dfree(c->d_task);
+    dfree(c->d_tvw); dfree(c->d_argmin_part); dfree(c->d_count); dfree(c->d_task); dfree(c->d_swap_stats);
     dfree(c->d_h_dist); dfree(c->d_h_obj); dfree(c->d_h_idx); dfree(c->d_h_val); dfree(c->d_n_resp);
     for (int k = 0; k < 2; ++k) {
       if (c->s_copy[k]) cudaStreamDestroy(c->s_copy[k]);

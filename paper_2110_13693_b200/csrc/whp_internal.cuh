@@ -121,6 +121,8 @@ struct whp_ctx {
   int64_t* d_dist_scratch = nullptr; // [fast_cap]
   uint32_t* d_planes = nullptr;      // [fast_cap][S][8 planes][KW] bit-sliced class counters
   unsigned long long* d_task = nullptr;  // [2] work-stealing counter
+  unsigned long long* d_swap_stats = nullptr;  // [2] batches / picks scored from their picks
+  bool swap_stats = false;                     // whp_set_swap_stats
   int64_t fast_cap = 0, fast_plane_words = 0;
   int32_t fast_pitch = 0;
   int smem_optin = 0;

@@ -487,14 +487,16 @@ whp_swaps_chain_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo,
 constexpr int kSwapWarps = 8;
 constexpr int kStage = 1024;  // positions of pre / orec staged per block
 
+template <bool STATS>  // STATS: also count the batches / picks scored from their picks
 __global__ void __launch_bounds__(kSwapWarps * 32)
 whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start, int32_t W,
                  int32_t rlo, int32_t rhi, int64_t n_nb, int64_t* __restrict__ d_dist,
-                 double* __restrict__ d_obj) {
+                 double* __restrict__ d_obj, unsigned long long* __restrict__ stats) {
   __shared__ warp_sets sets_all[kSwapWarps];
   __shared__ int32_t s_pre[kStage + 1];
   __shared__ uint32_t s_orec[kStage];
   __shared__ int32_t s_nxt[kStage];
+  uint32_t n_scored = 0, n_scored_picks = 0;  // stats: batches / picks scored from their picks
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
@@ -576,6 +578,11 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
       add_classes();
       D += score_batch(T, sets, q, __ldg(B.bstart + bj), __ldg(B.bstart + bj + 1));
       add_classes();
+      if (STATS) {
+        n_scored += 2;
+        n_scored_picks += (uint32_t)(q.pre_at(__ldg(B.bstart + bi + 1)) - q.pre_at(__ldg(B.bstart + bi)) +
+                                     q.pre_at(__ldg(B.bstart + bj + 1)) - q.pre_at(__ldg(B.bstart + bj)));
+      }
     } else {
       const int32_t b0 = slip ? bi - 1 : bi;
       int32_t p = __ldg(B.bstart + b0);
@@ -639,6 +646,7 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
         } else {
           D += score_batch(T, sets, q, p, e);
           add_classes();
+          if (STATS) { n_scored += 1; n_scored_picks += (uint32_t)(q.pre_at(e) - q.pre_at(p)); }
         }
         p = e;
         if (p >= n) { b_end = nb; break; }
@@ -657,6 +665,10 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
       if (d_obj) d_obj[nn] = __dadd_rn((double)D, phi);
     }
   }
+  if (STATS && lane == 0) {
+    atomicAdd(stats, (unsigned long long)n_scored);
+    atomicAdd(stats + 1, (unsigned long long)n_scored_picks);
+  }
 }
 
 // ------------------------------------------------------------------------------ NEXT-4: moves
@@ -666,13 +678,15 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
 // coincides with a base boundary. The orders between pi and pj only shift by one position, so a
 // new batch that lies between them and ends where the base criterion ends it is the tabulated
 // batch of its (shifted) base start; after M the rest is one chain look-up, as for swaps.
+template <bool STATS>
 __global__ void __launch_bounds__(kSwapWarps * 32)
 whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start, int32_t W,
                  int32_t rlo, int32_t rhi, int64_t n_nb, int64_t* __restrict__ d_dist,
-                 double* __restrict__ d_obj) {
+                 double* __restrict__ d_obj, unsigned long long* __restrict__ stats) {
   __shared__ warp_sets sets_all[kSwapWarps];
   __shared__ int32_t s_pre[kStage + 1];
   __shared__ uint32_t s_orec[kStage];
+  uint32_t n_scored = 0, n_scored_picks = 0;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
@@ -737,6 +751,7 @@ whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
         r[6] += (int32_t)((c1.z >> lane) & 1u); r[7] += (int32_t)((c1.w >> lane) & 1u);
       } else {
         D += score_batch(T, sets, q, p, e);
+        if (STATS) { n_scored += 1; n_scored_picks += (uint32_t)(q.pre_at(e) - q.pre_at(p)); }
         __syncwarp();
 #pragma unroll
         for (int w = 0; w < 8; ++w) r[w] += (int32_t)((sets->cmask[w] >> lane) & 1u);
@@ -761,6 +776,10 @@ whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
       if (d_dist) d_dist[nn] = D;
       if (d_obj) d_obj[nn] = __dadd_rn((double)D, phi);
     }
+  }
+  if (STATS && lane == 0) {
+    atomicAdd(stats, (unsigned long long)n_scored);
+    atomicAdd(stats + 1, (unsigned long long)n_scored_picks);
   }
 }
 
@@ -861,8 +880,13 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
   int64_t blocks = (n_nb + kSwapWarps - 1) / kSwapWarps;
   const int64_t cap = (int64_t)c->num_sms * 8;
   if (blocks > cap) blocks = cap;
-  whp_swaps_kernel<<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(T, c->base, win_start, win_len,
-                                                                 rlo, rhi, n_nb, d_dist, d_obj);
+  if (c->swap_stats && (e = cudaMemsetAsync(c->d_swap_stats, 0, 16, st)) != cudaSuccess) return e;
+  if (c->swap_stats)
+    whp_swaps_kernel<true><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
+        T, c->base, win_start, win_len, rlo, rhi, n_nb, d_dist, d_obj, c->d_swap_stats);
+  else
+    whp_swaps_kernel<false><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
+        T, c->base, win_start, win_len, rlo, rhi, n_nb, d_dist, d_obj, nullptr);
   c->launches += 1;
   return cudaGetLastError();
 }
@@ -877,8 +901,13 @@ cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win
   int64_t blocks = (n_nb + kSwapWarps - 1) / kSwapWarps;
   const int64_t cap = (int64_t)c->num_sms * 8;
   if (blocks > cap) blocks = cap;
-  whp_moves_kernel<<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(T, c->base, win_start, win_len,
-                                                                 rlo, rhi, n_nb, d_dist, d_obj);
+  if (c->swap_stats && (e = cudaMemsetAsync(c->d_swap_stats, 0, 16, st)) != cudaSuccess) return e;
+  if (c->swap_stats)
+    whp_moves_kernel<true><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
+        T, c->base, win_start, win_len, rlo, rhi, n_nb, d_dist, d_obj, c->d_swap_stats);
+  else
+    whp_moves_kernel<false><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
+        T, c->base, win_start, win_len, rlo, rhi, n_nb, d_dist, d_obj, nullptr);
   c->launches += 1;
   return cudaGetLastError();
 }

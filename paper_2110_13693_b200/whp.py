@@ -24,7 +24,7 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
            "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move",
-           "whp_probe_l2_read", "whp_max_batches"]
+           "whp_probe_l2_read", "whp_max_batches", "whp_set_swap_stats", "whp_get_swap_stats"]
 
 
 class WhpError(RuntimeError):
@@ -60,6 +60,8 @@ def lib():
         L.whp_eval_moves.argtypes = [vp, vp, i32, i32, vp, vp, vp]
         L.whp_apply_move.argtypes = [vp, vp, i32, i32, vp, vp]
         L.whp_probe_l2_read.argtypes = [vp, i64, i32, vp]
+        L.whp_set_swap_stats.argtypes = [vp, i32]
+        L.whp_get_swap_stats.argtypes = [vp, vp, vp, vp]
         L.whp_max_batches.argtypes = [vp]
         L.whp_max_batches.restype = i64
         L.whp_launch_count.argtypes = [vp]
@@ -249,6 +251,17 @@ class Context:
         ms = C.c_float(0.0)
         self._check(lib().whp_probe_l2_read(self._h, nbytes, reps, C.byref(ms)))
         return nbytes * reps / (ms.value * 1e-3) / 1e9
+
+    def set_swap_stats(self, enable=True):
+        self._check(lib().whp_set_swap_stats(self._h, 1 if enable else 0))
+
+    def get_swap_stats(self, stream=None):
+        """(batches, picks) scored from their picks by the latest eval_swaps / eval_moves call
+        made while the statistics were enabled."""
+        b, k = C.c_int64(0), C.c_int64(0)
+        self._check(lib().whp_get_swap_stats(self._h, C.addressof(b), C.addressof(k),
+                                             _stream(stream)))
+        return b.value, k.value
 
     def max_batches(self) -> int:
         return int(lib().whp_max_batches(self._h))

@@ -180,6 +180,28 @@ def test_swaps_on_long_plans(torch_cuda, n_orders, s, Wn, margin):
     ctx.close()
 
 
+def test_swap_stats_count_the_batches_scored_from_their_picks(torch_cuda):
+    """One-item orders, C = 5: carts are exactly 5 positions and every boundary stays. A swap
+    inside a cart changes nothing (no batch scored); a swap across carts rescores exactly the two
+    carts (10 picks). Window of 20 positions = 4 carts: 40 pairs inside a cart, 150 across."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    from test_gpu_parity import _random_problem
+    pb = _random_problem(5, NA=12, S=9, K=10, n_skus=80, n_orders=50, qmax=1, C=5)
+    ctx = whp.Context.from_problem(pb)
+    base = torch.from_numpy(W.base_perm(1, pb.n_orders)).cuda()
+    d, o = gpu_swaps(torch, ctx, base, 0, 20)
+    assert ctx.get_swap_stats() == (0, 0)          # off by default
+    ctx.set_swap_stats(True)
+    d2, o2 = gpu_swaps(torch, ctx, base, 0, 20)
+    assert ctx.get_swap_stats() == (300, 1500)
+    assert torch.equal(d, d2) and torch.equal(o, o2)
+    d3, o3 = gpu_swaps(torch, ctx, base, 5, 5)      # one cart: nothing to rescore
+    assert ctx.get_swap_stats() == (0, 0)
+    ctx.set_swap_stats(False)
+    ctx.close()
+
+
 def test_smaller_opening_order_slips_into_previous_cart(torch_cuda):
     """q = [2,1,3,1], C = 4: swapping positions 2 and 3 (both in the second batch) lets the
     1-item order join the first cart — the incremental evaluator must restart one batch early."""
