@@ -113,6 +113,33 @@ __device__ __forceinline__ int64_t score_batch(const whp_tables& T, warp_sets* s
   const int32_t base0 = q.pre_at(s);
   const int32_t load = q.pre_at(e) - base0;
   uint32_t kmax = 0, kmin = 0xffffffffu;
+  const int32_t npos = e - s;
+  if (npos <= 32) {
+    // one position per lane: its relative prefix (ascending over the lanes) and order record;
+    // an item finds its position by a binary search over the lanes (shuffles, no table access)
+    const int32_t mine = lane < npos ? q.pre_at(s + lane) - base0 : 0x7fffffff;
+    const uint32_t my_orec = lane < npos ? q.orec_at(s + lane) : 0u;
+    for (int32_t t0 = 0; t0 < load; t0 += 32) {
+      const int32_t t = t0 + lane;
+      int l = 0;  // largest lane with mine <= t (mine of lane 0 is 0)
+#pragma unroll
+      for (int step = 16; step >= 1; step >>= 1) {
+        const int32_t v = __shfl_sync(WHP_FULL, mine, (l + step) & 31);
+        if (l + step < 32 && v <= t) l += step;
+      }
+      const uint32_t orec = __shfl_sync(WHP_FULL, my_orec, l);
+      const int32_t first = __shfl_sync(WHP_FULL, mine, l);
+      if (t < load) {
+        const uint32_t pr = __ldg(T.pick_rec + (orec >> WHP_Q_BITS) + (t - first));
+        kmax = max(kmax, pr);
+        kmin = min(kmin, pr);
+        const uint32_t a = WHP_PICK_AISLE(pr);
+        const uint32_t c = pr & WHP_PICK_CLASS_MASK;
+        atomicOr(&sets->amask[a >> 5], 1u << (a & 31));
+        atomicOr(&sets->cmask[c >> 5], 1u << (c & 31));
+      }
+    }
+  } else
   for (int32_t t0 = 0; t0 < load; t0 += 32) {
     const int32_t t = t0 + lane;
     if (t < load) {
@@ -509,7 +536,9 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
     const int32_t bw = __ldg(B.bop + win_start);
     lo = __ldg(B.bstart + (bw > 0 ? bw - 1 : 0));
   }
-  const int32_t cnt = min(kStage, n - lo);
+  // (what a neighbour reads lies between that start and a cart or two past the window; anything
+  // further goes through the accessors' global-memory path)
+  const int32_t cnt = min(min(kStage, n - lo), win_start + W + 3 * T.C + 32 - lo);
   for (int k = threadIdx.x; k <= cnt; k += blockDim.x) s_pre[k] = __ldg(B.pre + lo + k);
   for (int k = threadIdx.x; k < cnt; k += blockDim.x) s_orec[k] = __ldg(B.orec + lo + k);
   for (int k = threadIdx.x; k < cnt; k += blockDim.x) s_nxt[k] = __ldg(B.nxt + lo + k);
