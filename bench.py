@@ -135,9 +135,36 @@ def run_ours(args):
     s_ev = {k: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
             for k in range(0, args.steps, ev_every)}
 
+    # The two halves of a step are independent (the neighbourhood pass works on the trajectory
+    # plan, not on the evaluated candidates), so with --overlap 1 they run on two streams, each
+    # with its own context ("one context per stream", include/whp.h): the small kernels of
+    # whp_eval_swaps fill the SMs that K1 (one warp per scheduler) leaves idle.
+    overlap = bool(args.overlap)
+    ctx_nb = whp.Context.from_problem(pb, device=local_rank) if overlap else ctx
+    main = torch.cuda.current_stream()
+    side = torch.cuda.Stream(device=dev, priority=-1) if overlap else main
+    fork_ev, join_ev = torch.cuda.Event(), torch.cuda.Event()
+
+    def neighbourhood_half(timed_index):
+        s = (it_counter[0] * stride) % (n - Wn + 1)
+        if timed_index is not None:
+            s_ev[timed_index][0].record()
+        ctx_nb.eval_swaps(base, s, Wn, dist=sdist, obj=sobj)
+        if timed_index is not None:
+            s_ev[timed_index][1].record()
+        ctx_nb.argmin(sobj, sidx)
+        ctx_nb.apply_swap(base, s, Wn, sidx)
+        it_counter[0] += 1
+
     def step(timed_index=None):
         if timed_index not in k_ev:
             timed_index = None
+        if overlap:
+            fork_ev.record(main)
+            side.wait_event(fork_ev)
+            with torch.cuda.stream(side):
+                neighbourhood_half(timed_index)
+                join_ev.record(side)
         if timed_index is not None:
             k_ev[timed_index][0].record()
         ctx.eval_candidates(perms, dist=dist, penalty=pen, obj=obj, n_batches=nbat,
@@ -145,15 +172,10 @@ def run_ours(args):
         if timed_index is not None:
             k_ev[timed_index][1].record()
         ctx.argmin(obj, idx, val)
-        s = (it_counter[0] * stride) % (n - Wn + 1)
-        if timed_index is not None:
-            s_ev[timed_index][0].record()
-        ctx.eval_swaps(base, s, Wn, dist=sdist, obj=sobj)
-        if timed_index is not None:
-            s_ev[timed_index][1].record()
-        ctx.argmin(sobj, sidx)
-        ctx.apply_swap(base, s, Wn, sidx)
-        it_counter[0] += 1
+        if overlap:
+            main.wait_event(join_ev)
+        else:
+            neighbourhood_half(timed_index)
 
     def timed_run():
         sampler = harness.ClockSampler(local_rank, args.clock_period_ms).start().wait_first() if rank == 0 else None
@@ -163,7 +185,7 @@ def run_ours(args):
             step()
         torch.cuda.synchronize()
         harness.barrier(world)
-        launches0 = ctx.launch_count()
+        launches0 = ctx.launch_count() + (ctx_nb.launch_count() if overlap else 0)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         e0.record()
@@ -174,7 +196,7 @@ def run_ours(args):
         harness.barrier(world)
         ms = e0.elapsed_time(e1)
         clocks = sampler.stop() if sampler else None
-        return ms, clocks, ctx.launch_count() - launches0
+        return ms, clocks, ctx.launch_count() + (ctx_nb.launch_count() if overlap else 0) - launches0
 
     ms, clocks, launches = timed_run()
     redo = harness.max_over_ranks(1.0 if (rank == 0 and harness.clocks_rejected(clocks)) else 0.0,
@@ -313,7 +335,10 @@ def run_ours(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "int64+f64", "data": "synthetic",
         "picks_per_s": value * pb.n_items,
-        "config": config_dict(pb, n_cand, world, wl_nb),
+        "config": dict(config_dict(pb, n_cand, world, wl_nb),
+                       streams=("candidate evaluation + argmin and neighbourhood pass + argmin + "
+                                "apply on two streams, one context each, joined every step")
+                       if overlap else "one stream, the calls of a step back to back"),
         "neighbourhood": {"ms_per_iteration_eval_swaps": s_ms,
                           "neighbours_per_s": nn / (s_ms * 1e-3),
                           "iterations_per_s": 1.0 / (s_ms * 1e-3),
@@ -350,6 +375,8 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--overlap", type=int, default=1, choices=[0, 1],
+                    help="1: candidate evaluation and neighbourhood pass of a step on two streams")
     ap.add_argument("--clock-period-ms", type=int, default=50,
                     help="nvidia-smi sampling period during the timed region")
     args = ap.parse_args()
