@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — one JSON line for the candidate picking-plan evaluation path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--overlap 0|1]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
         --master-port P bench.py --gpus N --steps K --warmup W
 
@@ -10,6 +10,8 @@ workload (BASELINE.json configs[2] + configs[3], "paper" / "neighbourhood" in wo
     whp_eval_candidates on 16,384 candidate plans (a1–a5)  -> whp_argmin (a7)
     whp_eval_swaps on the 32,640-neighbour window of the trajectory plan (a6) -> whp_argmin
     -> whp_apply_swap (the trajectory of configs[3] advances one iteration per step).
+The two lines are independent of each other; with --overlap 1 (default) they run on two streams,
+one context each, forked and joined by events inside every step.
 `value` = candidate plans per second over the whole step, inputs resident in HBM. Multi-GPU:
 candidates are independent, so each rank evaluates its own 16,384 plans (weak scaling), no
 data-path collective; time = max over ranks. `--impl reference` times the oracle (oracle/, a
@@ -209,6 +211,23 @@ def run_ours(args):
     k_ms = float(np.mean([a.elapsed_time(b) for a, b in k_ev.values()]))
     s_ms = float(np.mean([a.elapsed_time(b) for a, b in s_ev.values()]))
     k_ms_max = harness.max_over_ranks(k_ms, world, dev)
+    s_span_ms = s_ms
+    if overlap:
+        # under overlap the events on the side stream span the wait behind K2 as well: the
+        # neighbourhood figures come from 50 further iterations of the trajectory run alone
+        torch.cuda.synchronize()
+        alone = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                 for _ in range(50)]
+        for a, b in alone:
+            s = (it_counter[0] * stride) % (n - Wn + 1)
+            a.record()
+            ctx_nb.eval_swaps(base, s, Wn, dist=sdist, obj=sobj)
+            b.record()
+            ctx_nb.argmin(sobj, sidx)
+            ctx_nb.apply_swap(base, s, Wn, sidx)
+            it_counter[0] += 1
+        torch.cuda.synchronize()
+        s_ms = float(np.mean([a.elapsed_time(b) for a, b in alone]))
     ms_per_step = ms / args.steps
     value = n_cand * world / (ms_per_step * 1e-3)
 
@@ -340,6 +359,7 @@ def run_ours(args):
                                 "apply on two streams, one context each, joined every step")
                        if overlap else "one stream, the calls of a step back to back"),
         "neighbourhood": {"ms_per_iteration_eval_swaps": s_ms,
+                          "ms_span_on_side_stream_in_step": s_span_ms,
                           "neighbours_per_s": nn / (s_ms * 1e-3),
                           "iterations_per_s": 1.0 / (s_ms * 1e-3),
                           "rescored_batches_per_neighbour": sw_batches / nn,
