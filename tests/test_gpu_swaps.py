@@ -492,3 +492,63 @@ def test_moves_paper_scale_sampled(torch_cuda):
         one = oracle.eval_candidates(pb, seq)
         assert d[k] == one["dist"][0] and o[k] == one["obj"][0]
     ctx.close()
+
+
+def test_two_contexts_on_two_streams_as_bench_issues_a_step(torch_cuda):
+    """bench.py's step (--overlap 1): candidate evaluation + argmin on one stream, neighbourhood
+    pass + argmin + apply on a second stream with a context of its own ("one context per
+    stream", include/whp.h), forked and joined by events every step. Both halves must still
+    equal the oracle: all candidates bit for bit, the trajectory move for move."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid")
+    n = pb.n_orders
+    ctx, ctx_nb = whp.Context.from_problem(pb), whp.Context.from_problem(pb)
+    n_cand, Wn, stride, n_iter = 1024, 32, 16, 24
+    rows = W.perm_rows(3, n, np.arange(n_cand))
+    perms = torch.from_numpy(rows).cuda()
+    base = W.base_perm(5, n)
+    ref = oracle.eval_candidates(pb, rows)
+    ref_tr = oracle.swap_trajectory(pb, base, Wn, stride, n_iter)
+
+    nn = Wn * (Wn - 1) // 2
+    perm = torch.from_numpy(base.copy()).cuda()
+    dist = torch.zeros(n_cand, dtype=torch.int64, device="cuda")
+    pen = torch.zeros(n_cand, dtype=torch.float64, device="cuda")
+    obj = torch.zeros(n_cand, dtype=torch.float64, device="cuda")
+    nbat = torch.zeros(n_cand, dtype=torch.int32, device="cuda")
+    bhash = torch.zeros(n_cand, dtype=torch.int64, device="cuda")
+    best = torch.zeros(n_iter, dtype=torch.int64, device="cuda")
+    sd = torch.zeros(nn, dtype=torch.int64, device="cuda")
+    so = torch.zeros(nn, dtype=torch.float64, device="cuda")
+    move = torch.zeros(n_iter, dtype=torch.int64, device="cuda")
+    mval = torch.zeros(n_iter, dtype=torch.float64, device="cuda")
+    main, side = torch.cuda.current_stream(), torch.cuda.Stream(priority=-1)
+    fork_ev, join_ev = torch.cuda.Event(), torch.cuda.Event()
+    torch.cuda.synchronize()
+    for it in range(n_iter):
+        s = (it * stride) % (n - Wn + 1)
+        fork_ev.record(main)
+        side.wait_event(fork_ev)
+        with torch.cuda.stream(side):
+            ctx_nb.eval_swaps(perm, s, Wn, sd, so)
+            ctx_nb.argmin(so, move[it:it + 1], mval[it:it + 1])
+            ctx_nb.apply_swap(perm, s, Wn, move[it:it + 1])
+            join_ev.record(side)
+        dist.fill_(-1)
+        ctx.eval_candidates(perms, dist=dist, penalty=pen, obj=obj, n_batches=nbat,
+                            batch_hash=bhash)
+        ctx.argmin(obj, best[it:it + 1])
+        main.wait_event(join_ev)
+    torch.cuda.synchronize()
+    assert np.array_equal(dist.cpu().numpy(), ref["dist"])
+    assert np.array_equal(obj.cpu().numpy(), ref["obj"])
+    assert np.array_equal(pen.cpu().numpy(), ref["penalty"])
+    assert np.array_equal(nbat.cpu().numpy(), ref["n_batches"])
+    assert np.array_equal(bhash.cpu().numpy().view(np.uint64), ref["batch_hash"])
+    assert np.all(best.cpu().numpy() == oracle.argmin(ref["obj"]))
+    assert np.array_equal(move.cpu().numpy(), ref_tr["move"])
+    assert np.array_equal(mval.cpu().numpy(), ref_tr["obj"])
+    assert np.array_equal(perm.cpu().numpy(), ref_tr["perm"])
+    ctx.close()
+    ctx_nb.close()
