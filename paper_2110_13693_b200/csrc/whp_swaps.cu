@@ -552,13 +552,28 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   for (int64_t nn = (int64_t)blockIdx.x * kSwapWarps + warp; nn < n_nb;
        nn += (int64_t)gridDim.x * kSwapWarps) {
     // neighbour index -> (i', j'), row i' starts at i'(2W-i'-1)/2
-    const double wm = 2.0 * W - 1.0;
-    int64_t i = (int64_t)floor((wm - sqrt(wm * wm - 8.0 * (double)nn)) * 0.5);
-    i = max((int64_t)0, min(i, (int64_t)W - 2));
-    while (i > 0 && i * (2 * (int64_t)W - i - 1) / 2 > nn) --i;
-    while ((i + 1) * (2 * (int64_t)W - i - 2) / 2 <= nn) ++i;
-    const int64_t j = i + 1 + (nn - i * (2 * (int64_t)W - i - 1) / 2);
-    const int32_t pi = win_start + (int32_t)i, pj = win_start + (int32_t)j;
+    // (an estimate of the row by a square root, made exact by the two integer loops; windows
+    // below 32,768 positions — W^2 < 2^30 — take 32-bit arithmetic and a float estimate)
+    int32_t pi, pj;
+    if (W < 32768) {
+      const int32_t n32 = (int32_t)nn, w2 = 2 * W;
+      const float wm = (float)(w2 - 1);
+      int32_t i = (int32_t)((wm - sqrtf(fmaxf(wm * wm - 8.0f * (float)n32, 0.0f))) * 0.5f);
+      i = max(0, min(i, W - 2));
+      while (i > 0 && i * (w2 - i - 1) / 2 > n32) --i;
+      while ((i + 1) * (w2 - i - 2) / 2 <= n32) ++i;
+      pi = win_start + i;
+      pj = pi + 1 + (n32 - i * (w2 - i - 1) / 2);
+    } else {
+      const double wm = 2.0 * W - 1.0;
+      int64_t i = (int64_t)floor((wm - sqrt(wm * wm - 8.0 * (double)nn)) * 0.5);
+      i = max((int64_t)0, min(i, (int64_t)W - 2));
+      while (i > 0 && i * (2 * (int64_t)W - i - 1) / 2 > nn) --i;
+      while ((i + 1) * (2 * (int64_t)W - i - 2) / 2 <= nn) ++i;
+      const int64_t j = i + 1 + (nn - i * (2 * (int64_t)W - i - 1) / 2);
+      pi = win_start + (int32_t)i;
+      pj = win_start + (int32_t)j;
+    }
     const int32_t bi = __ldg(B.bop + pi), bj = __ldg(B.bop + pj);
     swap_seq q{B.pre, B.orec, s_pre, s_orec, lo, (uint32_t)(cnt + 1), (uint32_t)cnt, pi, pj, 0};
     const int32_t qi = (int32_t)(q.orec_at(pj) & WHP_Q_MASK);  // orec_at swaps: this is q(pi)
@@ -734,7 +749,9 @@ whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   const int64_t D_base = B.totals[0];
   for (int64_t nn = (int64_t)blockIdx.x * kSwapWarps + warp; nn < n_nb;
        nn += (int64_t)gridDim.x * kSwapWarps) {
-    const int32_t i = (int32_t)(nn / (W - 1));
+    // (32-bit division when the neighbourhood has fewer than 2^31 moves)
+    const int32_t i = n_nb <= 0x7fffffff ? (int32_t)((uint32_t)nn / (uint32_t)(W - 1))
+                                         : (int32_t)(nn / (W - 1));
     const int32_t jr = (int32_t)(nn - (int64_t)i * (W - 1));
     const int32_t j = jr < i ? jr : jr + 1;
     const int32_t pi = win_start + i, pj = win_start + j;
