@@ -552,3 +552,36 @@ def test_two_contexts_on_two_streams_as_bench_issues_a_step(torch_cuda):
     assert np.array_equal(perm.cpu().numpy(), ref_tr["perm"])
     ctx.close()
     ctx_nb.close()
+
+
+def test_neighbour_index_decode_at_row_boundaries_of_a_4000_wide_window(torch_cuda):
+    """The neighbour kernel turns n into (i', j') by a float square-root estimate made exact by
+    integer correction loops (32-bit below 32,768 positions). At W = 4,000 — the whole
+    paper-scale plan, 7,998,000 swaps — (2W-1)^2 no longer fits a float mantissa, so the estimate
+    is off near the row boundaries: the first and last neighbour of many rows, and random ones,
+    against the oracle on the materialised plans."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("paper")
+    ctx = whp.Context.from_problem(pb)
+    n = pb.n_orders
+    base = W.base_perm(6, n)
+    rng = np.random.default_rng(21)
+    rows = np.unique(np.concatenate([np.arange(0, 6), np.arange(n - 8, n - 1), [1000, 2047, 2048, 2896, 3000],
+                                     rng.integers(0, n - 1, 60)]))
+    i = np.concatenate([rows, rows, rng.integers(0, n - 1, 150)])
+    j = np.concatenate([rows + 1, np.full(len(rows), n - 1), np.zeros(150, dtype=np.int64)])
+    j[2 * len(rows):] = rng.integers(i[2 * len(rows):] + 1, n)
+    idx = i * (2 * n - i - 1) // 2 + (j - i - 1)
+    plans = np.repeat(base[None, :], len(i), axis=0)
+    plans[np.arange(len(i)), i], plans[np.arange(len(i)), j] = base[j], base[i]
+    nn = n * (n - 1) // 2
+    d = torch.zeros(nn, dtype=torch.int64, device="cuda")
+    o = torch.zeros(nn, dtype=torch.float64, device="cuda")
+    ctx.eval_swaps(torch.from_numpy(base).cuda(), 0, n, d, o)
+    torch.cuda.synchronize()
+    ref = oracle.eval_candidates(pb, plans)
+    sel = torch.from_numpy(idx).cuda()
+    assert np.array_equal(d[sel].cpu().numpy(), ref["dist"])
+    assert np.array_equal(o[sel].cpu().numpy(), ref["obj"])
+    ctx.close()
