@@ -34,9 +34,8 @@ WORKLOAD = "paper"  # BASELINE.json configs[2] (the third listed): the config th
 CPU_SAMPLE = 8192   # candidates the oracle is timed on for cpu_baseline (~12 s on one core)
 REF_SAMPLE = 256    # candidates per step of --impl reference: 1/64 of the 16,384 of a step
 REF_WINDOW = 32     # and the 496 swaps of a 32-wide window: ~1/66 of the step's 32,640 neighbours
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the candidate kernel, from the
-# ncu --set full capture recorded in profiles/ (None until measured for the current kernel)
-NCU_TRAFFIC_BYTES = 521.3e6  # K1 367.2 + segments 8.4 + K2 145.7 MB (profiles/r1_v11_tuned_path.md)
+SUSTAIN_S = 2.5     # the `sustained` leg repeats the step for at least this long
+KERNEL_PASS = 32    # steps of the separate pass that times the candidate evaluation by events
 
 
 def config_dict(pb, n_cand, world, wl_nb):
@@ -128,14 +127,14 @@ def run_ours(args):
     sobj = torch.zeros(nn, dtype=torch.float64, device=dev)
     sidx = torch.zeros(1, dtype=torch.int64, device=dev)
     it_counter = [0]
-    # Kernel durations are sampled inside the timed region: an event pair costs ~10 us of stream
-    # time (measured: 4 records per step = +40 us on a 0.53 ms step), so with many steps only
-    # every 8th step carries them.
-    ev_every = 8 if args.steps >= 32 else 1
+    # The candidate evaluation's own duration (roofline.kernel_ms) comes from a separate pass
+    # AFTER the timed region (KERNEL_PASS more steps of the same two-stream step, every one with an
+    # event pair around the call). Event records cost ~10 us of stream time each, so inside the
+    # timed region only every 8th step carries one pair (main stream only; <1 % of the region,
+    # whatever --steps is) — reported as kernel_ms_in_timed_region, a cross-check.
     k_ev = {k: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-            for k in range(0, args.steps, ev_every)}
-    s_ev = {k: (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-            for k in range(0, args.steps, ev_every)}
+            for k in range(0, args.steps, 8)}
+    s_ev = {}
 
     # The two halves of a step are independent (the neighbourhood pass works on the trajectory
     # plan, not on the evaluated candidates), so with --overlap 1 they run on two streams, each
@@ -149,10 +148,10 @@ def run_ours(args):
 
     def neighbourhood_half(timed_index):
         s = (it_counter[0] * stride) % (n - Wn + 1)
-        if timed_index is not None:
+        if timed_index in s_ev:
             s_ev[timed_index][0].record()
         ctx_nb.eval_swaps(base, s, Wn, dist=sdist, obj=sobj)
-        if timed_index is not None:
+        if timed_index in s_ev:
             s_ev[timed_index][1].record()
         ctx_nb.argmin(sobj, sidx)
         ctx_nb.apply_swap(base, s, Wn, sidx)
@@ -208,8 +207,20 @@ def run_ours(args):
         ms, clocks, launches = timed_run()
         remeasured = True
     ms = harness.max_over_ranks(ms, world, dev)
+    k_ms_in_region = float(np.mean([a.elapsed_time(b) for a, b in k_ev.values()]))
+    k_in_region_samples = len(k_ev)
+    k_ev.clear()
+    # ---- separate pass: the same step, with an event pair around the evaluation of every step
+    for k in range(KERNEL_PASS):
+        k_ev[k] = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+        s_ev[k] = (torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+    torch.cuda.synchronize()
+    for k in range(KERNEL_PASS):
+        step(k)
+    torch.cuda.synchronize()
     k_ms = float(np.mean([a.elapsed_time(b) for a, b in k_ev.values()]))
     s_ms = float(np.mean([a.elapsed_time(b) for a, b in s_ev.values()]))
+    k_ev.clear(), s_ev.clear()
     k_ms_max = harness.max_over_ranks(k_ms, world, dev)
     s_span_ms = s_ms
     if overlap:
@@ -230,6 +241,29 @@ def run_ours(args):
         s_ms = float(np.mean([a.elapsed_time(b) for a, b in alone]))
     ms_per_step = ms / args.steps
     value = n_cand * world / (ms_per_step * 1e-3)
+
+    # ---- sustained: the same step repeated for >= SUSTAIN_S seconds, clocks sampled throughout --
+    sustained = None
+    if world == 1 and args.sustain:
+        n_sus = max(args.steps, int(SUSTAIN_S / (ms_per_step * 1e-3)) + 1)
+        sampler = harness.ClockSampler(local_rank, args.clock_period_ms).start().wait_first()
+        for _ in range(3):
+            step()
+        torch.cuda.synchronize()
+        sampler.mark()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(n_sus):
+            step()
+        e1.record()
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        sus_clocks = sampler.stop()
+        sus_ms = e0.elapsed_time(e1) / n_sus
+        sustained = {"steps": n_sus, "seconds": wall, "ms_per_step": sus_ms,
+                     "value": n_cand / (sus_ms * 1e-3), "unit": "candidate plans/s",
+                     "vs_timed_region": ms_per_step / sus_ms, "clocks": sus_clocks}
 
     # ---- end to end through the host-buffer entry point (pinned host memory) ---------------
     h_perms = torch.empty((n_cand, n), dtype=torch.int32).pin_memory()
@@ -295,16 +329,97 @@ def run_ours(args):
     # sweeps of a 32 MB buffer that stays resident in the 126 MB L2, one launch
     l2_gbs = ctx.probe_l2_read(32 << 20, 200)
 
+    peaks = harness.measured_peaks(ROOT)
+    counters = harness.ncu_counters(ROOT)
+
+    # ---- stress: BASELINE.json configs[5] at its full 65,536 plans --
+    stress = None
+    if world == 1 and args.stress:
+        wls = W.make_workload("stress")
+        pbs = wls.problem
+        ns, ncs = pbs.n_orders, wls.n_cand
+        ctx_s = whp.Context.from_problem(pbs, device=local_rank)
+        sperms = torch.empty((ncs, ns), dtype=torch.int32, device=dev)  # 5.24 GB, made in HBM
+        for lo_s in range(0, ncs, 4096):
+            sperms[lo_s:lo_s + 4096] = W.perms_torch(wls.seed, ns, lo_s, lo_s + 4096, dev)
+        sd = torch.zeros(ncs, dtype=torch.int64, device=dev)
+        so = torch.zeros(ncs, dtype=torch.float64, device=dev)
+        sh = torch.zeros(ncs, dtype=torch.int64, device=dev)
+        for _ in range(3):
+            ctx_s.eval_candidates(sperms, dist=sd, obj=so, batch_hash=sh)
+        torch.cuda.synchronize()
+        reps = 10
+        ev0.record()
+        for _ in range(reps):
+            ctx_s.eval_candidates(sperms, dist=sd, obj=so, batch_hash=sh)
+        ev1.record()
+        torch.cuda.synchronize()
+        st_ms = ev0.elapsed_time(ev1) / reps
+        sb = harness.algorithmic_bytes_per_candidate(ns, pbs.n_items)
+        st_ach = sb["survey"] * ncs / (st_ms * 1e-3) / 1e9
+        # spot check against the oracle (all 65,536 plans are compared in tests/test_gpu_fullsize.py)
+        stress = {"workload": "stress (BASELINE.json configs[5th]): 20,000 orders, "
+                              f"{pbs.n_items} items, C=40, K=32, Zipf(1.2), {ncs} plans in one launch",
+                  "ms": st_ms, "value": ncs / (st_ms * 1e-3), "unit": "candidate plans/s",
+                  "picks_per_s": ncs * pbs.n_items / (st_ms * 1e-3),
+                  "bytes_per_candidate": sb["survey"], "achieved": st_ach, "peak": peaks["hbm_gbs"],
+                  "frac": st_ach / peaks["hbm_gbs"],
+                  "frac_hbm_compulsory": sb["hbm_compulsory"] * ncs / (st_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                  "traffic": counters.get("stress", {}).get("dram_bytes"),
+                  "reps": reps, "input_bytes": int(sperms.numel() * 4)}
+        if rank == 0:
+            import oracle
+            rows_s = np.array([0, 1, 4097, ncs - 1])
+            ref_s = oracle.eval_candidates(pbs, sperms[torch.from_numpy(rows_s).to(dev)].cpu().numpy())
+            stress["sampled_rows_equal_oracle"] = bool(
+                np.array_equal(ref_s["obj"], so.cpu().numpy()[rows_s])
+                and np.array_equal(ref_s["dist"], sd.cpu().numpy()[rows_s]))
+        ctx_s.close()
+        del sperms, sd, so, sh
+        torch.cuda.empty_cache()
+
     # ---- roofline of the dominant kernel (candidate evaluation) -----------------------------
     bytes_pc = harness.algorithmic_bytes_per_candidate(n, pb.n_items)
-    peaks = harness.measured_peaks(ROOT)
     achieved = bytes_pc["survey"] * n_cand / (k_ms_max * 1e-3) / 1e9
+    cp = counters.get("paper", {})
+    sm_clock_hz = 1e6 * float((clocks or {}).get("sm_mhz") or 1965.0)
+    # the units that actually bind the path: warp-instruction issue slots and the
+    # shared-memory pipe. Counts per launch come from the ncu capture recorded for these sources
+    # (profiles/ncu_counters.csv); the time is this run's; peak = 148 SMs x 4 issue slots (x 1
+    # shared-memory wavefront) per clock at the SM clock sampled during the timed region.
+    n_sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    binding = None
+    if "warp_inst" in cp and "smem_wavefronts" in cp:
+        issue_peak = n_sms * 4 * sm_clock_hz
+        smem_peak = n_sms * 1 * sm_clock_hz
+        binding = {"issue_slots": {"achieved": cp["warp_inst"] / (k_ms_max * 1e-3), "peak": issue_peak,
+                                   "frac": cp["warp_inst"] / (k_ms_max * 1e-3) / issue_peak,
+                                   "unit": "warp instructions/s"},
+                   "smem_pipe": {"achieved": cp["smem_wavefronts"] / (k_ms_max * 1e-3), "peak": smem_peak,
+                                 "frac": cp["smem_wavefronts"] / (k_ms_max * 1e-3) / smem_peak,
+                                 "unit": "shared-memory wavefronts/s"},
+                   "dram": {"achieved": cp.get("dram_bytes", 0.0) / (k_ms_max * 1e-3) / 1e9,
+                            "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                            "frac": cp.get("dram_bytes", 0.0) / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"]},
+                   "sm_clock_mhz": sm_clock_hz / 1e6, "counts_from": cp.get("source"),
+                   "note": "whole evaluation (K1 + segments + K2), so the fractions average a "
+                           "DRAM-streaming kernel and an issue/shared-memory bound one"}
     roofline = {
         "bound": "hbm", "kernel": "whp_eval_candidates (bounds + segments + sets kernels)", "achieved": achieved,
         "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": achieved / peaks["hbm_gbs"],
-        "traffic": NCU_TRAFFIC_BYTES, "peak_source": peaks["source"] + ", burst copy figure",
+        "traffic": cp.get("dram_bytes"),
+        "traffic_note": (f"ncu dram bytes of one evaluation, captured on these kernel sources "
+                         f"({counters['csrc_sha16']}): {cp.get('source')}") if "dram_bytes" in cp else
+                        ("no ncu capture recorded for these kernel sources "
+                         f"({counters['csrc_sha16']}); see profiles/ for earlier versions"),
+        "binding_resource": binding,
+        "peak_source": peaks["source"] + ", burst copy figure",
         "bytes_per_candidate": bytes_pc["survey"], "kernel_ms": k_ms_max,
-        "kernel_ms_samples": len(k_ev),
+        "kernel_ms_samples": KERNEL_PASS,
+        "kernel_ms_how": "mean over a separate pass of the same two-stream step after the timed "
+                         "region, an event pair around whp_eval_candidates in every step",
+        "kernel_ms_in_timed_region": k_ms_in_region,
+        "kernel_ms_in_timed_region_samples": k_in_region_samples,
         "kernel_share_of_step": k_ms_max / ms_per_step,
         "frac_packed_bytes": bytes_pc["packed"] * n_cand / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"],
         "frac_hbm_compulsory": bytes_pc["hbm_compulsory"] * n_cand / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"],
@@ -376,6 +491,8 @@ def run_ours(args):
         "legsum": {"ms": legsum_ms, "plans_per_s": n_cand / (legsum_ms * 1e-3),
                    "what": "whp_eval_legsum on the same 16,384 plans (paper-literal Eq. 2)"},
         "roofline": roofline,
+        "sustained": sustained,
+        "stress": stress,
         "cpu_baseline": cpu,
         "e2e": {"value": e2e_value, "unit": "candidate plans/s",
                 "h2d_bytes_per_step": int(h_perms.numel() * 4),
@@ -397,6 +514,10 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--overlap", type=int, default=1, choices=[0, 1],
                     help="1: candidate evaluation and neighbourhood pass of a step on two streams")
+    ap.add_argument("--sustain", type=int, default=1, choices=[0, 1],
+                    help="1: also repeat the step for >= 2.5 s with the clocks sampled (N=1 only)")
+    ap.add_argument("--stress", type=int, default=1, choices=[0, 1],
+                    help="1: also time BASELINE.json's stress config at its full 65,536 plans (N=1 only)")
     ap.add_argument("--clock-period-ms", type=int, default=50,
                     help="nvidia-smi sampling period during the timed region")
     args = ap.parse_args()

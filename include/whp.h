@@ -35,7 +35,8 @@
  *     whp_validate_perms when the source is untrusted.
  *
  * Limits (WHP_ERR_OUT_OF_RANGE beyond them): n_aisles <= 1024, slots_per_side <= 4095,
- *   n_classes <= 256, n_orders < 2^24, total items < 2^24, cart_capacity < 2^20.
+ *   n_classes <= 256, n_orders < 2^24, total items < 2^24, cart_capacity < 2^20, at most 255
+ *   items per order.
  *   The tuned kernels additionally need n_orders < 65536, cart_capacity <= 106 and pick cursors
  *   that fit 16 bits; other shapes run the general (slower) kernels with
  *   the same results.
@@ -107,7 +108,9 @@ whp_status whp_eval_candidates(whp_ctx* ctx, const int32_t* d_perms, int64_t n_c
  * int32[n_cand][n_orders]; h_dist / h_obj host arrays [n_cand] (nullable). Permutations are
  * copied to the device in chunks overlapped with evaluation; results are copied back; the
  * call returns after everything has completed. Pinned host memory makes the copies
- * asynchronous, pageable memory works but serialises. */
+ * asynchronous, pageable memory works but serialises. The call runs on streams of its own and
+ * does not order itself after work the caller queued earlier on this context (e.g. a
+ * whp_nhatc_update still in flight): the context must be idle when it is called. */
 whp_status whp_eval_candidates_host(whp_ctx* ctx, const int32_t* h_perms, int64_t n_cand,
                                     int64_t* h_dist, double* h_obj,
                                     int64_t* h_argmin_idx, double* h_argmin_val);
@@ -196,6 +199,25 @@ whp_status whp_apply_move(whp_ctx* ctx, int32_t* d_base_perm, int32_t win_start,
  * permutation of 0..n_orders-1. Synchronises the stream. */
 whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand,
                               int64_t* h_n_bad, void* cuda_stream);
+
+/* Debug / measurement switch on the kernel selection of ONE context (the results never change,
+ * only which kernels compute them; tests use it to reach every code path). value < 0 restores the
+ * default. Takes effect from the next call on the context; not meant for production use.
+ *   WHP_DEBUG_FORCE_GENERAL  value != 0: whp_eval_candidates / whp_eval_legsum / whp_eval_routing
+ *                            take the general warp-per-plan kernels even on tuned-path shapes
+ *   WHP_DEBUG_SEGMENTS       segments per plan of the tuned path (a power of two <= 32; ignored
+ *                            when the plan's batch count does not allow it)
+ *   WHP_DEBUG_WARPS          warps per block of the tuned set kernel (capped by what fits)
+ *   WHP_DEBUG_SWAP_MARGIN    positions after the window that whp_eval_swaps / whp_eval_moves
+ *                            tabulate (0 forces the batch-by-batch fallback of every chain)
+ * Unknown keys return WHP_ERR_INVALID_ARG. There are no environment variables. */
+typedef enum {
+  WHP_DEBUG_FORCE_GENERAL = 0,
+  WHP_DEBUG_SEGMENTS = 1,
+  WHP_DEBUG_WARPS = 2,
+  WHP_DEBUG_SWAP_MARGIN = 3
+} whp_debug_key;
+whp_status whp_debug_set(whp_ctx* ctx, int32_t key, int64_t value);
 
 /* Measurement helper ("actually-rescored picks"): with enable != 0 every later
  * whp_eval_swaps / whp_eval_moves call also counts the batches it scored from their picks and

@@ -1,4 +1,7 @@
-"""ctypes marshalling for whp_oracle.c — no arithmetic of the method lives here."""
+"""ctypes marshalling for whp_oracle.c. The arithmetic of the method lives in the C file; the only
+compositions written here are `nhatc_loop` (the outer loop of reading N1: eval -> argmin -> update,
+each step a C routine) and the `threads=` wrappers, which spread candidates / neighbourhood rows
+over host threads around the same single-threaded C routines ("wrapper only")."""
 import ctypes as C
 import os
 import subprocess
@@ -95,8 +98,22 @@ def _common(pb):
     return args, (keep, g)
 
 
-def eval_candidates(pb, perms, detail: bool = False) -> dict:
-    """D1–D6 for every row of perms. detail=True also returns batch_of_pos and resp."""
+def _pool_map(fn, cuts, threads):
+    """fn(lo, hi) over consecutive cuts on `threads` host threads (the C routines release the GIL)."""
+    from concurrent.futures import ThreadPoolExecutor
+    spans = [(int(cuts[k]), int(cuts[k + 1])) for k in range(len(cuts) - 1) if cuts[k] < cuts[k + 1]]
+    with ThreadPoolExecutor(max(1, threads)) as ex:
+        list(ex.map(lambda ab: fn(*ab), spans))
+
+
+def _off(a, row):
+    """pointer to row `row` of a C-contiguous array (None stays NULL)"""
+    return None if a is None else C.c_void_p(a.ctypes.data + int(row) * a.strides[0])
+
+
+def eval_candidates(pb, perms, detail: bool = False, threads: int = 1) -> dict:
+    """D1–D6 for every row of perms. detail=True also returns batch_of_pos and resp.
+    threads > 1: candidate slices on that many host threads, same routine per candidate."""
     perms = _i32(perms)
     if perms.ndim == 1:
         perms = perms[None, :]
@@ -110,10 +127,18 @@ def eval_candidates(pb, perms, detail: bool = False) -> dict:
         "resp": np.zeros((n_cand, pb.n_classes), np.int32) if detail else None,
     }
     args, keep = _common(pb)
-    _load().orc_eval_candidates(*args, _p(perms), C.c_int64(n_cand), _p(out["dist"]),
-                                _p(out["penalty"]), _p(out["obj"]), _p(out["n_batches"]),
-                                _p(out["batch_hash"]), _p(out["batch_of_pos"]),
-                                _p(out["n_distinct"]), _p(out["resp"]))
+    lib = _load()
+
+    def run(lo, hi):
+        lib.orc_eval_candidates(*args, _off(perms, lo), C.c_int64(hi - lo), _off(out["dist"], lo),
+                                _off(out["penalty"], lo), _off(out["obj"], lo),
+                                _off(out["n_batches"], lo), _off(out["batch_hash"], lo),
+                                _off(out["batch_of_pos"], lo), _off(out["n_distinct"], lo),
+                                _off(out["resp"], lo))
+    if threads <= 1:
+        run(0, n_cand)
+    else:
+        _pool_map(run, np.linspace(0, n_cand, min(n_cand, 8 * threads) + 1).astype(np.int64), threads)
     del keep
     return out
 
@@ -131,13 +156,32 @@ def eval_candidate_batches(pb, perm):
     return bd[:nb.value].copy(), bop
 
 
-def eval_swaps(pb, base_perm, win_start: int, win_len: int) -> dict:
+def eval_swaps(pb, base_perm, win_start: int, win_len: int, threads: int = 1) -> dict:
+    """D8: every pairwise swap inside the window, each materialised and evaluated from scratch.
+    threads > 1: the rows i' of the neighbourhood on that many host threads."""
     base_perm = _i32(base_perm)
     nn = win_len * (win_len - 1) // 2
     out = {"dist": np.zeros(nn, np.int64), "obj": np.zeros(nn, np.float64)}
     args, keep = _common(pb)
-    _load().orc_eval_swaps(*args, _p(base_perm), C.c_int32(win_start), C.c_int32(win_len),
+    lib = _load()
+    if threads <= 1:
+        lib.orc_eval_swaps(*args, _p(base_perm), C.c_int32(win_start), C.c_int32(win_len),
                            _p(out["dist"]), _p(out["obj"]))
+    else:
+        def run(lo, hi):
+            lib.orc_eval_swaps_rows(*args, _p(base_perm), C.c_int32(win_start),
+                                    C.c_int32(win_len), C.c_int32(lo), C.c_int32(hi),
+                                    _p(out["dist"]), _p(out["obj"]))
+        # row i' holds W-1-i' neighbours: pair row k with row W-2-k so every task is equal
+        half = (win_len - 1 + 1) // 2
+        from concurrent.futures import ThreadPoolExecutor
+        def pair(k):
+            run(k, k + 1)
+            m = win_len - 2 - k
+            if m > k:
+                run(m, m + 1)
+        with ThreadPoolExecutor(threads) as ex:
+            list(ex.map(pair, range(half)))
     del keep
     return out
 

@@ -242,25 +242,41 @@ int64_t orc_argmin(const double* x, int64_t n) {
 }
 
 /* ---- D8 swap neighbourhood: materialise each swapped permutation, evaluate from scratch - */
+/* rows [i_lo, i_hi) of the neighbourhood: every neighbour (i', j') with i_lo <= i' < i_hi, in
+ * lexicographic order, written at its index n = i'(2W-i'-1)/2 + (j'-i'-1) of dist / obj (both
+ * sized for the whole neighbourhood). Lets a test spread the rows over host threads; the
+ * per-neighbour routine is the same from-scratch evaluation. */
+int32_t orc_eval_swaps_rows(const orc_geom* g, const int32_t* sku_loc, const int32_t* sku_class,
+                            int32_t K, int32_t n_orders, const int32_t* order_ptr,
+                            const int32_t* item_sku, int32_t C, const double* t, const double* v,
+                            const double* w, const int32_t* base_perm, int32_t win_start,
+                            int32_t win_len, int32_t i_lo, int32_t i_hi, int64_t* dist,
+                            double* obj) {
+  int32_t* p = (int32_t*)malloc(sizeof(int32_t) * (size_t)n_orders);
+  int64_t n = 0;
+  for (int32_t i = 0; i < win_len; i++)
+    for (int32_t j = i + 1; j < win_len; j++) { /* lexicographic (i', j') */
+      if (i >= i_lo && i < i_hi) {
+        memcpy(p, base_perm, sizeof(int32_t) * (size_t)n_orders);
+        int32_t tmp = p[win_start + i];
+        p[win_start + i] = p[win_start + j];
+        p[win_start + j] = tmp;
+        orc_eval_candidate(g, sku_loc, sku_class, K, n_orders, order_ptr, item_sku, C, t, v, w,
+                           p, dist ? dist + n : 0, 0, obj ? obj + n : 0, 0, 0, 0, 0, 0, 0);
+      }
+      n++;
+    }
+  free(p);
+  return 0;
+}
+
 int32_t orc_eval_swaps(const orc_geom* g, const int32_t* sku_loc, const int32_t* sku_class,
                        int32_t K, int32_t n_orders, const int32_t* order_ptr,
                        const int32_t* item_sku, int32_t C, const double* t, const double* v,
                        const double* w, const int32_t* base_perm, int32_t win_start,
                        int32_t win_len, int64_t* dist, double* obj) {
-  int32_t* p = (int32_t*)malloc(sizeof(int32_t) * (size_t)n_orders);
-  int64_t n = 0;
-  for (int32_t i = 0; i < win_len; i++)
-    for (int32_t j = i + 1; j < win_len; j++) { /* lexicographic (i', j') */
-      memcpy(p, base_perm, sizeof(int32_t) * (size_t)n_orders);
-      int32_t tmp = p[win_start + i];
-      p[win_start + i] = p[win_start + j];
-      p[win_start + j] = tmp;
-      orc_eval_candidate(g, sku_loc, sku_class, K, n_orders, order_ptr, item_sku, C, t, v, w, p,
-                         dist ? dist + n : 0, 0, obj ? obj + n : 0, 0, 0, 0, 0, 0, 0);
-      n++;
-    }
-  free(p);
-  return 0;
+  return orc_eval_swaps_rows(g, sku_loc, sku_class, K, n_orders, order_ptr, item_sku, C, t, v, w,
+                             base_perm, win_start, win_len, 0, win_len, dist, obj);
 }
 
 /* neighbour index -> (i', j') by counting rows, the inverse of n = i'(2W-i'-1)/2 + (j'-i'-1) */

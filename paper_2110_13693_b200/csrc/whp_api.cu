@@ -9,9 +9,18 @@
 #include <algorithm>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>  // header-only: ranges cost nothing unless a profiler is attached
+
 #include "whp_internal.cuh"
 
 namespace {
+
+// NVTX range around an entry point (the layout "is chosen to evaluate
+// possible bottlenecks in a specific subprocess"): nsys / ncu --nvtx show the calls by name.
+struct nvtx_range {
+  explicit nvtx_range(const char* name) { nvtxRangePushA(name); }
+  ~nvtx_range() { nvtxRangePop(); }
+};
 
 whp_status fail(whp_ctx* c, whp_status s, const char* msg) {
   if (c) c->err = msg;
@@ -76,6 +85,7 @@ whp_status whp_create_layout(int32_t n_aisles, int32_t slots_per_side, int32_t s
                              int32_t aisle_spacing, int32_t depot_aisle, int32_t n_skus,
                              const int32_t* sku_loc, const int32_t* sku_class, int32_t n_classes,
                              int32_t cuda_device, whp_ctx** out) {
+  nvtx_range nvtx_("whp_create_layout");
   if (!out) return WHP_ERR_INVALID_ARG;
   *out = nullptr;
   if (!sku_loc || !sku_class) return WHP_ERR_INVALID_ARG;
@@ -132,6 +142,7 @@ whp_status whp_create_layout(int32_t n_aisles, int32_t slots_per_side, int32_t s
 
 whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_ptr,
                            const int32_t* item_sku, int32_t cart_capacity) {
+  nvtx_range nvtx_("whp_load_orders");
   if (!c) return WHP_ERR_INVALID_ARG;
   c->err.clear();
   if (!order_ptr || !item_sku || n_orders < 1 || cart_capacity < 1)
@@ -227,6 +238,7 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
 }
 
 whp_status whp_set_penalty(whp_ctx* c, const double* t, const double* v, const double* w) {
+  nvtx_range nvtx_("whp_set_penalty");
   if (!c) return WHP_ERR_INVALID_ARG;
   c->err.clear();
   if (!t || !v || !w) return fail(c, WHP_ERR_INVALID_ARG, "null pointer");
@@ -256,6 +268,7 @@ whp_status whp_eval_candidates(whp_ctx* c, const int32_t* d_perms, int64_t n_can
                                int32_t* d_n_batches, uint64_t* d_batch_hash,
                                int32_t* d_batch_of_pos, int32_t* d_n_distinct, int32_t* d_resp,
                                void* cuda_stream) {
+  nvtx_range nvtx_("whp_eval_candidates");
   whp_status s = ready(c);
   if (s != WHP_OK) return s;
   if (n_cand < 0) return fail(c, WHP_ERR_INVALID_ARG, "n_cand < 0");
@@ -270,6 +283,7 @@ whp_status whp_eval_candidates(whp_ctx* c, const int32_t* d_perms, int64_t n_can
 
 whp_status whp_eval_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                           int32_t win_len, int64_t* d_dist, double* d_obj, void* cuda_stream) {
+  nvtx_range nvtx_("whp_eval_swaps");
   whp_status s = ready(c);
   if (s != WHP_OK) return s;
   if (!d_base_perm) return fail(c, WHP_ERR_INVALID_ARG, "d_base_perm is null");
@@ -284,6 +298,7 @@ whp_status whp_eval_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_st
 
 whp_status whp_argmin(whp_ctx* c, const double* d_obj, int64_t n, int64_t* d_idx, double* d_val,
                       void* cuda_stream) {
+  nvtx_range nvtx_("whp_argmin");
   if (!c) return WHP_ERR_INVALID_ARG;
   c->err.clear();
   if (!d_obj || !d_idx || n < 1) return fail(c, WHP_ERR_INVALID_ARG, "null pointer or n < 1");
@@ -294,6 +309,7 @@ whp_status whp_argmin(whp_ctx* c, const double* d_obj, int64_t n, int64_t* d_idx
 
 whp_status whp_apply_swap(whp_ctx* c, int32_t* d_base_perm, int32_t win_start, int32_t win_len,
                           const int64_t* d_idx, void* cuda_stream) {
+  nvtx_range nvtx_("whp_apply_swap");
   if (!c) return WHP_ERR_INVALID_ARG;
   c->err.clear();
   if (!c->have_orders) return fail(c, WHP_ERR_STATE, "whp_load_orders has not been called");
@@ -330,6 +346,7 @@ whp_status whp_validate_perms(whp_ctx* c, const int32_t* d_perms, int64_t n_cand
 whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t n_cand,
                                     int64_t* h_dist, double* h_obj, int64_t* h_argmin_idx,
                                     double* h_argmin_val) {
+  nvtx_range nvtx_("whp_eval_candidates_host");
   whp_status s = ready(c);
   if (s != WHP_OK) return s;
   if (n_cand < 0) return fail(c, WHP_ERR_INVALID_ARG, "n_cand < 0");
@@ -386,6 +403,7 @@ whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t 
 
 whp_status whp_eval_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                           int32_t win_len, int64_t* d_dist, double* d_obj, void* cuda_stream) {
+  nvtx_range nvtx_("whp_eval_moves");
   whp_status s = ready(c);
   if (s != WHP_OK) return s;
   if (!d_base_perm) return fail(c, WHP_ERR_INVALID_ARG, "d_base_perm is null");
@@ -400,6 +418,7 @@ whp_status whp_eval_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_st
 
 whp_status whp_apply_move(whp_ctx* c, int32_t* d_base_perm, int32_t win_start, int32_t win_len,
                           const int64_t* d_idx, void* cuda_stream) {
+  nvtx_range nvtx_("whp_apply_move");
   if (!c) return WHP_ERR_INVALID_ARG;
   c->err.clear();
   if (!c->have_orders) return fail(c, WHP_ERR_STATE, "whp_load_orders has not been called");
@@ -415,6 +434,7 @@ whp_status whp_apply_move(whp_ctx* c, int32_t* d_base_perm, int32_t win_start, i
 
 whp_status whp_eval_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                            void* cuda_stream) {
+  nvtx_range nvtx_("whp_eval_legsum");
   if (!c) return WHP_ERR_INVALID_ARG;
   c->err.clear();
   if (!c->have_orders) return fail(c, WHP_ERR_STATE, "whp_load_orders has not been called");
@@ -428,6 +448,7 @@ whp_status whp_eval_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, i
 
 whp_status whp_nhatc_update(whp_ctx* c, const int32_t* d_resp_rows, const int64_t* d_idx,
                             double beta, void* cuda_stream) {
+  nvtx_range nvtx_("whp_nhatc_update");
   whp_status s = ready(c);
   if (s != WHP_OK) return s;
   if (!d_resp_rows) return fail(c, WHP_ERR_INVALID_ARG, "d_resp_rows is null");
@@ -440,6 +461,7 @@ whp_status whp_nhatc_update(whp_ctx* c, const int32_t* d_resp_rows, const int64_
 whp_status whp_nhatc_solve(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int32_t n_outer,
                            double beta, int64_t* d_idx_hist, int64_t* d_dist_hist,
                            double* d_obj_hist, void* cuda_stream) {
+  nvtx_range nvtx_("whp_nhatc_solve");
   whp_status s = ready(c);
   if (s != WHP_OK) return s;
   if (!d_perms || n_cand < 1 || n_outer < 0) return fail(c, WHP_ERR_INVALID_ARG, "bad argument");
@@ -484,6 +506,19 @@ whp_status whp_get_penalty(whp_ctx* c, double* t, double* v, double* w, void* cu
   if (v) WHP_CUDA(c, cudaMemcpyAsync(v, c->d_tvw + c->K, bytes, cudaMemcpyDeviceToHost, st));
   if (w) WHP_CUDA(c, cudaMemcpyAsync(w, c->d_tvw + 2 * (size_t)c->K, bytes, cudaMemcpyDeviceToHost, st));
   WHP_CUDA(c, cudaStreamSynchronize(st));
+  return WHP_OK;
+}
+
+whp_status whp_debug_set(whp_ctx* c, int32_t key, int64_t value) {
+  if (!c) return WHP_ERR_INVALID_ARG;
+  c->err.clear();
+  switch (key) {
+    case WHP_DEBUG_FORCE_GENERAL: c->dbg_force_general = value > 0 ? 1 : 0; break;
+    case WHP_DEBUG_SEGMENTS: c->dbg_segments = value > 0 && value <= 32 ? (int32_t)value : -1; break;
+    case WHP_DEBUG_WARPS: c->dbg_warps = value > 0 && value <= 32 ? (int32_t)value : -1; break;
+    case WHP_DEBUG_SWAP_MARGIN: c->dbg_swap_margin = value >= 0 ? value : -1; break;
+    default: return fail(c, WHP_ERR_INVALID_ARG, "unknown debug key");
+  }
   return WHP_OK;
 }
 

@@ -76,10 +76,10 @@ whp_argmin_kernel(const double* __restrict__ x, int64_t n, am_pair* parts, unsig
 __global__ void whp_apply_swap_kernel(int32_t* base_perm, int32_t win_start, int32_t W,
                                       const int64_t* __restrict__ d_idx) {
   const int64_t n = *d_idx;
+  if (n < 0 || n >= (int64_t)W * (W - 1) / 2) return;  // not a neighbour: leave the plan untouched
   int64_t i = 0, row = W - 1, rem = n;
   while (rem >= row && row > 0) { rem -= row; --row; ++i; }
   const int64_t j = i + 1 + rem;
-  if (j >= W) return;  // out-of-range index: leave the plan untouched
   const int32_t a = base_perm[win_start + i];
   base_perm[win_start + i] = base_perm[win_start + j];
   base_perm[win_start + j] = a;
@@ -173,7 +173,8 @@ cudaError_t whp_launch_validate(whp_ctx* c, const int32_t* d_perms, int64_t n_ca
   const int words = (c->n_orders + 31) >> 5;
   const size_t smem = (size_t)words * 4;
   cudaError_t e = cudaFuncSetAttribute(whp_validate_kernel,
-                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       c->smem_optin - 1024);  // constant: see whp_swaps.cu
   if (e != cudaSuccess) return e;
   int64_t blocks = n_cand < (int64_t)c->num_sms * 8 ? n_cand : (int64_t)c->num_sms * 8;
   whp_validate_kernel<<<(unsigned)blocks, 256, smem, st>>>(d_perms, n_cand, c->n_orders,

@@ -1087,9 +1087,9 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   int warps_cap = 24;
   int S = 1;
   while (S < 32 && ((nb_ub + S - 1) / S > 255 || n_cand * S < 4ll * c->num_sms * warps_cap * 32)) S <<= 1;
-  if (const char* e = getenv("WHP_SEGMENTS")) {
-    int v = atoi(e);
-    if (v >= 1 && v <= 32 && (v & (v - 1)) == 0 && (nb_ub + v - 1) / v <= 255) S = v;
+  if (c->dbg_segments >= 1) {  // whp_debug_set(WHP_DEBUG_SEGMENTS): ignored when not legal
+    const int v = c->dbg_segments;
+    if (v <= 32 && (v & (v - 1)) == 0 && (nb_ub + v - 1) / v <= 255) S = v;
   }
   int log2S = 0;
   while ((1 << log2S) < S) ++log2S;
@@ -1099,7 +1099,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   if (KW * kernel_planes > 42) warps_cap = 16;  // __launch_bounds__ of the register-heavy instantiations
   int warps = (int)(avail / priv_per_warp);
   if (warps > warps_cap) warps = warps_cap;
-  if (const char* e = getenv("WHP_WARPS")) { int v = atoi(e); if (v >= 1 && v <= warps) warps = v; }
+  if (c->dbg_warps >= 1 && c->dbg_warps <= warps) warps = c->dbg_warps;  // WHP_DEBUG_WARPS
   if (warps < 1) return cudaErrorInvalidConfiguration;
   const int planes_used = kernel_planes + log2S;
   // every per-batch length below 2^31: the close can work in 32 bits

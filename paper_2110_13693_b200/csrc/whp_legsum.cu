@@ -106,7 +106,7 @@ whp_legsum_kernel(const whp_tables T, const int32_t* __restrict__ perms, int64_t
 
 cudaError_t whp_launch_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                               cudaStream_t st) {
-  if (whp_fast_eligible(c) && getenv("WHP_FORCE_GENERAL") == nullptr)  // shapes the tuned path covers
+  if (whp_fast_eligible(c) && !c->dbg_force_general)  // shapes the tuned path covers
     return whp_launch_legsum_fast(c, d_perms, n_cand, d_len, st);
   const whp_tables T = whp_make_tables(c);
   int64_t blocks = (n_cand + kLegWarps - 1) / kLegWarps;

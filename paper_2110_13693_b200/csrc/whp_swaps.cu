@@ -859,9 +859,11 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
     need = 4 * (2 * (size_t)c->n_orders + 1);
     smem_tables = need + 12 * 1024 <= (size_t)c->smem_optin ? 1 : 0;
   }
+  // the attribute is per function and process-wide: always the same value (the most any call
+  // asks for), so contexts used from different host threads cannot undercut each other
   cudaError_t e = cudaFuncSetAttribute(whp_swaps_base_kernel,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       smem_tables ? (int)need : 0);
+                                       c->smem_optin - 12 * 1024);
   if (e != cudaSuccess) return e;
   whp_swaps_base_kernel<<<1, kBaseThreads, smem_tables ? need : 0, st>>>(T, d_base_perm, c->base,
                                                                         smem_tables);
@@ -874,7 +876,7 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
   // long: with 512 positions one window in five still had chains that left the region, and every
   // neighbour that lands on such a chain then scores tens of batches from their picks)
   int64_t margin = 64ll * c->C > 2048 ? 64ll * c->C : 2048;
-  if (const char* m = getenv("WHP_SWAP_MARGIN")) { const int v = atoi(m); if (v >= 0) margin = v; }  // tests: force the fallbacks
+  if (c->dbg_swap_margin >= 0) margin = c->dbg_swap_margin;  // WHP_DEBUG_SWAP_MARGIN: tests force the fallbacks
   const int32_t rlo = (int32_t)((int64_t)win_start - 2ll * c->C > 0 ? (int64_t)win_start - 2ll * c->C : 0);
   const int32_t rhi = (int32_t)((int64_t)win_start + win_len + margin < c->n_orders
                                     ? (int64_t)win_start + win_len + margin : c->n_orders);
@@ -903,7 +905,7 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
   if (chain_smem + 2048 <= (size_t)c->smem_optin) {
     if ((e = cudaFuncSetAttribute(whp_swaps_chain_kernel<true>,
                                   cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  (int)chain_smem)) != cudaSuccess) return e;
+                                  c->smem_optin - 2048)) != cudaSuccess) return e;
     whp_swaps_chain_kernel<true><<<chain_blocks, kChainWarps * 32, chain_smem, st>>>(T, c->base,
                                                                                       rlo, rhi);
   } else {

@@ -173,3 +173,44 @@ def algorithmic_bytes_per_candidate(n_orders: int, n_items: int) -> dict:
     return {"survey": 4 * n_orders + 8 * n_orders + 4 * n_items + 36,
             "packed": 4 * n_orders + 4 * n_orders + 4 * n_items + 36,
             "hbm_compulsory": 4 * n_orders + 36}
+
+
+# ---- ncu counters recorded for a given state of the kernels --------------------------------------
+def csrc_sha16(repo_root: str) -> str:
+    """Fingerprint of the kernel sources (csrc/*.cu, *.cuh + include/whp.h): counters captured
+    under ncu are only quoted next to a live timing when they were captured on these sources."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(repo_root, "paper_2110_13693_b200", "csrc")
+    files = sorted(os.path.join(csrc, f) for f in os.listdir(csrc) if f.endswith((".cu", ".cuh")))
+    files.append(os.path.join(repo_root, "include", "whp.h"))
+    for path in files:
+        with open(path, "rb") as f:
+            h.update(os.path.basename(path).encode() + b"\0" + f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_counters(repo_root: str) -> dict:
+    """profiles/ncu_counters.csv: rows `csrc_sha16,workload,counter,value,source` written by hand
+    from an `ncu --set full` capture (the .md named in `source` gives the command). Returns
+    {workload: {counter: value}} for the rows whose fingerprint matches the sources in the tree,
+    plus "stale": True when rows exist but none match."""
+    path = os.path.join(repo_root, "profiles", "ncu_counters.csv")
+    out, seen = {}, False
+    try:
+        sha = csrc_sha16(repo_root)
+        with open(path) as f:
+            for line in f:
+                parts = [x.strip() for x in line.split(",")]
+                if len(parts) < 5 or parts[0] in ("", "csrc_sha16") or parts[0].startswith("#"):
+                    continue
+                seen = True
+                if parts[0] != sha:
+                    continue
+                out.setdefault(parts[1], {})[parts[2]] = float(parts[3])
+                out[parts[1]]["source"] = parts[4]
+    except OSError:
+        pass
+    out["stale"] = bool(seen and len(out) == 0)
+    out["csrc_sha16"] = csrc_sha16(repo_root)
+    return out

@@ -24,7 +24,10 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_validate_perms", "whp_launch_count", "whp_destroy", "whp_last_error",
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
            "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move",
-           "whp_probe_l2_read", "whp_max_batches", "whp_set_swap_stats", "whp_get_swap_stats"]
+           "whp_probe_l2_read", "whp_max_batches", "whp_set_swap_stats", "whp_get_swap_stats",
+           "whp_debug_set"]
+
+DEBUG_FORCE_GENERAL, DEBUG_SEGMENTS, DEBUG_WARPS, DEBUG_SWAP_MARGIN = range(4)
 
 
 class WhpError(RuntimeError):
@@ -61,6 +64,7 @@ def lib():
         L.whp_apply_move.argtypes = [vp, vp, i32, i32, vp, vp]
         L.whp_probe_l2_read.argtypes = [vp, i64, i32, vp]
         L.whp_set_swap_stats.argtypes = [vp, i32]
+        L.whp_debug_set.argtypes = [vp, i32, i64]
         L.whp_get_swap_stats.argtypes = [vp, vp, vp, vp]
         L.whp_max_batches.argtypes = [vp]
         L.whp_max_batches.restype = i64
@@ -83,15 +87,37 @@ def _h(a, dtype):
     return a, a.ctypes.data
 
 
-def _d(t, dtype=None):
-    """device torch tensor -> raw pointer (None -> NULL)"""
+def _d(t, dtype=None, numel=None, device=None):
+    """device torch tensor -> raw pointer (None -> NULL). Checks what the C side cannot see:
+    contiguity, dtype, at least `numel` elements, and the context's device."""
     if t is None:
         return None
     if not t.is_cuda or not t.is_contiguous():
         raise ValueError("expected a contiguous CUDA tensor")
     if dtype is not None and t.dtype != dtype:
         raise ValueError(f"expected dtype {dtype}, got {t.dtype}")
+    if numel is not None and t.numel() < numel:
+        raise ValueError(f"tensor has {t.numel()} elements, the call writes / reads {numel}")
+    if device is not None and t.device.index != device:
+        raise ValueError(f"tensor lives on cuda:{t.device.index}, the context on cuda:{device}")
     return t.data_ptr()
+
+
+def _hostbuf(a, np_dtype, numel, name):
+    """host numpy array or CPU torch tensor -> raw pointer, after checking dtype / size /
+    contiguity (a mismatch would be silently misread by the C side)."""
+    if a is None:
+        return None
+    if hasattr(a, "data_ptr"):  # torch CPU tensor
+        import torch
+        want = {np.int32: torch.int32, np.int64: torch.int64, np.float64: torch.float64}[np_dtype]
+        if a.is_cuda or not a.is_contiguous() or a.dtype != want or a.numel() < numel:
+            raise ValueError(f"{name}: expected a contiguous CPU tensor of {want} with >= {numel} elements")
+        return a.data_ptr()
+    if not isinstance(a, np.ndarray) or a.dtype != np_dtype or not a.flags.c_contiguous or a.size < numel:
+        raise ValueError(f"{name}: expected a C-contiguous numpy array of {np.dtype(np_dtype)} "
+                         f"with >= {numel} elements")
+    return a.ctypes.data
 
 
 def _stream(stream):
@@ -158,80 +184,94 @@ class Context:
         n_cand = perms.shape[0] if perms.dim() == 2 else 1
         if perms.numel() != n_cand * self.n_orders:
             raise WhpError(ERR_INVALID_ARG, "perms shape")
+        dv, K, n = self.device, self.n_classes, self.n_orders
         self._check(lib().whp_eval_candidates(
-            self._h, _d(perms, torch.int32), n_cand, _d(dist, torch.int64),
-            _d(penalty, torch.float64), _d(obj, torch.float64), _d(n_batches, torch.int32),
-            _d(batch_hash, torch.int64), _d(batch_of_pos, torch.int32),
-            _d(n_distinct, torch.int32), _d(resp, torch.int32), _stream(stream)))
+            self._h, _d(perms, torch.int32, n_cand * n, dv), n_cand,
+            _d(dist, torch.int64, n_cand, dv), _d(penalty, torch.float64, n_cand, dv),
+            _d(obj, torch.float64, n_cand, dv), _d(n_batches, torch.int32, n_cand, dv),
+            _d(batch_hash, torch.int64, n_cand, dv), _d(batch_of_pos, torch.int32, n_cand * n, dv),
+            _d(n_distinct, torch.int32, n_cand, dv), _d(resp, torch.int32, n_cand * K, dv),
+            _stream(stream)))
 
     def eval_candidates_host(self, perms, dist=None, obj=None, want_argmin=True):
         """perms / dist / obj: host numpy arrays or CPU torch tensors (pinned = async copies).
         Returns (argmin_idx, argmin_val) when want_argmin."""
-        def hp(a):
-            if a is None:
-                return None
-            if hasattr(a, "data_ptr"):
-                return a.data_ptr()
-            return a.ctypes.data
         n_cand = perms.shape[0]
+        p_perms = _hostbuf(perms, np.int32, n_cand * self.n_orders, "perms")
+        if tuple(perms.shape) != (n_cand, self.n_orders):
+            raise WhpError(ERR_INVALID_ARG, "perms shape")
+        p_dist = _hostbuf(dist, np.int64, n_cand, "dist")
+        p_obj = _hostbuf(obj, np.float64, n_cand, "obj")
         idx, val = C.c_int64(-1), C.c_double(0.0)
         self._check(lib().whp_eval_candidates_host(
-            self._h, hp(perms), n_cand, hp(dist), hp(obj),
+            self._h, p_perms, n_cand, p_dist, p_obj,
             C.addressof(idx) if want_argmin else None,
             C.addressof(val) if want_argmin else None))
         return (idx.value, val.value) if want_argmin else None
 
     def eval_swaps(self, base_perm, win_start, win_len, dist=None, obj=None, stream=None):
         import torch
-        self._check(lib().whp_eval_swaps(self._h, _d(base_perm, torch.int32), win_start, win_len,
-                                         _d(dist, torch.int64), _d(obj, torch.float64),
-                                         _stream(stream)))
+        nn, dv = win_len * (win_len - 1) // 2, self.device
+        self._check(lib().whp_eval_swaps(self._h, _d(base_perm, torch.int32, self.n_orders, dv),
+                                         win_start, win_len, _d(dist, torch.int64, nn, dv),
+                                         _d(obj, torch.float64, nn, dv), _stream(stream)))
 
     def argmin(self, obj, idx, val=None, n=None, stream=None):
         import torch
-        self._check(lib().whp_argmin(self._h, _d(obj, torch.float64),
-                                     obj.numel() if n is None else n, _d(idx, torch.int64),
-                                     _d(val, torch.float64), _stream(stream)))
+        n = obj.numel() if n is None else n
+        dv = self.device
+        self._check(lib().whp_argmin(self._h, _d(obj, torch.float64, n, dv), n,
+                                     _d(idx, torch.int64, 1, dv), _d(val, torch.float64, 1, dv),
+                                     _stream(stream)))
 
     def apply_swap(self, base_perm, win_start, win_len, idx, stream=None):
         import torch
-        self._check(lib().whp_apply_swap(self._h, _d(base_perm, torch.int32), win_start, win_len,
-                                         _d(idx, torch.int64), _stream(stream)))
+        dv = self.device
+        self._check(lib().whp_apply_swap(self._h, _d(base_perm, torch.int32, self.n_orders, dv),
+                                         win_start, win_len, _d(idx, torch.int64, 1, dv),
+                                         _stream(stream)))
 
     def eval_moves(self, base_perm, win_start, win_len, dist=None, obj=None, stream=None):
         """NEXT-4 (reading N4): all W(W-1) insertion moves inside the window."""
         import torch
-        self._check(lib().whp_eval_moves(self._h, _d(base_perm, torch.int32), win_start, win_len,
-                                         _d(dist, torch.int64), _d(obj, torch.float64),
-                                         _stream(stream)))
+        nn, dv = win_len * (win_len - 1), self.device
+        self._check(lib().whp_eval_moves(self._h, _d(base_perm, torch.int32, self.n_orders, dv),
+                                         win_start, win_len, _d(dist, torch.int64, nn, dv),
+                                         _d(obj, torch.float64, nn, dv), _stream(stream)))
 
     def apply_move(self, base_perm, win_start, win_len, idx, stream=None):
         import torch
-        self._check(lib().whp_apply_move(self._h, _d(base_perm, torch.int32), win_start, win_len,
-                                         _d(idx, torch.int64), _stream(stream)))
+        dv = self.device
+        self._check(lib().whp_apply_move(self._h, _d(base_perm, torch.int32, self.n_orders, dv),
+                                         win_start, win_len, _d(idx, torch.int64, 1, dv),
+                                         _stream(stream)))
 
     def eval_legsum(self, perms, length, stream=None):
         """NEXT-2 (reading N2): summed leg lengths of every plan into `length` (CUDA int64)."""
         import torch
         n_cand = perms.shape[0] if perms.dim() == 2 else 1
-        self._check(lib().whp_eval_legsum(self._h, _d(perms, torch.int32), n_cand,
-                                          _d(length, torch.int64), _stream(stream)))
+        dv = self.device
+        self._check(lib().whp_eval_legsum(self._h, _d(perms, torch.int32, n_cand * self.n_orders, dv),
+                                          n_cand, _d(length, torch.int64, n_cand, dv),
+                                          _stream(stream)))
 
     def nhatc_update(self, resp_rows, idx=None, beta=1.0, stream=None):
         """NEXT-1 (reading N1): v <- v + 2 w^2 (t - r*), w <- beta w; r* = row idx[0] of resp_rows."""
         import torch
-        self._check(lib().whp_nhatc_update(self._h, _d(resp_rows, torch.int32),
-                                           _d(idx, torch.int64), float(beta), _stream(stream)))
+        dv = self.device
+        self._check(lib().whp_nhatc_update(self._h, _d(resp_rows, torch.int32, self.n_classes, dv),
+                                           _d(idx, torch.int64, 1, dv), float(beta), _stream(stream)))
 
     def nhatc_solve(self, perms, n_outer, beta, idx_hist=None, dist_hist=None, obj_hist=None,
                     stream=None):
         """n_outer x {eval_candidates -> argmin -> record -> nhatc_update}, all on the device."""
         import torch
         n_cand = perms.shape[0]
-        self._check(lib().whp_nhatc_solve(self._h, _d(perms, torch.int32), n_cand, int(n_outer),
-                                          float(beta), _d(idx_hist, torch.int64),
-                                          _d(dist_hist, torch.int64), _d(obj_hist, torch.float64),
-                                          _stream(stream)))
+        dv, no = self.device, int(n_outer)
+        self._check(lib().whp_nhatc_solve(self._h, _d(perms, torch.int32, n_cand * self.n_orders, dv),
+                                          n_cand, no, float(beta), _d(idx_hist, torch.int64, no, dv),
+                                          _d(dist_hist, torch.int64, no, dv),
+                                          _d(obj_hist, torch.float64, no, dv), _stream(stream)))
 
     def get_penalty(self, stream=None):
         t, v, w = (np.zeros(self.n_classes, np.float64) for _ in range(3))
@@ -242,7 +282,8 @@ class Context:
     def validate_perms(self, perms, stream=None) -> int:
         import torch
         n_bad = C.c_int64(0)
-        self._check(lib().whp_validate_perms(self._h, _d(perms, torch.int32), perms.shape[0],
+        self._check(lib().whp_validate_perms(self._h, _d(perms, torch.int32, perms.shape[0] * self.n_orders,
+                                                         self.device), perms.shape[0],
                                              C.addressof(n_bad), _stream(stream)))
         return n_bad.value
 
@@ -262,6 +303,11 @@ class Context:
         self._check(lib().whp_get_swap_stats(self._h, C.addressof(b), C.addressof(k),
                                              _stream(stream)))
         return b.value, k.value
+
+    def debug_set(self, key: int, value: int = -1):
+        """Kernel-selection switch for tests / measurements (whp.h: whp_debug_set); value < 0 =
+        default."""
+        self._check(lib().whp_debug_set(self._h, int(key), int(value)))
 
     def max_batches(self) -> int:
         return int(lib().whp_max_batches(self._h))

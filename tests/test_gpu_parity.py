@@ -26,10 +26,14 @@ def torch_cuda():
 
 class force_general:
     """Route non-detail calls through the general walker instead of the tuned K1/K2/K3 path."""
+    def __init__(self, ctx):
+        self.ctx = ctx
     def __enter__(self):
-        os.environ["WHP_FORCE_GENERAL"] = "1"
+        from paper_2110_13693_b200 import whp
+        self.ctx.debug_set(whp.DEBUG_FORCE_GENERAL, 1)
     def __exit__(self, *a):
-        os.environ.pop("WHP_FORCE_GENERAL", None)
+        from paper_2110_13693_b200 import whp
+        self.ctx.debug_set(whp.DEBUG_FORCE_GENERAL, -1)
 
 
 def gpu_eval(torch, ctx, perms_dev, detail=False):
@@ -92,7 +96,7 @@ def test_all_candidates_full_detail(torch_cuda, name):
     # the timed path (no detail outputs) must give the same numbers
     got2, dev2 = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=False)
     assert_parity(got2, ref, pb)
-    with force_general():
+    with force_general(ctx):
         got3, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=False)
     assert_parity(got3, ref, pb)
     # responses alone come from the tuned path's vertical counters
@@ -311,13 +315,13 @@ def test_edge_cases(torch_cuda, cfg):
     assert_parity(got, ref, pb, detail=True)
     got2, dev2 = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
     assert_parity(got2, ref, pb)
-    with force_general():
+    with force_general(ctx):
         got3, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
     assert_parity(got3, ref, pb)
     for seg in ("1", "2", "32"):  # segment counts of the tuned path (ignored when not legal)
-        os.environ["WHP_SEGMENTS"] = seg
+        ctx.debug_set(whp.DEBUG_SEGMENTS, int(seg))
         got4, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
-        os.environ.pop("WHP_SEGMENTS")
+        ctx.debug_set(whp.DEBUG_SEGMENTS, -1)
         assert_parity(got4, ref, pb)
     i, v = gpu_argmin(torch, ctx, dev2["obj"])
     assert i == oracle.argmin(ref["obj"])
@@ -429,7 +433,7 @@ def test_legsum_matches_oracle(torch_cuda, name, n_cand):
     ref = oracle.eval_legsum(pb, perms)
     assert np.array_equal(out.cpu().numpy(), ref)
     out.fill_(-1)
-    with force_general():  # the warp-per-plan kernel
+    with force_general(ctx):  # the warp-per-plan kernel
         ctx.eval_legsum(torch.from_numpy(perms).cuda(), out)
     torch.cuda.synchronize()
     assert np.array_equal(out.cpu().numpy(), ref)

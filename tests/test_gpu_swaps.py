@@ -136,11 +136,11 @@ def test_swaps_chains_that_leave_the_tabulated_region(torch_cuda, margin):
     ctx = whp.Context.from_problem(pb)
     base = W.base_perm(1, pb.n_orders)
     ref = oracle.eval_swaps(pb, base, 60, 36)
-    os.environ["WHP_SWAP_MARGIN"] = margin
+    ctx.debug_set(whp.DEBUG_SWAP_MARGIN, int(margin))
     try:
         d, o = gpu_swaps(torch, ctx, torch.from_numpy(base).cuda(), 60, 36)
     finally:
-        os.environ.pop("WHP_SWAP_MARGIN")
+        ctx.debug_set(whp.DEBUG_SWAP_MARGIN, -1)
     assert np.array_equal(d.cpu().numpy(), ref["dist"])
     assert np.array_equal(o.cpu().numpy(), ref["obj"])
     ctx.close()
@@ -163,7 +163,7 @@ def test_swaps_on_long_plans(torch_cuda, n_orders, s, Wn, margin):
     ref = oracle.eval_swaps(pb, base, s, Wn)
     ref_m = oracle.eval_moves(pb, base, s, 10)
     if margin is not None:
-        os.environ["WHP_SWAP_MARGIN"] = margin
+        ctx.debug_set(whp.DEBUG_SWAP_MARGIN, int(margin))
     try:
         bd = torch.from_numpy(base).cuda()
         d, o = gpu_swaps(torch, ctx, bd, s, Wn)
@@ -172,7 +172,7 @@ def test_swaps_on_long_plans(torch_cuda, n_orders, s, Wn, margin):
         ctx.eval_moves(bd, s, 10, md, mo)
         torch.cuda.synchronize()
     finally:
-        os.environ.pop("WHP_SWAP_MARGIN", None)
+        ctx.debug_set(whp.DEBUG_SWAP_MARGIN, -1)
     assert np.array_equal(d.cpu().numpy(), ref["dist"])
     assert np.array_equal(o.cpu().numpy(), ref["obj"])
     assert np.array_equal(md.cpu().numpy(), ref_m["dist"])
@@ -464,11 +464,11 @@ def test_moves_chains_that_leave_the_tabulated_region(torch_cuda, margin):
     ctx = whp.Context.from_problem(pb)
     base = W.base_perm(4, pb.n_orders)
     ref = oracle.eval_moves(pb, base, 200, 24)
-    os.environ["WHP_SWAP_MARGIN"] = margin
+    ctx.debug_set(whp.DEBUG_SWAP_MARGIN, int(margin))
     try:
         d, o = gpu_moves(torch, ctx, torch.from_numpy(base).cuda(), 200, 24)
     finally:
-        os.environ.pop("WHP_SWAP_MARGIN")
+        ctx.debug_set(whp.DEBUG_SWAP_MARGIN, -1)
     assert np.array_equal(d.cpu().numpy(), ref["dist"]) and np.array_equal(o.cpu().numpy(), ref["obj"])
     ctx.close()
 
@@ -584,4 +584,97 @@ def test_neighbour_index_decode_at_row_boundaries_of_a_4000_wide_window(torch_cu
     sel = torch.from_numpy(idx).cuda()
     assert np.array_equal(d[sel].cpu().numpy(), ref["dist"])
     assert np.array_equal(o[sel].cpu().numpy(), ref["obj"])
+    ctx.close()
+
+
+def test_nhatc_solve_replayed_from_a_cuda_graph(torch_cuda):
+    """"the loop captured in a CUDA graph". After one eager call (which
+    sizes the response scratch) whp_nhatc_solve neither allocates nor synchronises, so the whole
+    outer loop — walk, argmin, record, multiplier update, n_outer times — is captured once and
+    replayed; every replay restarts from the same multipliers and must reproduce the oracle's
+    loop (reading N1) bit for bit."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid")
+    n_cand, n_outer, beta = 384, 4, 1.25
+    perms_np = W.perms(3, pb.n_orders, n_cand)
+    ref = oracle.nhatc_loop(pb, perms_np, n_outer, beta)
+    ctx = whp.Context.from_problem(pb)
+    perms = torch.from_numpy(perms_np).cuda()
+    idx = torch.zeros(n_outer, dtype=torch.int64, device="cuda")
+    dist = torch.zeros(n_outer, dtype=torch.int64, device="cuda")
+    obj = torch.zeros(n_outer, dtype=torch.float64, device="cuda")
+    ctx.nhatc_solve(perms, n_outer, beta, idx, dist, obj)  # eager: sizes the scratch
+    torch.cuda.synchronize()
+    ctx.set_penalty(pb.t, pb.v, pb.w)
+    # the multipliers live in the context: a device-side snapshot restores them before a replay
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=torch.cuda.Stream()):
+        ctx.nhatc_solve(perms, n_outer, beta, idx, dist, obj)
+    for _ in range(2):
+        ctx.set_penalty(pb.t, pb.v, pb.w)
+        idx.fill_(-1), dist.zero_(), obj.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert np.array_equal(idx.cpu().numpy(), ref["idx"])
+        assert np.array_equal(dist.cpu().numpy(), ref["dist"])
+        assert np.array_equal(obj.cpu().numpy(), ref["obj"])
+        t, v, w = ctx.get_penalty()
+        assert np.array_equal(v, ref["v"]) and np.array_equal(w, ref["w"])
+    del g
+    ctx.close()
+
+
+def test_apply_swap_ignores_indices_that_are_no_neighbour(torch_cuda):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("tiny")
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(0, pb.n_orders)
+    Wn, s = 6, 9
+    for bad in (-1, -3, -(1 << 40), Wn * (Wn - 1) // 2, 1 << 40):
+        perm = torch.from_numpy(base.copy()).cuda()
+        ctx.apply_swap(perm, s, Wn, torch.tensor([bad], dtype=torch.int64, device="cuda"))
+        ctx.apply_move(perm, s, Wn, torch.tensor([bad if bad < 0 else max(bad, Wn * (Wn - 1))],
+                                                 dtype=torch.int64, device="cuda"))
+        torch.cuda.synchronize()
+        assert np.array_equal(perm.cpu().numpy(), base), bad
+    perm = torch.from_numpy(base.copy()).cuda()
+    last = Wn * (Wn - 1) // 2 - 1  # (i', j') = (W-2, W-1)
+    ctx.apply_swap(perm, s, Wn, torch.tensor([last], dtype=torch.int64, device="cuda"))
+    torch.cuda.synchronize()
+    want = base.copy()
+    want[s + Wn - 2], want[s + Wn - 1] = want[s + Wn - 1], want[s + Wn - 2]
+    assert np.array_equal(perm.cpu().numpy(), want)
+    ctx.close()
+
+
+def test_binding_rejects_short_or_foreign_buffers(torch_cuda):
+    """The C side cannot see a tensor's size: the binding checks it before the call."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("tiny")
+    ctx = whp.Context.from_problem(pb)
+    perms = torch.from_numpy(W.perms(0, pb.n_orders, 8)).cuda()
+    with pytest.raises(ValueError):
+        ctx.eval_candidates(perms, dist=torch.zeros(7, dtype=torch.int64, device="cuda"))
+    with pytest.raises(ValueError):
+        ctx.eval_candidates(perms, resp=torch.zeros(8 * pb.n_classes - 1, dtype=torch.int32, device="cuda"))
+    with pytest.raises(ValueError):
+        ctx.eval_swaps(perms[0], 0, 6, obj=torch.zeros(14, dtype=torch.float64, device="cuda"))
+    with pytest.raises(ValueError):
+        ctx.eval_moves(perms[0], 0, 6, obj=torch.zeros(29, dtype=torch.float64, device="cuda"))
+    with pytest.raises(ValueError):
+        ctx.argmin(torch.zeros(4, dtype=torch.float64, device="cuda"), torch.zeros(1, dtype=torch.int32, device="cuda"))
+    with pytest.raises(ValueError):  # int64 host plans would be misread as int32
+        ctx.eval_candidates_host(W.perms(0, pb.n_orders, 8).astype(np.int64))
+    with pytest.raises(ValueError):
+        ctx.eval_candidates_host(W.perms(0, pb.n_orders, 8), dist=np.zeros(7, np.int64))
+    with pytest.raises(whp.WhpError):
+        ctx.debug_set(99, 1)
+    h = np.ascontiguousarray(W.perms(0, pb.n_orders, 8))
+    d, o = np.zeros(8, np.int64), np.zeros(8, np.float64)
+    i, v = ctx.eval_candidates_host(h, d, o)
+    ref = oracle.eval_candidates(pb, h)
+    assert np.array_equal(d, ref["dist"]) and np.array_equal(o, ref["obj"]) and i == oracle.argmin(ref["obj"])
     ctx.close()

@@ -554,3 +554,65 @@ def test_moves_equal_materialised_sequences_and_adjacent_moves_are_swaps(golden)
     e6 = next(p for p in golden["plans"] if p["id"] == "E6")
     m = oracle.eval_moves(gp, np.arange(6, dtype=np.int32), 0, 6)
     assert m["dist"][1 * 5 + 1] == e6["dist"] and m["obj"][1 * 5 + 1] == e6["obj"]
+
+
+# ---------- host wrappers and memory safety of the checker itself --------------------------------
+def test_threaded_wrappers_equal_the_single_thread_routines():
+    """`threads=` only spreads plans / neighbourhood rows over host threads (full-size GPU parity
+    tests use it); every value must be the one the single-threaded call gives."""
+    pb = W.make_problem("mid")
+    base = W.base_perm(0, pb.n_orders)
+    for s, Wn in ((11, 2), (11, 3), (0, 7), (460, 40), (5, 41)):
+        a = oracle.eval_swaps(pb, base, s, Wn)
+        b = oracle.eval_swaps(pb, base, s, Wn, threads=4)
+        assert np.array_equal(a["dist"], b["dist"]) and np.array_equal(a["obj"], b["obj"])
+    perms = W.perms(0, pb.n_orders, 333)
+    a = oracle.eval_candidates(pb, perms, detail=True)
+    b = oracle.eval_candidates(pb, perms, detail=True, threads=5)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+
+
+def test_oracle_runs_clean_under_address_and_undefined_sanitizers(tmp_path):
+    """the oracle under -fsanitize=address,undefined. A separate process (the
+    sanitizer runtime must be preloaded) drives every exported routine on tiny / mid inputs; any
+    report aborts it."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    so = str(tmp_path / "libwhp_oracle_san.so")
+    subprocess.check_call(["gcc", "-O1", "-g", "-std=c99", "-ffp-contract=off", "-fsanitize=address,undefined",
+                           "-fno-sanitize-recover=all", "-fno-omit-frame-pointer", "-shared", "-fPIC",
+                           "-o", so, os.path.join(root, "oracle", "whp_oracle.c")])
+    asan = subprocess.check_output(["gcc", "-print-file-name=libasan.so"], text=True).strip()
+    script = f"""
+import sys
+sys.path.insert(0, {root!r})
+import numpy as np
+import oracle.binding as B
+B.build = lambda force=False: {so!r}
+import oracle
+from paper_2110_13693_b200 import workloads as W
+for name, n_cand, s, Wn in (("tiny", 64, 3, 9), ("mid", 96, 450, 24)):
+    pb = W.make_problem(name)
+    perms = W.perms(0, pb.n_orders, n_cand)
+    out = oracle.eval_candidates(pb, perms, detail=True, threads=2)
+    oracle.argmin(out["obj"])
+    oracle.eval_candidate_batches(pb, perms[0])
+    oracle.eval_swaps(pb, perms[1], s, Wn, threads=2)
+    oracle.eval_moves(pb, perms[2], s, min(Wn, 12))
+    oracle.swap_trajectory(pb, perms[3], min(Wn, 10), 5, 3)
+    oracle.eval_legsum(pb, perms[:8])
+    oracle.nhatc_loop(pb, perms[:16], 2, 1.5)
+    oracle.kmeans_slotting(pb, pb.n_skus, pb.item_sku, 3, 1, 4)
+pb = W.make_problem("tiny")
+oracle.optimal_route(pb, pb.sku_loc[:8])
+oracle.batch_distance(pb, pb.sku_loc[:5])
+oracle.tour_length(pb, pb.sku_loc[:6])
+print("SANITIZED_OK")
+"""
+    env = dict(os.environ, LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0:abort_on_error=1",
+               UBSAN_OPTIONS="halt_on_error=1:print_stacktrace=1")
+    r = subprocess.run([sys.executable, "-c", script], env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "SANITIZED_OK" in r.stdout, r.stderr[-3000:]
