@@ -34,6 +34,7 @@ WORKLOAD = "paper"  # BASELINE.json configs[2] (the third listed): the config th
 CPU_SAMPLE = 8192   # candidates the oracle is timed on for cpu_baseline (~12 s on one core)
 REF_SAMPLE = 256    # candidates per step of --impl reference: 1/64 of the 16,384 of a step
 REF_WINDOW = 32     # and the 496 swaps of a 32-wide window: ~1/66 of the step's 32,640 neighbours
+LEGS = ("step", "sustained", "e2e", "next", "stress", "cpu")  # --legs; "step" is the contract line
 SUSTAIN_S = 2.5     # the `sustained` leg repeats the step for at least this long
 KERNEL_PASS = 32    # steps of the separate pass that times the candidate evaluation by events
 
@@ -96,6 +97,54 @@ def run_reference(args):
     return 0
 
 
+def stress_leg(torch, whp, dev, local_rank, peaks, counters):
+    """BASELINE.json configs[5] at its full 65,536 plans: one launch
+    of whp_eval_candidates over 5.24 GB of plans generated in HBM, timed by CUDA events."""
+    import oracle
+    wls = W.make_workload("stress")
+    pbs = wls.problem
+    ns, ncs = pbs.n_orders, wls.n_cand
+    ctx_s = whp.Context.from_problem(pbs, device=local_rank)
+    sperms = torch.empty((ncs, ns), dtype=torch.int32, device=dev)
+    for lo_s in range(0, ncs, 4096):
+        sperms[lo_s:lo_s + 4096] = W.perms_torch(wls.seed, ns, lo_s, lo_s + 4096, dev)
+    sd = torch.zeros(ncs, dtype=torch.int64, device=dev)
+    so = torch.zeros(ncs, dtype=torch.float64, device=dev)
+    sh = torch.zeros(ncs, dtype=torch.int64, device=dev)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(3):
+        ctx_s.eval_candidates(sperms, dist=sd, obj=so, batch_hash=sh)
+    torch.cuda.synchronize()
+    reps = 10
+    ev0.record()
+    for _ in range(reps):
+        ctx_s.eval_candidates(sperms, dist=sd, obj=so, batch_hash=sh)
+    ev1.record()
+    torch.cuda.synchronize()
+    st_ms = ev0.elapsed_time(ev1) / reps
+    sb = harness.algorithmic_bytes_per_candidate(ns, pbs.n_items)
+    st_ach = sb["survey"] * ncs / (st_ms * 1e-3) / 1e9
+    # spot check against the oracle (all 65,536 plans are compared in tests/test_gpu_fullsize.py)
+    rows_s = np.array([0, 1, 4097, ncs - 1])
+    ref_s = oracle.eval_candidates(pbs, sperms[torch.from_numpy(rows_s).to(dev)].cpu().numpy())
+    stress = {"workload": "stress (BASELINE.json configs[5th]): 20,000 orders, "
+                          f"{pbs.n_items} items, C=40, K=32, Zipf(1.2), {ncs} plans in one launch",
+              "ms": st_ms, "value": ncs / (st_ms * 1e-3), "unit": "candidate plans/s",
+              "picks_per_s": ncs * pbs.n_items / (st_ms * 1e-3),
+              "bytes_per_candidate": sb["survey"], "achieved": st_ach, "peak": peaks["hbm_gbs"],
+              "unit_achieved": "GB/s", "frac": st_ach / peaks["hbm_gbs"],
+              "frac_hbm_compulsory": sb["hbm_compulsory"] * ncs / (st_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+              "traffic": counters.get("stress", {}).get("dram_bytes"),
+              "reps": reps, "input_bytes": int(sperms.numel() * 4),
+              "sampled_rows_equal_oracle": bool(
+                  np.array_equal(ref_s["obj"], so.cpu().numpy()[rows_s])
+                  and np.array_equal(ref_s["dist"], sd.cpu().numpy()[rows_s]))}
+    ctx_s.close()
+    del sperms, sd, so, sh
+    torch.cuda.empty_cache()
+    return stress
+
+
 def run_ours(args):
     import torch
     if not torch.cuda.is_available():
@@ -105,6 +154,20 @@ def run_ours(args):
     rank, local_rank, world = harness.init_dist("nccl")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
+    legs = set(LEGS) if args.legs == "all" else set(args.legs.split(","))
+    if not legs <= set(LEGS):
+        raise SystemExit(f"--legs takes a comma list of {LEGS}")
+    if not args.sustain:
+        legs.discard("sustained")
+    if not args.stress:
+        legs.discard("stress")
+    if "step" not in legs:  # profiling runs: only the stress launch (no JSON contract line)
+        if rank == 0 and "stress" in legs:
+            print(json.dumps({"impl": "ours", "legs": sorted(legs),
+                              "stress": stress_leg(torch, whp, dev, local_rank,
+                                                   harness.measured_peaks(ROOT),
+                                                   harness.ncu_counters(ROOT))}))
+        return 0
 
     wl = W.make_workload(WORKLOAD)
     wl_nb = W.make_workload("neighbourhood")
@@ -244,7 +307,7 @@ def run_ours(args):
 
     # ---- sustained: the same step repeated for >= SUSTAIN_S seconds, clocks sampled throughout --
     sustained = None
-    if world == 1 and args.sustain:
+    if world == 1 and "sustained" in legs:
         n_sus = max(args.steps, int(SUSTAIN_S / (ms_per_step * 1e-3)) + 1)
         sampler = harness.ClockSampler(local_rank, args.clock_period_ms).start().wait_first()
         for _ in range(3):
@@ -266,117 +329,94 @@ def run_ours(args):
                      "vs_timed_region": ms_per_step / sus_ms, "clocks": sus_clocks}
 
     # ---- end to end through the host-buffer entry point (pinned host memory) ---------------
-    h_perms = torch.empty((n_cand, n), dtype=torch.int32).pin_memory()
-    h_perms.copy_(perms)
-    h_dist = torch.zeros(n_cand, dtype=torch.int64).pin_memory()
-    h_obj = torch.zeros(n_cand, dtype=torch.float64).pin_memory()
-    for _ in range(max(1, min(args.warmup, 2))):
-        ctx.eval_candidates_host(h_perms, h_dist, h_obj)
-    torch.cuda.synchronize()
-    harness.barrier(world)
-    e2e_steps = max(1, min(args.steps, 10))
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        e_idx, e_val = ctx.eval_candidates_host(h_perms, h_dist, h_obj)
-    torch.cuda.synchronize()
-    e2e_s = harness.max_over_ranks(time.perf_counter() - t0, world, dev)
-    harness.barrier(world)
-    e2e_value = n_cand * world * e2e_steps / e2e_s
-    torch.cuda.synchronize()
-    same = bool(np.array_equal(h_obj.numpy(), obj.cpu().numpy()) and e_idx == int(idx.item()))
+    e2e = None
+    if "e2e" in legs:
+        h_perms = torch.empty((n_cand, n), dtype=torch.int32).pin_memory()
+        h_perms.copy_(perms)
+        h_dist = torch.zeros(n_cand, dtype=torch.int64).pin_memory()
+        h_obj = torch.zeros(n_cand, dtype=torch.float64).pin_memory()
+        for _ in range(max(1, min(args.warmup, 2))):
+            ctx.eval_candidates_host(h_perms, h_dist, h_obj)
+        torch.cuda.synchronize()
+        harness.barrier(world)
+        e2e_steps = max(1, min(args.steps, 10))
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e_idx, e_val = ctx.eval_candidates_host(h_perms, h_dist, h_obj)
+        torch.cuda.synchronize()
+        e2e_s = harness.max_over_ranks(time.perf_counter() - t0, world, dev)
+        harness.barrier(world)
+        torch.cuda.synchronize()
+        e2e = {"value": n_cand * world * e2e_steps / e2e_s, "unit": "candidate plans/s",
+               "h2d_bytes_per_step": int(h_perms.numel() * 4),
+               "d2h_bytes_per_step": int(n_cand * 16 + 16),
+               "api": "whp_eval_candidates_host (pinned host buffers, chunked copy/compute overlap)",
+               "matches_device_path": bool(np.array_equal(h_obj.numpy(), obj.cpu().numpy())
+                                           and e_idx == int(idx.item()))}
+        del h_perms
 
-    # ---- NEXT-1: the NHATC outer loop around the solve, on the device (not part of the step) ---
-    n_outer = 5
-    idx_h = torch.zeros(n_outer, dtype=torch.int64, device=dev)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ctx.nhatc_solve(perms, 1, 1.25, idx_h)  # warm-up (allocates the response scratch)
-    torch.cuda.synchronize()
-    ev0.record()
-    ctx.nhatc_solve(perms, n_outer, 1.25, idx_h)
-    ev1.record()
-    torch.cuda.synchronize()
-    nhatc_ms = ev0.elapsed_time(ev1) / n_outer
-    ctx.set_penalty(pb.t, pb.v, pb.w)  # restore the multipliers
+    nexts, l2_gbs = {}, None
+    if "next" in legs:
+        # ---- NEXT-1: the NHATC outer loop around the solve, on the device (not part of the step)
+        n_outer = 5
+        idx_h = torch.zeros(n_outer, dtype=torch.int64, device=dev)
+        ctx.nhatc_solve(perms, 1, 1.25, idx_h)  # warm-up (allocates the response scratch)
+        torch.cuda.synchronize()
+        ev0.record()
+        ctx.nhatc_solve(perms, n_outer, 1.25, idx_h)
+        ev1.record()
+        torch.cuda.synchronize()
+        nhatc_ms = ev0.elapsed_time(ev1) / n_outer
+        ctx.set_penalty(pb.t, pb.v, pb.w)  # restore the multipliers
+        nexts["nhatc_outer_loop"] = {
+            "ms_per_outer_iteration": nhatc_ms, "n_outer": n_outer,
+            "what": "whp_nhatc_solve: 16,384 plans walked once (D, r), then per outer iteration "
+                    "penalty -> argmin -> multiplier update, device only; mean over the call"}
 
-    # ---- NEXT-2: leg sums of the same plans (not part of the step) -----------------------------
-    leg = torch.zeros(n_cand, dtype=torch.int64, device=dev)
-    ctx.eval_legsum(perms, leg)
-    torch.cuda.synchronize()
-    ev0.record()
-    ctx.eval_legsum(perms, leg)
-    ev1.record()
-    torch.cuda.synchronize()
-    legsum_ms = ev0.elapsed_time(ev1)
+        # ---- NEXT-2: leg sums of the same plans (not part of the step) -------------------------
+        leg = torch.zeros(n_cand, dtype=torch.int64, device=dev)
+        ctx.eval_legsum(perms, leg)
+        torch.cuda.synchronize()
+        ev0.record()
+        ctx.eval_legsum(perms, leg)
+        ev1.record()
+        torch.cuda.synchronize()
+        legsum_ms = ev0.elapsed_time(ev1)
+        nexts["legsum"] = {"ms": legsum_ms, "plans_per_s": n_cand / (legsum_ms * 1e-3),
+                           "what": "whp_eval_legsum on the same 16,384 plans (paper-literal Eq. 2)"}
 
-    # ---- NEXT-4: insertion-move neighbourhood of the trajectory plan (not part of the step) ---
-    mW = 128
-    mobj = torch.zeros(mW * (mW - 1), dtype=torch.float64, device=dev)
-    ctx.eval_moves(base, 0, mW, None, mobj)
-    torch.cuda.synchronize()
-    ev0.record()
-    ctx.eval_moves(base, 0, mW, None, mobj)
-    ev1.record()
-    torch.cuda.synchronize()
-    moves_ms = ev0.elapsed_time(ev1)
+        # ---- NEXT-4: insertion-move neighbourhood of the trajectory plan (not part of the step)
+        mW = 128
+        mobj = torch.zeros(mW * (mW - 1), dtype=torch.float64, device=dev)
+        ctx.eval_moves(base, 0, mW, None, mobj)
+        torch.cuda.synchronize()
+        ev0.record()
+        ctx.eval_moves(base, 0, mW, None, mobj)
+        ev1.record()
+        torch.cuda.synchronize()
+        moves_ms = ev0.elapsed_time(ev1)
+        nexts["moves"] = {"ms": moves_ms, "neighbours": mW * (mW - 1),
+                          "neighbours_per_s": mW * (mW - 1) / (moves_ms * 1e-3),
+                          "what": "whp_eval_moves, all insertion moves of a 128-wide window"}
 
-    # ---- picks actually rescored by one neighbourhood pass (untimed, counted)
-    ctx.set_swap_stats(True)
-    ctx.eval_swaps(base, 0, Wn, dist=sdist, obj=sobj)
-    sw_batches, sw_picks = ctx.get_swap_stats()
-    ctx.set_swap_stats(False)
+        # ---- picks actually rescored by one neighbourhood pass (untimed, counted)
+        ctx.set_swap_stats(True)
+        ctx.eval_swaps(base, 0, Wn, dist=sdist, obj=sobj)
+        sw_batches, sw_picks = ctx.get_swap_stats()
+        ctx.set_swap_stats(False)
+        nexts["rescored"] = {"rescored_batches_per_neighbour": sw_batches / nn,
+                             "rescored_picks_per_neighbour": sw_picks / nn,
+                             "rescored_picks_per_s": sw_picks / (s_ms * 1e-3)}
 
-    # ---- measured L2 read bandwidth (not in MEASURED_PEAKS.json): 200 read-only
-    # sweeps of a 32 MB buffer that stays resident in the 126 MB L2, one launch
-    l2_gbs = ctx.probe_l2_read(32 << 20, 200)
+        # ---- measured L2 read bandwidth (not in MEASURED_PEAKS.json): 200
+        # read-only sweeps of a 32 MB buffer that stays resident in the 126 MB L2, one launch
+        l2_gbs = ctx.probe_l2_read(32 << 20, 200)
 
     peaks = harness.measured_peaks(ROOT)
     counters = harness.ncu_counters(ROOT)
 
-    # ---- stress: BASELINE.json configs[5] at its full 65,536 plans --
-    stress = None
-    if world == 1 and args.stress:
-        wls = W.make_workload("stress")
-        pbs = wls.problem
-        ns, ncs = pbs.n_orders, wls.n_cand
-        ctx_s = whp.Context.from_problem(pbs, device=local_rank)
-        sperms = torch.empty((ncs, ns), dtype=torch.int32, device=dev)  # 5.24 GB, made in HBM
-        for lo_s in range(0, ncs, 4096):
-            sperms[lo_s:lo_s + 4096] = W.perms_torch(wls.seed, ns, lo_s, lo_s + 4096, dev)
-        sd = torch.zeros(ncs, dtype=torch.int64, device=dev)
-        so = torch.zeros(ncs, dtype=torch.float64, device=dev)
-        sh = torch.zeros(ncs, dtype=torch.int64, device=dev)
-        for _ in range(3):
-            ctx_s.eval_candidates(sperms, dist=sd, obj=so, batch_hash=sh)
-        torch.cuda.synchronize()
-        reps = 10
-        ev0.record()
-        for _ in range(reps):
-            ctx_s.eval_candidates(sperms, dist=sd, obj=so, batch_hash=sh)
-        ev1.record()
-        torch.cuda.synchronize()
-        st_ms = ev0.elapsed_time(ev1) / reps
-        sb = harness.algorithmic_bytes_per_candidate(ns, pbs.n_items)
-        st_ach = sb["survey"] * ncs / (st_ms * 1e-3) / 1e9
-        # spot check against the oracle (all 65,536 plans are compared in tests/test_gpu_fullsize.py)
-        stress = {"workload": "stress (BASELINE.json configs[5th]): 20,000 orders, "
-                              f"{pbs.n_items} items, C=40, K=32, Zipf(1.2), {ncs} plans in one launch",
-                  "ms": st_ms, "value": ncs / (st_ms * 1e-3), "unit": "candidate plans/s",
-                  "picks_per_s": ncs * pbs.n_items / (st_ms * 1e-3),
-                  "bytes_per_candidate": sb["survey"], "achieved": st_ach, "peak": peaks["hbm_gbs"],
-                  "frac": st_ach / peaks["hbm_gbs"],
-                  "frac_hbm_compulsory": sb["hbm_compulsory"] * ncs / (st_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                  "traffic": counters.get("stress", {}).get("dram_bytes"),
-                  "reps": reps, "input_bytes": int(sperms.numel() * 4)}
-        if rank == 0:
-            import oracle
-            rows_s = np.array([0, 1, 4097, ncs - 1])
-            ref_s = oracle.eval_candidates(pbs, sperms[torch.from_numpy(rows_s).to(dev)].cpu().numpy())
-            stress["sampled_rows_equal_oracle"] = bool(
-                np.array_equal(ref_s["obj"], so.cpu().numpy()[rows_s])
-                and np.array_equal(ref_s["dist"], sd.cpu().numpy()[rows_s]))
-        ctx_s.close()
-        del sperms, sd, so, sh
-        torch.cuda.empty_cache()
+    stress = stress_leg(torch, whp, dev, local_rank, peaks, counters) if (world == 1 and "stress" in legs) else None
 
     # ---- roofline of the dominant kernel (candidate evaluation) -----------------------------
     bytes_pc = harness.algorithmic_bytes_per_candidate(n, pb.n_items)
@@ -423,14 +463,15 @@ def run_ours(args):
         "kernel_share_of_step": k_ms_max / ms_per_step,
         "frac_packed_bytes": bytes_pc["packed"] * n_cand / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"],
         "frac_hbm_compulsory": bytes_pc["hbm_compulsory"] * n_cand / (k_ms_max * 1e-3) / 1e9 / peaks["hbm_gbs"],
-        "l2_read_gbs_measured": l2_gbs, "frac_of_l2_read_peak": achieved / l2_gbs,
+        "l2_read_gbs_measured": l2_gbs,
+        "frac_of_l2_read_peak": achieved / l2_gbs if l2_gbs else None,
     }
 
     if rank != 0:
         return 0
     # ---- CPU baseline: the oracle on a bounded sample, rank 0 at N=1 only -------------------
     cpu = None
-    if world == 1:
+    if world == 1 and "cpu" in legs:
         import oracle
         sample = W.perm_rows(wl.seed, n, np.arange(CPU_SAMPLE))
         t0 = time.perf_counter()
@@ -473,32 +514,22 @@ def run_ours(args):
                        streams=("candidate evaluation + argmin and neighbourhood pass + argmin + "
                                 "apply on two streams, one context each, joined every step")
                        if overlap else "one stream, the calls of a step back to back"),
-        "neighbourhood": {"ms_per_iteration_eval_swaps": s_ms,
-                          "ms_span_on_side_stream_in_step": s_span_ms,
-                          "neighbours_per_s": nn / (s_ms * 1e-3),
-                          "iterations_per_s": 1.0 / (s_ms * 1e-3),
-                          "rescored_batches_per_neighbour": sw_batches / nn,
-                          "rescored_picks_per_neighbour": sw_picks / nn,
-                          "rescored_picks_per_s": sw_picks / (s_ms * 1e-3)},
-        "nhatc_outer_loop": {"ms_per_outer_iteration": nhatc_ms,
-                             "n_outer": n_outer,
-                             "what": "whp_nhatc_solve: 16,384 plans walked once (D, r), then per "
-                                     "outer iteration penalty -> argmin -> multiplier update, "
-                                     "device only; mean over the call"},
-        "moves": {"ms": moves_ms, "neighbours": mW * (mW - 1),
-                  "neighbours_per_s": mW * (mW - 1) / (moves_ms * 1e-3),
-                  "what": "whp_eval_moves, all insertion moves of a 128-wide window"},
-        "legsum": {"ms": legsum_ms, "plans_per_s": n_cand / (legsum_ms * 1e-3),
-                   "what": "whp_eval_legsum on the same 16,384 plans (paper-literal Eq. 2)"},
+        "neighbourhood": dict({"ms_per_iteration_eval_swaps": s_ms,
+                               "ms_span_on_side_stream_in_step": s_span_ms,
+                               "neighbours_per_s": nn / (s_ms * 1e-3),
+                               "iterations_per_s": 1.0 / (s_ms * 1e-3)}, **nexts.pop("rescored", {})),
+        **nexts,
         "roofline": roofline,
         "sustained": sustained,
         "stress": stress,
         "cpu_baseline": cpu,
-        "e2e": {"value": e2e_value, "unit": "candidate plans/s",
-                "h2d_bytes_per_step": int(h_perms.numel() * 4),
-                "d2h_bytes_per_step": int(n_cand * 16 + 16),
-                "api": "whp_eval_candidates_host (pinned host buffers, chunked copy/compute overlap)",
-                "matches_device_path": same},
+        "e2e": e2e,
+        "legs": sorted(legs),
+        "notes": ["the --impl reference arm (the oracle) re-evaluates every swap neighbour from "
+                  "scratch while this arm rescans only the affected batches: the driver's "
+                  "ours/reference ratio mixes that algorithmic gain with the hardware's",
+                  "roofline.frac is SURVEY.md 8(d)'s nominal gathered bytes against the HBM copy "
+                  "peak; roofline.binding_resource gives the units that really bind the path"],
         "gpu_launches": int(launches),
         "clocks": clocks, "remeasured_for_clocks": remeasured,
     }
@@ -514,6 +545,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--overlap", type=int, default=1, choices=[0, 1],
                     help="1: candidate evaluation and neighbourhood pass of a step on two streams")
+    ap.add_argument("--legs", default="all",
+                    help="comma list of step,sustained,e2e,next,stress,cpu (default all; profiling "
+                         "runs use --legs step or --legs stress)")
     ap.add_argument("--sustain", type=int, default=1, choices=[0, 1],
                     help="1: also repeat the step for >= 2.5 s with the clocks sampled (N=1 only)")
     ap.add_argument("--stress", type=int, default=1, choices=[0, 1],

@@ -5,7 +5,12 @@ hot path). Only tests/, __graft_entry__.smoke() and bench.py's cp
 --impl reference legs may import this package; the product package never does.
 """
 from .binding import (  # noqa: F401
+    LARGEST_GAP,
+    RETURN,
+    S_SHAPE,
     argmin,
+    batch_largest_gap_distance,
+    batch_return_distance,
     batch_distance,
     build,
     decode_neighbour,
@@ -13,6 +18,7 @@ from .binding import (  # noqa: F401
     eval_candidates,
     eval_legsum,
     eval_moves,
+    eval_routing,
     eval_swaps,
     kmeans_slotting,
     nhatc_loop,

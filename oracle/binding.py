@@ -38,6 +38,8 @@ def _load():
         _lib.orc_penalty.restype = C.c_double
         _lib.orc_argmin.restype = C.c_int64
         _lib.orc_tour_length.restype = C.c_int64
+        _lib.orc_batch_return_distance.restype = C.c_int64
+        _lib.orc_batch_largest_gap_distance.restype = C.c_int64
     return _lib
 
 
@@ -272,5 +274,45 @@ def eval_moves(pb, base_perm, win_start: int, win_len: int) -> dict:
     args, keep = _common(pb)
     _load().orc_eval_moves(*args, _p(base_perm), C.c_int32(win_start), C.c_int32(win_len),
                            _p(out["dist"]), _p(out["obj"]))
+    del keep
+    return out
+
+
+S_SHAPE, RETURN, LARGEST_GAP = 0, 1, 2  # routing policies (D4, readings N5 and N6)
+
+
+def batch_return_distance(geom, locs) -> int:
+    """NEXT-2 (reading N5): return routing of one cart."""
+    locs = _i32(locs)
+    return int(_load().orc_batch_return_distance(C.byref(_geom(geom)), _p(locs), C.c_int32(len(locs))))
+
+
+def batch_largest_gap_distance(geom, locs) -> int:
+    """NEXT-2 (reading N6): largest-gap routing of one cart."""
+    locs = _i32(locs)
+    return int(_load().orc_batch_largest_gap_distance(C.byref(_geom(geom)), _p(locs),
+                                                      C.c_int32(len(locs))))
+
+
+def eval_routing(pb, perms, policy: int, threads: int = 1) -> dict:
+    """D and J = D + phi of every plan with the carts routed by `policy` (0 S-shape, 1 return,
+    2 largest gap); batching, responses and penalty as in eval_candidates."""
+    perms = _i32(perms)
+    if perms.ndim == 1:
+        perms = perms[None, :]
+    n_cand = perms.shape[0]
+    out = {"dist": np.zeros(n_cand, np.int64), "obj": np.zeros(n_cand, np.float64)}
+    args, keep = _common(pb)
+    lib = _load()
+
+    def run(lo, hi):
+        st = lib.orc_eval_routing(*args, C.c_int32(policy), _off(perms, lo), C.c_int64(hi - lo),
+                                  _off(out["dist"], lo), _off(out["obj"], lo))
+        if st != 0:
+            raise ValueError("eval_routing: unknown policy")
+    if threads <= 1:
+        run(0, n_cand)
+    else:
+        _pool_map(run, np.linspace(0, n_cand, min(n_cand, 8 * threads) + 1).astype(np.int64), threads)
     del keep
     return out

@@ -21,11 +21,14 @@
  * hand-worked step, special cases and exact rationals; leg sums N2 by hand-worked tours, the
  * one-pick closed form and min-over-orderings = exhaustive optimum; K-means slotting N3 by a
  * hand-worked example and nearest-centroid / SSE / exact-mean / contiguity invariants;
- * insertion moves N4 against independently materialised sequences, swaps and E6.
+ * insertion moves N4 against independently materialised sequences, swaps and E6; the return and
+ * largest-gap routing policies N5 / N6 by hand-worked batches, the one-aisle closed form,
+ * explicitly constructed tours (every pick on the tour, legs summed with an independent
+ * metric), the exhaustive optimum as a lower bound and a brute-force search over entry depths.
  * "Parity unpinned" BY THE PAPER (it prints no formula for them): the choice of r_k (Q9), the
  * geometry constants (Q2–Q3), the update rule N1, the tour convention N2, the K-means details
- * N3 and the move definition N4 — they are pinned only to DESIGN.md's readings and hand-worked
- * examples.
+ * N3, the move definition N4 and the routing policies N5 / N6 — they are pinned only to
+ * DESIGN.md's readings and hand-worked examples.
  */
 #include <stdint.h>
 #include <stdlib.h>
@@ -488,5 +491,131 @@ int32_t orc_eval_moves(const orc_geom* g, const int32_t* sku_loc, const int32_t*
       n++;
     }
   free(p);
+  return 0;
+}
+
+
+/* ---- NEXT-2, second half: return and largest-gap routing on the per-aisle depth table -----------
+ * PAPER.md:125-132 (§5 Eq. 2): subproblem 2 minimises the travelled distance of "a sequence of
+ * picking positions"; BASELINE.json north_star routes every cart with the S-shape heuristic (D4)
+ * and asks for "max-depth tables". SURVEY.md §8(f) NEXT-2 names two more routing policies over
+ * the same carts. DESIGN.md readings (the classical definitions of these heuristics in a
+ * two-cross-aisle layout; the paper prints none):
+ *   N5 return       the cart enters every visited aisle from the FRONT cross-aisle, walks to the
+ *                   aisle's deepest pick and comes back:  dist_b = H + 2 * sum_{a in V_b} maxdepth_a
+ *   N6 largest gap  one visited aisle: as N5. Otherwise the first (a_min) and last (a_max) visited
+ *                   aisles are traversed completely (out along the back cross-aisle, home along
+ *                   the front one) and every visited aisle in between is entered from the back
+ *                   and / or the front so that its LARGEST GAP — the largest of: front cross-aisle
+ *                   to the shallowest pick, between depth-adjacent picks, deepest pick to the back
+ *                   cross-aisle — is the stretch not walked:
+ *                     dist_b = H + 2A + 2 * sum_{a in V_b, a_min < a < a_max} (A - gap*_a)
+ * with H the horizontal term of D4 (depot -> a_min -> a_max -> depot along the cross-aisles) and
+ * A the aisle length. Both are lengths of real tours that visit every pick (pinned by building
+ * them). policy: 0 = S-shape (D4), 1 = return (N5), 2 = largest gap (N6). */
+static int64_t horizontal_term(const orc_geom* g, int32_t a_min, int32_t a_max) {
+  int64_t a0 = g->depot_aisle, P = g->aisle_spacing;
+  return P * (iabs64(a0 - a_min) + ((int64_t)a_max - a_min) + iabs64((int64_t)a_max - a0));
+}
+
+int64_t orc_batch_return_distance(const orc_geom* g, const int32_t* locs, int32_t n) {
+  if (n <= 0) return 0;
+  int32_t* aisles = (int32_t*)malloc(sizeof(int32_t) * (size_t)n);
+  for (int32_t i = 0; i < n; i++) aisles[i] = loc_aisle(g, locs[i]);
+  int32_t m = sort_unique(aisles, n); /* V_b */
+  int64_t deep = 0;
+  for (int32_t k = 0; k < m; k++) { /* the per-aisle max-depth table */
+    int64_t maxdepth = 0;
+    for (int32_t i = 0; i < n; i++)
+      if (loc_aisle(g, locs[i]) == aisles[k] && loc_depth(g, locs[i]) > maxdepth)
+        maxdepth = loc_depth(g, locs[i]);
+    deep += maxdepth;
+  }
+  int64_t H = horizontal_term(g, aisles[0], aisles[m - 1]);
+  free(aisles);
+  return H + 2 * deep;
+}
+
+/* largest gap of one aisle given the depths of its picks (repeats allowed, n >= 1) */
+static int64_t largest_gap(const orc_geom* g, int32_t* depths, int32_t n) {
+  int32_t k = sort_unique(depths, n);
+  int64_t best = depths[0];                      /* front cross-aisle (y = 0) to the first pick */
+  for (int32_t i = 1; i < k; i++)
+    if ((int64_t)depths[i] - depths[i - 1] > best) best = (int64_t)depths[i] - depths[i - 1];
+  if (aisle_len(g) - depths[k - 1] > best) best = aisle_len(g) - depths[k - 1]; /* to the back */
+  return best;
+}
+
+int64_t orc_batch_largest_gap_distance(const orc_geom* g, const int32_t* locs, int32_t n) {
+  if (n <= 0) return 0;
+  int32_t* aisles = (int32_t*)malloc(sizeof(int32_t) * (size_t)n);
+  int32_t* depths = (int32_t*)malloc(sizeof(int32_t) * (size_t)n);
+  for (int32_t i = 0; i < n; i++) aisles[i] = loc_aisle(g, locs[i]);
+  int32_t m = sort_unique(aisles, n);
+  int64_t H = horizontal_term(g, aisles[0], aisles[m - 1]);
+  int64_t A = aisle_len(g), Vt;
+  if (m == 1) {
+    int64_t maxdepth = 0;
+    for (int32_t i = 0; i < n; i++)
+      if (loc_depth(g, locs[i]) > maxdepth) maxdepth = loc_depth(g, locs[i]);
+    Vt = 2 * maxdepth;
+  } else {
+    Vt = 2 * A; /* first and last visited aisle, traversed completely */
+    for (int32_t k = 1; k + 1 < m; k++) {
+      int32_t nd = 0;
+      for (int32_t i = 0; i < n; i++)
+        if (loc_aisle(g, locs[i]) == aisles[k]) depths[nd++] = loc_depth(g, locs[i]);
+      Vt += 2 * (A - largest_gap(g, depths, nd));
+    }
+  }
+  free(aisles); free(depths);
+  return H + Vt;
+}
+
+/* D1, D2, D5, D6 as in orc_eval_candidate, the cart length by `policy`. perms[n_cand][n_orders];
+ * dist, obj nullable. Returns 1 on an unknown policy. */
+int32_t orc_eval_routing(const orc_geom* g, const int32_t* sku_loc, const int32_t* sku_class,
+                         int32_t K, int32_t n_orders, const int32_t* order_ptr,
+                         const int32_t* item_sku, int32_t C, const double* t, const double* v,
+                         const double* w, int32_t policy, const int32_t* perms, int64_t n_cand,
+                         int64_t* dist, double* obj) {
+  if (policy < 0 || policy > 2) return 1;
+  int32_t n_items = order_ptr[n_orders];
+  int32_t* locs = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n_items > 0 ? n_items : 1));
+  int32_t* cls = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n_items > 0 ? n_items : 1));
+  int32_t* r = (int32_t*)malloc(sizeof(int32_t) * (size_t)K);
+  for (int64_t c = 0; c < n_cand; c++) {
+    const int32_t* perm = perms + c * n_orders;
+    for (int32_t k = 0; k < K; k++) r[k] = 0;
+    int64_t D = 0;
+    int32_t load = 0, n = 0;
+    for (int32_t pos = 0; pos <= n_orders; pos++) {
+      int32_t q = 0;
+      if (pos < n_orders) q = order_ptr[perm[pos] + 1] - order_ptr[perm[pos]];
+      if (pos == n_orders || (load > 0 && load + q > C)) { /* D2: the cart is closed */
+        if (n > 0) {
+          D += policy == 0 ? orc_batch_distance(g, locs, n)
+             : policy == 1 ? orc_batch_return_distance(g, locs, n)
+                           : orc_batch_largest_gap_distance(g, locs, n);
+          int32_t kc = sort_unique(cls, n); /* K_b */
+          for (int32_t i = 0; i < kc; i++) r[cls[i]] += 1; /* D5 */
+        }
+        load = 0; n = 0;
+      }
+      if (pos < n_orders) {
+        int32_t o = perm[pos];
+        for (int32_t it = order_ptr[o]; it < order_ptr[o + 1]; it++) {
+          locs[n] = sku_loc[item_sku[it]];
+          cls[n] = sku_class[item_sku[it]];
+          n++;
+        }
+        load += q;
+      }
+    }
+    double phi = orc_penalty(K, r, t, v, w); /* D6 */
+    if (dist) dist[c] = D;
+    if (obj) obj[c] = (double)D + phi;
+  }
+  free(locs); free(cls); free(r);
   return 0;
 }

@@ -605,14 +605,172 @@ for name, n_cand, s, Wn in (("tiny", 64, 3, 9), ("mid", 96, 450, 24)):
     oracle.swap_trajectory(pb, perms[3], min(Wn, 10), 5, 3)
     oracle.eval_legsum(pb, perms[:8])
     oracle.nhatc_loop(pb, perms[:16], 2, 1.5)
+    for pol in (0, 1, 2):
+        oracle.eval_routing(pb, perms[:8], pol, threads=2)
     oracle.kmeans_slotting(pb, pb.n_skus, pb.item_sku, 3, 1, 4)
 pb = W.make_problem("tiny")
 oracle.optimal_route(pb, pb.sku_loc[:8])
 oracle.batch_distance(pb, pb.sku_loc[:5])
 oracle.tour_length(pb, pb.sku_loc[:6])
+oracle.batch_return_distance(pb, pb.sku_loc[:9])
+oracle.batch_largest_gap_distance(pb, pb.sku_loc[:9])
 print("SANITIZED_OK")
 """
     env = dict(os.environ, LD_PRELOAD=asan, ASAN_OPTIONS="detect_leaks=0:abort_on_error=1",
                UBSAN_OPTIONS="halt_on_error=1:print_stacktrace=1")
     r = subprocess.run([sys.executable, "-c", script], env=env, capture_output=True, text=True, timeout=600)
     assert r.returncode == 0 and "SANITIZED_OK" in r.stdout, r.stderr[-3000:]
+
+
+# ---------- NEXT-2, second half: return and largest-gap routing (readings N5, N6) ------------------
+def _aisle_table(geom, locs):
+    """{aisle: sorted distinct depths} — the per-aisle depth table, with python sets."""
+    tab = {}
+    for l in locs:
+        a, y = _point(geom, l)
+        tab.setdefault(a, set()).add(y)
+    return {a: sorted(ys) for a, ys in tab.items()}
+
+
+def _tour_len_and_cover(geom, way, locs):
+    """Length of the closed walk through the waypoints under the independent D0 metric, and
+    whether every pick lies on one of its in-aisle segments."""
+    total = sum(_walk(geom, way[i], way[i + 1]) for i in range(len(way) - 1))
+    covered = set()
+    for (a1, y1), (a2, y2) in zip(way[:-1], way[1:]):
+        if a1 == a2:
+            for l in locs:
+                a, y = _point(geom, l)
+                if a == a1 and min(y1, y2) <= y <= max(y1, y2):
+                    covered.add(l)
+    return total, covered == set(locs)
+
+
+def _return_tour(geom, locs):
+    NA, S, p, P, a0 = geom
+    tab = _aisle_table(geom, locs)
+    way = [(a0, 0)]
+    # depot -> leftmost visited aisle -> sweep to the rightmost -> depot, all along the front
+    for a in sorted(tab):
+        way += [(a, 0), (a, tab[a][-1]), (a, 0)]
+    way.append((a0, 0))
+    return way
+
+
+def _largest_gap_tour(geom, locs):
+    NA, S, p, P, a0 = geom
+    A = (S + 1) * p
+    tab = _aisle_table(geom, locs)
+    aisles = sorted(tab)
+    if len(aisles) == 1:
+        a = aisles[0]
+        return [(a0, 0), (a, 0), (a, tab[a][-1]), (a, 0), (a0, 0)]
+    first, last, mid = aisles[0], aisles[-1], aisles[1:-1]
+    cut = {}
+    for a in mid:  # (front reach, back reach) around the largest gap; ties -> first
+        ys = [0] + tab[a] + [A]
+        k = max(range(len(ys) - 1), key=lambda i: (ys[i + 1] - ys[i], -i))
+        cut[a] = (ys[k], ys[k + 1])
+    def front_entry(a):
+        return [(a, 0), (a, cut[a][0]), (a, 0)] if cut[a][0] > 0 else []
+    way = [(a0, 0)]
+    for a in reversed([x for x in mid if x <= a0]):  # on the way out along the front cross-aisle
+        way += front_entry(a)
+    way += [(first, 0), (first, A)]
+    for a in mid:  # along the back cross-aisle
+        if cut[a][1] < A:
+            way += [(a, A), (a, cut[a][1]), (a, A)]
+    way += [(last, A), (last, 0)]
+    for a in reversed([x for x in mid if x > a0]):  # home along the front cross-aisle
+        way += front_entry(a)
+    way.append((a0, 0))
+    return way
+
+
+def test_routing_golden(golden):
+    geom = TINY
+    r = golden["routing"]
+    for ex in r["batches"]:
+        assert oracle.batch_return_distance(geom, ex["locs"]) == ex["return"], ex["id"]
+        assert oracle.batch_largest_gap_distance(geom, ex["locs"]) == ex["largest_gap"], ex["id"]
+    pb = _golden_problem(golden)
+    perm = np.array([p for p in golden["plans"] if p["id"] == r["plan"]][0]["perm"], np.int32)
+    ret = oracle.eval_routing(pb, perm, oracle.RETURN)
+    lg = oracle.eval_routing(pb, perm, oracle.LARGEST_GAP)
+    assert int(ret["dist"][0]) == r["return_total"] and float(ret["obj"][0]) == r["return_obj"]
+    assert int(lg["dist"][0]) == r["largest_gap_total"] and float(lg["obj"][0]) == r["largest_gap_obj"]
+
+
+@pytest.mark.parametrize("geom", [TINY, (7, 9, 2, 5, 3), (20, 50, 1, 3, 0), (12, 30, 3, 4, 11)])
+def test_routing_equals_explicit_tours_that_visit_every_pick(geom):
+    """N5 / N6 are lengths of real walks: build each tour waypoint by waypoint, check that every
+    pick lies on it, and add its legs with the test's own D0 metric."""
+    NA, S, p, P, a0 = geom
+    rng = np.random.default_rng(hash(geom) % (1 << 31))
+    for trial in range(150):
+        n = int(rng.integers(1, 13))
+        locs = rng.integers(0, 2 * NA * S, n).tolist()
+        if trial % 5 == 0:  # few aisles, many picks per aisle
+            aisles = rng.integers(0, NA, 2)
+            locs = [int(a) * 2 * S + int(x) for a, x in zip(rng.choice(aisles, n), rng.integers(0, 2 * S, n))]
+        for tour, fn in ((_return_tour, oracle.batch_return_distance),
+                         (_largest_gap_tour, oracle.batch_largest_gap_distance)):
+            length, covered = _tour_len_and_cover(geom, tour(geom, locs), locs)
+            assert covered, (geom, locs, tour.__name__)
+            assert fn(geom, locs) == length, (geom, locs, tour.__name__)
+
+
+def test_routing_closed_forms_bounds_and_invariances():
+    rng = np.random.default_rng(5)
+    for geom in (TINY, (6, 8, 2, 5, 2)):
+        NA, S, p, P, a0 = geom
+        A = (S + 1) * p
+        for loc in range(2 * NA * S):  # one pick: the m = 1 closed form of north_star (P1)
+            a, y = _point(geom, loc)
+            assert oracle.batch_return_distance(geom, [loc]) == 2 * abs(a - a0) * P + 2 * y
+            assert oracle.batch_largest_gap_distance(geom, [loc]) == 2 * abs(a - a0) * P + 2 * y
+        for _ in range(200):
+            locs = rng.integers(0, 2 * NA * S, int(rng.integers(1, 8))).tolist()
+            ret, lg = oracle.batch_return_distance(geom, locs), oracle.batch_largest_gap_distance(geom, locs)
+            opt = _brute_route(geom, locs)
+            assert ret >= opt and lg >= opt  # both are tours: never below the exhaustive optimum
+            # invariant to order, repeats and the side of the aisle (P4)
+            shuffled = list(rng.permutation(locs + locs[:2]))
+            flipped = [l + S if (l % (2 * S)) < S else l - S for l in locs]
+            for other in (shuffled, flipped):
+                assert oracle.batch_return_distance(geom, other) == ret
+                assert oracle.batch_largest_gap_distance(geom, other) == lg
+            # the table the policies read: return = H + 2 * sum of the per-aisle maxima
+            tab = _aisle_table(geom, locs)
+            H = P * (abs(a0 - min(tab)) + (max(tab) - min(tab)) + abs(max(tab) - a0))
+            assert ret == H + 2 * sum(ys[-1] for ys in tab.values())
+            # largest gap of an aisle = the best way to reach all its picks by one walk in from
+            # the front and one in from the back: brute force over where the two walks stop
+            if len(tab) >= 3:
+                want = H + 2 * A
+                for a in sorted(tab)[1:-1]:
+                    ys = tab[a]
+                    want += min(2 * f + 2 * (A - b) for f, b in zip([0] + ys, ys + [A]))
+                assert lg == want
+
+
+def test_routing_evaluator_shares_batching_and_penalty_with_the_s_shape_path():
+    """Policy 0 of eval_routing is D4: it must reproduce eval_candidates (which pins the new
+    function's batching, responses and penalty); the other policies differ only in the cart
+    lengths, recomputed here per cart from python-side batching."""
+    for name in ("tiny", "mid"):
+        pb = W.make_problem(name)
+        perms = W.perms(1, pb.n_orders, 24)
+        ref = oracle.eval_candidates(pb, perms)
+        s0 = oracle.eval_routing(pb, perms, oracle.S_SHAPE, threads=3)
+        assert np.array_equal(s0["dist"], ref["dist"]) and np.array_equal(s0["obj"], ref["obj"])
+        for pol, fn in ((oracle.RETURN, oracle.batch_return_distance),
+                        (oracle.LARGEST_GAP, oracle.batch_largest_gap_distance)):
+            out = oracle.eval_routing(pb, perms, pol)
+            for c in range(6):
+                bop, batches, r = _py_plan(pb, perms[c])
+                D = sum(fn(pb, b) for b in batches)
+                assert out["dist"][c] == D
+                assert out["obj"][c] == float(D) + ref["penalty"][c]
+    with pytest.raises(ValueError):
+        oracle.eval_routing(W.make_problem("tiny"), W.perms(1, 20, 2), 3)
