@@ -163,6 +163,29 @@ whp_status whp_get_penalty(whp_ctx* ctx, double* t, double* v, double* w, void* 
 whp_status whp_eval_legsum(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                            void* cuda_stream);
 
+/* Routing policies of a cart: the S-shape of D4 (BASELINE.json north_star), and the
+ * two further heuristics SURVEY.md §8(f) NEXT-2 names, as read in N5 / N6:
+ *   WHP_ROUTE_RETURN       enter every visited aisle from the front cross-aisle, walk to its
+ *                          deepest pick and come back: H + 2 * sum over visited aisles of maxdepth
+ *   WHP_ROUTE_LARGEST_GAP  one visited aisle: as return; else traverse the first and the last
+ *                          visited aisle and enter every aisle in between from the back and / or
+ *                          the front so that its largest gap is not walked:
+ *                          H + 2A + 2 * sum over inner visited aisles of (A - largest gap)
+ * (H = horizontal term of D4, A = aisle length). */
+typedef enum {
+  WHP_ROUTE_S_SHAPE = 0,
+  WHP_ROUTE_RETURN = 1,
+  WHP_ROUTE_LARGEST_GAP = 2
+} whp_route_policy;
+
+/* D and J = (double)D + phi of every plan with its carts routed by `policy`; batching (D2),
+ * responses (D5) and penalty (D6) as in whp_eval_candidates, of which policy 0 is a synonym.
+ * d_perms DEVICE int32 [n_cand][n_orders]; d_dist int64 / d_obj double DEVICE [n_cand], nullable.
+ * Policies 1 and 2 keep the cart's (aisle, depth) list in shared memory and need
+ * cart_capacity <= 1024 (WHP_ERR_OUT_OF_RANGE beyond); an unknown policy is WHP_ERR_INVALID_ARG. */
+whp_status whp_eval_routing(whp_ctx* ctx, const int32_t* d_perms, int64_t n_cand, int32_t policy,
+                            int64_t* d_dist, double* d_obj, void* cuda_stream);
+
 /* ---- NEXT-3: subproblem 3 (§5: product placement by picking frequency, "e.g.
  * K-means clustering"; reading N3 of DESIGN.md) ------------------------------------------- */
 

@@ -446,6 +446,27 @@ whp_status whp_eval_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, i
   return WHP_OK;
 }
 
+whp_status whp_eval_routing(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int32_t policy,
+                            int64_t* d_dist, double* d_obj, void* cuda_stream) {
+  nvtx_range nvtx_("whp_eval_routing");
+  whp_status s = ready(c);
+  if (s != WHP_OK) return s;
+  if (n_cand < 0) return fail(c, WHP_ERR_INVALID_ARG, "n_cand < 0");
+  if (policy < WHP_ROUTE_S_SHAPE || policy > WHP_ROUTE_LARGEST_GAP)
+    return fail(c, WHP_ERR_INVALID_ARG, "unknown routing policy");
+  if (n_cand == 0) return WHP_OK;
+  if (!d_perms) return fail(c, WHP_ERR_INVALID_ARG, "d_perms is null");
+  device_guard dg(c->device);
+  if (policy == WHP_ROUTE_S_SHAPE) {
+    whp_eval_out out{d_dist, nullptr, d_obj, nullptr, nullptr, nullptr, nullptr, nullptr};
+    WHP_CUDA(c, whp_launch_eval(c, d_perms, n_cand, out, (cudaStream_t)cuda_stream));
+    return WHP_OK;
+  }
+  if (c->C > 1024) return fail(c, WHP_ERR_OUT_OF_RANGE, "return / largest-gap routing needs cart_capacity <= 1024");
+  WHP_CUDA(c, whp_launch_route(c, d_perms, n_cand, policy, d_dist, d_obj, (cudaStream_t)cuda_stream));
+  return WHP_OK;
+}
+
 whp_status whp_nhatc_update(whp_ctx* c, const int32_t* d_resp_rows, const int64_t* d_idx,
                             double beta, void* cuda_stream) {
   nvtx_range nvtx_("whp_nhatc_update");

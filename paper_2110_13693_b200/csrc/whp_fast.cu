@@ -439,6 +439,15 @@ __device__ __forceinline__ void step_cursor(uint32_t rec, uint32_t& cur, uint32_
       : "r"(rec), "r"(v_end), "r"(pb), "r"(ringbase), "r"(ring_mask));
 }
 
+// if (p) {a, b} = the aligned record pair at ptr (ld.global.nc.v2) — predicated, never a branch.
+// Pick tables that do not fit shared memory are gathered through L1 / L2, where a warp-wide
+// gather costs one tag look-up per lane (the L1TEX unit is what saturates: 91 % at stress scale):
+// every order starts at an even index, so one 8-byte load serves two consecutive steps.
+__device__ __forceinline__ void ldg_pair_if(uint32_t& a, uint32_t& b, const uint32_t* ptr, bool p) {
+  asm volatile("{ .reg .pred pq; setp.ne.u32 pq, %3, 0; @pq ld.global.nc.v2.u32 {%0, %1}, [%2]; }"
+               : "+r"(a), "+r"(b) : "l"(ptr), "r"((uint32_t)p));
+}
+
 // if (p) v = ld.shared.u16 [a] — predicated, never a branch; idle lanes cost no bank cycle
 __device__ __forceinline__ void lds16_if(uint32_t& v, uint32_t a, bool p) {
   asm volatile("{ .reg .pred pq; setp.ne.u32 pq, %2, 0; @pq ld.shared.u16 %0, [%1]; }"
@@ -563,7 +572,9 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         cur = SMEM_TABLES ? pb : 0u;
       }
       uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));
-      uint32_t rec = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
+      uint32_t pair_lo = 0, pair_hi = 0;  // !SMEM_TABLES: the aligned record pair that holds cur
+      if (!SMEM_TABLES) ldg_pair_if(pair_lo, pair_hi, pick_fast + cur, true);  // cur is even here
+      uint32_t rec = SMEM_TABLES ? lds32(cur) : pair_lo;
       uint32_t kmax = 0, kmin = 0xffffffffu;
       // Branch-free step: every lane runs Cmax steps. A lane that has finished its batch stays
       // on the batch's final pick and re-inserts it (set inserts and max are idempotent); a
@@ -583,9 +594,12 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
           nxt = more ? first_of_next : nxt;
           v = more ? v + 2 : v;
           lds16_if(n_c16, ringbase + (v & P.ring_mask), more);  // the look-ahead cursor
+          // a new pair is needed exactly when the cursor moved on to an even index (the next
+          // pair of this order, or the first pick of the next order)
+          ldg_pair_if(pair_lo, pair_hi, pick_fast + nxt, (nxt != cur) && !(nxt & 1u));
           cur = nxt;
         }
-        const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
+        const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : ((cur & 1u) ? pair_hi : pair_lo);
         // ---- this step's pick
         kmax = max(kmax, rec);
         if (!DEPOT0) kmin = min(kmin, rec);

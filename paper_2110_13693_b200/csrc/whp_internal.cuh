@@ -177,6 +177,8 @@ cudaError_t whp_launch_legsum_fast(whp_ctx* c, const int32_t* d_perms, int64_t n
                                    cudaStream_t st);
 cudaError_t whp_launch_legsum(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int64_t* d_len,
                               cudaStream_t st);
+cudaError_t whp_launch_route(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int32_t policy,
+                             int64_t* d_dist, double* d_obj, cudaStream_t st);
 cudaError_t whp_launch_l2_probe(whp_ctx* c, int64_t bytes, int32_t reps, float* ms);
 cudaError_t whp_launch_validate(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
                                 cudaStream_t st);

@@ -25,8 +25,9 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
            "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move",
            "whp_probe_l2_read", "whp_max_batches", "whp_set_swap_stats", "whp_get_swap_stats",
-           "whp_debug_set"]
+           "whp_debug_set", "whp_eval_routing"]
 
+ROUTE_S_SHAPE, ROUTE_RETURN, ROUTE_LARGEST_GAP = range(3)
 DEBUG_FORCE_GENERAL, DEBUG_SEGMENTS, DEBUG_WARPS, DEBUG_SWAP_MARGIN = range(4)
 
 
@@ -59,6 +60,7 @@ def lib():
         L.whp_nhatc_solve.argtypes = [vp, vp, i64, i32, C.c_double, vp, vp, vp, vp]
         L.whp_get_penalty.argtypes = [vp, vp, vp, vp, vp]
         L.whp_eval_legsum.argtypes = [vp, vp, i64, vp, vp]
+        L.whp_eval_routing.argtypes = [vp, vp, i64, i32, vp, vp, vp]
         L.whp_kmeans_slotting.argtypes = [i32, i32, i32, i32, vp, i32, i32, i32, i32, i32, vp, vp, vp, vp]
         L.whp_eval_moves.argtypes = [vp, vp, i32, i32, vp, vp, vp]
         L.whp_apply_move.argtypes = [vp, vp, i32, i32, vp, vp]
@@ -254,6 +256,16 @@ class Context:
         self._check(lib().whp_eval_legsum(self._h, _d(perms, torch.int32, n_cand * self.n_orders, dv),
                                           n_cand, _d(length, torch.int64, n_cand, dv),
                                           _stream(stream)))
+
+    def eval_routing(self, perms, policy, dist=None, obj=None, stream=None):
+        """NEXT-2 (readings N5 / N6): D and J of every plan with its carts routed by `policy`
+        (ROUTE_S_SHAPE, ROUTE_RETURN, ROUTE_LARGEST_GAP)."""
+        import torch
+        n_cand = perms.shape[0] if perms.dim() == 2 else 1
+        dv = self.device
+        self._check(lib().whp_eval_routing(self._h, _d(perms, torch.int32, n_cand * self.n_orders, dv),
+                                           n_cand, int(policy), _d(dist, torch.int64, n_cand, dv),
+                                           _d(obj, torch.float64, n_cand, dv), _stream(stream)))
 
     def nhatc_update(self, resp_rows, idx=None, beta=1.0, stream=None):
         """NEXT-1 (reading N1): v <- v + 2 w^2 (t - r*), w <- beta w; r* = row idx[0] of resp_rows."""

@@ -603,7 +603,7 @@ def test_api_errors_and_nullable_outputs(torch_cuda):
         ctx.eval_swaps(perms[0], 0, 1, obj=obj)
     assert e.value.status == whp.ERR_INVALID_ARG
     with pytest.raises(whp.WhpError) as e:
-        ctx.eval_swaps(perms[0], 15, 6, obj=obj)
+        ctx.eval_swaps(perms[0], 15, 6, obj=torch.zeros(15, dtype=torch.float64, device="cuda"))
     assert e.value.status == whp.ERR_OUT_OF_RANGE
     bad = perms.clone()
     bad[2, 0] = bad[2, 1]
