@@ -365,7 +365,24 @@ def run_ours(args):
                "api": "whp_eval_candidates_host (pinned host buffers, chunked copy/compute overlap)",
                "matches_device_path": bool(np.array_equal(h_obj.numpy(), obj.cpu().numpy())
                                            and e_idx == int(idx.item()))}
-        del h_perms
+        # the same through whp_eval_candidates_host16: 16-bit order ids, half the bytes over PCIe
+        h16 = torch.from_numpy(perms.cpu().numpy().astype(np.uint16).view(np.int16)).pin_memory()
+        for _ in range(2):
+            ctx.eval_candidates_host(h16, h_dist, h_obj)
+        torch.cuda.synchronize()
+        harness.barrier(world)
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            e_idx16, _ = ctx.eval_candidates_host(h16, h_dist, h_obj)
+        torch.cuda.synchronize()
+        e16_s = harness.max_over_ranks(time.perf_counter() - t0, world, dev)
+        harness.barrier(world)
+        e2e["uint16_ids"] = {"value": n_cand * world * e2e_steps / e16_s, "unit": "candidate plans/s",
+                             "h2d_bytes_per_step": int(h16.numel() * 2),
+                             "api": "whp_eval_candidates_host16",
+                             "matches_device_path": bool(np.array_equal(h_obj.numpy(), obj.cpu().numpy())
+                                                         and e_idx16 == int(idx.item()))}
+        del h_perms, h16
 
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     nexts, l2_gbs = {}, None

@@ -115,6 +115,15 @@ whp_status whp_eval_candidates_host(whp_ctx* ctx, const int32_t* h_perms, int64_
                                     int64_t* h_dist, double* h_obj,
                                     int64_t* h_argmin_idx, double* h_argmin_val);
 
+/* The same with 16-bit order ids (h_perms host uint16[n_cand][n_orders]): half the bytes over
+ * PCIe, which is what bounds the host-buffer path; the first kernel reads 16-bit tiles. Legal only
+ * on shapes of the tuned kernels (n_orders < 65536, ...: WHP_ERR_OUT_OF_RANGE otherwise — use the
+ * int32 call). PAPER.md:125 ("evaluating the permutations of different picking sequences");
+ * BASELINE.json configs[3] states int32 ids, so the int32 call stays the reference entry point. */
+whp_status whp_eval_candidates_host16(whp_ctx* ctx, const uint16_t* h_perms, int64_t n_cand,
+                                      int64_t* h_dist, double* h_obj,
+                                      int64_t* h_argmin_idx, double* h_argmin_val);
+
 /* a6 (D8): all W(W-1)/2 pairwise swaps of positions inside [win_start, win_start+win_len)
  * of d_base_perm (DEVICE int32[n_orders]); neighbour n <-> (i',j'), 0 <= i' < j' < W,
  * n = i'(2W-i'-1)/2 + (j'-i'-1); value = D2–D6 of the swapped sequence. Only the batches a

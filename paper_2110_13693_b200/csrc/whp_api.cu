@@ -53,7 +53,7 @@ void free_orders(whp_ctx* c) {
   dfree(c->base.cls_at); dfree(c->base.dtail); dfree(c->base.bF); dfree(c->base.rtail);
   c->rtail_rows = 0;
   dfree(c->d_stage[0]); dfree(c->d_stage[1]);
-  c->stage_rows = 0;
+  c->stage_bytes = 0;
   dfree(c->d_bmask); dfree(c->d_cstream); dfree(c->d_nb); dfree(c->d_dist_scratch);
   dfree(c->d_planes); dfree(c->d_segstart); dfree(c->d_perm_pad);
   c->perm_pad_bytes = 0;
@@ -343,28 +343,32 @@ whp_status whp_validate_perms(whp_ctx* c, const int32_t* d_perms, int64_t n_cand
   return WHP_OK;
 }
 
-whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t n_cand,
-                                    int64_t* h_dist, double* h_obj, int64_t* h_argmin_idx,
-                                    double* h_argmin_val) {
-  nvtx_range nvtx_("whp_eval_candidates_host");
+// Shared by the two host-buffer entry points: elem = bytes of an order id (4, or 2 for host16).
+static whp_status eval_host(whp_ctx* c, const void* h_perms, size_t elem, int64_t n_cand,
+                            int64_t* h_dist, double* h_obj, int64_t* h_argmin_idx,
+                            double* h_argmin_val) {
   whp_status s = ready(c);
   if (s != WHP_OK) return s;
   if (n_cand < 0) return fail(c, WHP_ERR_INVALID_ARG, "n_cand < 0");
   if (n_cand == 0) return WHP_OK;
   if (!h_perms) return fail(c, WHP_ERR_INVALID_ARG, "h_perms is null");
+  const bool perm16 = elem == 2;
+  if (perm16 && !whp_fast_eligible(c))
+    return fail(c, WHP_ERR_OUT_OF_RANGE, "16-bit plans need a shape of the tuned path (whp.h limits): use whp_eval_candidates_host");
   device_guard dg(c->device);
   // staging: two device buffers of `rows` plans each (~32 MB), results for all plans
-  const int64_t row_bytes = 4ll * c->n_orders;
+  const int64_t row_bytes = (int64_t)elem * c->n_orders;
   int64_t rows = (32ll << 20) / row_bytes;
   if (rows < 1) rows = 1;
   if (rows > n_cand) rows = n_cand;
-  if (c->stage_rows < rows) {
+  if (c->stage_bytes < rows * row_bytes) {
     dfree(c->d_stage[0]); dfree(c->d_stage[1]);
+    c->stage_bytes = 0;
     WHP_CUDA(c, cudaMalloc(&c->d_stage[0], (size_t)(rows * row_bytes)));
     WHP_CUDA(c, cudaMalloc(&c->d_stage[1], (size_t)(rows * row_bytes)));
-    c->stage_rows = rows;
+    c->stage_bytes = rows * row_bytes;
   }
-  rows = c->stage_rows < n_cand ? c->stage_rows : n_cand;
+  rows = c->stage_bytes / row_bytes < n_cand ? c->stage_bytes / row_bytes : n_cand;
   if (c->h_out_cap < n_cand) {
     dfree(c->d_h_dist); dfree(c->d_h_obj);
     WHP_CUDA(c, cudaMalloc(&c->d_h_dist, 8 * (size_t)n_cand));
@@ -377,13 +381,16 @@ whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t 
     const int b = (int)(chunk & 1);
     const int64_t nr = (n_cand - lo < rows) ? n_cand - lo : rows;
     if (chunk >= 2) WHP_CUDA(c, cudaStreamWaitEvent(c->s_copy[b], c->ev_done[b], 0));
-    WHP_CUDA(c, cudaMemcpyAsync(c->d_stage[b], h_perms + lo * c->n_orders,
+    WHP_CUDA(c, cudaMemcpyAsync(c->d_stage[b], (const char*)h_perms + lo * row_bytes,
                                 (size_t)(nr * row_bytes), cudaMemcpyHostToDevice, c->s_copy[b]));
     WHP_CUDA(c, cudaEventRecord(c->ev_copied[b], c->s_copy[b]));
     WHP_CUDA(c, cudaStreamWaitEvent(c->s_exec, c->ev_copied[b], 0));
     whp_eval_out out{c->d_h_dist + lo, nullptr, c->d_h_obj + lo, nullptr, nullptr, nullptr,
                      nullptr, nullptr};
-    WHP_CUDA(c, whp_launch_eval(c, c->d_stage[b], nr, out, c->s_exec));
+    if (perm16)
+      WHP_CUDA(c, whp_launch_eval_fast(c, c->d_stage[b], nr, out, c->s_exec, true));
+    else
+      WHP_CUDA(c, whp_launch_eval(c, (const int32_t*)c->d_stage[b], nr, out, c->s_exec));
     WHP_CUDA(c, cudaEventRecord(c->ev_done[b], c->s_exec));
   }
   if (h_argmin_idx || h_argmin_val) {
@@ -399,6 +406,20 @@ whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t 
     WHP_CUDA(c, cudaMemcpyAsync(h_obj, c->d_h_obj, 8 * (size_t)n_cand, cudaMemcpyDeviceToHost, c->s_exec));
   WHP_CUDA(c, cudaStreamSynchronize(c->s_exec));
   return WHP_OK;
+}
+
+whp_status whp_eval_candidates_host(whp_ctx* c, const int32_t* h_perms, int64_t n_cand,
+                                    int64_t* h_dist, double* h_obj, int64_t* h_argmin_idx,
+                                    double* h_argmin_val) {
+  nvtx_range nvtx_("whp_eval_candidates_host");
+  return eval_host(c, h_perms, 4, n_cand, h_dist, h_obj, h_argmin_idx, h_argmin_val);
+}
+
+whp_status whp_eval_candidates_host16(whp_ctx* c, const uint16_t* h_perms, int64_t n_cand,
+                                      int64_t* h_dist, double* h_obj, int64_t* h_argmin_idx,
+                                      double* h_argmin_val) {
+  nvtx_range nvtx_("whp_eval_candidates_host16");
+  return eval_host(c, h_perms, 2, n_cand, h_dist, h_obj, h_argmin_idx, h_argmin_val);
 }
 
 whp_status whp_eval_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,

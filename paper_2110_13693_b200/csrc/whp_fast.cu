@@ -45,6 +45,9 @@ __device__ __forceinline__ int4 lds128(uint32_t a) {
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) {
   asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v));
 }
+__device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
+  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w));
+}
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
 }
@@ -107,18 +110,38 @@ __device__ __forceinline__ void tma_tile_2d(uint32_t dst, const CUtensorMap* tm,
 // order records of the positions of a word (ids from the staged chunk, records from the order
 // table in shared memory). FULL: all 32 positions, straight-line code; otherwise only the first
 // n4 groups of four exist and the others get record 0 (q = 0: no effect on the recurrence).
-template <bool FULL>
+// U16: the plans hold 16-bit order ids; a 128-byte tile row is then two words (64 positions) and
+// `half` selects the word (chunks 4 half .. 4 half + 3, eight ids each).
+template <bool FULL, bool U16>
 __device__ __forceinline__ void gather_word(uint32_t (&r)[32], uint32_t row, uint32_t swz,
-                                            uint32_t sorec0, int n4, int left = 32) {
+                                            uint32_t sorec0, int n4, int left = 32, int half = 0) {
   // row = address of this lane's 128-byte row of the tile; 16-byte chunk g lives at g ^ (lane & 7)
+  if (U16) {
 #pragma unroll
-  for (int g = 0; g < 8; ++g) {
-    if (FULL || g < n4) {
-      const int4 v = lds128(row + ((16 * g) ^ swz));
-      r[4 * g + 0] = lds32(sorec0 + 4 * v.x); r[4 * g + 1] = lds32(sorec0 + 4 * v.y);
-      r[4 * g + 2] = lds32(sorec0 + 4 * v.z); r[4 * g + 3] = lds32(sorec0 + 4 * v.w);
-    } else {
-      r[4 * g + 0] = 0u; r[4 * g + 1] = 0u; r[4 * g + 2] = 0u; r[4 * g + 3] = 0u;
+    for (int g = 0; g < 4; ++g) {
+      if (FULL || 2 * g < n4) {
+        const int4 v = lds128(row + ((16 * (g + 4 * half)) ^ swz));
+        const uint32_t w4[4] = {(uint32_t)v.x, (uint32_t)v.y, (uint32_t)v.z, (uint32_t)v.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          r[8 * g + 2 * j] = lds32(sorec0 + ((w4[j] << 2) & 0x3fffcu));
+          r[8 * g + 2 * j + 1] = lds32(sorec0 + ((w4[j] >> 14) & 0x3fffcu));
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) r[8 * g + j] = 0u;
+      }
+    }
+  } else {
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      if (FULL || g < n4) {
+        const int4 v = lds128(row + ((16 * g) ^ swz));
+        r[4 * g + 0] = lds32(sorec0 + 4 * v.x); r[4 * g + 1] = lds32(sorec0 + 4 * v.y);
+        r[4 * g + 2] = lds32(sorec0 + 4 * v.z); r[4 * g + 3] = lds32(sorec0 + 4 * v.w);
+      } else {
+        r[4 * g + 0] = 0u; r[4 * g + 1] = 0u; r[4 * g + 2] = 0u; r[4 * g + 3] = 0u;
+      }
     }
   }
   if (!FULL) {  // a plan whose length is no multiple of 4: the tile is zero-filled past its end
@@ -171,7 +194,9 @@ __device__ __forceinline__ uint32_t recur_word(const uint32_t (&r)[32], uint32_t
   return ~__brev(rev);
 }
 
-template <int kWarps>  // warps per block: they share the order table (a warp = 32 plans)
+// kWarps: warps per block, they share the order table (a warp = 32 plans). U16: the plan matrix
+// holds 16-bit order ids (whp_eval_candidates_host16): a tile is then 32 plans x 64 positions.
+template <int kWarps, bool U16>
 __global__ void __launch_bounds__(32 * kWarps)
 whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_cs,
                   const uint32_t* __restrict__ order_fast,
@@ -194,10 +219,11 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();
   const int64_t row0 = ((int64_t)blockIdx.x * kWarps + wq) * 32;  // first plan of this warp
-  auto issue = [&](int w) {  // one lane: tile of word w into stage w mod kStages
-    const uint32_t bar = bars + 8 * (w % kStages);
+  const int nt = U16 ? (nw + 1) >> 1 : nw;  // tiles of a plan
+  auto issue = [&](int t) {  // one lane: tile t into stage t mod kStages
+    const uint32_t bar = bars + 8 * (t % kStages);
     mbar_expect_tx(bar, kTileBytes);
-    tma_tile_2d(tiles + (w % kStages) * kTileBytes, &tmap, 32 * w, (int32_t)row0, bar);
+    tma_tile_2d(tiles + (t % kStages) * kTileBytes, &tmap, (U16 ? 64 : 32) * t, (int32_t)row0, bar);
   };
   if (threadIdx.x == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
     const uint32_t table_bytes = 4u * (uint32_t)((n_orders + 3) & ~3);  // the table is padded
@@ -205,19 +231,23 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     bulk_g2s(sorec0, order_fast, table_bytes, bar_table);
   }
   if (lane == 0)
-    for (int w = 0; w < kStages && w < nw; ++w) issue(w);
+    for (int t = 0; t < kStages && t < nt; ++t) issue(t);
   const int64_t c = row0 + lane;
   const bool have = c < n_cand;  // rows past the end arrive zero-filled: order 0, never written
   uint32_t* __restrict__ bm = bmask + (have ? c : 0) * bm_pitch;
   uint4* __restrict__ cs = reinterpret_cast<uint4*>(cstream + (have ? c : 0) * cs_pitch);
   const uint32_t rowoff = lane * 128, swz = (lane & 7) << 4;
-  auto tile_row = [&](int w) { return tiles + (w % kStages) * kTileBytes + rowoff; };
-  auto wait_word = [&](int w) { mbar_wait(bars + 8 * (w % kStages), (w / kStages) & 1); };
-  auto refill = [&](int w) {  // word w is consumed by every lane: its stage takes word w + kStages
+  auto tile_of = [&](int w) { return U16 ? w >> 1 : w; };
+  auto tile_row = [&](int w) { return tiles + (tile_of(w) % kStages) * kTileBytes + rowoff; };
+  auto wait_word = [&](int w) {
+    mbar_wait(bars + 8 * (tile_of(w) % kStages), (tile_of(w) / kStages) & 1);
+  };
+  auto refill = [&](int w) {  // word w is consumed by every lane: its stage takes the next tile
     // (the tile was only READ, and every value read has been used: no proxy fence is needed
     // before the async proxy overwrites it)
+    if (U16 && !(w & 1)) return;  // the tile's second word is still to come
     __syncwarp();
-    if (lane == 0 && w + kStages < nw) issue(w + kStages);
+    if (lane == 0 && tile_of(w) + kStages < nt) issue(tile_of(w) + kStages);
   };
   uint32_t room = (uint32_t)C;
   uint32_t ra[32], rb[32];
@@ -226,7 +256,7 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   const int n_full = n_orders >> 5;            // words with all 32 positions
   // pairs of words (2k, 2k+1) whose successor 2k+2 is full too: the straight-line path
   const int KF = n_full > 0 ? (n_full - 1) >> 1 : 0;
-  if (n_full > 0) gather_word<true>(ra, tile_row(0), swz, sorec0, 8);
+  if (n_full > 0) gather_word<true, U16>(ra, tile_row(0), swz, sorec0, 8, 32, 0);
 #pragma unroll 1
   for (int k = 0; k < KF; ++k) {
     const int w = 2 * k;
@@ -236,14 +266,14 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     __syncwarp();
     // word w runs its recurrence while word w+1 is gathered
     wait_word(w + 1);
-    gather_word<true>(rb, tile_row(w + 1), swz, sorec0, 8);
+    gather_word<true, U16>(rb, tile_row(w + 1), swz, sorec0, 8, 32, 1);
     uint32_t bits = recur_word<true, true>(ra, (uint32_t)C, room, nullptr, otile + rowoff, swz, 0, 8, have);
     if (k == 0) bits |= 1u;  // batch 0 starts at position 0
     const uint32_t bits_even = bits;
     refill(w);
     // word w+1 runs its recurrence while word w+2 is gathered
     wait_word(w + 2);
-    gather_word<true>(ra, tile_row(w + 2), swz, sorec0, 8);
+    gather_word<true, U16>(ra, tile_row(w + 2), swz, sorec0, 8, 32, 0);
     bits = recur_word<true, true>(rb, (uint32_t)C, room, nullptr, otile + rowoff, swz, 1, 8, have);
     if (have) *reinterpret_cast<uint2*>(bm + w) = make_uint2(bits_even, bits);
     refill(w + 1);
@@ -259,7 +289,7 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     const int n4 = min(8, (left + 3) >> 2);
     if (w > 2 * KF || n_full == 0) {
       wait_word(w);
-      gather_word<false>(ra, tile_row(w), swz, sorec0, n4, left);
+      gather_word<false, U16>(ra, tile_row(w), swz, sorec0, n4, left, w & 1);
     }
     uint32_t bits = recur_word<false, false>(ra, (uint32_t)C, room, cs + 4 * w, 0u, 0u, 0, n4, have);
     if (w == 0) bits |= 1u;
@@ -454,6 +484,9 @@ __device__ __forceinline__ void lds16_if(uint32_t& v, uint32_t a, bool p) {
                : "+r"(v) : "r"(a), "r"((uint32_t)p));
 }
 
+// SMEM_TABLES false: the pick table does not fit shared memory and is gathered through L1 / L2
+// (the shared memory the private state leaves free is L1: 32 warps instead of 24 leave 10 KB of it
+// and the stress evaluation goes from 10.6 to 17.5 ms, the L1 hit rate from 52 % to 2 %).
 template <bool SMEM_TABLES, bool DEPOT0, int KW, int kPlanes>
 __global__ void __launch_bounds__(KW * kPlanes <= 42 ? 768 : 512, 1)  // counter registers: KW x planes
 whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restrict__ pick_fast,
@@ -576,6 +609,7 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       if (!SMEM_TABLES) ldg_pair_if(pair_lo, pair_hi, pick_fast + cur, true);  // cur is even here
       uint32_t rec = SMEM_TABLES ? lds32(cur) : pair_lo;
       uint32_t kmax = 0, kmin = 0xffffffffu;
+      uint32_t cset = 0;  // KW == 1: class set of the batch
       // Branch-free step: every lane runs Cmax steps. A lane that has finished its batch stays
       // on the batch's final pick and re-inserts it (set inserts and max are idempotent); a
       // lane without a batch walks to the end of order 0 and stays there — its sets are
@@ -595,7 +629,9 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
           v = more ? v + 2 : v;
           lds16_if(n_c16, ringbase + (v & P.ring_mask), more);  // the look-ahead cursor
           // a new pair is needed exactly when the cursor moved on to an even index (the next
-          // pair of this order, or the first pick of the next order)
+          // pair of this order, or the first pick of the next order). Measured and not kept:
+          // fetching the next order's first pair one order ahead (12.9 ms against 12.2 ms for
+          // the 65,536 stress plans: the extra loads cost more than the hidden latency saves)
           ldg_pair_if(pair_lo, pair_hi, pick_fast + nxt, (nxt != cur) && !(nxt & 1u));
           cur = nxt;
         }
@@ -605,8 +641,12 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         if (!DEPOT0) kmin = min(kmin, rec);
         const uint32_t aaddr = abase | ((rec >> 20) & amask);
         sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 22));
-        const uint32_t caddr = cbase | (rec & 0x380u);
-        sts32(caddr, lds32(caddr) | one_shl_wrap(rec));
+        if (KW == 1) {  // up to 32 classes: the batch's class set is one register
+          cset |= one_shl_wrap(rec);
+        } else {
+          const uint32_t caddr = cbase | (rec & 0x380u);
+          sts32(caddr, lds32(caddr) | one_shl_wrap(rec));
+        }
         rec = rec_next;
       }
       {  // refill the slots of the chunks this batch finished; waited for two batches later
@@ -650,8 +690,13 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
 #pragma unroll
       for (int w = 0; w < KW; ++w) {
         // lanes without a batch j ran the steps on a dummy pick: their set is discarded
-        uint32_t carry = lds32(cbase + w * 128);
-        sts32(cbase + w * 128, 0u);
+        uint32_t carry;
+        if (KW == 1) {
+          carry = cset;
+        } else {
+          carry = lds32(cbase + w * 128);
+          sts32(cbase + w * 128, 0u);
+        }
         if (!live) carry = 0u;
 #pragma unroll
         for (int pp = 0; pp < kPlanes; ++pp) {
@@ -1005,8 +1050,9 @@ static cudaError_t ensure_fast_scratch(whp_ctx* c, int64_t n_cand, int64_t plane
 }
 
 // K1 (batch boundaries, cursor stream) and the segment starts of every plan
-static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int S,
-                                              int log2S, int32_t* n_batches_out, cudaStream_t st) {
+static cudaError_t launch_bounds_and_segments(whp_ctx* c, const void* d_perms, int64_t n_cand, int S,
+                                              int log2S, int32_t* n_batches_out, cudaStream_t st,
+                                              bool perm16 = false) {
   const int32_t bm_pitch = fast_bm_pitch(c), cs_pitch = fast_cs_pitch(c), ss_pitch = kSsPitch;
   {
     cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
@@ -1018,9 +1064,10 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms
     if (!encode) return cudaErrorNotSupported;
     // TMA needs a 16-byte aligned matrix with a row pitch that is a multiple of 16 bytes:
     // otherwise the plans are first copied into a padded scratch matrix
-    size_t pitch_bytes = 4 * (size_t)c->n_orders;
-    if ((c->n_orders & 3) != 0 || ((uintptr_t)d_perms & 15u) != 0) {
-      pitch_bytes = 4 * (((size_t)c->n_orders + 3) & ~(size_t)3);
+    const size_t elem = perm16 ? 2 : 4;  // bytes of an order id
+    size_t pitch_bytes = elem * (size_t)c->n_orders;
+    if ((pitch_bytes & 15u) != 0 || ((uintptr_t)d_perms & 15u) != 0) {
+      pitch_bytes = (pitch_bytes + 15) & ~(size_t)15;
       if (c->perm_pad_bytes < pitch_bytes * (size_t)n_cand) {
         if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return e;
         cudaFree(c->d_perm_pad);
@@ -1029,8 +1076,8 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms
         if ((e = cudaMalloc(&c->d_perm_pad, pitch_bytes * (size_t)n_cand)) != cudaSuccess) return e;
         c->perm_pad_bytes = pitch_bytes * (size_t)n_cand;
       }
-      if ((e = cudaMemcpy2DAsync(c->d_perm_pad, pitch_bytes, d_perms, 4 * (size_t)c->n_orders,
-                                 4 * (size_t)c->n_orders, (size_t)n_cand, cudaMemcpyDeviceToDevice,
+      if ((e = cudaMemcpy2DAsync(c->d_perm_pad, pitch_bytes, d_perms, elem * (size_t)c->n_orders,
+                                 elem * (size_t)c->n_orders, (size_t)n_cand, cudaMemcpyDeviceToDevice,
                                  st)) != cudaSuccess)
         return e;
       d_perms = c->d_perm_pad;
@@ -1038,9 +1085,10 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms
     CUtensorMap tmap;
     const cuuint64_t gdim[2] = {(cuuint64_t)c->n_orders, (cuuint64_t)n_cand};
     const cuuint64_t gstride[1] = {(cuuint64_t)pitch_bytes};
-    const cuuint32_t box[2] = {32, 32};
+    const cuuint32_t box[2] = {perm16 ? 64u : 32u, 32};  // 128 bytes x 32 plans
     const cuuint32_t estr[2] = {1, 1};
-    if (encode(&tmap, CU_TENSOR_MAP_DATA_TYPE_INT32, 2, (void*)d_perms, gdim, gstride, box, estr,
+    if (encode(&tmap, perm16 ? CU_TENSOR_MAP_DATA_TYPE_UINT16 : CU_TENSOR_MAP_DATA_TYPE_INT32, 2,
+               (void*)d_perms, gdim, gstride, box, estr,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
@@ -1054,17 +1102,22 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms
                CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return cudaErrorInvalidValue;
     const unsigned blocks = (unsigned)((n_cand + 32 * kw1 - 1) / (32 * kw1));
-#define WHP_LAUNCH_BOUNDS(KW1)                                                                  \
+#define WHP_LAUNCH_BOUNDS_T(KW1, U16V)                                                          \
   do {                                                                                          \
-    cudaFuncSetAttribute(whp_bounds_kernel<KW1>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
-                         c->smem_optin - 1024);                                                 \
-    whp_bounds_kernel<KW1><<<blocks, 32 * KW1, smem, st>>>(                                     \
+    cudaFuncSetAttribute(whp_bounds_kernel<KW1, U16V>,                                          \
+                         cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin - 1024);    \
+    whp_bounds_kernel<KW1, U16V><<<blocks, 32 * KW1, smem, st>>>(                               \
         tmap, tmap_cs, c->d_order_fast, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch,        \
         c->d_cstream, cs_pitch);                                                                \
+  } while (0)
+#define WHP_LAUNCH_BOUNDS(KW1)                                                                  \
+  do {                                                                                          \
+    if (perm16) WHP_LAUNCH_BOUNDS_T(KW1, true); else WHP_LAUNCH_BOUNDS_T(KW1, false);           \
   } while (0)
     if (kw1 == 1) WHP_LAUNCH_BOUNDS(1);
     else if (kw1 == 2) WHP_LAUNCH_BOUNDS(2);
     else WHP_LAUNCH_BOUNDS(4);
+#undef WHP_LAUNCH_BOUNDS_T
 #undef WHP_LAUNCH_BOUNDS
     c->launches += 1;
     if ((e = cudaGetLastError()) != cudaSuccess) return e;
@@ -1077,8 +1130,8 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const int32_t* d_perms
   return cudaSuccess;
 }
 
-cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
-                                 const whp_eval_out& out, cudaStream_t st) {
+cudaError_t whp_launch_eval_fast(whp_ctx* c, const void* d_perms, int64_t n_cand,
+                                 const whp_eval_out& out, cudaStream_t st, bool perm16) {
   const whp_tables T = whp_make_tables(c);
   const int64_t nb_ub = nb_upper_bound(c);
   const int32_t bm_pitch = fast_bm_pitch(c), cs_pitch = fast_cs_pitch(c), ss_pitch = kSsPitch;
@@ -1122,7 +1175,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_c
   const int fits32 = worst < (1ll << 31) ? 1 : 0;
   cudaError_t e0 = ensure_fast_scratch(c, n_cand, (int64_t)kPlaneRow * KW, st);
   if (e0 != cudaSuccess) return e0;
-  if ((e0 = launch_bounds_and_segments(c, d_perms, n_cand, S, log2S, out.n_batches, st)) != cudaSuccess)
+  if ((e0 = launch_bounds_and_segments(c, d_perms, n_cand, S, log2S, out.n_batches, st, perm16)) != cudaSuccess)
     return e0;
   // K2
   {

@@ -127,8 +127,8 @@ struct whp_ctx {
   int32_t fast_pitch = 0;
   int smem_optin = 0;
   // host-path staging (whp_eval_candidates_host)
-  int32_t* d_stage[2] = {nullptr, nullptr};
-  int64_t stage_rows = 0;
+  void* d_stage[2] = {nullptr, nullptr};
+  int64_t stage_bytes = 0;
   int64_t* d_h_dist = nullptr;
   double* d_h_obj = nullptr;
   int64_t h_out_cap = 0;
@@ -154,8 +154,9 @@ whp_tables whp_make_tables(const whp_ctx* c);
 cudaError_t whp_launch_eval(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
                             const whp_eval_out& out, cudaStream_t st);
 bool whp_fast_eligible(const whp_ctx* c);
-cudaError_t whp_launch_eval_fast(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
-                                 const whp_eval_out& out, cudaStream_t st);
+// perm16: d_perms holds uint16 order ids (tuned path only)
+cudaError_t whp_launch_eval_fast(whp_ctx* c, const void* d_perms, int64_t n_cand,
+                                 const whp_eval_out& out, cudaStream_t st, bool perm16 = false);
 cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                              int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st);
 cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,

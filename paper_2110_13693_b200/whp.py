@@ -25,7 +25,7 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
            "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move",
            "whp_probe_l2_read", "whp_max_batches", "whp_set_swap_stats", "whp_get_swap_stats",
-           "whp_debug_set", "whp_eval_routing"]
+           "whp_debug_set", "whp_eval_routing", "whp_eval_candidates_host16"]
 
 ROUTE_S_SHAPE, ROUTE_RETURN, ROUTE_LARGEST_GAP = range(3)
 DEBUG_FORCE_GENERAL, DEBUG_SEGMENTS, DEBUG_WARPS, DEBUG_SWAP_MARGIN = range(4)
@@ -52,6 +52,7 @@ def lib():
         L.whp_set_penalty.argtypes = [vp, vp, vp, vp]
         L.whp_eval_candidates.argtypes = [vp, vp, i64] + [vp] * 8 + [vp]
         L.whp_eval_candidates_host.argtypes = [vp, vp, i64, vp, vp, vp, vp]
+        L.whp_eval_candidates_host16.argtypes = [vp, vp, i64, vp, vp, vp, vp]
         L.whp_eval_swaps.argtypes = [vp, vp, i32, i32, vp, vp, vp]
         L.whp_argmin.argtypes = [vp, vp, i64, vp, vp, vp]
         L.whp_apply_swap.argtypes = [vp, vp, i32, i32, vp, vp]
@@ -197,15 +198,25 @@ class Context:
 
     def eval_candidates_host(self, perms, dist=None, obj=None, want_argmin=True):
         """perms / dist / obj: host numpy arrays or CPU torch tensors (pinned = async copies).
+        int32 plans go through whp_eval_candidates_host, uint16 plans (numpy uint16, torch
+        uint16 / int16 bit patterns) through whp_eval_candidates_host16.
         Returns (argmin_idx, argmin_val) when want_argmin."""
         n_cand = perms.shape[0]
-        p_perms = _hostbuf(perms, np.int32, n_cand * self.n_orders, "perms")
         if tuple(perms.shape) != (n_cand, self.n_orders):
             raise WhpError(ERR_INVALID_ARG, "perms shape")
+        is16 = (perms.dtype == np.uint16) if isinstance(perms, np.ndarray) else \
+            (str(perms.dtype) in ("torch.uint16", "torch.int16"))
+        fn = lib().whp_eval_candidates_host16 if is16 else lib().whp_eval_candidates_host
+        if is16 and not isinstance(perms, np.ndarray):
+            if perms.is_cuda or not perms.is_contiguous():
+                raise ValueError("perms: expected a contiguous CPU tensor")
+            p_perms = perms.data_ptr()
+        else:
+            p_perms = _hostbuf(perms, np.uint16 if is16 else np.int32, n_cand * self.n_orders, "perms")
         p_dist = _hostbuf(dist, np.int64, n_cand, "dist")
         p_obj = _hostbuf(obj, np.float64, n_cand, "obj")
         idx, val = C.c_int64(-1), C.c_double(0.0)
-        self._check(lib().whp_eval_candidates_host(
+        self._check(fn(
             self._h, p_perms, n_cand, p_dist, p_obj,
             C.addressof(idx) if want_argmin else None,
             C.addressof(val) if want_argmin else None))

@@ -658,3 +658,48 @@ def test_host_buffer_entry_point(torch_cuda):
     assert (i2, v2) == (i, v) and np.array_equal(pd.numpy(), ref["dist"])
     assert np.array_equal(po.numpy(), ref["obj"])
     ctx.close()
+
+
+# ---- host-buffer entry points (int32 and uint16 order ids) -------------------------------------------
+@pytest.mark.parametrize("n_orders,n_cand", [(500, 700), (64, 33), (97, 5), (36, 1), (4000, 300), (130, 64)])
+def test_host_entry_points_int32_and_uint16(torch_cuda, n_orders, n_cand):
+    """whp_eval_candidates_host / _host16 (chunked copies overlapped with evaluation) equal the
+    oracle; the 16-bit call runs K1 on 16-bit tiles (64 positions per tile row), including plan
+    lengths that are no multiple of 8 (padded copy) and of 64 (partial last tile)."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    if n_orders == 4000:
+        pb = W.make_problem("paper")
+    elif n_orders == 500:
+        pb = W.make_problem("mid")
+    else:
+        pb = _random_problem(9, NA=70, S=12, K=70, n_skus=400, n_orders=n_orders, qmax=5, C=11, depot=3)
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perm_rows(3, pb.n_orders, np.arange(n_cand))
+    ref = oracle.eval_candidates(pb, perms)
+    for arr in (perms, perms.astype(np.uint16)):
+        d, o = np.zeros(n_cand, np.int64), np.zeros(n_cand, np.float64)
+        i, v = ctx.eval_candidates_host(np.ascontiguousarray(arr), d, o)
+        assert np.array_equal(d, ref["dist"]) and np.array_equal(o, ref["obj"]), arr.dtype
+        assert i == oracle.argmin(ref["obj"]) and v == ref["obj"][i]
+    # pinned torch buffers, 16-bit ids as int16 bit patterns
+    h16 = torch.from_numpy(perms.astype(np.uint16).view(np.int16)).pin_memory()
+    hd = torch.zeros(n_cand, dtype=torch.int64).pin_memory()
+    ho = torch.zeros(n_cand, dtype=torch.float64).pin_memory()
+    i, v = ctx.eval_candidates_host(h16, hd, ho)
+    assert np.array_equal(hd.numpy(), ref["dist"]) and np.array_equal(ho.numpy(), ref["obj"])
+    ctx.close()
+
+
+def test_host16_needs_a_tuned_path_shape(torch_cuda):
+    from paper_2110_13693_b200 import whp
+    pb = _random_problem(4, NA=50, S=40, K=70, n_skus=3000, n_orders=300, qmax=4, C=200)  # C > 106
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perm_rows(8, pb.n_orders, np.arange(6))
+    with pytest.raises(whp.WhpError) as e:
+        ctx.eval_candidates_host(perms.astype(np.uint16), np.zeros(6, np.int64))
+    assert e.value.status == whp.ERR_OUT_OF_RANGE
+    d = np.zeros(6, np.int64)
+    ctx.eval_candidates_host(perms, d)  # the int32 call takes any shape
+    assert np.array_equal(d, oracle.eval_candidates(pb, perms)["dist"])
+    ctx.close()
