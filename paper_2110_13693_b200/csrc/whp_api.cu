@@ -356,42 +356,61 @@ static whp_status eval_host(whp_ctx* c, const void* h_perms, size_t elem, int64_
   if (perm16 && !whp_fast_eligible(c))
     return fail(c, WHP_ERR_OUT_OF_RANGE, "16-bit plans need a shape of the tuned path (whp.h limits): use whp_eval_candidates_host");
   device_guard dg(c->device);
-  // staging: two device buffers of `rows` plans each (~32 MB), results for all plans
+  // Staging: the plans of one pass (up to 1 GiB of them) go to one device buffer in ~16 MB
+  // pieces, ALL enqueued on the copy stream before the first evaluation is launched — the host
+  // work of a launch (two tensor-map encodings, four launches) would otherwise sit between two
+  // copies and leave PCIe idle. Piece k is evaluated as soon as its copy has landed, so only the
+  // last piece's evaluation is not hidden behind a copy.
   const int64_t row_bytes = (int64_t)elem * c->n_orders;
-  int64_t rows = (32ll << 20) / row_bytes;
+  int64_t rows = (16ll << 20) / row_bytes;
   if (rows < 1) rows = 1;
-  if (rows > n_cand) rows = n_cand;
-  if (c->stage_bytes < rows * row_bytes) {
-    dfree(c->d_stage[0]); dfree(c->d_stage[1]);
+  int64_t pass_rows = (1ll << 30) / row_bytes;
+  if (pass_rows < rows) pass_rows = rows;
+  if (pass_rows > n_cand) pass_rows = n_cand;
+  if (c->stage_bytes < pass_rows * row_bytes) {
+    dfree(c->d_stage[0]);
     c->stage_bytes = 0;
-    WHP_CUDA(c, cudaMalloc(&c->d_stage[0], (size_t)(rows * row_bytes)));
-    WHP_CUDA(c, cudaMalloc(&c->d_stage[1], (size_t)(rows * row_bytes)));
-    c->stage_bytes = rows * row_bytes;
+    WHP_CUDA(c, cudaMalloc(&c->d_stage[0], (size_t)(pass_rows * row_bytes)));
+    c->stage_bytes = pass_rows * row_bytes;
   }
-  rows = c->stage_bytes / row_bytes < n_cand ? c->stage_bytes / row_bytes : n_cand;
+  const int64_t pieces = (pass_rows + rows - 1) / rows;
+  while ((int64_t)c->ev_piece.size() < pieces) {
+    cudaEvent_t ev = nullptr;
+    WHP_CUDA(c, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+    c->ev_piece.push_back(ev);
+  }
   if (c->h_out_cap < n_cand) {
     dfree(c->d_h_dist); dfree(c->d_h_obj);
     WHP_CUDA(c, cudaMalloc(&c->d_h_dist, 8 * (size_t)n_cand));
     WHP_CUDA(c, cudaMalloc(&c->d_h_obj, 8 * (size_t)n_cand));
     c->h_out_cap = n_cand;
   }
-  // pipeline: copy chunk k+1 (alternating copy streams) while chunk k is evaluated
-  int64_t chunk = 0;
-  for (int64_t lo = 0; lo < n_cand; lo += rows, ++chunk) {
-    const int b = (int)(chunk & 1);
-    const int64_t nr = (n_cand - lo < rows) ? n_cand - lo : rows;
-    if (chunk >= 2) WHP_CUDA(c, cudaStreamWaitEvent(c->s_copy[b], c->ev_done[b], 0));
-    WHP_CUDA(c, cudaMemcpyAsync(c->d_stage[b], (const char*)h_perms + lo * row_bytes,
-                                (size_t)(nr * row_bytes), cudaMemcpyHostToDevice, c->s_copy[b]));
-    WHP_CUDA(c, cudaEventRecord(c->ev_copied[b], c->s_copy[b]));
-    WHP_CUDA(c, cudaStreamWaitEvent(c->s_exec, c->ev_copied[b], 0));
-    whp_eval_out out{c->d_h_dist + lo, nullptr, c->d_h_obj + lo, nullptr, nullptr, nullptr,
-                     nullptr, nullptr};
-    if (perm16)
-      WHP_CUDA(c, whp_launch_eval_fast(c, c->d_stage[b], nr, out, c->s_exec, true));
-    else
-      WHP_CUDA(c, whp_launch_eval(c, (const int32_t*)c->d_stage[b], nr, out, c->s_exec));
-    WHP_CUDA(c, cudaEventRecord(c->ev_done[b], c->s_exec));
+  for (int64_t pass_lo = 0; pass_lo < n_cand; pass_lo += pass_rows) {
+    const int64_t pass_n = (n_cand - pass_lo < pass_rows) ? n_cand - pass_lo : pass_rows;
+    if (pass_lo > 0) {  // the buffer is reused: the previous pass must have been evaluated
+      WHP_CUDA(c, cudaEventRecord(c->ev_done[0], c->s_exec));
+      WHP_CUDA(c, cudaStreamWaitEvent(c->s_copy[0], c->ev_done[0], 0));
+    }
+    int64_t k = 0;
+    for (int64_t lo = 0; lo < pass_n; lo += rows, ++k) {
+      const int64_t nr = (pass_n - lo < rows) ? pass_n - lo : rows;
+      WHP_CUDA(c, cudaMemcpyAsync((char*)c->d_stage[0] + lo * row_bytes,
+                                  (const char*)h_perms + (pass_lo + lo) * row_bytes,
+                                  (size_t)(nr * row_bytes), cudaMemcpyHostToDevice, c->s_copy[0]));
+      WHP_CUDA(c, cudaEventRecord(c->ev_piece[(size_t)k], c->s_copy[0]));
+    }
+    k = 0;
+    for (int64_t lo = 0; lo < pass_n; lo += rows, ++k) {
+      const int64_t nr = (pass_n - lo < rows) ? pass_n - lo : rows;
+      WHP_CUDA(c, cudaStreamWaitEvent(c->s_exec, c->ev_piece[(size_t)k], 0));
+      whp_eval_out out{c->d_h_dist + pass_lo + lo, nullptr, c->d_h_obj + pass_lo + lo, nullptr,
+                       nullptr, nullptr, nullptr, nullptr};
+      const void* src = (const char*)c->d_stage[0] + lo * row_bytes;
+      if (perm16)
+        WHP_CUDA(c, whp_launch_eval_fast(c, src, nr, out, c->s_exec, true));
+      else
+        WHP_CUDA(c, whp_launch_eval(c, (const int32_t*)src, nr, out, c->s_exec));
+    }
   }
   if (h_argmin_idx || h_argmin_val) {
     WHP_CUDA(c, whp_launch_argmin(c, c->d_h_obj, n_cand, c->d_h_idx, c->d_h_val, c->s_exec));
@@ -602,6 +621,7 @@ void whp_destroy(whp_ctx* c) {
     free_orders(c);
     dfree(c->d_tvw); dfree(c->d_argmin_part); dfree(c->d_count); dfree(c->d_task); dfree(c->d_swap_stats);
     dfree(c->d_h_dist); dfree(c->d_h_obj); dfree(c->d_h_idx); dfree(c->d_h_val); dfree(c->d_n_resp);
+    for (cudaEvent_t ev : c->ev_piece) cudaEventDestroy(ev);
     for (int k = 0; k < 2; ++k) {
       if (c->s_copy[k]) cudaStreamDestroy(c->s_copy[k]);
       if (c->ev_copied[k]) cudaEventDestroy(c->ev_copied[k]);

@@ -5,6 +5,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "../../include/whp.h"
 
@@ -140,6 +141,7 @@ struct whp_ctx {
   cudaStream_t s_copy[2] = {nullptr, nullptr};
   cudaStream_t s_exec = nullptr;
   cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_done[2] = {nullptr, nullptr};
+  std::vector<cudaEvent_t> ev_piece;  // one per staged piece of whp_eval_candidates_host
   int num_sms = 148;
   int64_t launches = 0;
   // whp_debug_set: kernel-selection overrides for tests and measurements (-1 / 0 = default)

@@ -98,7 +98,14 @@ def test_all_candidates_full_detail(torch_cuda, name):
     assert_parity(got2, ref, pb)
     with force_general(ctx):
         got3, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda(), detail=False)
+        # resp / batch_of_pos without n_distinct: the general kernel without its distinct-location scan
+        resp_g = torch.full((wl.n_cand, pb.n_classes), -1, dtype=torch.int32, device="cuda")
+        bop_g = torch.full((wl.n_cand, pb.n_orders), -1, dtype=torch.int32, device="cuda")
+        ctx.eval_candidates(torch.from_numpy(perms).cuda(), resp=resp_g, batch_of_pos=bop_g)
+        torch.cuda.synchronize()
     assert_parity(got3, ref, pb)
+    assert np.array_equal(resp_g.cpu().numpy(), ref["resp"])
+    assert np.array_equal(bop_g.cpu().numpy(), ref["batch_of_pos"])
     # responses alone come from the tuned path's vertical counters
     resp = torch.full((wl.n_cand, pb.n_classes), -1, dtype=torch.int32, device="cuda")
     ctx.eval_candidates(torch.from_numpy(perms).cuda(), resp=resp)
