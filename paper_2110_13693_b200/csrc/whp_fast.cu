@@ -991,6 +991,8 @@ static size_t bounds_smem_bytes(const whp_ctx* c, int warps = 1) {
 // them fit, else two or four warps that share one copy of the order table
 static int bounds_warps(const whp_ctx* c) {
   const size_t cap = (size_t)c->smem_optin;
+  if (c->dbg_k1_warps == 1 || c->dbg_k1_warps == 2 || c->dbg_k1_warps == 4)  // WHP_DEBUG_K1_WARPS
+    if (bounds_smem_bytes(c, c->dbg_k1_warps) + 1024 <= cap) return c->dbg_k1_warps;
   if (4 * (bounds_smem_bytes(c, 1) + 1024) <= cap) return 1;
   if (2 * (bounds_smem_bytes(c, 2) + 1024) <= cap) return 2;
   if (bounds_smem_bytes(c, 4) + 1024 <= cap) return 4;

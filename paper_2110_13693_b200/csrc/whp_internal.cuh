@@ -145,7 +145,7 @@ struct whp_ctx {
   int num_sms = 148;
   int64_t launches = 0;
   // whp_debug_set: kernel-selection overrides for tests and measurements (-1 / 0 = default)
-  int32_t dbg_force_general = 0, dbg_segments = -1, dbg_warps = -1;
+  int32_t dbg_force_general = 0, dbg_segments = -1, dbg_warps = -1, dbg_k1_warps = -1;
   int64_t dbg_swap_margin = -1;
   std::string err;
 };

@@ -28,7 +28,7 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_debug_set", "whp_eval_routing", "whp_eval_candidates_host16"]
 
 ROUTE_S_SHAPE, ROUTE_RETURN, ROUTE_LARGEST_GAP = range(3)
-DEBUG_FORCE_GENERAL, DEBUG_SEGMENTS, DEBUG_WARPS, DEBUG_SWAP_MARGIN = range(4)
+DEBUG_FORCE_GENERAL, DEBUG_SEGMENTS, DEBUG_WARPS, DEBUG_SWAP_MARGIN, DEBUG_K1_WARPS = range(5)
 
 
 class WhpError(RuntimeError):

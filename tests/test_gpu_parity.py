@@ -350,6 +350,11 @@ def test_tuned_path_word_and_warp_tails(torch_cuda, n_orders, n_cand):
     got, dev = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
     ref = oracle.eval_candidates(pb, perms, detail=True)
     assert_parity(got, ref, pb)
+    for kw in (2, 4):  # K1 blocks of two / four warps sharing the order table
+        ctx.debug_set(whp.DEBUG_K1_WARPS, kw)
+        got_k, _ = gpu_eval(torch, ctx, torch.from_numpy(perms).cuda())
+        assert_parity(got_k, ref, pb)
+    ctx.debug_set(whp.DEBUG_K1_WARPS, -1)
     # batch_of_pos alone stays on the tuned path (derived from K1's boundary mask)
     bop = torch.full((n_cand, pb.n_orders), -1, dtype=torch.int32, device="cuda")
     d2 = torch.zeros(n_cand, dtype=torch.int64, device="cuda")
