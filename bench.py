@@ -418,11 +418,12 @@ def run_ours(args):
         # ---- NEXT-2, second half: return / largest-gap routing of the same plans ---------------
         nexts["routing"] = {"what": "whp_eval_routing on the same 16,384 plans (readings N5, N6): "
                                     "D and J with the carts routed by the policy"}
+        r_obj = torch.zeros(n_cand, dtype=torch.float64, device=dev)
         for pol, pname in ((whp.ROUTE_RETURN, "return"), (whp.ROUTE_LARGEST_GAP, "largest_gap")):
-            ctx.eval_routing(perms, pol, leg, obj)
+            ctx.eval_routing(perms, pol, leg, r_obj)
             torch.cuda.synchronize()
             ev0.record()
-            ctx.eval_routing(perms, pol, leg, obj)
+            ctx.eval_routing(perms, pol, leg, r_obj)
             ev1.record()
             torch.cuda.synchronize()
             r_ms = ev0.elapsed_time(ev1)
