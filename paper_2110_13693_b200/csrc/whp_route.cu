@@ -6,9 +6,10 @@
 // Both policies need more than the S-shape's (number of aisles, deepest pick of the last aisle):
 // return needs the deepest pick of EVERY visited aisle, largest gap every distinct depth of every
 // aisle strictly between the first and the last. The table kept per open cart is therefore the
-// list of its picks' (aisle, depth) keys — at most C entries, in shared memory — sorted at the
-// cart's close: in registers by a 32-lane bitonic network of shuffles when C <= 32 (every config
-// of BASELINE.json but the stress one), else by a bitonic network over the shared-memory list.
+// list of its picks' (aisle, depth) keys — at most C entries — sorted at the cart's close: when
+// C <= 32 (every config of BASELINE.json but the stress one) the keys live one per lane in
+// registers and a 32-lane bitonic network of shuffles sorts them (whp_route32_kernel); else the
+// list sits in shared memory and a bitonic network runs over it (whp_route_kernel).
 // In sorted order an aisle is a run of equal high bits; its deepest pick is the run's last key and
 // its gaps are differences of neighbours.
 //
@@ -211,6 +212,142 @@ whp_route_kernel(const whp_tables T, const int32_t* __restrict__ perms, int64_t 
   }
 }
 
+
+// ---------------------------------------------------------------------- carts of up to 32 picks
+// C <= 32 (every configuration of BASELINE.json but the stress one): the open cart's keys never
+// leave the registers. A tile part's picks are flattened over the lanes (item i of the part
+// belongs to the last position whose item prefix is <= i: a five-step search by shuffles, then
+// one pick load per lane), lane t of the cart holds key t; at the close the 32-lane bitonic
+// network sorts them, runs of equal aisles are found by comparing neighbours (shuffles), the
+// largest gap of a run by a segmented max-scan, and the cart's distinct classes by match_any
+// (one leader per class bumps r_k). No shared memory but the r_k counters.
+// len_t: int32_t when every per-cart quantity provably fits 31 bits (host check), else int64_t.
+template <int POLICY, typename len_t>
+__global__ void __launch_bounds__(kRouteWarps * 32)
+whp_route32_kernel(const whp_tables T, const int32_t* __restrict__ perms, int64_t n_cand,
+                   int64_t* __restrict__ dist_out, double* __restrict__ obj_out) {
+  __shared__ int32_t r_all[kRouteWarps][WHP_MAX_CLASSES];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  int32_t* r = r_all[warp];
+  const len_t A = (len_t)T.g.aisle_len, pitch = (len_t)T.g.slot_pitch;
+  const int64_t a0 = T.g.depot_aisle;
+  for (int64_t cand = (int64_t)blockIdx.x * kRouteWarps + warp; cand < n_cand;
+       cand += (int64_t)gridDim.x * kRouteWarps) {
+    for (int k = lane; k < T.K; k += 32) r[k] = 0;
+    __syncwarp();
+    const int32_t* row = perms + cand * T.n_orders;
+    int32_t load = 0, nkeys = 0;
+    uint32_t key = kPadKey, cls = 0;  // this lane's pick of the open cart (lane < nkeys)
+    int64_t D = 0;
+
+    auto close_cart = [&]() {
+      __syncwarp();  // the previous cart's r_k updates (other lanes) are done
+      const int n = nkeys;
+      const bool mine = lane < n;
+      // D5: one leader per distinct class of the cart
+      const uint32_t act = __ballot_sync(WHP_FULL, mine);
+      if (mine) {
+        const uint32_t same = __match_any_sync(act, cls);
+        if ((int)(__ffs(same) - 1) == lane) r[cls] += 1;
+      }
+      // D3 on sorted keys
+      const uint32_t sk = sort32(key);
+      const int32_t a = (int32_t)(sk >> 12);
+      const len_t y = (len_t)(sk & 0xfffu) * pitch;
+      const uint32_t up = __shfl_up_sync(WHP_FULL, sk, 1), dn = __shfl_down_sync(WHP_FULL, sk, 1);
+      const bool first = mine && (lane == 0 || (int32_t)(up >> 12) != a);
+      const bool last = mine && (lane == n - 1 || (int32_t)(dn >> 12) != a);
+      const int32_t a_min = __shfl_sync(WHP_FULL, a, 0), a_max = __shfl_sync(WHP_FULL, a, n - 1);
+      const int64_t H = (int64_t)T.g.aisle_spacing *
+                        (llabs(a0 - a_min) + ((int64_t)a_max - a_min) + llabs((int64_t)a_max - a0));
+      len_t part = 0;
+      if (POLICY == 1 || a_min == a_max) {
+        if (last) part = 2 * y;  // deepest pick of every visited aisle
+      } else {
+        // largest gap of every run: front cross-aisle -> first pick, between neighbours, and
+        // (at the run's last key) deepest pick -> back cross-aisle; segmented max-scan
+        const len_t yup = (len_t)(up & 0xfffu) * pitch;
+        len_t g = mine ? (first ? y : y - yup) : 0;
+        if (last) g = max(g, A - y);
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          const len_t og = __shfl_up_sync(WHP_FULL, g, d);
+          const int32_t oa = __shfl_up_sync(WHP_FULL, a, d);
+          if (lane >= d && oa == a) g = max(g, og);
+        }
+        if (last && a != a_min && a != a_max) part = 2 * (A - g);
+        if (lane == 0) part += 2 * A;  // first and last visited aisle, traversed completely
+      }
+#pragma unroll
+      for (int o = 16; o >= 1; o >>= 1) part += __shfl_xor_sync(WHP_FULL, part, o);
+      D += H + (int64_t)part;
+      key = kPadKey;
+      nkeys = 0;
+    };
+
+    for (int32_t tile = 0; tile < T.n_orders; tile += 32) {
+      const int32_t pos = tile + lane;
+      const int nvalid = min(32, T.n_orders - tile);
+      const bool valid = lane < nvalid;
+      uint32_t orec = 0;
+      if (valid) orec = __ldg(T.order_rec + __ldg(row + pos));
+      const int32_t q = valid ? (int32_t)(orec & WHP_Q_MASK) : 0;
+      const int32_t incl = whp_warp_incl_scan(q);
+      const int32_t excl = incl - q;
+      int32_t cur = -load;
+      uint32_t starts = (load == 0) ? 1u : 0u;
+      int from = (load == 0) ? 1 : 0;
+      while (from < 32) {
+        const uint32_t viol =
+            __ballot_sync(WHP_FULL, valid && (incl - cur > T.C)) & (WHP_FULL << from);
+        if (!viol) break;
+        const int p = __ffs(viol) - 1;
+        starts |= 1u << p;
+        cur = __shfl_sync(WHP_FULL, excl, p);
+        from = p + 1;
+      }
+      int lo = 0;
+      while (lo < nvalid) {
+        if ((starts >> lo) & 1u) {
+          if (load > 0 || lo > 0) close_cart();
+        }
+        const uint32_t rest = (lo + 1 < 32) ? (starts & (WHP_FULL << (lo + 1))) : 0u;
+        const int hi = rest ? min(__ffs(rest) - 1, nvalid) : nvalid;
+        const int32_t excl_lo = __shfl_sync(WHP_FULL, excl, lo);
+        const int32_t items = __shfl_sync(WHP_FULL, incl, hi - 1) - excl_lo;
+        // item i = lane - nkeys of this part: its position j in [lo, hi) is the last one with
+        // excl_j - excl_lo <= i (excl ascends over the lanes)
+        const int32_t i = lane - nkeys;
+        int j = lo;
+#pragma unroll
+        for (int step = 16; step >= 1; step >>= 1) {
+          const int jj = j + step;
+          const int32_t e = __shfl_sync(WHP_FULL, excl, jj & 31);
+          if (jj < hi && e - excl_lo <= i) j = jj;
+        }
+        const uint32_t orec_j = __shfl_sync(WHP_FULL, orec, j);
+        const int32_t excl_j = __shfl_sync(WHP_FULL, excl, j);
+        if (i >= 0 && i < items) {
+          const uint32_t pr = __ldg(T.pick_rec + (orec_j >> WHP_Q_BITS) + (i - (excl_j - excl_lo)));
+          key = pr >> WHP_PICK_SLOT_SHIFT;  // aisle << 12 | slot1
+          cls = pr & WHP_PICK_CLASS_MASK;
+        }
+        nkeys += items;
+        lo = hi;
+      }
+      load = nkeys;
+    }
+    if (load > 0) close_cart();
+    __syncwarp();
+    const double phi = whp_penalty(T, r);
+    if (lane == 0) {
+      if (dist_out) dist_out[cand] = D;
+      if (obj_out) obj_out[cand] = __dadd_rn((double)D, phi);
+    }
+    __syncwarp();
+  }
+}
+
 }  // namespace
 
 cudaError_t whp_launch_route(whp_ctx* c, const int32_t* d_perms, int64_t n_cand, int32_t policy,
@@ -232,7 +369,19 @@ cudaError_t whp_launch_route(whp_ctx* c, const int32_t* d_perms, int64_t n_cand,
     whp_route_kernel<POL, REG><<<(unsigned)blocks, kRouteWarps * 32, smem, st>>>(                \
         T, d_perms, n_cand, p2max, d_dist, d_obj);                                               \
   } while (0)
-  if (policy == WHP_ROUTE_RETURN) {
+  if (reg_sort && !c->dbg_force_general) {  // carts of up to 32 picks: keys stay in registers
+    // a cart's vertical travel is at most 2 A per pick (+ 2 A): 32-bit lengths when that fits
+    const bool fits32 = 68ll * c->g.aisle_len < (1ll << 31);
+#define WHP_LAUNCH_ROUTE32(POL, LEN)                                                             \
+  whp_route32_kernel<POL, LEN><<<(unsigned)blocks, kRouteWarps * 32, 0, st>>>(T, d_perms, n_cand, \
+                                                                             d_dist, d_obj)
+    if (policy == WHP_ROUTE_RETURN) {
+      if (fits32) WHP_LAUNCH_ROUTE32(1, int32_t); else WHP_LAUNCH_ROUTE32(1, int64_t);
+    } else {
+      if (fits32) WHP_LAUNCH_ROUTE32(2, int32_t); else WHP_LAUNCH_ROUTE32(2, int64_t);
+    }
+#undef WHP_LAUNCH_ROUTE32
+  } else if (policy == WHP_ROUTE_RETURN) {
     if (reg_sort) WHP_LAUNCH_ROUTE(1, true); else WHP_LAUNCH_ROUTE(1, false);
   } else {
     if (reg_sort) WHP_LAUNCH_ROUTE(2, true); else WHP_LAUNCH_ROUTE(2, false);

@@ -33,14 +33,20 @@ def gpu_routing(torch, ctx, perms_dev, policy):
     return d.cpu().numpy(), o.cpu().numpy()
 
 
-def check(torch, ctx, pb, perms, policies=(0, 1, 2)):
+def check(torch, ctx, pb, perms, policies=(0, 1, 2), both_kernels=True):
+    """Carts of up to 32 picks run the register-resident kernel; `force general` selects the
+    shared-memory-list kernel (the only one for larger carts), so both are checked."""
+    from paper_2110_13693_b200 import whp
     dev = torch.from_numpy(perms).cuda()
     for pol in policies:
-        d, o = gpu_routing(torch, ctx, dev, pol)
         ref = oracle.eval_routing(pb, perms, pol, threads=CORES)
-        bad = np.flatnonzero((d != ref["dist"]) | (o != ref["obj"]))
-        assert bad.size == 0, f"policy {pol}: {bad.size} plans differ, first {bad[:5]}"
-        assert np.all(np.abs(o - ref["obj"]) <= 1e-9 * np.abs(ref["obj"]))
+        for general in ((0, 1) if both_kernels else (0,)):
+            ctx.debug_set(whp.DEBUG_FORCE_GENERAL, general)
+            d, o = gpu_routing(torch, ctx, dev, pol)
+            ctx.debug_set(whp.DEBUG_FORCE_GENERAL, -1)
+            bad = np.flatnonzero((d != ref["dist"]) | (o != ref["obj"]))
+            assert bad.size == 0, f"policy {pol} general {general}: {bad.size} plans differ, first {bad[:5]}"
+            assert np.all(np.abs(o - ref["obj"]) <= 1e-9 * np.abs(ref["obj"]))
 
 
 @pytest.mark.parametrize("name", ["tiny", "mid"])
@@ -104,6 +110,7 @@ ROUTE_EDGE = [
     dict(NA=8, S=12, K=40, n_skus=100, n_orders=129, qmax=5, C=70),        # many picks per aisle
     dict(NA=5, S=9, K=3, n_skus=30, n_orders=32, qmax=4, C=1000),          # one cart holds all
     dict(NA=12, S=100, K=9, n_skus=1100, n_orders=300, qmax=20, C=1024, depot=6),
+    dict(NA=20, S=50, K=9, n_skus=300, n_orders=100, qmax=5, C=20, pitch=1000000, spacing=7),  # 64-bit cart lengths
 ]
 
 
