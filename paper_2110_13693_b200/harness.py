@@ -176,17 +176,19 @@ def algorithmic_bytes_per_candidate(n_orders: int, n_items: int) -> dict:
 
 
 # ---- ncu counters recorded for a given state of the kernels --------------------------------------
+EVAL_PATH_SOURCES = ("whp_fast.cu", "whp_eval.cu", "whp_walk.cuh", "whp_internal.cuh")
+
+
 def csrc_sha16(repo_root: str) -> str:
-    """Fingerprint of the kernel sources (csrc/*.cu, *.cuh + include/whp.h): counters captured
-    under ncu are only quoted next to a live timing when they were captured on these sources."""
+    """Fingerprint of the sources of the candidate-evaluation kernels (K1, segments, K2, K3 and
+    their launcher): counters captured under ncu are only quoted next to a live timing when they
+    were captured on these sources."""
     import hashlib
     h = hashlib.sha256()
     csrc = os.path.join(repo_root, "paper_2110_13693_b200", "csrc")
-    files = sorted(os.path.join(csrc, f) for f in os.listdir(csrc) if f.endswith((".cu", ".cuh")))
-    files.append(os.path.join(repo_root, "include", "whp.h"))
-    for path in files:
-        with open(path, "rb") as f:
-            h.update(os.path.basename(path).encode() + b"\0" + f.read())
+    for name in EVAL_PATH_SOURCES:
+        with open(os.path.join(csrc, name), "rb") as f:
+            h.update(name.encode() + b"\0" + f.read())
     return h.hexdigest()[:16]
 
 
