@@ -45,9 +45,6 @@ __device__ __forceinline__ int4 lds128(uint32_t a) {
 __device__ __forceinline__ void sts32(uint32_t a, uint32_t v) {
   asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v));
 }
-__device__ __forceinline__ void sts128(uint32_t a, uint4 v) {
-  asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w));
-}
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src));
 }
@@ -153,9 +150,8 @@ __device__ __forceinline__ void gather_word(uint32_t (&r)[32], uint32_t row, uin
 
 // The next-fit recurrence over one word, on room = C - load:  room' = umin(room - q, C - q)
 // (room < q wraps room - q above C - q: a new batch opens) — ONE dependent instruction per
-// position (a fused add-min); everything else hangs off the chain: e = q - 1 - room is
-// non-negative exactly when a batch opens, and a funnel shift collects the 32 sign bits, first
-// position last. Writes the 16-bit cursors (bits 8..23 of the order records) of the first n4
+// position (a fused add-min); everything else hangs off the chain: d = room - q is negative
+// exactly when a batch opens, and a funnel shift collects the 32 sign bits, first position last. Writes the 16-bit cursors (bits 8..23 of the order records) of the first n4
 // groups of four positions.
 // TILE: the cursors go to this lane's 128-byte row of a shared-memory tile (two words per
 // row, 16-byte chunk c at c ^ (lane & 7)) that a TMA tile store writes out; otherwise straight
@@ -172,8 +168,8 @@ __device__ __forceinline__ uint32_t recur_word(const uint32_t (&r)[32], uint32_t
     // use up to the loads (it would stall on the shared-memory latency there)
     asm volatile("" : "+r"(ri));
     const uint32_t q = ri & WHP_Q_MASK;
-    const uint32_t e = q - room - 1u;  // sign bit clear <=> room < q
-    rev = __funnelshift_l(e, rev, 1);  // (rev << 1) | (e >> 31)
+    const uint32_t d = room - q;       // wraps (sign bit set) <=> room < q: a batch opens here
+    rev = __funnelshift_l(d, rev, 1);  // (rev << 1) | (d >> 31)
     room = min(room + (0u - q), C - q);
   }
 #pragma unroll
@@ -191,7 +187,7 @@ __device__ __forceinline__ uint32_t recur_word(const uint32_t (&r)[32], uint32_t
       }
     }
   }
-  return ~__brev(rev);
+  return __brev(rev);
 }
 
 // kWarps: warps per block, they share the order table (a warp = 32 plans). U16: the plan matrix
@@ -1057,6 +1053,9 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const void* d_perms, i
                                               bool perm16 = false) {
   const int32_t bm_pitch = fast_bm_pitch(c), cs_pitch = fast_cs_pitch(c), ss_pitch = kSsPitch;
   {
+    // (Folding this reset into the segments kernel saves 1 us of the evaluation alone and costs
+    // 13 us of bench.py's two-stream step: K1 then reaches the SMs before the other stream's
+    // one-block base kernel, whose 92 KB of shared memory no longer fit beside K1's blocks.)
     cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
     const int kw1 = bounds_warps(c);
