@@ -89,3 +89,47 @@ def test_bench_reference_arm_prints_one_json_line():
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle"
     assert line["value"] > 0 and line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_ncu_counters_are_quoted_only_for_the_sources_they_were_captured_on(tmp_path):
+    """bench.py prints roofline.traffic / binding_resource from profiles/ncu_counters.csv only while
+    the evaluation-path sources hash to the fingerprint stored beside the counters."""
+    import shutil
+    root = tmp_path / "repo"
+    csrc = root / "paper_2110_13693_b200" / "csrc"
+    csrc.mkdir(parents=True)
+    (root / "profiles").mkdir()
+    for name in harness.EVAL_PATH_SOURCES:
+        shutil.copy(os.path.join(ROOT, "paper_2110_13693_b200", "csrc", name), csrc / name)
+    sha = harness.csrc_sha16(str(root))
+    assert sha == harness.csrc_sha16(ROOT) and len(sha) == 16
+    (root / "profiles" / "ncu_counters.csv").write_text(
+        "csrc_sha16,workload,counter,value,source\n# comment\n"
+        f"{sha},paper,dram_bytes,521.0e6,profiles/x.md\n{sha},paper,warp_inst,2.5e8,profiles/x.md\n"
+        "0123456789abcdef,paper,dram_bytes,1.0,profiles/old.md\n")
+    c = harness.ncu_counters(str(root))
+    assert c["paper"]["dram_bytes"] == 521.0e6 and c["paper"]["warp_inst"] == 2.5e8
+    assert c["paper"]["source"] == "profiles/x.md" and not c["stale"]
+    with open(csrc / "whp_fast.cu", "a") as f:
+        f.write("// edited\n")
+    c2 = harness.ncu_counters(str(root))
+    assert "paper" not in c2 and c2["stale"] and c2["csrc_sha16"] != sha
+    os.remove(root / "profiles" / "ncu_counters.csv")
+    c3 = harness.ncu_counters(str(root))
+    assert "paper" not in c3 and not c3["stale"]
+
+
+def test_binding_constants_match_the_header():
+    """whp.py mirrors the enums of include/whp.h by value."""
+    import re
+    from paper_2110_13693_b200 import whp
+    text = open(os.path.join(ROOT, "include", "whp.h")).read()
+    enums = dict((k, int(v)) for k, v in re.findall(r"\b(WHP_[A-Z0-9_]+)\s*=\s*(\d+)", text))
+    for name, value in enums.items():
+        if name.startswith("WHP_DEBUG_"):
+            assert getattr(whp, name[4:]) == value, name
+        elif name.startswith("WHP_ROUTE_"):
+            assert getattr(whp, name[4:]) == value, name
+        elif name.startswith("WHP_ERR_") or name == "WHP_OK":
+            assert getattr(whp, name[4:]) == value, name
+    assert enums["WHP_DEBUG_K1_WARPS"] == 4 and enums["WHP_ROUTE_LARGEST_GAP"] == 2
