@@ -715,3 +715,67 @@ def test_host16_needs_a_tuned_path_shape(torch_cuda):
     ctx.eval_candidates_host(perms, d)  # the int32 call takes any shape
     assert np.array_equal(d, oracle.eval_candidates(pb, perms)["dist"])
     ctx.close()
+
+
+def test_host_entry_point_in_several_passes(torch_cuda):
+    """More than 1 GiB of plans: whp_eval_candidates_host stages them in several passes through one
+    buffer (the copy stream waits for the previous pass to be evaluated). 600,000 mid-scale plans
+    (1.2 GB of int32 ids): argmin and sampled rows against the oracle, every row against the
+    device-resident call."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    wl = W.make_workload("mid")
+    pb = wl.problem
+    n, n_cand = pb.n_orders, 600_000
+    ctx = whp.Context.from_problem(pb)
+    perms_dev = torch.empty((n_cand, n), dtype=torch.int32, device="cuda")
+    for lo in range(0, n_cand, 100_000):
+        perms_dev[lo:lo + 100_000] = W.perms_torch(wl.seed, n, lo, lo + 100_000, "cuda")
+    d_dev = torch.zeros(n_cand, dtype=torch.int64, device="cuda")
+    o_dev = torch.zeros(n_cand, dtype=torch.float64, device="cuda")
+    i_dev = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ctx.eval_candidates(perms_dev, dist=d_dev, obj=o_dev)
+    ctx.argmin(o_dev, i_dev)
+    h = perms_dev.cpu().numpy()
+    assert h.nbytes > (1 << 30)
+    d, o = np.zeros(n_cand, np.int64), np.zeros(n_cand, np.float64)
+    i, v = ctx.eval_candidates_host(h, d, o)
+    assert np.array_equal(d, d_dev.cpu().numpy()) and np.array_equal(o, o_dev.cpu().numpy())
+    assert i == int(i_dev.item())
+    rows = np.unique(np.concatenate([[0, 1, n_cand - 1, 536_870, 536_871],  # around the pass boundary
+                                     (W.stream_u64(3, 5, 300) % np.uint64(n_cand)).astype(np.int64)]))
+    ref = oracle.eval_candidates(pb, h[rows])
+    assert np.array_equal(d[rows], ref["dist"]) and np.array_equal(o[rows], ref["obj"])
+    assert np.array_equal(h[rows], W.perm_rows(wl.seed, n, rows))
+    one = oracle.eval_candidates(pb, h[i])
+    assert one["obj"][0] == v
+    # the 16-bit call takes one pass for the same plans (1.2 GB / 2)
+    d16, o16 = np.zeros(n_cand, np.int64), np.zeros(n_cand, np.float64)
+    i16, v16 = ctx.eval_candidates_host(h.astype(np.uint16), d16, o16)
+    assert np.array_equal(d16, d) and np.array_equal(o16, o) and i16 == i and v16 == v
+    ctx.close()
+
+
+def test_routing_and_host_calls_under_cuda_graph_rules(torch_cuda):
+    """whp_eval_routing is capturable after one eager call (it allocates nothing); a replay gives
+    the oracle's values."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = W.make_problem("mid")
+    perms_np = W.perm_rows(2, pb.n_orders, np.arange(200))
+    perms = torch.from_numpy(perms_np).cuda()
+    ctx = whp.Context.from_problem(pb)
+    d = torch.zeros(200, dtype=torch.int64, device="cuda")
+    o = torch.zeros(200, dtype=torch.float64, device="cuda")
+    ctx.eval_routing(perms, whp.ROUTE_LARGEST_GAP, d, o)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=torch.cuda.Stream()):
+        ctx.eval_routing(perms, whp.ROUTE_LARGEST_GAP, d, o)
+    d.zero_(), o.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    ref = oracle.eval_routing(pb, perms_np, oracle.LARGEST_GAP)
+    assert np.array_equal(d.cpu().numpy(), ref["dist"]) and np.array_equal(o.cpu().numpy(), ref["obj"])
+    del g
+    ctx.close()
