@@ -136,6 +136,31 @@ whp_status whp_eval_swaps(whp_ctx* ctx, const int32_t* d_base_perm, int32_t win_
 whp_status whp_argmin(whp_ctx* ctx, const double* d_obj, int64_t n, int64_t* d_idx,
                       double* d_val, void* cuda_stream);
 
+/* a7 (D7) again, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it): the ONE entry point that allocates nothing — no
+ * context (creating one allocates), no cudaMalloc / cudaFree / allocating library routine, only a
+ * 4-byte cudaMemsetAsync and one kernel on cuda_stream of the CURRENT device. Same result as
+ * whp_argmin: *d_idx = index of the minimum of d_obj[0..n) (DEVICE double), ties -> lowest
+ * index; *d_val (nullable) its value. d_idx int64*, d_val double* are DEVICE scalars.
+ *   - The per-block partial results live in a static __device__ array of
+ *     WHP_ARGMIN_STATIC_SCRATCH_BYTES that every GPU loading the library holds until exit; it has
+ *     room for 4096 blocks of 4096 values, so n <= WHP_ARGMIN_STATIC_MAX_N. A larger n returns
+ *     WHP_ERR_OUT_OF_RANGE (nothing is launched; use whp_argmin); n < 1 or a null d_obj / d_idx
+ *     WHP_ERR_INVALID_ARG; a failing CUDA call WHP_ERR_CUDA. Text: whp_static_last_error().
+ *   - ALL calls on a device share that array. Calls ordered on one stream (or otherwise
+ *     serialised) are fine — the array is re-initialised by every call; calls that OVERLAP on the
+ *     GPU (different streams, no dependency) race on it and return garbage.
+ *   - whp_argmin_static_setup() resolves the array's device address for the current device
+ *     (cudaGetSymbolAddress, once per device). whp_argmin_static does the same on its first call
+ *     per device; call the set-up beforehand when that first call would fall inside a stream
+ *     capture. Device ordinals 0..63. */
+#define WHP_ARGMIN_STATIC_MAX_N 16777216LL      /* 4096 blocks x 4096 values */
+#define WHP_ARGMIN_STATIC_SCRATCH_BYTES 65792   /* 4096 x 16 B pairs + a 256 B ticket line */
+whp_status whp_argmin_static_setup(void);
+whp_status whp_argmin_static(const double* d_obj, int64_t n, int64_t* d_idx, double* d_val,
+                             void* cuda_stream);
+const char* whp_static_last_error(void); /* of the calling thread's latest *_static call; "" when none */
+
 /* D8 trajectory step: decode neighbour *d_idx (DEVICE int64, as written by whp_argmin over
  * a whp_eval_swaps result with the same window) and exchange the two positions of
  * d_base_perm in place, on the device, so a search loop needs no host round trip. */

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libwhp.so")
-SOURCES = ["whp_api.cu", "whp_eval.cu", "whp_fast.cu", "whp_swaps.cu", "whp_argmin.cu", "whp_nhatc.cu", "whp_legsum.cu", "whp_kmeans.cu", "whp_route.cu"]
+SOURCES = ["whp_api.cu", "whp_eval.cu", "whp_fast.cu", "whp_swaps.cu", "whp_argmin.cu", "whp_nhatc.cu", "whp_legsum.cu", "whp_kmeans.cu", "whp_route.cu", "whp_static.cu"]
 HEADERS = ["whp_internal.cuh", "whp_walk.cuh", os.path.join("..", "..", "include", "whp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--fmad=false",  # D6: every fp64 product and sum individually rounded

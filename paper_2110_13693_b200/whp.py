@@ -25,10 +25,12 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_version", "whp_nhatc_update", "whp_nhatc_solve", "whp_get_penalty",
            "whp_eval_legsum", "whp_kmeans_slotting", "whp_eval_moves", "whp_apply_move",
            "whp_probe_l2_read", "whp_max_batches", "whp_set_swap_stats", "whp_get_swap_stats",
-           "whp_debug_set", "whp_eval_routing", "whp_eval_candidates_host16"]
+           "whp_debug_set", "whp_eval_routing", "whp_eval_candidates_host16",
+           "whp_argmin_static_setup", "whp_argmin_static", "whp_static_last_error"]
 
 ROUTE_S_SHAPE, ROUTE_RETURN, ROUTE_LARGEST_GAP = range(3)
 DEBUG_FORCE_GENERAL, DEBUG_SEGMENTS, DEBUG_WARPS, DEBUG_SWAP_MARGIN, DEBUG_K1_WARPS = range(5)
+ARGMIN_STATIC_MAX_N = 4096 * 4096  # WHP_ARGMIN_STATIC_MAX_N
 
 
 class WhpError(RuntimeError):
@@ -78,6 +80,10 @@ def lib():
         L.whp_last_error.argtypes = [vp]
         L.whp_last_error.restype = C.c_char_p
         L.whp_version.restype = C.c_char_p
+        L.whp_argmin_static_setup.argtypes = []
+        L.whp_argmin_static.argtypes = [vp, i64, vp, vp, vp]
+        L.whp_static_last_error.argtypes = []
+        L.whp_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -364,6 +370,29 @@ def kmeans_slotting(n_aisles, slots_per_side, depot_aisle, n_skus, item_sku, k, 
     if st != OK:
         raise WhpError(st, "whp_kmeans_slotting")
     return out
+
+
+def _check_static(st):
+    if st != OK:
+        raise WhpError(st, lib().whp_static_last_error().decode())
+
+
+def argmin_static_setup():
+    """whp_argmin_static_setup: resolve the static scratch's address on torch's current device
+    (once per device; needed beforehand only when the first whp_argmin_static would be captured)."""
+    _check_static(lib().whp_argmin_static_setup())
+
+
+def argmin_static(obj, idx, val=None, n=None, stream=None):
+    """whp_argmin_static: D7 without a context and without any allocation, n <=
+    ARGMIN_STATIC_MAX_N; the tensors must live on torch's current device. Calls that overlap on
+    the GPU race on the shared static scratch."""
+    import torch
+    n = obj.numel() if n is None else n
+    dv = torch.cuda.current_device()
+    _check_static(lib().whp_argmin_static(_d(obj, torch.float64, n, dv), n,
+                                          _d(idx, torch.int64, 1, dv),
+                                          _d(val, torch.float64, 1, dv), _stream(stream)))
 
 
 def version() -> str:
