@@ -227,126 +227,176 @@ __device__ __forceinline__ V block_excl_scan(V x, V* ws, V& total) {
   return ws[warp] + incl - x;
 }
 
+// Segment table of the boundary search (phase C below): the plan is cut into n_seg segments of
+// seg_len >= C positions; a batch spans at most C positions, so the first batch start at or after
+// a segment's first position is one of its first C positions.
+constexpr int kMaxSegEntries = 8192;
+
+// SMEM: pre / nxt / mark live in shared memory (and pre, nxt are copied out for the later
+// kernels); otherwise they are the global tables themselves (mark = B.bop before it is ranked).
+template <bool SMEM>
 __global__ void __launch_bounds__(kBaseThreads)
 whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
-                      const whp_base_tables B, int smem_tables) {
+                      const whp_base_tables B, int32_t seg_len, int32_t n_seg) {
   extern __shared__ __align__(16) uint8_t dyn[];
   __shared__ int32_t s_scan32[33];
-  __shared__ int32_t s_nb;
   const int tid = threadIdx.x;
-  const int32_t n = T.n_orders;
-  // item-count prefix and "next batch start" tables: shared memory when they fit
-  int32_t* pre = smem_tables ? reinterpret_cast<int32_t*>(dyn) : B.pre;
-  int32_t* nxt = smem_tables ? reinterpret_cast<int32_t*>(dyn) + (n + 1) : B.nxt;
+  const int32_t n = T.n_orders, C = T.C;
+  const int32_t n4 = (n + 4) & ~3;  // >= n + 1, a multiple of four (16-byte rows)
+  int32_t* pre = SMEM ? reinterpret_cast<int32_t*>(dyn) : B.pre;
+  int32_t* nxt = SMEM ? reinterpret_cast<int32_t*>(dyn) + n4 : B.nxt;
+  int32_t* mark = SMEM ? reinterpret_cast<int32_t*>(dyn) + 2 * n4 : B.bop;
+  int32_t* seg_exit = reinterpret_cast<int32_t*>(dyn) + (SMEM ? 3 * n4 : 0);  // [n_seg][C]
+  int32_t* seg_entry = seg_exit + (n_seg > 0 ? n_seg * C : 0);                // [n_seg]
 
   // ---- A: order record of every position; exclusive prefix of the item counts (four
   // consecutive positions per thread: the dependent global loads of a round overlap)
+  const bool vec = (reinterpret_cast<uintptr_t>(base_perm) & 15u) == 0;
   int32_t carry = 0;
   for (int32_t p0 = 0; p0 < n; p0 += 4 * kBaseThreads) {
     const int32_t pb = p0 + 4 * tid;
-    uint32_t orec[4];
+    const bool full = pb + 3 < n;
+    uint32_t orec[4] = {0u, 0u, 0u, 0u};
+    if (full && vec) {
+      const int4 o = __ldg(reinterpret_cast<const int4*>(base_perm + pb));
+      orec[0] = __ldg(T.order_rec + o.x); orec[1] = __ldg(T.order_rec + o.y);
+      orec[2] = __ldg(T.order_rec + o.z); orec[3] = __ldg(T.order_rec + o.w);
+    } else {
 #pragma unroll
-    for (int k = 0; k < 4; ++k) orec[k] = (pb + k < n) ? __ldg(T.order_rec + __ldg(base_perm + pb + k)) : 0u;
+      for (int k = 0; k < 4; ++k)
+        if (pb + k < n) orec[k] = __ldg(T.order_rec + __ldg(base_perm + pb + k));
+    }
     int32_t qs[4], sum = 0;
 #pragma unroll
     for (int k = 0; k < 4; ++k) { qs[k] = sum; sum += (int32_t)(orec[k] & WHP_Q_MASK); }
     int32_t tot;
-    const int32_t ex = block_excl_scan<int32_t>(sum, s_scan32, tot);
+    const int32_t ex = carry + block_excl_scan<int32_t>(sum, s_scan32, tot);
+    if (full) {
+      const int4 pv = make_int4(ex + qs[0], ex + qs[1], ex + qs[2], ex + qs[3]);
+      *reinterpret_cast<uint4*>(B.orec + pb) = make_uint4(orec[0], orec[1], orec[2], orec[3]);
+      *reinterpret_cast<int4*>(B.pre + pb) = pv;
+      if (SMEM) *reinterpret_cast<int4*>(pre + pb) = pv;
+    } else {
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
-      if (pb + k < n) {
-        B.orec[pb + k] = orec[k];
-        pre[pb + k] = carry + ex + qs[k];
-        if (smem_tables) B.pre[pb + k] = carry + ex + qs[k];
-      }
+      for (int k = 0; k < 4; ++k)
+        if (pb + k < n) {
+          B.orec[pb + k] = orec[k];
+          B.pre[pb + k] = ex + qs[k];
+          if (SMEM) pre[pb + k] = ex + qs[k];
+        }
+    }
     carry += tot;
   }
-  if (tid == 0) { pre[n] = carry; B.pre[n] = carry; }
+  if (tid == 0) { pre[n] = carry; if (SMEM) B.pre[n] = carry; }
   __syncthreads();
 
-  // ---- B: nxt[p] = where the batch that opens at p ends (binary search in p+1 .. p+C)
-  for (int32_t p = tid; p < n; p += kBaseThreads) {
-    const int32_t lim = pre[p] + T.C;
-    int32_t lo = p + 1, hi = min(n, p + T.C);  // pre[lo] <= lim always (q <= C)
+  // ---- B: nxt[p] = where the batch that opens at p ends: the largest e <= min(n, p + C) with
+  // pre[e] <= pre[p] + C (q <= C, so e >= p + 1). A binary search for the first of a thread's four
+  // positions; nxt is monotone, so the others advance from their predecessor's answer.
+  for (int32_t p0 = 0; p0 < n; p0 += 4 * kBaseThreads) {
+    const int32_t pb = p0 + 4 * tid;
+    if (pb >= n) break;
+    int32_t nx[4] = {0, 0, 0, 0};
+    int32_t lim = pre[pb] + C;
+    int32_t lo = pb + 1, hi = min(n, pb + C);
     while (lo < hi) {
       const int32_t mid = (lo + hi + 1) >> 1;
       if (pre[mid] <= lim) lo = mid; else hi = mid - 1;
     }
-    nxt[p] = lo;
-    if (smem_tables) B.nxt[p] = lo;
-  }
-  __syncthreads();
-
-  // ---- C: the base boundaries = the positions reachable from 0 along nxt
-  if (smem_tables == 2) {
-    // pointer doubling: after round k, J = nxt^(2^(k+1)) and the marked positions are those at
-    // fewer than 2^(k+1) hops from 0; then a block scan ranks the marks (bstart, bop)
-    int32_t* J0 = reinterpret_cast<int32_t*>(dyn) + (2 * n + 1);
-    int32_t* J1 = J0 + n;
-    int32_t* mark = J1 + n;
-    for (int32_t p = tid; p < n; p += kBaseThreads) { J0[p] = nxt[p]; mark[p] = p == 0; }
-    __syncthreads();
-    int32_t* J = J0;
-    int32_t* Jn = J1;
-    for (;;) {
-      const bool done = J[0] >= n;  // 2^k hops from 0 leave the plan: every start is marked
-      for (int32_t p = tid; p < n; p += kBaseThreads)
-        if (mark[p] == 1) { const int32_t t = J[p]; if (t < n && mark[t] == 0) mark[t] = 2; }
-      __syncthreads();
-      for (int32_t p = tid; p < n; p += kBaseThreads) {
-        if (mark[p] == 2) mark[p] = 1;
-        const int32_t t = J[p];
-        Jn[p] = t < n ? J[t] : n;
-      }
-      __syncthreads();
-      if (done) break;
-      int32_t* tmp = J; J = Jn; Jn = tmp;
-    }
-    int32_t carry_b = 0;
-    for (int32_t p0 = 0; p0 < n; p0 += 4 * kBaseThreads) {  // four positions per thread
-      const int32_t pb = p0 + 4 * tid;
-      int32_t mk[4], before[4], sum = 0;
+    nx[0] = lo;
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        mk[k] = (pb + k < n) ? mark[pb + k] : 0;
-        before[k] = sum;
-        sum += mk[k];
+    for (int k = 1; k < 4; ++k)
+      if (pb + k < n) {
+        lim = pre[pb + k] + C;
+        lo = max(lo, pb + k + 1);
+        hi = min(n, pb + k + C);
+        while (lo < hi && pre[lo + 1] <= lim) ++lo;
+        nx[k] = lo;
       }
-      int32_t tot;
-      const int32_t ex = block_excl_scan<int32_t>(sum, s_scan32, tot);
+    if (pb + 3 < n) {
+      const int4 v = make_int4(nx[0], nx[1], nx[2], nx[3]);
+      *reinterpret_cast<int4*>(B.nxt + pb) = v;
+      if (SMEM) *reinterpret_cast<int4*>(nxt + pb) = v;
+      *reinterpret_cast<int4*>(mark + pb) = make_int4(0, 0, 0, 0);
+    } else {
 #pragma unroll
       for (int k = 0; k < 4; ++k)
         if (pb + k < n) {
-          const int32_t rank = carry_b + ex + before[k];
-          if (mk[k]) B.bstart[rank] = pb + k;
-          B.bop[pb + k] = rank + mk[k] - 1;
+          B.nxt[pb + k] = nx[k];
+          if (SMEM) nxt[pb + k] = nx[k];
+          mark[pb + k] = 0;
         }
-      carry_b += tot;
     }
-    if (tid == 0) { B.bstart[carry_b] = n; s_nb = carry_b; }
-  } else if (tid == 0) {  // one thread chases the boundaries
-    int32_t b = 0;
-    for (int32_t p = 0; p < n; p = nxt[p]) B.bstart[b++] = p;
-    B.bstart[b] = n;
-    s_nb = b;
   }
   __syncthreads();
-  const int32_t nb = s_nb;
-  if (smem_tables != 2)  // the chase left bstart only: batch of every position
-    for (int32_t b = tid; b < nb; b += kBaseThreads)
-      for (int32_t p = B.bstart[b]; p < B.bstart[b + 1]; ++p) B.bop[p] = b;
 
-  if (tid == 0) B.totals[1] = nb;
+  // ---- C: the base boundaries = the positions reachable from 0 along nxt.
+  if (n_seg > 0) {
+    // (1) for every segment s and every one of its first C positions: where a chain that passes
+    //     through that position enters the next segment
+    for (int32_t u = tid; u < n_seg * C; u += kBaseThreads) {
+      const int32_t s = u / C;
+      int32_t p = s * seg_len + (u - s * C);
+      const int32_t lim = min((s + 1) * seg_len, n);
+      while (p < lim) p = nxt[p];
+      seg_exit[u] = p;
+    }
+    __syncthreads();
+    // (2) one thread composes the segments: the first boundary of each
+    if (tid == 0) {
+      int32_t E = 0;
+      for (int32_t s = 0; s < n_seg; ++s) {
+        seg_entry[s] = E;
+        if (E < n) E = seg_exit[s * C + (E - s * seg_len)];
+      }
+    }
+    __syncthreads();
+    // (3) one thread per segment marks its boundaries
+    for (int32_t s = tid; s < n_seg; s += kBaseThreads) {
+      const int32_t lim = min((s + 1) * seg_len, n);
+      for (int32_t p = seg_entry[s]; p < lim; p = nxt[p]) mark[p] = 1;
+    }
+  } else if (tid == 0) {  // a table too large for shared memory: one thread chases the boundaries
+    for (int32_t p = 0; p < n; p = nxt[p]) mark[p] = 1;
+  }
+  __syncthreads();
+  // ---- D: a block scan ranks the marks (bstart[b], bop[p])
+  int32_t carry_b = 0;
+  for (int32_t p0 = 0; p0 < n; p0 += 4 * kBaseThreads) {  // four positions per thread
+    const int32_t pb = p0 + 4 * tid;
+    int32_t mk[4], before[4], sum = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      mk[k] = (pb + k < n) ? mark[pb + k] : 0;
+      before[k] = sum;
+      sum += mk[k];
+    }
+    int32_t tot;
+    const int32_t ex = carry_b + block_excl_scan<int32_t>(sum, s_scan32, tot);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (pb + k < n) {
+        const int32_t rank = ex + before[k];
+        if (mk[k]) B.bstart[rank] = pb + k;
+        B.bop[pb + k] = rank + mk[k] - 1;
+      }
+    carry_b += tot;
+  }
+  if (tid == 0) { B.bstart[carry_b] = n; B.totals[1] = carry_b; }
 }
 
 // Second half of the base pass, after whp_swaps_prep_kernel has scored the base batches
-// (dist_at / cls_at at their start positions). Block w < KW: the class-count prefix rpre[b][k] of
-// the 32 classes of word w, in three steps over chunks of 32 batches — the chunk's visit totals
-// (32 ballots, one warp per chunk), a running sum of the totals over the chunks per class, then
-// a running count inside every chunk with one coalesced row store per batch. Block KW: the
-// prefix of the batch lengths (bdist[nb] = D_base).
-__global__ void __launch_bounds__(kBaseThreads)
-whp_swaps_base2_kernel(const whp_tables T, const whp_base_tables B) {
+// (dist_at / cls_at at their start positions); blocks 0 .. KW of whp_swaps_tail_kernel.
+// Block w < KW: the class-count prefix rpre[b][k] of the 32 classes of word w, over chunks of 32
+// batches: lane j of the chunk's warp gets the ballot of class j over the chunk's batches, a
+// two-level running sum (chunks of a warp, then warps) gives the chunk's offset, and row b of the
+// chunk is offset + popc(ballot below b) — one coalesced row store per batch, no read-modify-write
+// of global memory. Block KW: the prefix of the batch lengths (bdist[nb] = D_base).
+// s_tab: [2 * 32 * chunk_cap + 1024] words of shared memory.
+constexpr int kBase2ChunkCap = 256;  // chunks (of 32 batches) the shared-memory path takes
+
+__device__ __forceinline__ void base2_role(const whp_tables& T, const whp_base_tables& B,
+                                           int32_t* s_tab, int32_t chunk_cap) {
   __shared__ int64_t s_scan64[33];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int32_t nb = (int32_t)B.totals[1];
@@ -368,6 +418,46 @@ whp_swaps_base2_kernel(const whp_tables T, const whp_base_tables B) {
   const bool mine = 32 * w + lane < T.K;
   const int32_t nchunks = (nb + 31) >> 5;
   int32_t* __restrict__ row = B.rpre + 32 * w + lane;
+  if (nchunks <= chunk_cap) {
+    int32_t* s_off = s_tab;                   // [chunk][class]: visits in the warp's chunks before
+    int32_t* s_msk = s_tab + 32 * chunk_cap;  // [chunk][class]: ballot of the class over the chunk
+    int32_t* s_seg = s_tab + 64 * chunk_cap;  // [warp][class]: visits in the warp's chunks
+    const int32_t per = (nchunks + 31) >> 5;  // chunks per warp
+    const int32_t c_lo = min(warp * per, nchunks), c_hi = min(c_lo + per, nchunks);
+    int32_t run = 0;
+    for (int32_t c = c_lo; c < c_hi; ++c) {
+      const int32_t b = 32 * c + lane;
+      const uint32_t word = (b < nb) ? B.cls_at[(int64_t)B.bstart[b] * 8 + w] : 0u;
+      uint32_t m = 0;
+#pragma unroll
+      for (int j = 0; j < 32; ++j) {
+        const uint32_t bal = __ballot_sync(WHP_FULL, (word >> j) & 1u);
+        if (lane == j) m = bal;
+      }
+      s_off[32 * c + lane] = run;
+      s_msk[32 * c + lane] = (int32_t)m;
+      run += __popc(m);
+    }
+    s_seg[32 * warp + lane] = run;
+    __syncthreads();
+    int32_t off = 0;
+    for (int s2 = 0; s2 < warp; ++s2) off += s_seg[32 * s2 + lane];
+    if (warp == kBaseThreads / 32 - 1 && mine) {  // the last warp's offset + its own = the total
+      B.resp[32 * w + lane] = off + run;
+      row[(int64_t)nb * T.K] = off + run;
+    }
+    for (int32_t c = c_lo; c < c_hi; ++c) {
+      const int32_t base = off + s_off[32 * c + lane];
+      const uint32_t m = (uint32_t)s_msk[32 * c + lane];
+      const int nbb = min(32, nb - 32 * c);
+      if (mine)
+        for (int bb = 0; bb < nbb; ++bb)
+          row[(int64_t)(32 * c + bb) * T.K] = base + __popc(m & ((1u << bb) - 1u));
+    }
+    return;
+  }
+  // more batches than the shared-memory tables take: the chunk totals are parked in the rows
+  // themselves (row 32c+1, rewritten below) and one warp runs over the chunks
   for (int32_t c = warp; c < nchunks; c += kBaseThreads / 32) {
     const int32_t b = 32 * c + lane;
     const uint32_t word = (b < nb) ? B.cls_at[(int64_t)B.bstart[b] * 8 + w] : 0u;
@@ -377,7 +467,7 @@ whp_swaps_base2_kernel(const whp_tables T, const whp_base_tables B) {
       const int32_t pc = __popc(__ballot_sync(WHP_FULL, (word >> j) & 1u));
       if (lane == j) tot = pc;
     }
-    if (mine) row[(int64_t)(32 * c + 1) * T.K] = tot;  // parked in row 32c+1 (rewritten below)
+    if (mine) row[(int64_t)(32 * c + 1) * T.K] = tot;
   }
   __syncthreads();
   if (warp == 0 && mine) {
@@ -443,17 +533,29 @@ whp_swaps_prep_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
 // class visits, bF[p] = base batch that starts at F(p) (nb: the chain runs to the end of the plan;
 // -1: it leaves the region first). With T(p) = dtail[p] + (D_base - bdist[bF[p]]), any stretch
 // s -> t of one chain costs T(s) - T(t).
-constexpr int kChainWarps = 16;
+// Only the chains of the positions a neighbour can ask for are summed: the first new boundary
+// after the later swapped position lies at most C positions behind it, so p < chi = window end +
+// C + 1 (and once a chain has left the region, so has every later node of it).
+constexpr int kChainWarps = 8;  // warps of a block that walk one chain each
 
+// One launch after whp_swaps_prep_kernel: blocks 0 .. KW are the second half of the base pass
+// (base2_role), the others sum kChainWarps chains each. The two halves are independent.
 // STAGED: the hop records of the region sit in shared memory (a chain only moves forward, so a
 // block stages the rows from its own first position on); otherwise (a region too long for
 // shared memory) they are read from global memory.
 template <bool STAGED>
-__global__ void __launch_bounds__(kChainWarps * 32)
-whp_swaps_chain_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, int32_t rhi) {
-  // [cls_at: rows x 8][dist_at: rows (int64)][nxt: rows; negative: p is a base batch start]
+__global__ void __launch_bounds__(kBaseThreads)
+whp_swaps_tail_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, int32_t rhi,
+                      int32_t chi, int32_t chunk_cap) {
+  // chain blocks: [cls_at: rows x 8][dist_at: rows (int64)][nxt: rows; negative: p is a base
+  // batch start]; base2 blocks: see base2_role
   extern __shared__ __align__(16) uint8_t chain_smem[];
-  const int32_t r0 = rlo + blockIdx.x * kChainWarps;  // first position of this block
+  const int KW = (T.K + 31) >> 5;
+  if ((int)blockIdx.x <= KW) {
+    base2_role(T, B, reinterpret_cast<int32_t*>(chain_smem), chunk_cap);
+    return;
+  }
+  const int32_t r0 = rlo + ((int)blockIdx.x - KW - 1) * kChainWarps;  // first position of this block
   const int32_t rows = STAGED ? rhi - r0 : 0;
   uint4* s_cls = reinterpret_cast<uint4*>(chain_smem);
   int64_t* s_dist = reinterpret_cast<int64_t*>(chain_smem + 32 * (size_t)rows);
@@ -472,7 +574,7 @@ whp_swaps_chain_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo,
     __syncthreads();
   }
   const int32_t p0 = r0 + warp;
-  if (p0 >= rhi) return;
+  if (warp >= kChainWarps || p0 >= chi) return;
   int64_t D = 0;
   int32_t r[8];
 #pragma unroll
@@ -517,8 +619,9 @@ constexpr int kStage = 1024;  // positions of pre / orec staged per block
 template <bool STATS>  // STATS: also count the batches / picks scored from their picks
 __global__ void __launch_bounds__(kSwapWarps * 32)
 whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start, int32_t W,
-                 int32_t rlo, int32_t rhi, int64_t n_nb, int64_t* __restrict__ d_dist,
-                 double* __restrict__ d_obj, unsigned long long* __restrict__ stats) {
+                 int32_t rlo, int32_t rhi, int32_t chi, int64_t n_nb,
+                 int64_t* __restrict__ d_dist, double* __restrict__ d_obj,
+                 unsigned long long* __restrict__ stats) {
   __shared__ warp_sets sets_all[kSwapWarps];
   __shared__ int32_t s_pre[kStage + 1];
   __shared__ uint32_t s_orec[kStage];
@@ -633,7 +736,7 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
       int32_t b_end;
       for (;;) {
         // (1) past pj the rest of the rewalk is the chain of p, summed once per position
-        if (p > pj && p >= rlo && p < rhi) {
+        if (p > pj && p >= rlo && p < chi) {
           const int32_t bf = __ldg(B.bF + p);
           if (bf >= 0) {
             D += __ldg(B.dtail + p);
@@ -725,8 +828,9 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
 template <bool STATS>
 __global__ void __launch_bounds__(kSwapWarps * 32)
 whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start, int32_t W,
-                 int32_t rlo, int32_t rhi, int64_t n_nb, int64_t* __restrict__ d_dist,
-                 double* __restrict__ d_obj, unsigned long long* __restrict__ stats) {
+                 int32_t rlo, int32_t rhi, int32_t chi, int64_t n_nb,
+                 int64_t* __restrict__ d_dist, double* __restrict__ d_obj,
+                 unsigned long long* __restrict__ stats) {
   __shared__ warp_sets sets_all[kSwapWarps];
   __shared__ int32_t s_pre[kStage + 1];
   __shared__ uint32_t s_orec[kStage];
@@ -767,7 +871,7 @@ whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
     for (int w = 0; w < 8; ++w) r[w] = 0;
     int32_t b_end;
     for (;;) {
-      if (p > M && p >= rlo && p < rhi) {  // the rest is the chain of p
+      if (p > M && p >= rlo && p < chi) {  // the rest is the chain of p
         const int32_t bf = __ldg(B.bF + p);
         if (bf >= 0) {
           D += __ldg(B.dtail + p);
@@ -850,23 +954,32 @@ __global__ void whp_apply_move_kernel(int32_t* __restrict__ base_perm, int32_t w
 // neighbourhoods)
 static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const int32_t* d_base_perm,
                                         int32_t win_start, int32_t win_len, int32_t* rlo_out,
-                                        int32_t* rhi_out, cudaStream_t st) {
-  // shared-memory tables of the base pass: pre + nxt, and (mode 2) three more arrays for the
-  // pointer doubling that finds the base boundaries
-  size_t need = 4 * (5 * (size_t)c->n_orders + 1);
-  int smem_tables = 2;
-  if (need + 12 * 1024 > (size_t)c->smem_optin) {
-    need = 4 * (2 * (size_t)c->n_orders + 1);
-    smem_tables = need + 12 * 1024 <= (size_t)c->smem_optin ? 1 : 0;
-  }
+                                        int32_t* rhi_out, int32_t* chi_out, cudaStream_t st) {
+  // boundary search of the base pass: segments of seg_len >= C positions, about 1024 / C of them
+  // (one thread per (segment, entry position) pair); without a table (n_seg = 0) one thread chases
+  const int64_t n64 = c->n_orders, C64 = c->C;
+  int64_t seg_len = (n64 * C64 + kBaseThreads - 1) / kBaseThreads;
+  if (seg_len < C64) seg_len = C64;
+  if (seg_len > n64) seg_len = n64;  // C > n: one segment
+  int64_t n_seg = (n64 + seg_len - 1) / seg_len;
+  if (n_seg * C64 > kMaxSegEntries) n_seg = 0;
+  const size_t seg_bytes = 4 * (size_t)(n_seg * C64 + n_seg);
+  // shared-memory tables of the base pass: pre, nxt and the boundary marks, when they fit
+  const size_t n4 = ((size_t)c->n_orders + 4) & ~(size_t)3;
+  const size_t need = 12 * n4 + seg_bytes;
+  const bool smem_tables = need + 12 * 1024 <= (size_t)c->smem_optin;
   // the attribute is per function and process-wide: always the same value (the most any call
   // asks for), so contexts used from different host threads cannot undercut each other
-  cudaError_t e = cudaFuncSetAttribute(whp_swaps_base_kernel,
+  cudaError_t e = cudaFuncSetAttribute(whp_swaps_base_kernel<true>,
                                        cudaFuncAttributeMaxDynamicSharedMemorySize,
                                        c->smem_optin - 12 * 1024);
   if (e != cudaSuccess) return e;
-  whp_swaps_base_kernel<<<1, kBaseThreads, smem_tables ? need : 0, st>>>(T, d_base_perm, c->base,
-                                                                        smem_tables);
+  if (smem_tables)
+    whp_swaps_base_kernel<true><<<1, kBaseThreads, need, st>>>(T, d_base_perm, c->base,
+                                                               (int32_t)seg_len, (int32_t)n_seg);
+  else
+    whp_swaps_base_kernel<false><<<1, kBaseThreads, seg_bytes, st>>>(T, d_base_perm, c->base,
+                                                                     (int32_t)seg_len, (int32_t)n_seg);
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   // region of tabulated hypothetical batches: from two cart lengths before the window (the
@@ -887,11 +1000,11 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
                           kPrepWarps * 32, 0, st>>>(T, c->base, rlo, rhi);
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  whp_swaps_base2_kernel<<<(unsigned)((c->K + 31) / 32 + 1), kBaseThreads, 0, st>>>(T, c->base);
-  c->launches += 1;
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
-  // chain sums of the region (rtail grows with the region)
-  const int64_t rows = rhi - rlo;
+  // second half of the base pass and the chain sums of the positions a neighbour can ask for,
+  // in one launch (rtail grows with the window)
+  const int32_t chi = (int32_t)((int64_t)win_start + win_len + c->C + 1 < rhi
+                                    ? (int64_t)win_start + win_len + c->C + 1 : rhi);
+  const int64_t rows = chi - rlo;
   if (c->rtail_rows < rows) {
     if ((e = cudaStreamSynchronize(st)) != cudaSuccess) return e;
     cudaFree(c->base.rtail);
@@ -900,29 +1013,38 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
     if ((e = cudaMalloc(&c->base.rtail, 4 * (size_t)rows * (size_t)c->K)) != cudaSuccess) return e;
     c->rtail_rows = rows;
   }
-  const size_t chain_smem = 44 * (size_t)rows;
-  const unsigned chain_blocks = (unsigned)((rows + kChainWarps - 1) / kChainWarps);
+  int64_t chunk_cap = nb_max / 32 + 1;
+  if (chunk_cap > kBase2ChunkCap) chunk_cap = kBase2ChunkCap;
+  const size_t base2_smem = 4 * (64 * (size_t)chunk_cap + 1024);
+  const size_t chain_smem = 44 * (size_t)(rhi - rlo);
+  const unsigned tail_blocks = (unsigned)((c->K + 31) / 32 + 1 + (rows + kChainWarps - 1) / kChainWarps);
+  if ((e = cudaFuncSetAttribute(whp_swaps_tail_kernel<true>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                c->smem_optin - 2048)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(whp_swaps_tail_kernel<false>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                c->smem_optin - 2048)) != cudaSuccess) return e;
   if (chain_smem + 2048 <= (size_t)c->smem_optin) {
-    if ((e = cudaFuncSetAttribute(whp_swaps_chain_kernel<true>,
-                                  cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  c->smem_optin - 2048)) != cudaSuccess) return e;
-    whp_swaps_chain_kernel<true><<<chain_blocks, kChainWarps * 32, chain_smem, st>>>(T, c->base,
-                                                                                      rlo, rhi);
+    whp_swaps_tail_kernel<true><<<tail_blocks, kBaseThreads,
+                                  chain_smem > base2_smem ? chain_smem : base2_smem, st>>>(
+        T, c->base, rlo, rhi, chi, (int32_t)chunk_cap);
   } else {
-    whp_swaps_chain_kernel<false><<<chain_blocks, kChainWarps * 32, 0, st>>>(T, c->base, rlo, rhi);
+    whp_swaps_tail_kernel<false><<<tail_blocks, kBaseThreads, base2_smem, st>>>(
+        T, c->base, rlo, rhi, chi, (int32_t)chunk_cap);
   }
   c->launches += 1;
   if ((e = cudaGetLastError()) != cudaSuccess) return e;
   *rlo_out = rlo;
   *rhi_out = rhi;
+  *chi_out = chi;
   return cudaSuccess;
 }
 
 cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                              int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st) {
   const whp_tables T = whp_make_tables(c);
-  int32_t rlo, rhi;
-  cudaError_t e = launch_window_tables(c, T, d_base_perm, win_start, win_len, &rlo, &rhi, st);
+  int32_t rlo, rhi, chi;
+  cudaError_t e = launch_window_tables(c, T, d_base_perm, win_start, win_len, &rlo, &rhi, &chi, st);
   if (e != cudaSuccess) return e;
   const int64_t n_nb = (int64_t)win_len * (win_len - 1) / 2;
   int64_t blocks = (n_nb + kSwapWarps - 1) / kSwapWarps;
@@ -931,10 +1053,10 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
   if (c->swap_stats && (e = cudaMemsetAsync(c->d_swap_stats, 0, 16, st)) != cudaSuccess) return e;
   if (c->swap_stats)
     whp_swaps_kernel<true><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
-        T, c->base, win_start, win_len, rlo, rhi, n_nb, d_dist, d_obj, c->d_swap_stats);
+        T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, c->d_swap_stats);
   else
     whp_swaps_kernel<false><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
-        T, c->base, win_start, win_len, rlo, rhi, n_nb, d_dist, d_obj, nullptr);
+        T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, nullptr);
   c->launches += 1;
   return cudaGetLastError();
 }
@@ -942,8 +1064,8 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
 cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
                              int32_t win_len, int64_t* d_dist, double* d_obj, cudaStream_t st) {
   const whp_tables T = whp_make_tables(c);
-  int32_t rlo, rhi;
-  cudaError_t e = launch_window_tables(c, T, d_base_perm, win_start, win_len, &rlo, &rhi, st);
+  int32_t rlo, rhi, chi;
+  cudaError_t e = launch_window_tables(c, T, d_base_perm, win_start, win_len, &rlo, &rhi, &chi, st);
   if (e != cudaSuccess) return e;
   const int64_t n_nb = (int64_t)win_len * (win_len - 1);
   int64_t blocks = (n_nb + kSwapWarps - 1) / kSwapWarps;
@@ -952,10 +1074,10 @@ cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win
   if (c->swap_stats && (e = cudaMemsetAsync(c->d_swap_stats, 0, 16, st)) != cudaSuccess) return e;
   if (c->swap_stats)
     whp_moves_kernel<true><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
-        T, c->base, win_start, win_len, rlo, rhi, n_nb, d_dist, d_obj, c->d_swap_stats);
+        T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, c->d_swap_stats);
   else
     whp_moves_kernel<false><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
-        T, c->base, win_start, win_len, rlo, rhi, n_nb, d_dist, d_obj, nullptr);
+        T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, nullptr);
   c->launches += 1;
   return cudaGetLastError();
 }
