@@ -26,6 +26,32 @@
 
 namespace {
 
+// Programmatic dependent launch: the kernels of one whp_eval_swaps / whp_eval_moves call depend
+// on each other in a row. A kernel launched with launch_dependent() may become resident while its
+// predecessor still runs; it must pass dep_wait() — which returns once the predecessor grid has
+// completed and its writes are visible — before it touches anything the predecessor writes. The
+// predecessor allows that early start with dep_trigger() (all of its blocks are resident or done
+// by then, so the waiting blocks cannot starve it). Every thread of a dependent kernel calls
+// dep_wait(), so completion stays transitive along the row.
+__device__ __forceinline__ void dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void dep_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
+
+template <class... KArgs, class... Args>
+cudaError_t launch_dependent(void (*kernel)(KArgs...), unsigned grid, unsigned block, size_t smem,
+                             cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(block);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // The base plan with positions pi and pj exchanged (pi = pj = -1: the base plan itself), seen
 // through the base tables: pre = exclusive item-count prefix, orec = order record by position.
 // A window [lo, lo+cnt) of both tables may be staged in shared memory.
@@ -240,6 +266,7 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
                       const whp_base_tables B, int32_t seg_len, int32_t n_seg) {
   extern __shared__ __align__(16) uint8_t dyn[];
   __shared__ int32_t s_scan32[33];
+  dep_trigger();
   const int tid = threadIdx.x;
   const int32_t n = T.n_orders, C = T.C;
   const int32_t n4 = (n + 4) & ~3;  // >= n + 1, a multiple of four (16-byte rows)
@@ -507,6 +534,8 @@ whp_swaps_prep_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
   if (lane < 8) sets->cmask[lane] = 0;
+  dep_trigger();
+  dep_wait();
   __syncwarp();
   // warps 0 .. rows-1: the region positions; the others: the base batches (their starts)
   const int32_t g = blockIdx.x * kPrepWarps + warp;
@@ -550,6 +579,8 @@ whp_swaps_tail_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
   // chain blocks: [cls_at: rows x 8][dist_at: rows (int64)][nxt: rows; negative: p is a base
   // batch start]; base2 blocks: see base2_role
   extern __shared__ __align__(16) uint8_t chain_smem[];
+  dep_trigger();
+  dep_wait();
   const int KW = (T.K + 31) >> 5;
   if ((int)blockIdx.x <= KW) {
     base2_role(T, B, reinterpret_cast<int32_t*>(chain_smem), chunk_cap);
@@ -631,6 +662,7 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
   if (lane < 8) sets->cmask[lane] = 0;
+  dep_wait();
   const int32_t n = T.n_orders;
   const int32_t nb = (int32_t)B.totals[1];
   // stage the tables from the start of the batch before the window's first batch
@@ -839,6 +871,7 @@ whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
   if (lane < 8) sets->cmask[lane] = 0;
+  dep_wait();
   const int32_t n = T.n_orders;
   const int32_t nb = (int32_t)B.totals[1];
   int32_t lo;
@@ -996,10 +1029,10 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
   // hypothetical batches of the region and the base batches themselves
   int64_t nb_max = 2ll * c->n_items / ((int64_t)c->C + 1) + 1;
   if (nb_max > c->n_orders) nb_max = c->n_orders;
-  whp_swaps_prep_kernel<<<(unsigned)((rhi - rlo + nb_max + kPrepWarps - 1) / kPrepWarps),
-                          kPrepWarps * 32, 0, st>>>(T, c->base, rlo, rhi);
+  if ((e = launch_dependent(whp_swaps_prep_kernel,
+                            (unsigned)((rhi - rlo + nb_max + kPrepWarps - 1) / kPrepWarps),
+                            kPrepWarps * 32, 0, st, T, c->base, rlo, rhi)) != cudaSuccess) return e;
   c->launches += 1;
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
   // second half of the base pass and the chain sums of the positions a neighbour can ask for,
   // in one launch (rtail grows with the window)
   const int32_t chi = (int32_t)((int64_t)win_start + win_len + c->C + 1 < rhi
@@ -1024,16 +1057,15 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
   if ((e = cudaFuncSetAttribute(whp_swaps_tail_kernel<false>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 c->smem_optin - 2048)) != cudaSuccess) return e;
-  if (chain_smem + 2048 <= (size_t)c->smem_optin) {
-    whp_swaps_tail_kernel<true><<<tail_blocks, kBaseThreads,
-                                  chain_smem > base2_smem ? chain_smem : base2_smem, st>>>(
-        T, c->base, rlo, rhi, chi, (int32_t)chunk_cap);
-  } else {
-    whp_swaps_tail_kernel<false><<<tail_blocks, kBaseThreads, base2_smem, st>>>(
-        T, c->base, rlo, rhi, chi, (int32_t)chunk_cap);
-  }
+  if (chain_smem + 2048 <= (size_t)c->smem_optin)
+    e = launch_dependent(whp_swaps_tail_kernel<true>, tail_blocks, kBaseThreads,
+                         chain_smem > base2_smem ? chain_smem : base2_smem, st, T, c->base, rlo,
+                         rhi, chi, (int32_t)chunk_cap);
+  else
+    e = launch_dependent(whp_swaps_tail_kernel<false>, tail_blocks, kBaseThreads, base2_smem, st, T,
+                         c->base, rlo, rhi, chi, (int32_t)chunk_cap);
+  if (e != cudaSuccess) return e;
   c->launches += 1;
-  if ((e = cudaGetLastError()) != cudaSuccess) return e;
   *rlo_out = rlo;
   *rhi_out = rhi;
   *chi_out = chi;
@@ -1051,14 +1083,15 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
   const int64_t cap = (int64_t)c->num_sms * 8;
   if (blocks > cap) blocks = cap;
   if (c->swap_stats && (e = cudaMemsetAsync(c->d_swap_stats, 0, 16, st)) != cudaSuccess) return e;
-  if (c->swap_stats)
+  if (c->swap_stats)  // (the memset sits between the launches: no early start then)
     whp_swaps_kernel<true><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
         T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, c->d_swap_stats);
   else
-    whp_swaps_kernel<false><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
-        T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, nullptr);
+    e = launch_dependent(whp_swaps_kernel<false>, (unsigned)blocks, kSwapWarps * 32, 0, st, T,
+                         c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj,
+                         (unsigned long long*)nullptr);
   c->launches += 1;
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
@@ -1076,10 +1109,11 @@ cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win
     whp_moves_kernel<true><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
         T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, c->d_swap_stats);
   else
-    whp_moves_kernel<false><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
-        T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, nullptr);
+    e = launch_dependent(whp_moves_kernel<false>, (unsigned)blocks, kSwapWarps * 32, 0, st, T,
+                         c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj,
+                         (unsigned long long*)nullptr);
   c->launches += 1;
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t whp_launch_apply_move(whp_ctx* c, int32_t* d_base_perm, int32_t win_start,
