@@ -26,13 +26,17 @@
 
 namespace {
 
-// Programmatic dependent launch: the kernels of one whp_eval_swaps / whp_eval_moves call depend
-// on each other in a row. A kernel launched with launch_dependent() may become resident while its
-// predecessor still runs; it must pass dep_wait() — which returns once the predecessor grid has
-// completed and its writes are visible — before it touches anything the predecessor writes. The
-// predecessor allows that early start with dep_trigger() (all of its blocks are resident or done
-// by then, so the waiting blocks cannot starve it). Every thread of a dependent kernel calls
-// dep_wait(), so completion stays transitive along the row.
+// Programmatic dependent launch: the table kernels of one whp_eval_swaps / whp_eval_moves call
+// depend on each other in a row (base -> prep -> tail). A kernel launched with launch_dependent()
+// may become resident while its predecessor still runs; it must pass dep_wait() — which returns
+// once the predecessor grid has completed and its writes are visible — before it touches anything
+// the predecessor writes. The predecessor allows that early start with dep_trigger() (all of its
+// blocks are resident or done by then, so the waiting blocks cannot starve it). Every thread of a
+// dependent kernel calls dep_wait(), so completion stays transitive along the row.
+// The neighbour kernel itself is launched normally: as a third dependent it saves another 2 us
+// of the call alone (74.8 instead of 76.7 us at W = 256), but its 1184 blocks then sit resident
+// and idle on every SM while the tables are built, and a candidate evaluation running on
+// another stream loses 0.03 ms of a 0.43 ms step to that (profiles/r2_neighbourhood.md).
 __device__ __forceinline__ void dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void dep_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
 
@@ -318,26 +322,24 @@ whp_swaps_base_kernel(const whp_tables T, const int32_t* __restrict__ base_perm,
   __syncthreads();
 
   // ---- B: nxt[p] = where the batch that opens at p ends: the largest e <= min(n, p + C) with
-  // pre[e] <= pre[p] + C (q <= C, so e >= p + 1). A binary search for the first of a thread's four
-  // positions; nxt is monotone, so the others advance from their predecessor's answer.
+  // pre[e] <= pre[p] + C (q <= C, so e >= p + 1): a binary search; nxt is monotone, so the search
+  // of a thread's later positions starts at its predecessor's answer. (A linear advance from
+  // there is one step on average but its longest lane holds up the warp.)
   for (int32_t p0 = 0; p0 < n; p0 += 4 * kBaseThreads) {
     const int32_t pb = p0 + 4 * tid;
     if (pb >= n) break;
     int32_t nx[4] = {0, 0, 0, 0};
-    int32_t lim = pre[pb] + C;
-    int32_t lo = pb + 1, hi = min(n, pb + C);
-    while (lo < hi) {
-      const int32_t mid = (lo + hi + 1) >> 1;
-      if (pre[mid] <= lim) lo = mid; else hi = mid - 1;
-    }
-    nx[0] = lo;
+    int32_t lo = pb + 1;
 #pragma unroll
-    for (int k = 1; k < 4; ++k)
+    for (int k = 0; k < 4; ++k)
       if (pb + k < n) {
-        lim = pre[pb + k] + C;
+        const int32_t lim = pre[pb + k] + C;
         lo = max(lo, pb + k + 1);
-        hi = min(n, pb + k + C);
-        while (lo < hi && pre[lo + 1] <= lim) ++lo;
+        int32_t hi = min(n, pb + k + C);
+        while (lo < hi) {
+          const int32_t mid = (lo + hi + 1) >> 1;
+          if (pre[mid] <= lim) lo = mid; else hi = mid - 1;
+        }
         nx[k] = lo;
       }
     if (pb + 3 < n) {
@@ -534,8 +536,8 @@ whp_swaps_prep_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
   if (lane < 8) sets->cmask[lane] = 0;
-  dep_trigger();
   dep_wait();
+  dep_trigger();
   __syncwarp();
   // warps 0 .. rows-1: the region positions; the others: the base batches (their starts)
   const int32_t g = blockIdx.x * kPrepWarps + warp;
@@ -565,7 +567,15 @@ whp_swaps_prep_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
 // Only the chains of the positions a neighbour can ask for are summed: the first new boundary
 // after the later swapped position lies at most C positions behind it, so p < chi = window end +
 // C + 1 (and once a chain has left the region, so has every later node of it).
-constexpr int kChainWarps = 8;  // warps of a block that walk one chain each
+constexpr int kChainWarps = 4;  // warps of a block that walk one chain each
+
+template <int BYTES>
+__device__ __forceinline__ void stage_async(void* smem_dst, const void* gmem_src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"(
+                   (uint32_t)__cvta_generic_to_shared(smem_dst)),
+               "l"(gmem_src), "n"(BYTES)
+               : "memory");
+}
 
 // One launch after whp_swaps_prep_kernel: blocks 0 .. KW are the second half of the base pass
 // (base2_role), the others sum kChainWarps chains each. The two halves are independent.
@@ -577,9 +587,8 @@ __global__ void __launch_bounds__(kBaseThreads)
 whp_swaps_tail_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, int32_t rhi,
                       int32_t chi, int32_t chunk_cap) {
   // chain blocks: [cls_at: rows x 8][dist_at: rows (int64)][nxt: rows; negative: p is a base
-  // batch start]; base2 blocks: see base2_role
+  // batch start][bop: rows + 1]; base2 blocks: see base2_role
   extern __shared__ __align__(16) uint8_t chain_smem[];
-  dep_trigger();
   dep_wait();
   const int KW = (T.K + 31) >> 5;
   if ((int)blockIdx.x <= KW) {
@@ -591,17 +600,25 @@ whp_swaps_tail_kernel(const whp_tables T, const whp_base_tables B, int32_t rlo, 
   uint4* s_cls = reinterpret_cast<uint4*>(chain_smem);
   int64_t* s_dist = reinterpret_cast<int64_t*>(chain_smem + 32 * (size_t)rows);
   int32_t* s_nx = reinterpret_cast<int32_t*>(chain_smem + 40 * (size_t)rows);
+  int32_t* s_bop = reinterpret_cast<int32_t*>(chain_smem + 44 * (size_t)rows);  // bop[r0-1 .. rhi)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int32_t n = T.n_orders;
   if (STAGED) {
+    // asynchronous copies: every load of the block is in flight before the first one is awaited
+    const uint4* cls_src = reinterpret_cast<const uint4*>(B.cls_at + (int64_t)r0 * 8);
+    for (int32_t k = threadIdx.x; k < 2 * rows; k += blockDim.x) stage_async<16>(s_cls + k, cls_src + k);
     for (int32_t k = threadIdx.x; k < rows; k += blockDim.x) {
-      const int32_t p = r0 + k;
-      const bool start = p == 0 || B.bop[p] != B.bop[p - 1];
-      s_nx[k] = start ? -1 : B.nxt[p];
-      s_dist[k] = B.dist_at[p];
+      stage_async<8>(s_dist + k, B.dist_at + r0 + k);
+      stage_async<4>(s_nx + k, B.nxt + r0 + k);
     }
-    for (int32_t k = threadIdx.x; k < 2 * rows; k += blockDim.x)
-      s_cls[k] = reinterpret_cast<const uint4*>(B.cls_at + (int64_t)r0 * 8)[k];
+    for (int32_t k = threadIdx.x; k <= rows; k += blockDim.x) {
+      if (r0 + k > 0) stage_async<4>(s_bop + k, B.bop + r0 - 1 + k);
+      else s_bop[k] = -1;
+    }
+    asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+    __syncthreads();
+    for (int32_t k = threadIdx.x; k < rows; k += blockDim.x)
+      if (s_bop[k + 1] != s_bop[k]) s_nx[k] = -1;  // position r0 + k opens a base batch
     __syncthreads();
   }
   const int32_t p0 = r0 + warp;
@@ -662,7 +679,6 @@ whp_swaps_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
   if (lane < 8) sets->cmask[lane] = 0;
-  dep_wait();
   const int32_t n = T.n_orders;
   const int32_t nb = (int32_t)B.totals[1];
   // stage the tables from the start of the batch before the window's first batch
@@ -871,7 +887,6 @@ whp_moves_kernel(const whp_tables T, const whp_base_tables B, int32_t win_start,
   warp_sets* sets = &sets_all[warp];
   sets->amask[lane] = 0;
   if (lane < 8) sets->cmask[lane] = 0;
-  dep_wait();
   const int32_t n = T.n_orders;
   const int32_t nb = (int32_t)B.totals[1];
   int32_t lo;
@@ -1049,7 +1064,7 @@ static cudaError_t launch_window_tables(whp_ctx* c, const whp_tables& T, const i
   int64_t chunk_cap = nb_max / 32 + 1;
   if (chunk_cap > kBase2ChunkCap) chunk_cap = kBase2ChunkCap;
   const size_t base2_smem = 4 * (64 * (size_t)chunk_cap + 1024);
-  const size_t chain_smem = 44 * (size_t)(rhi - rlo);
+  const size_t chain_smem = 48 * (size_t)(rhi - rlo) + 16;
   const unsigned tail_blocks = (unsigned)((c->K + 31) / 32 + 1 + (rows + kChainWarps - 1) / kChainWarps);
   if ((e = cudaFuncSetAttribute(whp_swaps_tail_kernel<true>,
                                 cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1083,15 +1098,14 @@ cudaError_t whp_launch_swaps(whp_ctx* c, const int32_t* d_base_perm, int32_t win
   const int64_t cap = (int64_t)c->num_sms * 8;
   if (blocks > cap) blocks = cap;
   if (c->swap_stats && (e = cudaMemsetAsync(c->d_swap_stats, 0, 16, st)) != cudaSuccess) return e;
-  if (c->swap_stats)  // (the memset sits between the launches: no early start then)
+  if (c->swap_stats)
     whp_swaps_kernel<true><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
         T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, c->d_swap_stats);
   else
-    e = launch_dependent(whp_swaps_kernel<false>, (unsigned)blocks, kSwapWarps * 32, 0, st, T,
-                         c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj,
-                         (unsigned long long*)nullptr);
+    whp_swaps_kernel<false><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
+        T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, nullptr);
   c->launches += 1;
-  return e != cudaSuccess ? e : cudaGetLastError();
+  return cudaGetLastError();
 }
 
 cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win_start,
@@ -1109,11 +1123,10 @@ cudaError_t whp_launch_moves(whp_ctx* c, const int32_t* d_base_perm, int32_t win
     whp_moves_kernel<true><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
         T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, c->d_swap_stats);
   else
-    e = launch_dependent(whp_moves_kernel<false>, (unsigned)blocks, kSwapWarps * 32, 0, st, T,
-                         c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj,
-                         (unsigned long long*)nullptr);
+    whp_moves_kernel<false><<<(unsigned)blocks, kSwapWarps * 32, 0, st>>>(
+        T, c->base, win_start, win_len, rlo, rhi, chi, n_nb, d_dist, d_obj, nullptr);
   c->launches += 1;
-  return e != cudaSuccess ? e : cudaGetLastError();
+  return cudaGetLastError();
 }
 
 cudaError_t whp_launch_apply_move(whp_ctx* c, int32_t* d_base_perm, int32_t win_start,

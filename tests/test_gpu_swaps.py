@@ -149,11 +149,11 @@ def test_swaps_chains_that_leave_the_tabulated_region(torch_cuda, margin):
 @pytest.mark.parametrize("n_orders,s,Wn,margin", [(20000, 9000, 28, None), (20000, 9000, 28, "8000"),
                                                   (30000, 21000, 12, None), (30000, 29988, 12, "9000")])
 def test_swaps_on_long_plans(torch_cuda, n_orders, s, Wn, margin):
-    """Stress-size plans. 20,000 orders: the base pass keeps only two of its five tables in shared
-    memory and one thread chases the batch boundaries; 30,000 orders: no table fits. With a region
-    of 8,000+ positions the hop records (44 bytes a position) do not fit shared memory either, so
-    the chain kernel reads them from global memory. Swaps and insertion moves of a small window
-    against the oracle."""
+    """Stress-size plans: 20,000 and 30,000 orders are more than the base pass can keep in shared
+    memory (12 bytes a position), so its prefix, batch-end and boundary-mark tables are the global
+    ones. With a region of 8,000+ positions the hop records (48 bytes a position) do not fit
+    shared memory either, so the chain blocks read them from global memory. Swaps and insertion
+    moves of a small window against the oracle."""
     import os
     torch = torch_cuda
     from paper_2110_13693_b200 import whp
@@ -173,6 +173,37 @@ def test_swaps_on_long_plans(torch_cuda, n_orders, s, Wn, margin):
         torch.cuda.synchronize()
     finally:
         ctx.debug_set(whp.DEBUG_SWAP_MARGIN, -1)
+    assert np.array_equal(d.cpu().numpy(), ref["dist"])
+    assert np.array_equal(o.cpu().numpy(), ref["obj"])
+    assert np.array_equal(md.cpu().numpy(), ref_m["dist"])
+    assert np.array_equal(mo.cpu().numpy(), ref_m["obj"])
+    ctx.close()
+
+
+@pytest.mark.parametrize("cfg,s,Wn", [
+    # a cart of 9,000 items: the per-segment boundary table of the base pass (segments x C entries)
+    # is not built and one thread chases the boundaries
+    (dict(NA=30, S=40, K=50, n_skus=800, n_orders=300, qmax=255, C=9000), 100, 24),
+    # ~14,000 carts: more than the 8,192 whose class-count prefix (rpre) the base pass builds in
+    # shared memory, so the chunk totals go through global memory
+    (dict(NA=40, S=50, K=70, n_skus=900, n_orders=20000, qmax=3, C=3), 9000, 12),
+    (dict(NA=40, S=50, K=70, n_skus=900, n_orders=20000, qmax=3, C=3), 19988, 12),
+])
+def test_swaps_beyond_the_shared_memory_tables_of_the_base_pass(torch_cuda, cfg, s, Wn):
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    from test_gpu_parity import _random_problem
+    pb = _random_problem(21, **cfg)
+    ctx = whp.Context.from_problem(pb)
+    base = W.base_perm(4, pb.n_orders)
+    ref = oracle.eval_swaps(pb, base, s, Wn)
+    ref_m = oracle.eval_moves(pb, base, s, 8)
+    bd = torch.from_numpy(base).cuda()
+    d, o = gpu_swaps(torch, ctx, bd, s, Wn)
+    md = torch.zeros(56, dtype=torch.int64, device="cuda")
+    mo = torch.zeros(56, dtype=torch.float64, device="cuda")
+    ctx.eval_moves(bd, s, 8, md, mo)
+    torch.cuda.synchronize()
     assert np.array_equal(d.cpu().numpy(), ref["dist"])
     assert np.array_equal(o.cpu().numpy(), ref["obj"])
     assert np.array_equal(md.cpu().numpy(), ref_m["dist"])
