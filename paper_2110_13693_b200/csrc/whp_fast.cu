@@ -636,12 +636,16 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         kmax = max(kmax, rec);
         if (!DEPOT0) kmin = min(kmin, rec);
         const uint32_t aaddr = abase | ((rec >> 20) & amask);
-        sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 22));
         if (KW == 1) {  // up to 32 classes: the batch's class set is one register
+          sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 22));
           cset |= one_shl_wrap(rec);
         } else {
+          // the aisle word and the class word are different words: both loads go out before
+          // either store, so a step waits for one shared-memory round trip instead of two
           const uint32_t caddr = cbase | (rec & 0x380u);
-          sts32(caddr, lds32(caddr) | one_shl_wrap(rec));
+          const uint32_t aw = lds32(aaddr), cw = lds32(caddr);
+          sts32(aaddr, aw | one_shl_wrap(rec >> 22));
+          sts32(caddr, cw | one_shl_wrap(rec));
         }
         rec = rec_next;
       }
