@@ -560,11 +560,18 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
     // ---- cursor stream of this lane through its private cp.async ring: chunk c (cursors of
     // positions 8c..8c+7) lives at ring offset (16 c) mod ring
     const uint4* __restrict__ cs = reinterpret_cast<const uint4*>(cstream + cand * P.cs_pitch);
+    // the last chunk this lane reads: the one that holds the first position of the next segment
+    // (a third of the ring traffic used to be chunks fetched past the end of the lane's run)
+    int c_last;
+    {
+      const int p_next = __shfl_down_sync(WHP_FULL, p, 1);
+      c_last = min((seg == P.S - 1 || lane == 31 ? T.n_orders : p_next) >> 3, n8 - 1);
+    }
     int lo_prev;  // first chunk that was resident when the newest refill group was issued
     {
       const int c0 = p >> 3;
       for (int k = 0; k < chunks; ++k)
-        cp_async16(ringbase + (((c0 + k) << 4) & P.ring_mask), cs + min(c0 + k, n8 - 1));
+        if (c0 + k <= c_last) cp_async16(ringbase + (((c0 + k) << 4) & P.ring_mask), cs + c0 + k);
       cp_async_commit();
       lo_prev = c0 - chunks;
     }
@@ -652,11 +659,10 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       {  // refill the slots of the chunks this batch finished; waited for two batches later
         const int nf = live ? (p >> 3) - (p0 >> 3) : 0;
         const int nfmax = __reduce_max_sync(WHP_FULL, nf);
-        for (int i = 0; i < nfmax; ++i)
-          if (i < nf) {
-            const int c = (p0 >> 3) + i;
-            cp_async16(ringbase + ((c << 4) & P.ring_mask), cs + min(c + chunks, n8 - 1));
-          }
+        for (int i = 0; i < nfmax; ++i) {
+          const int c = (p0 >> 3) + i;
+          if (i < nf && c + chunks <= c_last) cp_async16(ringbase + ((c << 4) & P.ring_mask), cs + c + chunks);
+        }
         cp_async_commit();
         if (live) lo_prev = p0 >> 3;
       }
@@ -832,11 +838,16 @@ whp_legs_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
     uint32_t bw = __ldg(bm + wi) & (WHP_FULL << (p & 31));
     uint32_t bw_next = __ldg(bm + min(wi + 1, P.bm_pitch - 1));
     const uint4* __restrict__ cs = reinterpret_cast<const uint4*>(cstream + cand * P.cs_pitch);
+    int c_last;  // the last chunk this lane reads (as in K2)
+    {
+      const int p_next = __shfl_down_sync(WHP_FULL, p, 1);
+      c_last = min((seg == P.S - 1 || lane == 31 ? T.n_orders : p_next) >> 3, n8 - 1);
+    }
     int lo_prev;
     {
       const int c0 = p >> 3;
       for (int k = 0; k < chunks; ++k)
-        cp_async16(ringbase + (((c0 + k) << 4) & P.ring_mask), cs + min(c0 + k, n8 - 1));
+        if (c0 + k <= c_last) cp_async16(ringbase + (((c0 + k) << 4) & P.ring_mask), cs + c0 + k);
       cp_async_commit();
       lo_prev = c0 - chunks;
     }
@@ -907,11 +918,10 @@ whp_legs_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       {
         const int nf = live ? (p >> 3) - (p0 >> 3) : 0;
         const int nfmax = __reduce_max_sync(WHP_FULL, nf);
-        for (int i = 0; i < nfmax; ++i)
-          if (i < nf) {
-            const int c = (p0 >> 3) + i;
-            cp_async16(ringbase + ((c << 4) & P.ring_mask), cs + min(c + chunks, n8 - 1));
-          }
+        for (int i = 0; i < nfmax; ++i) {
+          const int c = (p0 >> 3) + i;
+          if (i < nf && c + chunks <= c_last) cp_async16(ringbase + ((c << 4) & P.ring_mask), cs + c + chunks);
+        }
         cp_async_commit();
         if (live) lo_prev = p0 >> 3;
       }
