@@ -56,6 +56,12 @@ __device__ __forceinline__ uint32_t one_shl_wrap(uint32_t n) {
   uint32_t r; asm("shf.l.wrap.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(0u), "r"(1u), "r"(n)); return r;
 }
 
+// Programmatic dependent launch (as in whp_swaps.cu): K2 may become resident — and stage its pick
+// table — while the segments kernel drains; it passes dep_wait() before it reads anything K1 or
+// the segments kernel wrote.
+__device__ __forceinline__ void dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void dep_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
+
 // ------------------------------------------------------------------------------------------ K1
 // Next-fit batching (D2) is a sequential recurrence along the plan: one thread per plan, one
 // warp per block. The plans of a warp are 32 consecutive rows of the permutation matrix, so one
@@ -303,6 +309,7 @@ whp_segments_kernel(const uint32_t* __restrict__ bmask, int32_t bm_pitch, int32_
                     int64_t n_cand, int32_t S, int32_t log2S, int32_t* __restrict__ nb_scratch,
                     int32_t* __restrict__ n_batches_out, int32_t* __restrict__ segstart,
                     int32_t ss_pitch) {
+  dep_trigger();
   const int lane = threadIdx.x & 31;
   const int64_t c = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   if (c >= n_cand) return;
@@ -523,6 +530,7 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
   const int n8 = P.cs_pitch >> 3;  // 16-byte chunks per cursor-stream row
   for (int w = 0; w < P.aw_words; ++w) sts32(abase + w * 128, 0u);
   for (int w = 0; w < KW; ++w) sts32(cbase + w * 128, 0u);
+  dep_wait();  // everything above reads only the pick table: it overlaps the segments kernel
 
   __shared__ unsigned long long s_task[32];
   for (;;) {
@@ -1208,10 +1216,21 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const void* d_perms, int64_t n_cand
   do {                                                                                           \
     cudaFuncSetAttribute(whp_sets_kernel<ST, D0, KWV, PLV>,                                      \
                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(c->smem_optin - 1024)); \
-    whp_sets_kernel<ST, D0, KWV, PLV><<<(unsigned)blocks, warps * 32, smem, st>>>(               \
-        T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand,          \
-        c->d_dist_scratch, c->d_planes, out.batch_hash, c->d_task, out.dist, out.penalty,      \
-        out.obj, out.resp);                                                                      \
+    cudaLaunchConfig_t cfg{};                                                                    \
+    cfg.gridDim = dim3((unsigned)blocks);                                                        \
+    cfg.blockDim = dim3(warps * 32);                                                             \
+    cfg.dynamicSmemBytes = smem;                                                                 \
+    cfg.stream = st;                                                                             \
+    cudaLaunchAttribute attr[1];                                                                 \
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                             \
+    attr[0].val.programmaticStreamSerializationAllowed = 1;                                      \
+    cfg.attrs = attr;                                                                            \
+    cfg.numAttrs = 1;                                                                            \
+    cudaLaunchKernelEx(&cfg, whp_sets_kernel<ST, D0, KWV, PLV>, T, P,                            \
+                       (const uint32_t*)c->d_pick_fast, (const uint16_t*)c->d_cstream,           \
+                       (const uint32_t*)c->d_bmask, (const int32_t*)c->d_nb,                     \
+                       (const int32_t*)c->d_segstart, n_cand, c->d_dist_scratch, c->d_planes,    \
+                       out.batch_hash, c->d_task, out.dist, out.penalty, out.obj, out.resp);     \
   } while (0)
 #define WHP_LAUNCH_SETS(ST, D0, KWV)                                                             \
   do {                                                                                           \
