@@ -174,6 +174,8 @@ def run_ours(args):
     pb = wl.problem
     n, n_cand = pb.n_orders, wl.n_cand
     ctx = whp.Context.from_problem(pb, device=local_rank)
+    if args.k1_warps:
+        ctx.debug_set(4, args.k1_warps)  # WHP_DEBUG_K1_WARPS
     lo, hi = harness.weak_rows(n_cand, rank)
     perms = W.perms_torch(wl.seed, n, lo, hi, dev)  # resident in HBM before the clock starts
     dist = torch.zeros(n_cand, dtype=torch.int64, device=dev)
@@ -568,7 +570,8 @@ def run_ours(args):
         "config": dict(config_dict(pb, n_cand, world, wl_nb),
                        streams=("candidate evaluation + argmin and neighbourhood pass + argmin + "
                                 "apply on two streams, one context each, joined every step")
-                       if overlap else "one stream, the calls of a step back to back"),
+                       if overlap else "one stream, the calls of a step back to back",
+                       k1_warps=args.k1_warps or "library default"),
         "neighbourhood": dict({"ms_per_iteration_eval_swaps": s_ms,
                                "ms_span_on_side_stream_in_step": s_span_ms,
                                "neighbours_per_s": nn / (s_ms * 1e-3),
@@ -607,6 +610,9 @@ def main():
                     help="1: also repeat the step for >= 2.5 s with the clocks sampled (N=1 only)")
     ap.add_argument("--stress", type=int, default=1, choices=[0, 1],
                     help="1: also time BASELINE.json's stress config at its full 65,536 plans (N=1 only)")
+    ap.add_argument("--k1-warps", type=int, default=0, choices=[0, 1, 2, 4],
+                    help="warps per block of the boundary kernel (whp_debug_set WHP_DEBUG_K1_WARPS; "
+                         "0 = the library's choice): the block-shape table of profiles/r2_head.md")
     ap.add_argument("--clock-period-ms", type=int, default=50,
                     help="nvidia-smi sampling period during the timed region")
     args = ap.parse_args()

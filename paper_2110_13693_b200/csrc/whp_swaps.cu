@@ -1,16 +1,20 @@
 // whp_swaps.cu — whp_eval_swaps (a6, D8): pairwise-swap neighbourhood of a base plan with
 // rescoring limited to the batches a swap can affect.
 //
-//   base pass   whp_swaps_base_kernel (one block): item-count prefix pre[p], order record per
-//               position, nxt[p] = end of the batch that would open at p, and the base batch
-//               starts (pointer doubling along nxt + a block scan: bstart[b], bop[p]).
+//   tables      whp_swaps_base_kernel (one block): item-count prefix pre[p], order record per
+//               position, nxt[p] = end of the batch that would open at p (binary search), and the
+//               base batch starts: the plan is cut into segments of >= C positions, every
+//               segment tabulates where a chain that enters it at its k-th position leaves it,
+//               one thread composes the segments' entry points, one thread per segment marks
+//               its boundaries, a block scan ranks them (bstart[b], bop[p]).
 //               whp_swaps_prep_kernel (multi-block): the hypothetical batch [p, nxt[p]) of every
 //               position of the window region and of every base batch start, one warp per batch
 //               with its picks flattened over the lanes (dist_at[p], cls_at[p]).
-//               whp_swaps_base2_kernel (one block): prefix of the base batch lengths bdist[b],
-//               class-count prefix rpre[b][k], base D, phi, J.
-//               whp_swaps_chain_kernel: per region position the sums along its chain
-//               p -> nxt[p] -> ... up to where it meets the base plan (dtail, rtail, bF).
+//               whp_swaps_tail_kernel (one launch, two block roles): the second half of the base
+//               pass — prefix of the base batch lengths bdist[b], class-count prefix rpre[b][k],
+//               base D, phi, J — and, per region position a neighbour can ask for, the sums along
+//               its chain p -> nxt[p] -> ... up to where it meets the base plan (dtail, rtail, bF).
+//               prep and tail are programmatic dependents of their predecessor.
 //   neighbours  one warp per swap (pi,pj). Next-fit only looks forward, so batches before the
 //               one holding pi are untouched — except that when pi opens its batch a smaller
 //               order may slip into the previous cart, so the rewalk then starts one batch
@@ -36,7 +40,7 @@ namespace {
 // The neighbour kernel itself is launched normally: as a third dependent it saves another 2 us
 // of the call alone (74.8 instead of 76.7 us at W = 256), but its 1184 blocks then sit resident
 // and idle on every SM while the tables are built, and a candidate evaluation running on
-// another stream loses 0.03 ms of a 0.43 ms step to that (profiles/r2_neighbourhood.md).
+// another stream loses 0.03 ms of a 0.43 ms step to that (profiles/r2_head.md).
 __device__ __forceinline__ void dep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void dep_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
 
