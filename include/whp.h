@@ -269,13 +269,16 @@ whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_ca
  *                            tabulate (0 forces the batch-by-batch fallback of every chain)
  *   WHP_DEBUG_K1_WARPS       warps per block of the tuned boundary kernel (1, 2 or 4: they share
  *                            one copy of the order table; ignored when it does not fit)
+ *   WHP_DEBUG_NO_FOURS       value != 0: pick tables that do not fit shared memory are read by the
+ *                            pair-load variant of the set kernel instead of the four-aligned one
  * Unknown keys return WHP_ERR_INVALID_ARG. There are no environment variables. */
 typedef enum {
   WHP_DEBUG_FORCE_GENERAL = 0,
   WHP_DEBUG_SEGMENTS = 1,
   WHP_DEBUG_WARPS = 2,
   WHP_DEBUG_SWAP_MARGIN = 3,
-  WHP_DEBUG_K1_WARPS = 4
+  WHP_DEBUG_K1_WARPS = 4,
+  WHP_DEBUG_NO_FOURS = 5
 } whp_debug_key;
 whp_status whp_debug_set(whp_ctx* ctx, int32_t key, int64_t value);
 

@@ -47,6 +47,7 @@ void dfree(T*& p) { if (p) { cudaFree(p); p = nullptr; } }
 
 void free_orders(whp_ctx* c) {
   dfree(c->d_order_rec); dfree(c->d_pick_rec); dfree(c->d_pick_fast); dfree(c->d_order_fast);
+  dfree(c->d_pick_f4); dfree(c->d_order_fast4);
   dfree(c->base.bstart); dfree(c->base.bop); dfree(c->base.bdist);
   dfree(c->base.resp); dfree(c->base.totals); dfree(c->base.pre);
   dfree(c->base.orec); dfree(c->base.rpre); dfree(c->base.nxt); dfree(c->base.dist_at);
@@ -233,6 +234,31 @@ whp_status whp_load_orders(whp_ctx* c, int32_t n_orders, const int32_t* order_pt
   WHP_CUDA(c, cudaMalloc(&c->d_order_fast, 4 * ofast.size()));
   WHP_CUDA(c, cudaMemcpy(c->d_pick_fast, pfast.data(), 4 * pfast.size(), cudaMemcpyHostToDevice));
   WHP_CUDA(c, cudaMemcpy(c->d_order_fast, ofast.data(), 4 * ofast.size(), cudaMemcpyHostToDevice));
+  // the four-aligned layout, for tables that cannot sit in shared memory beside K2's private state
+  // (built whenever the pair table takes more than half of it; the launch decides which is used)
+  if (fast_ok && 4 * pfast.size() > (size_t)c->smem_optin / 2) {
+    std::vector<uint32_t> ofast4((no + 3) & ~(size_t)3, 0u), pf4;
+    pf4.reserve((size_t)n_items + 3 * (size_t)n_orders);
+    bool ok4 = true;
+    for (int32_t o = 0; o < n_orders; ++o) {
+      const size_t cur = pf4.size() / 4;
+      if (cur > 0xffff) { ok4 = false; break; }
+      uint32_t r = 0;
+      for (int32_t i = order_ptr[o]; i < order_ptr[o + 1]; ++i) {
+        r = WHP_FAST_PACK(prec[i], i == order_ptr[o + 1] - 1);
+        pf4.push_back(r);
+      }
+      while (pf4.size() & 3) pf4.push_back(r);  // the order's last record again
+      pf4.back() |= WHP_FAST_LAST4;             // this four ends the order
+      ofast4[o] = ((uint32_t)cur << WHP_Q_BITS) | (uint32_t)(order_ptr[o + 1] - order_ptr[o]);
+    }
+    if (ok4) {
+      WHP_CUDA(c, cudaMalloc(&c->d_pick_f4, 4 * pf4.size()));
+      WHP_CUDA(c, cudaMalloc(&c->d_order_fast4, 4 * ofast4.size()));
+      WHP_CUDA(c, cudaMemcpy(c->d_pick_f4, pf4.data(), 4 * pf4.size(), cudaMemcpyHostToDevice));
+      WHP_CUDA(c, cudaMemcpy(c->d_order_fast4, ofast4.data(), 4 * ofast4.size(), cudaMemcpyHostToDevice));
+    }
+  }
   c->have_orders = true;
   return WHP_OK;
 }
@@ -579,6 +605,7 @@ whp_status whp_debug_set(whp_ctx* c, int32_t key, int64_t value) {
     case WHP_DEBUG_WARPS: c->dbg_warps = value > 0 && value <= 32 ? (int32_t)value : -1; break;
     case WHP_DEBUG_SWAP_MARGIN: c->dbg_swap_margin = value >= 0 ? value : -1; break;
     case WHP_DEBUG_K1_WARPS: c->dbg_k1_warps = value > 0 && value <= 4 ? (int32_t)value : -1; break;
+    case WHP_DEBUG_NO_FOURS: c->dbg_no_fours = value > 0 ? 1 : 0; break;
     default: return fail(c, WHP_ERR_INVALID_ARG, "unknown debug key");
   }
   return WHP_OK;

@@ -789,6 +789,289 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
   }
 }
 
+// ------------------------------------------------------------------------------------------ K2'
+// K2 for pick tables that do not fit shared memory (stress scale: 305 KB) and are gathered
+// through L1 / L2. The pair-load variant of whp_sets_kernel pays an L2 round trip per warp step
+// of ONE pick: the address of a lane's next load depends on the last-pick flag of the record it
+// is consuming, and with 32 lanes some lane needs a new pair at practically every step. Here the
+// table is the four-aligned layout (whp_internal.cuh: every order starts at a multiple of four
+// records and is padded to a multiple of four with copies of its last record — set inserts and
+// max are idempotent) and a step is one 16-byte load = four picks, so a batch takes as many
+// round trips as its longest lane has fours (~20 instead of C = 40 at stress scale) and the four
+// inserts of a step cover the latency of the next load. The last record of an order's last four
+// carries WHP_FAST_LAST4; a lane whose batch is exhausted keeps re-inserting its last four. The
+// step loop ends when no lane of the warp has a four left.
+__device__ __forceinline__ void ldg_four_if(uint4& q, const uint32_t* ptr, bool p) {
+  asm volatile("{ .reg .pred pq; setp.ne.u32 pq, %5, 0; @pq ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4]; }"
+               : "+r"(q.x), "+r"(q.y), "+r"(q.z), "+r"(q.w) : "l"(ptr), "r"((uint32_t)p));
+}
+
+template <bool DEPOT0, int KW, int kPlanes>
+__global__ void __launch_bounds__(KW * kPlanes <= 42 ? 768 : 512, 1)  // counter registers: KW x planes
+whp_sets4_kernel(const whp_tables T, const sets_params P, const uint32_t* __restrict__ pick_f4,
+                const uint16_t* __restrict__ cstream, const uint32_t* __restrict__ bmask,
+                const int32_t* __restrict__ nb_scratch, const int32_t* __restrict__ segstart,
+                int64_t n_cand, int64_t* __restrict__ dist_scratch,
+                uint32_t* __restrict__ planes_out, uint64_t* __restrict__ hash_out,
+                unsigned long long* __restrict__ task_counter, int64_t* __restrict__ o_dist,
+                double* __restrict__ o_pen, double* __restrict__ o_obj, int32_t* __restrict__ o_resp) {
+  extern __shared__ __align__(16) uint32_t smem[];
+  uint32_t* priv = smem;  // layout: [per-warp private words]
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int nwarps = blockDim.x >> 5;
+  // private state of a lane: aw_words aisle words and KW class words laid out [word][lane]
+  // (bank = lane), a warp's words aligned to their (power-of-two) size so that a word's
+  // address is base | offset; then the lane's cursor ring, lane-major, stride ring + 16 bytes
+  const int ring_stride = P.ring_mask + 1 + 16;
+  const uint32_t a_area = (smem_u32(priv) + P.awp * 128 - 1) & ~(uint32_t)(P.awp * 128 - 1);
+  const uint32_t c_area = a_area + nwarps * P.awp * 128;  // awp >= kwp: aligned as well
+  const uint32_t abase = a_area + warp * P.awp * 128 + lane * 4;
+  const uint32_t cbase = c_area + warp * P.kwp * 128 + lane * 4;
+  const uint32_t ringbase = c_area + nwarps * P.kwp * 128 + (warp * 32 + lane) * ring_stride;
+  const uint32_t amask = (uint32_t)(P.awp - 1) << 7;
+  const int chunks = (P.ring_mask + 1) >> 4;
+  const int64_t A = T.g.aisle_len;
+  const int64_t P2 = 2 * (int64_t)T.g.aisle_spacing;
+  const int n8 = P.cs_pitch >> 3;  // 16-byte chunks per cursor-stream row
+  for (int w = 0; w < P.aw_words; ++w) sts32(abase + w * 128, 0u);
+  for (int w = 0; w < KW; ++w) sts32(cbase + w * 128, 0u);
+  dep_wait();  // everything above reads only the pick table: it overlaps the segments kernel
+
+  __shared__ unsigned long long s_task[32];
+  for (;;) {
+    // claim the next warp task (32 consecutive (candidate, segment) pairs)
+    if (lane == 0) s_task[warp] = atomicAdd(task_counter, 1ull);
+    __syncwarp();
+    const int64_t task = (int64_t)s_task[warp];
+    __syncwarp();
+    if (task >= P.n_tasks) break;
+    const int64_t unit = task * 32 + lane;
+    const int64_t cand_raw = unit >> P.log2S;
+    const int seg = (int)(unit & (P.S - 1));
+    const bool have = cand_raw < n_cand;
+    const int64_t cand = have ? cand_raw : n_cand - 1;
+    int b_lo = 0, nbseg = 0;
+    if (have) {
+      const int nb = __ldg(nb_scratch + cand);
+      b_lo = (int)((int64_t)seg * nb >> P.log2S);
+      nbseg = (int)((int64_t)(seg + 1) * nb >> P.log2S) - b_lo;
+    }
+    const int nbmax = __reduce_max_sync(WHP_FULL, nbseg);
+    uint32_t pl[kPlanes][KW];
+#pragma unroll
+    for (int p = 0; p < kPlanes; ++p)
+#pragma unroll
+      for (int w = 0; w < KW; ++w) pl[p][w] = 0;
+
+    // ---- first batch of the segment: its start position comes from K1
+    const uint32_t* __restrict__ bm = bmask + cand * P.bm_pitch;
+    int p = __ldg(segstart + cand * P.ss_pitch + seg);
+    int wi = p >> 5;
+    uint32_t bw = __ldg(bm + wi) & (WHP_FULL << (p & 31));
+    uint32_t bw_next = __ldg(bm + min(wi + 1, P.bm_pitch - 1));
+
+    // ---- cursor stream of this lane through its private cp.async ring: chunk c (cursors of
+    // positions 8c..8c+7) lives at ring offset (16 c) mod ring
+    const uint4* __restrict__ cs = reinterpret_cast<const uint4*>(cstream + cand * P.cs_pitch);
+    // the last chunk this lane reads: the one that holds the first position of the next segment
+    // (a third of the ring traffic used to be chunks fetched past the end of the lane's run)
+    int c_last;
+    {
+      const int p_next = __shfl_down_sync(WHP_FULL, p, 1);
+      c_last = min((seg == P.S - 1 || lane == 31 ? T.n_orders : p_next) >> 3, n8 - 1);
+    }
+    int lo_prev;  // first chunk that was resident when the newest refill group was issued
+    {
+      const int c0 = p >> 3;
+      for (int k = 0; k < chunks; ++k)
+        if (c0 + k <= c_last) cp_async16(ringbase + (((c0 + k) << 4) & P.ring_mask), cs + c0 + k);
+      cp_async_commit();
+      lo_prev = c0 - chunks;
+    }
+
+    int64_t D = 0;
+    uint64_t hash = 0;
+    uint4 q4 = make_uint4(0u, 0u, 0u, 0u);
+    for (int j = 0; j < nbmax; ++j) {
+      int left = 0;  // orders of batch j
+      const int p0 = p;
+      if (j < nbseg) {
+        bw &= bw - 1;  // past my own start bit: the next set bit is the next batch (or the end)
+        while (bw == 0) {
+          ++wi;
+          bw = bw_next;
+          bw_next = __ldg(bm + min(wi + 1, P.bm_pitch - 1));
+        }
+        const int pe = 32 * wi + __ffs(bw) - 1;
+        hash += (uint64_t)(uint32_t)(p + 1) * (uint64_t)(uint32_t)(2 * (b_lo + j) + 1);
+        left = pe - p;
+        p = pe;
+      }
+      const bool live = left > 0;
+      // the newest refill group brought chunks lo_prev+chunks ..; everything older has landed
+      // after wait<1>. The batch reads cursors of positions p0 .. p (one ahead).
+      if (live && (p >> 3) >= lo_prev + chunks) cp_async_wait<0>(); else cp_async_wait<1>();
+      // ---- the batch's picks, four records per step
+      uint32_t v = 2u * (uint32_t)p0;                      // 2 x position of the next order
+      const uint32_t v_end = live ? 2u * (uint32_t)p : v;
+      uint32_t cur4 = lds16(ringbase + (v & P.ring_mask));  // the four being loaded
+      v += live ? 2u : 0u;
+      uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));  // first four of the next order
+      bool have = live;
+      // (a lane without a batch keeps the four of its previous batch: its sets are discarded)
+      ldg_four_if(q4, pick_f4 + 4 * (size_t)cur4, have);
+      uint32_t kmax = 0, kmin = 0xffffffffu;
+      uint32_t cset = 0;  // KW == 1: class set of the batch
+      auto insert = [&](uint32_t rec) {
+        kmax = max(kmax, rec);
+        if (!DEPOT0) kmin = min(kmin, rec);
+        const uint32_t aaddr = abase | ((rec >> 20) & amask);
+        sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 22));
+        if (KW == 1) {
+          cset |= one_shl_wrap(rec);
+        } else {
+          const uint32_t caddr = cbase | (rec & 0x380u);
+          sts32(caddr, lds32(caddr) | one_shl_wrap(rec));
+        }
+      };
+      while (__any_sync(WHP_FULL, have)) {
+        const uint32_t r0 = q4.x, r1 = q4.y, r2 = q4.z, r3 = q4.w;
+        // where the next four is: the next one of this order, the first one of the next order,
+        // or nowhere (then the lane stays on this four)
+        const bool last4 = (r3 & WHP_FAST_LAST4) != 0u;
+        const bool next_order = last4 && (v != v_end);
+        have = have && (!last4 || next_order);
+        cur4 = next_order ? n_c16 : cur4 + 1u;
+        v += next_order ? 2u : 0u;
+        lds16_if(n_c16, ringbase + (v & P.ring_mask), next_order);
+        ldg_four_if(q4, pick_f4 + 4 * (size_t)cur4, have);
+        insert(r0); insert(r1); insert(r2); insert(r3);
+      }
+      {  // refill the slots of the chunks this batch finished; waited for two batches later
+        const int nf = live ? (p >> 3) - (p0 >> 3) : 0;
+        const int nfmax = __reduce_max_sync(WHP_FULL, nf);
+        for (int i = 0; i < nfmax; ++i) {
+          const int c = (p0 >> 3) + i;
+          if (i < nf && c + chunks <= c_last) cp_async16(ringbase + ((c << 4) & P.ring_mask), cs + c + chunks);
+        }
+        cp_async_commit();
+        if (live) lo_prev = p0 >> 3;
+      }
+      // ---- close the batch: m = distinct aisles, D4; the sets are emptied for the next batch
+      int m = 0;
+#pragma unroll 4
+      for (int w = 0; w < P.aw_words; ++w) {
+        m += __popc(lds32(abase + w * 128));
+        sts32(abase + w * 128, 0u);
+      }
+      if (live) {
+        const uint32_t a_max = WHP_FAST_AISLE(kmax);
+        const uint32_t slot1 = WHP_FAST_SLOT1(kmax);
+        if (DEPOT0 && P.fits32) {
+          const uint32_t d2 = 2u * slot1 * (uint32_t)T.g.slot_pitch;
+          D += (uint32_t)P2 * a_max + (uint32_t)m * (uint32_t)A + ((m & 1) ? d2 - (uint32_t)A : 0u);
+        } else {
+          const int64_t d_last = (int64_t)slot1 * T.g.slot_pitch;
+          int64_t H;
+          if (DEPOT0) {
+            H = P2 * (int64_t)a_max;
+          } else {
+            const int64_t a_min = WHP_FAST_AISLE(kmin), a0 = T.g.depot_aisle;
+            H = (int64_t)T.g.aisle_spacing *
+                (llabs(a0 - a_min) + ((int64_t)a_max - a_min) + llabs((int64_t)a_max - a0));
+          }
+          D += H + ((m & 1) ? (int64_t)(m - 1) * A + 2 * d_last : (int64_t)m * A);
+        }
+      }
+      // the batch's class set goes into the vertical counters (D5)
+#pragma unroll
+      for (int w = 0; w < KW; ++w) {
+        // lanes without a batch j ran the steps on a dummy pick: their set is discarded
+        uint32_t carry;
+        if (KW == 1) {
+          carry = cset;
+        } else {
+          carry = lds32(cbase + w * 128);
+          sts32(cbase + w * 128, 0u);
+        }
+        if (!live) carry = 0u;
+#pragma unroll
+        for (int pp = 0; pp < kPlanes; ++pp) {
+          const uint32_t t2 = pl[pp][w] & carry;
+          pl[pp][w] ^= carry;
+          carry = t2;
+        }
+      }
+    }
+    cp_async_wait<0>();  // nothing of this task may still land in the ring
+    // ---- combine the S segment lanes of each candidate (D, hash); write the counters
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1)
+      if (o < P.S) {
+        D += __shfl_xor_sync(WHP_FULL, D, o);
+        hash += __shfl_xor_sync(WHP_FULL, hash, o);
+      }
+    const bool fused = P.S == 32;  // the warp is one plan: it finishes D6 itself (no K3)
+    if (have && seg == 0) {
+      if (!fused) dist_scratch[cand] = D;
+      if (hash_out) hash_out[cand] = hash;
+    }
+    double phi = 0.0;
+    // bit-sliced addition of the S lanes' vertical counters (one more plane per level)
+    {
+      uint32_t* __restrict__ po = planes_out + cand * (kPlaneRow * KW);
+#pragma unroll
+      for (int w = 0; w < KW; ++w) {
+        uint32_t a[kPlanes + 5];
+#pragma unroll
+        for (int pp = 0; pp < kPlanes + 5; ++pp) a[pp] = pp < kPlanes ? pl[pp][w] : 0u;
+#pragma unroll
+        for (int lvl = 0; lvl < 5; ++lvl) {
+          if ((1 << lvl) < P.S) {
+            uint32_t carry = 0;
+#pragma unroll
+            for (int pp = 0; pp < kPlanes + lvl; ++pp) {
+              const uint32_t b = __shfl_xor_sync(WHP_FULL, a[pp], 1 << lvl);
+              const uint32_t sum = a[pp] ^ b ^ carry;
+              carry = (a[pp] & b) | (carry & (a[pp] ^ b));
+              a[pp] = sum;
+            }
+            a[kPlanes + lvl] = carry;
+          }
+        }
+        if (fused) {
+          // every lane holds the plan's counters: lane l decodes r_k of class 32w + l and adds
+          // its term — ascending w, lane = k mod 32: the canonical accumulation of D6
+          uint32_t r = 0;
+#pragma unroll
+          for (int pp = 0; pp < kPlanes + 5; ++pp) r |= ((a[pp] >> lane) & 1u) << pp;
+          const int k = 32 * w + lane;
+          if (k < T.K) {
+            if (o_resp && have) o_resp[cand * T.K + k] = (int32_t)r;
+            const double c = __dsub_rn(__ldg(T.tvw + k), (double)r);
+            const double u = __dmul_rn(__ldg(T.tvw + 2 * T.K + k), c);
+            phi = __dadd_rn(phi, __dadd_rn(__dmul_rn(__ldg(T.tvw + T.K + k), c), __dmul_rn(u, u)));
+          }
+        } else if (have && seg == 0) {
+#pragma unroll
+          for (int pp = 0; pp < kPlanes + 5; ++pp)
+            if (pp < kPlanes + P.log2S) po[pp * KW + w] = a[pp];
+        }
+      }
+    }
+    if (fused) {
+#pragma unroll
+      for (int off = 16; off >= 1; off >>= 1) phi = __dadd_rn(phi, __shfl_xor_sync(WHP_FULL, phi, off));
+      if (have && lane == 0) {
+        if (o_dist) o_dist[cand] = D;
+        if (o_pen) o_pen[cand] = phi;
+        if (o_obj) o_obj[cand] = __dadd_rn((double)D, phi);
+      }
+    }
+    __syncwarp();
+  }
+}
+
 // ------------------------------------------------------------------------------------------ KL
 // NEXT-2 tuned: leg sums (reading N2) on the K1 outputs. Same decomposition as K2 — one lane per
 // (plan, segment), one pick per branch-free step — but a step only adds the leg from the previous
@@ -1072,7 +1355,8 @@ static cudaError_t ensure_fast_scratch(whp_ctx* c, int64_t n_cand, int64_t plane
 // K1 (batch boundaries, cursor stream) and the segment starts of every plan
 static cudaError_t launch_bounds_and_segments(whp_ctx* c, const void* d_perms, int64_t n_cand, int S,
                                               int log2S, int32_t* n_batches_out, cudaStream_t st,
-                                              bool perm16 = false) {
+                                              bool perm16 = false, const uint32_t* order_table = nullptr) {
+  if (!order_table) order_table = c->d_order_fast;  // else: cursors of the four-aligned layout
   const int32_t bm_pitch = fast_bm_pitch(c), cs_pitch = fast_cs_pitch(c), ss_pitch = kSsPitch;
   {
     // (Folding this reset into the segments kernel saves 1 us of the evaluation alone and costs
@@ -1130,7 +1414,7 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const void* d_perms, i
     cudaFuncSetAttribute(whp_bounds_kernel<KW1, U16V>,                                          \
                          cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin - 1024);    \
     whp_bounds_kernel<KW1, U16V><<<blocks, 32 * KW1, smem, st>>>(                               \
-        tmap, tmap_cs, c->d_order_fast, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch,        \
+        tmap, tmap_cs, order_table, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch,            \
         c->d_cstream, cs_pitch);                                                                \
   } while (0)
 #define WHP_LAUNCH_BOUNDS(KW1)                                                                  \
@@ -1172,6 +1456,8 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const void* d_perms, int64_t n_cand
   const size_t priv_per_warp = (size_t)(kwp + awp) * 128 + 32 * (size_t)(ring_bytes + 16);
   const size_t smem_max = (size_t)c->smem_optin - 1024 - (size_t)awp * 128;  // alignment slack
   const bool smem_tables = table_bytes + 4 * priv_per_warp <= smem_max;
+  // tables beyond shared memory: the four-aligned layout (K2')
+  const bool fours = !smem_tables && c->d_pick_f4 != nullptr && !c->dbg_no_fours;
   const size_t avail = smem_max - (smem_tables ? table_bytes : 0);
   // segments: few enough batches per segment for the counter planes, and >= 4 tasks per warp
   int warps_cap = 24;
@@ -1198,7 +1484,8 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const void* d_perms, int64_t n_cand
   const int fits32 = worst < (1ll << 31) ? 1 : 0;
   cudaError_t e0 = ensure_fast_scratch(c, n_cand, (int64_t)kPlaneRow * KW, st);
   if (e0 != cudaSuccess) return e0;
-  if ((e0 = launch_bounds_and_segments(c, d_perms, n_cand, S, log2S, out.n_batches, st, perm16)) != cudaSuccess)
+  if ((e0 = launch_bounds_and_segments(c, d_perms, n_cand, S, log2S, out.n_batches, st, perm16,
+                                       fours ? c->d_order_fast4 : nullptr)) != cudaSuccess)
     return e0;
   // K2
   {
@@ -1246,13 +1533,53 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const void* d_perms, int64_t n_cand
     else if (KW == 7) WHP_LAUNCH_SETS(ST, D0, 7);                                                \
     else WHP_LAUNCH_SETS(ST, D0, 8);                                                             \
   } while (0)
-    if (smem_tables && depot0) WHP_LAUNCH_SETS_KW(true, true);
+#define WHP_LAUNCH_SETS4_PL(D0, KWV, PLV)                                                        \
+  do {                                                                                           \
+    cudaFuncSetAttribute(whp_sets4_kernel<D0, KWV, PLV>,                                         \
+                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(c->smem_optin - 1024)); \
+    cudaLaunchConfig_t cfg{};                                                                    \
+    cfg.gridDim = dim3((unsigned)blocks);                                                        \
+    cfg.blockDim = dim3(warps * 32);                                                             \
+    cfg.dynamicSmemBytes = smem;                                                                 \
+    cfg.stream = st;                                                                             \
+    cudaLaunchAttribute attr[1];                                                                 \
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;                             \
+    attr[0].val.programmaticStreamSerializationAllowed = 1;                                      \
+    cfg.attrs = attr;                                                                            \
+    cfg.numAttrs = 1;                                                                            \
+    cudaLaunchKernelEx(&cfg, whp_sets4_kernel<D0, KWV, PLV>, T, P,                               \
+                       (const uint32_t*)c->d_pick_f4,                                            \
+                       (const uint16_t*)c->d_cstream, (const uint32_t*)c->d_bmask,               \
+                       (const int32_t*)c->d_nb, (const int32_t*)c->d_segstart, n_cand,           \
+                       c->d_dist_scratch, c->d_planes, out.batch_hash, c->d_task, out.dist,      \
+                       out.penalty, out.obj, out.resp);                                          \
+  } while (0)
+#define WHP_LAUNCH_SETS4(D0, KWV)                                                                \
+  do {                                                                                           \
+    if (kernel_planes == 4) WHP_LAUNCH_SETS4_PL(D0, KWV, 4);                                     \
+    else if (kernel_planes == 6) WHP_LAUNCH_SETS4_PL(D0, KWV, 6);                                \
+    else WHP_LAUNCH_SETS4_PL(D0, KWV, 8);                                                        \
+  } while (0)
+#define WHP_LAUNCH_SETS4_KW(D0)                                                                  \
+  do {                                                                                           \
+    if (KW == 1) WHP_LAUNCH_SETS4(D0, 1);                                                        \
+    else if (KW == 2) WHP_LAUNCH_SETS4(D0, 2);                                                   \
+    else if (KW == 4) WHP_LAUNCH_SETS4(D0, 4);                                                   \
+    else if (KW == 7) WHP_LAUNCH_SETS4(D0, 7);                                                   \
+    else WHP_LAUNCH_SETS4(D0, 8);                                                                \
+  } while (0)
+    if (fours && depot0) WHP_LAUNCH_SETS4_KW(true);
+    else if (fours) WHP_LAUNCH_SETS4_KW(false);
+    else if (smem_tables && depot0) WHP_LAUNCH_SETS_KW(true, true);
     else if (smem_tables) WHP_LAUNCH_SETS_KW(true, false);
     else if (depot0) WHP_LAUNCH_SETS_KW(false, true);
     else WHP_LAUNCH_SETS_KW(false, false);
 #undef WHP_LAUNCH_SETS_KW
 #undef WHP_LAUNCH_SETS
 #undef WHP_LAUNCH_SETS_PL
+#undef WHP_LAUNCH_SETS4_KW
+#undef WHP_LAUNCH_SETS4
+#undef WHP_LAUNCH_SETS4_PL
     c->launches += 1;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;

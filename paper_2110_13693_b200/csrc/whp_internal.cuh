@@ -27,10 +27,11 @@
 #define WHP_PICK_CLASS_MASK 0xffu
 
 // pick record of the tuned candidate path (whp_fast.cu), built from the record above:
-//   aisle[31:22] | slot1[21:10] | class>>5 [9:7] | 0 [6] | last-pick-of-its-order [5] | class&31 [4:0]
+//   aisle[31:22] | slot1[21:10] | class>>5 [9:7] | last-four [6] | last-pick-of-its-order [5] | class&31 [4:0]
 //   (rec >> 20) & (words-1)<<7 and rec & 0x380 are the byte offsets of the 32-aisle and the
 //   32-class occupancy words of a lane; (rec >> 22) mod 32 and rec mod 32 the bits inside them.
 #define WHP_FAST_LAST 0x20u
+#define WHP_FAST_LAST4 0x40u /* four-aligned layout: last record of the order's last four */
 #define WHP_FAST_PACK(rec, last)                                                              \
   ((WHP_PICK_AISLE(rec) << 22) | ((((rec) >> WHP_PICK_SLOT_SHIFT) & WHP_PICK_SLOT_MASK) << 10) | \
    ((((rec) & WHP_PICK_CLASS_MASK) >> 5) << 7) | ((last) ? WHP_FAST_LAST : 0u) | ((rec) & 31u))
@@ -104,6 +105,14 @@ struct whp_ctx {
   uint32_t* d_order_fast = nullptr;
   int32_t n_items_pad = 0;
   bool fast_tables_ok = false;
+  // second layout for pick tables that do not fit shared memory (K2 gathers them through L1 / L2,
+  // whp_sets4_kernel): every order's picks start at a multiple of FOUR and are padded to a
+  // multiple of four by repeating the order's last record (set inserts and max are idempotent);
+  // the last record of an order's last four carries WHP_FAST_LAST4;
+  // order_fast4 = (first_pick_index/4) << 8 | q. Null when the pair table is small or the
+  // four-cursors overflow 16 bits.
+  uint32_t* d_pick_f4 = nullptr;
+  uint32_t* d_order_fast4 = nullptr;
   double* d_tvw = nullptr;
   bool have_orders = false, have_penalty = false;
   // scratch
@@ -145,7 +154,7 @@ struct whp_ctx {
   int num_sms = 148;
   int64_t launches = 0;
   // whp_debug_set: kernel-selection overrides for tests and measurements (-1 / 0 = default)
-  int32_t dbg_force_general = 0, dbg_segments = -1, dbg_warps = -1, dbg_k1_warps = -1;
+  int32_t dbg_force_general = 0, dbg_segments = -1, dbg_warps = -1, dbg_k1_warps = -1, dbg_no_fours = 0;
   int64_t dbg_swap_margin = -1;
   std::string err;
 };

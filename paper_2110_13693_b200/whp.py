@@ -29,7 +29,7 @@ SYMBOLS = ["whp_create_layout", "whp_load_orders", "whp_set_penalty", "whp_eval_
            "whp_argmin_static_setup", "whp_argmin_static", "whp_static_last_error"]
 
 ROUTE_S_SHAPE, ROUTE_RETURN, ROUTE_LARGEST_GAP = range(3)
-DEBUG_FORCE_GENERAL, DEBUG_SEGMENTS, DEBUG_WARPS, DEBUG_SWAP_MARGIN, DEBUG_K1_WARPS = range(5)
+DEBUG_FORCE_GENERAL, DEBUG_SEGMENTS, DEBUG_WARPS, DEBUG_SWAP_MARGIN, DEBUG_K1_WARPS, DEBUG_NO_FOURS = range(6)
 ARGMIN_STATIC_MAX_N = 4096 * 4096  # WHP_ARGMIN_STATIC_MAX_N
 
 

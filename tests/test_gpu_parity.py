@@ -246,6 +246,45 @@ def test_stress_full_size_sampled_oracle(torch_cuda):
     ctx.close()
 
 
+BIG_TABLES = [
+    # pick tables beyond shared memory (the tuned path gathers them through L1 / L2)
+    dict(NA=400, S=250, K=32, n_skus=20000, n_orders=16000, qmax=5, C=40),              # stress-like
+    dict(NA=400, S=250, K=200, n_skus=20000, n_orders=12000, qmax=7, C=30, depot=123),  # 7 class words
+    dict(NA=1024, S=100, K=64, n_skus=9000, n_orders=30000, qmax=1, C=17, pitch=2),     # one-pick orders
+    dict(NA=90, S=4095, K=256, n_skus=9000, n_orders=9000, qmax=13, C=64, spacing=9),   # many fours an order
+]
+
+
+@pytest.mark.parametrize("cfg", BIG_TABLES, ids=lambda c: "-".join(f"{k}{v}" for k, v in c.items()))
+def test_tables_beyond_shared_memory_both_set_kernels(torch_cuda, cfg):
+    """The four-aligned set kernel (default) and the pair-load variant (WHP_DEBUG_NO_FOURS) both
+    equal the oracle, with every segment count, on candidate counts that leave warp tails."""
+    torch = torch_cuda
+    from paper_2110_13693_b200 import whp
+    pb = _random_problem(23, **cfg)
+    ctx = whp.Context.from_problem(pb)
+    perms = W.perm_rows(5, pb.n_orders, np.arange(37))
+    ref = oracle.eval_candidates(pb, perms, detail=True)
+    d_perms = torch.from_numpy(perms).cuda()
+    for no_fours in (0, 1):
+        ctx.debug_set(whp.DEBUG_NO_FOURS, no_fours)
+        for seg in (-1, 8, 32):
+            ctx.debug_set(whp.DEBUG_SEGMENTS, seg)
+            got, _ = gpu_eval(torch, ctx, d_perms)
+            assert_parity(got, ref, pb)
+            resp = torch.zeros((37, pb.n_classes), dtype=torch.int32, device="cuda")
+            ctx.eval_candidates(d_perms, resp=resp)
+            torch.cuda.synchronize()
+            assert np.array_equal(resp.cpu().numpy(), ref["resp"])
+    ctx.debug_set(whp.DEBUG_NO_FOURS, -1)
+    ctx.debug_set(whp.DEBUG_SEGMENTS, -1)
+    leg = torch.full((37,), -1, dtype=torch.int64, device="cuda")
+    ctx.eval_legsum(d_perms, leg)  # the leg kernel keeps the pair layout
+    torch.cuda.synchronize()
+    assert np.array_equal(leg.cpu().numpy(), oracle.eval_legsum(pb, perms))
+    ctx.close()
+
+
 def test_more_orders_than_the_tuned_path_indexes(torch_cuda):
     """66,000 orders: positions no longer fit the 16-bit cursors, so evaluation, leg sums and the
     neighbourhood all take their general kernels (and the swap base pass runs without
