@@ -610,7 +610,7 @@ def main():
                     help="1: also repeat the step for >= 2.5 s with the clocks sampled (N=1 only)")
     ap.add_argument("--stress", type=int, default=1, choices=[0, 1],
                     help="1: also time BASELINE.json's stress config at its full 65,536 plans (N=1 only)")
-    ap.add_argument("--k1-warps", type=int, default=0, choices=[0, 1, 2, 4],
+    ap.add_argument("--k1-warps", type=int, default=0, choices=[0, 1, 2, 4, 5],
                     help="warps per block of the boundary kernel (whp_debug_set WHP_DEBUG_K1_WARPS; "
                          "0 = the library's choice): the block-shape table of profiles/r2_head.md")
     ap.add_argument("--clock-period-ms", type=int, default=50,

@@ -267,7 +267,7 @@ whp_status whp_validate_perms(whp_ctx* ctx, const int32_t* d_perms, int64_t n_ca
  *   WHP_DEBUG_WARPS          warps per block of the tuned set kernel (capped by what fits)
  *   WHP_DEBUG_SWAP_MARGIN    positions after the window that whp_eval_swaps / whp_eval_moves
  *                            tabulate (0 forces the batch-by-batch fallback of every chain)
- *   WHP_DEBUG_K1_WARPS       warps per block of the tuned boundary kernel (1, 2 or 4: they share
+ *   WHP_DEBUG_K1_WARPS       warps per block of the tuned boundary kernel (1, 2, 4 or 5: they share
  *                            one copy of the order table; ignored when it does not fit)
  *   WHP_DEBUG_NO_FOURS       value != 0: pick tables that do not fit shared memory are read by the
  *                            pair-load variant of the set kernel instead of the four-aligned one

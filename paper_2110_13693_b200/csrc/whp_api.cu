@@ -604,7 +604,7 @@ whp_status whp_debug_set(whp_ctx* c, int32_t key, int64_t value) {
     case WHP_DEBUG_SEGMENTS: c->dbg_segments = value > 0 && value <= 32 ? (int32_t)value : -1; break;
     case WHP_DEBUG_WARPS: c->dbg_warps = value > 0 && value <= 32 ? (int32_t)value : -1; break;
     case WHP_DEBUG_SWAP_MARGIN: c->dbg_swap_margin = value >= 0 ? value : -1; break;
-    case WHP_DEBUG_K1_WARPS: c->dbg_k1_warps = value > 0 && value <= 4 ? (int32_t)value : -1; break;
+    case WHP_DEBUG_K1_WARPS: c->dbg_k1_warps = value > 0 && value <= 5 ? (int32_t)value : -1; break;
     case WHP_DEBUG_NO_FOURS: c->dbg_no_fours = value > 0 ? 1 : 0; break;
     default: return fail(c, WHP_ERR_INVALID_ARG, "unknown debug key");
   }

@@ -72,6 +72,7 @@ __device__ __forceinline__ void dep_trigger() { asm volatile("griddepcontrol.lau
 // the order ids of word w+1 leave the tile and their order records are gathered from the table
 // in shared memory — so that a lone warp per scheduler keeps issuing.
 constexpr int kStages = 7;           // tiles (words) in flight per warp
+constexpr int kStagesWide = 5;       // ... of the five-warp block (multi-wave launches, see bounds_shape)
 constexpr int kTileBytes = 32 * 128; // 32 rows x 32 positions x 4 B
 
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -198,34 +199,35 @@ __device__ __forceinline__ uint32_t recur_word(const uint32_t (&r)[32], uint32_t
 
 // kWarps: warps per block, they share the order table (a warp = 32 plans). U16: the plan matrix
 // holds 16-bit order ids (whp_eval_candidates_host16): a tile is then 32 plans x 64 positions.
-template <int kWarps, bool U16>
+// kSt: tiles in flight per warp.
+template <int kWarps, bool U16, int kSt>
 __global__ void __launch_bounds__(32 * kWarps)
 whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap tmap_cs,
                   const uint32_t* __restrict__ order_fast,
                   int32_t n_orders, int32_t C, int64_t n_cand, uint32_t* __restrict__ bmask,
                   int32_t bm_pitch, uint16_t* __restrict__ cstream, int32_t cs_pitch) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  // per warp: [tiles: kStages x 4 KB, 1 KB aligned (swizzle)][cursor tiles: 2 x 4 KB]; then
-  // the order table shared by the block's warps and the mbarriers (kStages per warp + 1)
+  // per warp: [tiles: kSt x 4 KB, 1 KB aligned (swizzle)][cursor tiles: 2 x 4 KB]; then
+  // the order table shared by the block's warps and the mbarriers (kSt per warp + 1)
   const int nw = (n_orders + 31) >> 5;
   const int lane = threadIdx.x & 31, wq = threadIdx.x >> 5;
   const uint32_t area = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  const uint32_t tiles = area + wq * (kStages + 2) * kTileBytes;
-  const uint32_t otiles = tiles + kStages * kTileBytes;  // 32 rows x 64 cursors, two of them
-  const uint32_t sorec0 = area + kWarps * (kStages + 2) * kTileBytes;
+  const uint32_t tiles = area + wq * (kSt + 2) * kTileBytes;
+  const uint32_t otiles = tiles + kSt * kTileBytes;  // 32 rows x 64 cursors, two of them
+  const uint32_t sorec0 = area + kWarps * (kSt + 2) * kTileBytes;
   const uint32_t bar_table = sorec0 + 4u * (uint32_t)((n_orders + 3) & ~3);
-  const uint32_t bars = bar_table + 8 + 8 * kStages * wq;
+  const uint32_t bars = bar_table + 8 + 8 * kSt * wq;
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages * kWarps + 1; ++s) mbar_init(bar_table + 8 * s, 1);
+    for (int s = 0; s < kSt * kWarps + 1; ++s) mbar_init(bar_table + 8 * s, 1);
   }
   asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   __syncthreads();
   const int64_t row0 = ((int64_t)blockIdx.x * kWarps + wq) * 32;  // first plan of this warp
   const int nt = U16 ? (nw + 1) >> 1 : nw;  // tiles of a plan
-  auto issue = [&](int t) {  // one lane: tile t into stage t mod kStages
-    const uint32_t bar = bars + 8 * (t % kStages);
+  auto issue = [&](int t) {  // one lane: tile t into stage t mod kSt
+    const uint32_t bar = bars + 8 * (t % kSt);
     mbar_expect_tx(bar, kTileBytes);
-    tma_tile_2d(tiles + (t % kStages) * kTileBytes, &tmap, (U16 ? 64 : 32) * t, (int32_t)row0, bar);
+    tma_tile_2d(tiles + (t % kSt) * kTileBytes, &tmap, (U16 ? 64 : 32) * t, (int32_t)row0, bar);
   };
   if (threadIdx.x == 0) {  // the order table: one bulk copy (n_orders is a multiple of 4)
     const uint32_t table_bytes = 4u * (uint32_t)((n_orders + 3) & ~3);  // the table is padded
@@ -233,23 +235,23 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
     bulk_g2s(sorec0, order_fast, table_bytes, bar_table);
   }
   if (lane == 0)
-    for (int t = 0; t < kStages && t < nt; ++t) issue(t);
+    for (int t = 0; t < kSt && t < nt; ++t) issue(t);
   const int64_t c = row0 + lane;
   const bool have = c < n_cand;  // rows past the end arrive zero-filled: order 0, never written
   uint32_t* __restrict__ bm = bmask + (have ? c : 0) * bm_pitch;
   uint4* __restrict__ cs = reinterpret_cast<uint4*>(cstream + (have ? c : 0) * cs_pitch);
   const uint32_t rowoff = lane * 128, swz = (lane & 7) << 4;
   auto tile_of = [&](int w) { return U16 ? w >> 1 : w; };
-  auto tile_row = [&](int w) { return tiles + (tile_of(w) % kStages) * kTileBytes + rowoff; };
+  auto tile_row = [&](int w) { return tiles + (tile_of(w) % kSt) * kTileBytes + rowoff; };
   auto wait_word = [&](int w) {
-    mbar_wait(bars + 8 * (tile_of(w) % kStages), (tile_of(w) / kStages) & 1);
+    mbar_wait(bars + 8 * (tile_of(w) % kSt), (tile_of(w) / kSt) & 1);
   };
   auto refill = [&](int w) {  // word w is consumed by every lane: its stage takes the next tile
     // (the tile was only READ, and every value read has been used: no proxy fence is needed
     // before the async proxy overwrites it)
     if (U16 && !(w & 1)) return;  // the tile's second word is still to come
     __syncwarp();
-    if (lane == 0 && tile_of(w) + kStages < nt) issue(tile_of(w) + kStages);
+    if (lane == 0 && tile_of(w) + kSt < nt) issue(tile_of(w) + kSt);
   };
   uint32_t room = (uint32_t)C;
   uint32_t ra[32], rb[32];
@@ -922,11 +924,16 @@ whp_sets4_kernel(const whp_tables T, const sets_params P, const uint32_t* __rest
       ldg_four_if(q4, pick_f4 + 4 * (size_t)cur4, have);
       uint32_t kmax = 0, kmin = 0xffffffffu;
       uint32_t cset = 0;  // KW == 1: class set of the batch
+      int m = 0;          // distinct aisles of the batch
       auto insert = [&](uint32_t rec) {
         kmax = max(kmax, rec);
         if (!DEPOT0) kmin = min(kmin, rec);
+        // the distinct aisles are counted as they arrive (the close then only clears the words:
+        // this kernel is bound by the L1 data pipe, and the count costs no wavefront here)
         const uint32_t aaddr = abase | ((rec >> 20) & amask);
-        sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 22));
+        const uint32_t aold = lds32(aaddr), anew = aold | one_shl_wrap(rec >> 22);
+        m += (anew != aold) ? 1 : 0;
+        sts32(aaddr, anew);
         if (KW == 1) {
           cset |= one_shl_wrap(rec);
         } else {
@@ -958,12 +965,8 @@ whp_sets4_kernel(const whp_tables T, const sets_params P, const uint32_t* __rest
         if (live) lo_prev = p0 >> 3;
       }
       // ---- close the batch: m = distinct aisles, D4; the sets are emptied for the next batch
-      int m = 0;
 #pragma unroll 4
-      for (int w = 0; w < P.aw_words; ++w) {
-        m += __popc(lds32(abase + w * 128));
-        sts32(abase + w * 128, 0u);
-      }
+      for (int w = 0; w < P.aw_words; ++w) sts32(abase + w * 128, 0u);
       if (live) {
         const uint32_t a_max = WHP_FAST_AISLE(kmax);
         const uint32_t slot1 = WHP_FAST_SLOT1(kmax);
@@ -1284,18 +1287,24 @@ whp_finish_kernel(const whp_tables T, int64_t n_cand, const int64_t* __restrict_
 // upper bound on the number of batches of any plan (derived in whp_load_orders)
 static int64_t nb_upper_bound(const whp_ctx* c) { return c->nb_ub; }
 
+static int bounds_stages(int warps) { return warps == 5 ? kStagesWide : kStages; }
 static size_t bounds_smem_bytes(const whp_ctx* c, int warps = 1) {
-  return 1024 + (size_t)warps * (kStages + 2) * kTileBytes +
-         4 * (((size_t)c->n_orders + 3) & ~(size_t)3) + 8 * ((size_t)warps * kStages + 1);
+  const int st = bounds_stages(warps);
+  return 1024 + (size_t)warps * (st + 2) * kTileBytes +
+         4 * (((size_t)c->n_orders + 3) & ~(size_t)3) + 8 * ((size_t)warps * st + 1);
 }
 // K1 wants four resident warps per SM (one per scheduler): blocks of one warp when four of
 // them fit, else two or four warps that share one copy of the order table
-static int bounds_warps(const whp_ctx* c) {
+static int bounds_warps(const whp_ctx* c, int64_t n_cand) {
   const size_t cap = (size_t)c->smem_optin;
-  if (c->dbg_k1_warps == 1 || c->dbg_k1_warps == 2 || c->dbg_k1_warps == 4)  // WHP_DEBUG_K1_WARPS
+  if (c->dbg_k1_warps == 1 || c->dbg_k1_warps == 2 || c->dbg_k1_warps == 4 || c->dbg_k1_warps == 5)  // WHP_DEBUG_K1_WARPS
     if (bounds_smem_bytes(c, c->dbg_k1_warps) + 1024 <= cap) return c->dbg_k1_warps;
   if (4 * (bounds_smem_bytes(c, 1) + 1024) <= cap) return 1;
   if (2 * (bounds_smem_bytes(c, 2) + 1024) <= cap) return 2;
+  // one block per SM: when the launch takes several waves of four-warp blocks, five warps with
+  // five tiles in flight each make the waves fewer (a warp's time is set by its plan's serial
+  // recurrence, not by the tiles in flight: stress scale 4 -> 3 waves)
+  if (bounds_smem_bytes(c, 5) + 1024 <= cap && n_cand > 128ll * c->num_sms) return 5;
   if (bounds_smem_bytes(c, 4) + 1024 <= cap) return 4;
   if (bounds_smem_bytes(c, 2) + 1024 <= cap) return 2;
   return 1;
@@ -1364,7 +1373,7 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const void* d_perms, i
     // one-block base kernel, whose 92 KB of shared memory no longer fit beside K1's blocks.)
     cudaError_t e = cudaMemsetAsync(c->d_task, 0, 2 * sizeof(unsigned long long), st);
     if (e != cudaSuccess) return e;
-    const int kw1 = bounds_warps(c);
+    const int kw1 = bounds_warps(c, n_cand);
     const size_t smem = bounds_smem_bytes(c, kw1);
     // tensor map over this call's permutation matrix: [n_cand][n_orders] int32, box 32 x 32
     PFN_cuTensorMapEncodeTiled encode = tensor_map_encoder();
@@ -1411,9 +1420,10 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const void* d_perms, i
     const unsigned blocks = (unsigned)((n_cand + 32 * kw1 - 1) / (32 * kw1));
 #define WHP_LAUNCH_BOUNDS_T(KW1, U16V)                                                          \
   do {                                                                                          \
-    cudaFuncSetAttribute(whp_bounds_kernel<KW1, U16V>,                                          \
+    constexpr int kSt_ = KW1 == 5 ? kStagesWide : kStages;                                      \
+    cudaFuncSetAttribute(whp_bounds_kernel<KW1, U16V, kSt_>,                                    \
                          cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin - 1024);    \
-    whp_bounds_kernel<KW1, U16V><<<blocks, 32 * KW1, smem, st>>>(                               \
+    whp_bounds_kernel<KW1, U16V, kSt_><<<blocks, 32 * KW1, smem, st>>>(                         \
         tmap, tmap_cs, order_table, c->n_orders, c->C, n_cand, c->d_bmask, bm_pitch,            \
         c->d_cstream, cs_pitch);                                                                \
   } while (0)
@@ -1423,6 +1433,7 @@ static cudaError_t launch_bounds_and_segments(whp_ctx* c, const void* d_perms, i
   } while (0)
     if (kw1 == 1) WHP_LAUNCH_BOUNDS(1);
     else if (kw1 == 2) WHP_LAUNCH_BOUNDS(2);
+    else if (kw1 == 5) WHP_LAUNCH_BOUNDS(5);
     else WHP_LAUNCH_BOUNDS(4);
 #undef WHP_LAUNCH_BOUNDS_T
 #undef WHP_LAUNCH_BOUNDS
