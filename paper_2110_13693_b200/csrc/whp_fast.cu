@@ -623,6 +623,7 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       uint32_t rec = SMEM_TABLES ? lds32(cur) : pair_lo;
       uint32_t kmax = 0, kmin = 0xffffffffu;
       uint32_t cset = 0;  // KW == 1: class set of the batch
+      int m = 0;          // distinct aisles of the batch, counted as they arrive
       // Branch-free step: every lane runs Cmax steps. A lane that has finished its batch stays
       // on the batch's final pick and re-inserts it (set inserts and max are idempotent); a
       // lane without a batch walks to the end of order 0 and stays there — its sets are
@@ -654,14 +655,18 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         if (!DEPOT0) kmin = min(kmin, rec);
         const uint32_t aaddr = abase | ((rec >> 20) & amask);
         if (KW == 1) {  // up to 32 classes: the batch's class set is one register
-          sts32(aaddr, lds32(aaddr) | one_shl_wrap(rec >> 22));
+          const uint32_t aw = lds32(aaddr), an = aw | one_shl_wrap(rec >> 22);
+          m += (an != aw) ? 1 : 0;
+          sts32(aaddr, an);
           cset |= one_shl_wrap(rec);
         } else {
           // the aisle word and the class word are different words: both loads go out before
           // either store, so a step waits for one shared-memory round trip instead of two
           const uint32_t caddr = cbase | (rec & 0x380u);
           const uint32_t aw = lds32(aaddr), cw = lds32(caddr);
-          sts32(aaddr, aw | one_shl_wrap(rec >> 22));
+          const uint32_t an = aw | one_shl_wrap(rec >> 22);
+          m += (an != aw) ? 1 : 0;
+          sts32(aaddr, an);
           sts32(caddr, cw | one_shl_wrap(rec));
         }
         rec = rec_next;
@@ -677,12 +682,8 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
         if (live) lo_prev = p0 >> 3;
       }
       // ---- close the batch: m = distinct aisles, D4; the sets are emptied for the next batch
-      int m = 0;
 #pragma unroll 4
-      for (int w = 0; w < P.aw_words; ++w) {
-        m += __popc(lds32(abase + w * 128));
-        sts32(abase + w * 128, 0u);
-      }
+      for (int w = 0; w < P.aw_words; ++w) sts32(abase + w * 128, 0u);
       if (live) {
         const uint32_t a_max = WHP_FAST_AISLE(kmax);
         const uint32_t slot1 = WHP_FAST_SLOT1(kmax);
@@ -803,6 +804,13 @@ whp_sets_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
 // inserts of a step cover the latency of the next load. The last record of an order's last four
 // carries WHP_FAST_LAST4; a lane whose batch is exhausted keeps re-inserting its last four. The
 // step loop ends when no lane of the warp has a four left.
+__device__ __forceinline__ void lds64(uint32_t& lo, uint32_t& hi, uint32_t a) {
+  asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(lo), "=r"(hi) : "r"(a));
+}
+__device__ __forceinline__ void lds64_if(uint32_t& lo, uint32_t& hi, uint32_t a, bool p) {
+  asm volatile("{ .reg .pred pq; setp.ne.u32 pq, %3, 0; @pq ld.shared.v2.u32 {%0, %1}, [%2]; }"
+               : "+r"(lo), "+r"(hi) : "r"(a), "r"((uint32_t)p));
+}
 __device__ __forceinline__ void ldg_four_if(uint4& q, const uint32_t* ptr, bool p) {
   asm volatile("{ .reg .pred pq; setp.ne.u32 pq, %5, 0; @pq ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4]; }"
                : "+r"(q.x), "+r"(q.y), "+r"(q.z), "+r"(q.w) : "l"(ptr), "r"((uint32_t)p));
@@ -918,7 +926,14 @@ whp_sets4_kernel(const whp_tables T, const sets_params P, const uint32_t* __rest
       const uint32_t v_end = live ? 2u * (uint32_t)p : v;
       uint32_t cur4 = lds16(ringbase + (v & P.ring_mask));  // the four being loaded
       v += live ? 2u : 0u;
-      uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));  // first four of the next order
+      // look-ahead cursors come four at a time (one 8-byte read per four orders: a quarter of
+      // the lanes take part in it, so it costs about one wavefront instead of two)
+      uint32_t cw_lo, cw_hi;
+      lds64(cw_lo, cw_hi, ringbase + (v & P.ring_mask & ~6u));
+      auto cursor_at = [&](uint32_t vv) {  // the 16-bit cursor of position vv / 2 out of (cw_lo, cw_hi)
+        return __byte_perm(cw_lo, cw_hi, (vv & 6u) * 0x11u + 0x10u) & 0xffffu;
+      };
+      uint32_t n_c16 = cursor_at(v);  // first four of the next order
       bool have = live;
       // (a lane without a batch keeps the four of its previous batch: its sets are discarded)
       ldg_four_if(q4, pick_f4 + 4 * (size_t)cur4, have);
@@ -950,7 +965,8 @@ whp_sets4_kernel(const whp_tables T, const sets_params P, const uint32_t* __rest
         have = have && (!last4 || next_order);
         cur4 = next_order ? n_c16 : cur4 + 1u;
         v += next_order ? 2u : 0u;
-        lds16_if(n_c16, ringbase + (v & P.ring_mask), next_order);
+        lds64_if(cw_lo, cw_hi, ringbase + (v & P.ring_mask), next_order && (v & 6u) == 0u);
+        n_c16 = cursor_at(v);
         ldg_four_if(q4, pick_f4 + 4 * (size_t)cur4, have);
         insert(r0); insert(r1); insert(r2); insert(r3);
       }
@@ -1474,6 +1490,10 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const void* d_perms, int64_t n_cand
   int warps_cap = 24;
   int S = 1;
   while (S < 32 && ((nb_ub + S - 1) / S > 255 || n_cand * S < 4ll * c->num_sms * warps_cap * 32)) S <<= 1;
+  // every plan has at least n_items / C batches: with eight or more per lane a warp is one plan
+  // (S = 32) whatever the plan count, so K2 finishes D6 itself — no K3 launch and no counter
+  // round trip (stress scale: 9.79 -> 9.58 ms against S = 8)
+  if ((int64_t)c->n_items / c->C >= 256) S = 32;
   if (c->dbg_segments >= 1) {  // whp_debug_set(WHP_DEBUG_SEGMENTS): ignored when not legal
     const int v = c->dbg_segments;
     if (v <= 32 && (v & (v - 1)) == 0 && (nb_ub + v - 1) / v <= 255) S = v;
