@@ -1096,7 +1096,7 @@ whp_sets4_kernel(const whp_tables T, const sets_params P, const uint32_t* __rest
 // (plan, segment), one pick per branch-free step — but a step only adds the leg from the previous
 // pick (D0's walking metric); there are no sets. A cart starts and ends at the depot; a lane
 // that has finished its cart stays on its last pick (a zero leg).
-template <bool SMEM_TABLES>
+template <bool SMEM_TABLES, bool FOURS>
 __global__ void __launch_bounds__(1024, 1)
 whp_legs_kernel(const whp_tables T, const sets_params P, const uint32_t* __restrict__ pick_fast,
                 const uint16_t* __restrict__ cstream, const uint32_t* __restrict__ bmask,
@@ -1162,6 +1162,7 @@ whp_legs_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       lo_prev = c0 - chunks;
     }
     int64_t L = 0;
+    uint4 q4 = make_uint4(0u, 0u, 0u, 0u);
     for (int j = 0; j < nbmax; ++j) {
       int left = 0;
       const int p0 = p;
@@ -1178,35 +1179,12 @@ whp_legs_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
       }
       const bool live = left > 0;
       if (live && (p >> 3) >= lo_prev + chunks) cp_async_wait<0>(); else cp_async_wait<1>();
-      uint32_t v = live ? 2u * (uint32_t)p0 : 0u;
-      const uint32_t v_end = live ? 2u * (uint32_t)p : 0u;
-      uint32_t cur;
-      if (live) {
-        const uint32_t c16 = lds16(ringbase + (v & P.ring_mask));
-        cur = SMEM_TABLES ? pb + 8 * c16 : 2 * c16;
-        v += 2;
-      } else {
-        cur = SMEM_TABLES ? pb : 0u;
-      }
-      uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));
-      uint32_t rec = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
       // the cart sets out from the depot
       int32_t pa = a0;
       int64_t py = 0, Lb = 0;
       uint32_t Lb32 = 0;
       int32_t py32 = 0;
-#pragma unroll 2
-      for (int t = 0; t < Cmax; ++t) {
-        const uint32_t first_of_next = SMEM_TABLES ? pb + 8 * n_c16 : 2 * n_c16;
-        const bool last = (int32_t)(rec << 26) < 0;
-        const bool more = last && (v != v_end);
-        uint32_t nxt = last ? cur : cur + (SMEM_TABLES ? 4u : 1u);
-        nxt = more ? first_of_next : nxt;
-        v = more ? v + 2 : v;
-        lds16_if(n_c16, ringbase + (v & P.ring_mask), more);
-        cur = nxt;
-        const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
-        // ---- the leg from the previous point to this pick
+      auto walk = [&](uint32_t rec) {  // the leg from the previous point to this pick
         const int32_t a = (int32_t)WHP_FAST_AISLE(rec);
         if (P.fits32) {
           const int32_t y = (int32_t)WHP_FAST_SLOT1(rec) * (int32_t)pitch;
@@ -1223,7 +1201,58 @@ whp_legs_kernel(const whp_tables T, const sets_params P, const uint32_t* __restr
           py = y;
         }
         pa = a;
-        rec = rec_next;
+      };
+      if (FOURS) {
+        // the four-aligned table (as in whp_sets4_kernel): a step is one 16-byte load = four picks;
+        // padding copies and a lane whose cart is exhausted walk to the point they stand on
+        uint32_t v = 2u * (uint32_t)p0;
+        const uint32_t v_end = live ? 2u * (uint32_t)p : v;
+        uint32_t cur4 = lds16(ringbase + (v & P.ring_mask));
+        v += live ? 2u : 0u;
+        uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));
+        bool fresh = live;  // q4 holds (or is about to receive) a four that has not been walked
+        uint32_t stay = 0;  // the last pick walked
+        ldg_four_if(q4, pick_fast + 4 * (size_t)cur4, fresh);
+        while (__any_sync(WHP_FULL, fresh)) {
+          const uint32_t r0 = fresh ? q4.x : stay, r1 = fresh ? q4.y : stay;
+          const uint32_t r2 = fresh ? q4.z : stay, r3 = fresh ? q4.w : stay;
+          stay = r3;
+          const bool last4 = (r3 & WHP_FAST_LAST4) != 0u;
+          const bool next_order = last4 && (v != v_end);
+          fresh = fresh && (!last4 || next_order);
+          cur4 = next_order ? n_c16 : cur4 + 1u;
+          v += next_order ? 2u : 0u;
+          lds16_if(n_c16, ringbase + (v & P.ring_mask), next_order);
+          ldg_four_if(q4, pick_fast + 4 * (size_t)cur4, fresh);
+          walk(r0); walk(r1); walk(r2); walk(r3);
+        }
+      } else {
+        uint32_t v = live ? 2u * (uint32_t)p0 : 0u;
+        const uint32_t v_end = live ? 2u * (uint32_t)p : 0u;
+        uint32_t cur;
+        if (live) {
+          const uint32_t c16 = lds16(ringbase + (v & P.ring_mask));
+          cur = SMEM_TABLES ? pb + 8 * c16 : 2 * c16;
+          v += 2;
+        } else {
+          cur = SMEM_TABLES ? pb : 0u;
+        }
+        uint32_t n_c16 = lds16(ringbase + (v & P.ring_mask));
+        uint32_t rec = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
+  #pragma unroll 2
+        for (int t = 0; t < Cmax; ++t) {
+          const uint32_t first_of_next = SMEM_TABLES ? pb + 8 * n_c16 : 2 * n_c16;
+          const bool last = (int32_t)(rec << 26) < 0;
+          const bool more = last && (v != v_end);
+          uint32_t nxt = last ? cur : cur + (SMEM_TABLES ? 4u : 1u);
+          nxt = more ? first_of_next : nxt;
+          v = more ? v + 2 : v;
+          lds16_if(n_c16, ringbase + (v & P.ring_mask), more);
+          cur = nxt;
+          const uint32_t rec_next = SMEM_TABLES ? lds32(cur) : __ldg(pick_fast + cur);
+          walk(rec);
+          rec = rec_next;
+        }
       }
       {
         const int nf = live ? (p >> 3) - (p0 >> 3) : 0;
@@ -1656,7 +1685,9 @@ cudaError_t whp_launch_legsum_fast(whp_ctx* c, const int32_t* d_perms, int64_t n
   const int64_t worst = ((int64_t)c->C + 2) * ((int64_t)c->g.aisle_spacing * c->g.n_aisles + 2 * c->g.aisle_len);
   cudaError_t e = ensure_fast_scratch(c, n_cand, 0, st);
   if (e != cudaSuccess) return e;
-  if ((e = launch_bounds_and_segments(c, d_perms, n_cand, S, log2S, nullptr, st)) != cudaSuccess) return e;
+  const bool fours = !smem_tables && c->d_pick_f4 != nullptr && !c->dbg_no_fours;  // as in K2'
+  if ((e = launch_bounds_and_segments(c, d_perms, n_cand, S, log2S, nullptr, st, false,
+                                      fours ? c->d_order_fast4 : nullptr)) != cudaSuccess) return e;
   sets_params P{};
   P.S = S; P.log2S = log2S; P.ring_mask = ring_bytes - 1;
   P.bm_pitch = fast_bm_pitch(c); P.cs_pitch = fast_cs_pitch(c); P.ss_pitch = kSsPitch;
@@ -1666,12 +1697,16 @@ cudaError_t whp_launch_legsum_fast(whp_ctx* c, const int32_t* d_perms, int64_t n
   if (blocks > c->num_sms) blocks = c->num_sms;
   const size_t smem = (smem_tables ? table_bytes : 0) + priv_per_warp * warps;
   if (smem_tables) {
-    cudaFuncSetAttribute(whp_legs_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
-    whp_legs_kernel<true><<<(unsigned)blocks, warps * 32, smem, st>>>(
+    cudaFuncSetAttribute(whp_legs_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+    whp_legs_kernel<true, false><<<(unsigned)blocks, warps * 32, smem, st>>>(
         T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand, d_len, c->d_task);
+  } else if (fours) {
+    cudaFuncSetAttribute(whp_legs_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+    whp_legs_kernel<false, true><<<(unsigned)blocks, warps * 32, smem, st>>>(
+        T, P, c->d_pick_f4, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand, d_len, c->d_task);
   } else {
-    cudaFuncSetAttribute(whp_legs_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
-    whp_legs_kernel<false><<<(unsigned)blocks, warps * 32, smem, st>>>(
+    cudaFuncSetAttribute(whp_legs_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max);
+    whp_legs_kernel<false, false><<<(unsigned)blocks, warps * 32, smem, st>>>(
         T, P, c->d_pick_fast, c->d_cstream, c->d_bmask, c->d_nb, c->d_segstart, n_cand, d_len, c->d_task);
   }
   c->launches += 1;

@@ -276,12 +276,15 @@ def test_tables_beyond_shared_memory_both_set_kernels(torch_cuda, cfg):
             ctx.eval_candidates(d_perms, resp=resp)
             torch.cuda.synchronize()
             assert np.array_equal(resp.cpu().numpy(), ref["resp"])
-    ctx.debug_set(whp.DEBUG_NO_FOURS, -1)
     ctx.debug_set(whp.DEBUG_SEGMENTS, -1)
-    leg = torch.full((37,), -1, dtype=torch.int64, device="cuda")
-    ctx.eval_legsum(d_perms, leg)  # the leg kernel keeps the pair layout
-    torch.cuda.synchronize()
-    assert np.array_equal(leg.cpu().numpy(), oracle.eval_legsum(pb, perms))
+    want = oracle.eval_legsum(pb, perms)
+    for no_fours in (0, 1):  # the leg kernel has both layouts too
+        ctx.debug_set(whp.DEBUG_NO_FOURS, no_fours)
+        leg = torch.full((37,), -1, dtype=torch.int64, device="cuda")
+        ctx.eval_legsum(d_perms, leg)
+        torch.cuda.synchronize()
+        assert np.array_equal(leg.cpu().numpy(), want)
+    ctx.debug_set(whp.DEBUG_NO_FOURS, -1)
     ctx.close()
 
 
