@@ -304,6 +304,82 @@ whp_bounds_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constan
   if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // tiles still being read
 }
 
+// The register path of whp_segments_kernel: lane l owns the 4*W4 consecutive mask words from
+// 4*W4*l on (16-byte loads), so one warp scan over the lanes' totals ranks every word; a segment
+// then finds its lane by a shuffle binary search, the word inside that lane from the lane's
+// packed per-word counts, and the bit by clearing the lower ones.
+template <int W4>
+__device__ __forceinline__ void segments_in_registers(
+    const uint32_t* __restrict__ bm, int32_t bm_pitch, int32_t n_orders, int nw, int lane, int32_t S,
+    int32_t log2S, int64_t c, int32_t* __restrict__ nb_scratch, int32_t* __restrict__ n_batches_out,
+    int32_t* __restrict__ segstart, int32_t ss_pitch) {
+  constexpr int W = 4 * W4;
+  uint32_t x[W], pk[W4];
+  const int w0 = lane * W;
+  const int ws = n_orders >> 5;  // the word that also holds the end sentinel (n_orders % 32 != 0)
+  int tot = 0;
+#pragma unroll
+  for (int i4 = 0; i4 < W4; ++i4) {
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (w0 + 4 * i4 < bm_pitch) v = __ldg(reinterpret_cast<const uint4*>(bm + w0 + 4 * i4));
+    x[4 * i4 + 0] = v.x; x[4 * i4 + 1] = v.y; x[4 * i4 + 2] = v.z; x[4 * i4 + 3] = v.w;
+    pk[i4] = 0u;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int w = w0 + 4 * i4 + k;
+      uint32_t xi = x[4 * i4 + k];
+      if (w >= nw) xi = 0u;
+      else if (w == ws) xi &= (1u << (n_orders & 31)) - 1u;  // drop the end sentinel
+      x[4 * i4 + k] = xi;
+      const int pc = __popc(xi);
+      pk[i4] |= (uint32_t)pc << (8 * k);
+      tot += pc;
+    }
+  }
+  int incl = tot;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const int y = __shfl_up_sync(WHP_FULL, incl, d);
+    if (lane >= d) incl += y;
+  }
+  const int nb = __shfl_sync(WHP_FULL, incl, 31);
+  if (lane == 0) {
+    nb_scratch[c] = nb;
+    if (n_batches_out) n_batches_out[c] = nb;
+  }
+  const int target = (int)(((int64_t)lane * nb) >> log2S);  // lane = segment
+  int lo = 0, hi = 31;  // smallest lane whose inclusive count exceeds the target
+#pragma unroll
+  for (int it = 0; it < 5; ++it) {
+    const int mid = (lo + hi) >> 1;
+    const int im = __shfl_sync(WHP_FULL, incl, mid);
+    if (im > target) hi = mid; else lo = mid + 1;
+  }
+  int r = target - __shfl_sync(WHP_FULL, incl - tot, lo);  // rank inside that lane's words
+  int j = -1;
+#pragma unroll
+  for (int i4 = 0; i4 < W4; ++i4) {
+    const uint32_t p = __shfl_sync(WHP_FULL, pk[i4], lo);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int pc = (int)((p >> (8 * k)) & 0xffu);
+      if (j < 0) {
+        if (r < pc) j = 4 * i4 + k; else r -= pc;
+      }
+    }
+  }
+  uint32_t t = 0u;
+#pragma unroll
+  for (int i = 0; i < W; ++i) {
+    const uint32_t xi = __shfl_sync(WHP_FULL, x[i], lo);
+    if (i == j) t = xi;
+  }
+  if (lane < S && j >= 0) {
+    for (; r > 0; --r) t &= t - 1;
+    segstart[c * ss_pitch + lane] = 32 * (lo * W + j) + __ffs(t) - 1;
+  }
+}
+
 // One warp per plan: number of batches, and the first position of every segment (segment s
 // starts with batch floor(s * nb / S)).
 __global__ void __launch_bounds__(256)
@@ -323,49 +399,14 @@ whp_segments_kernel(const uint32_t* __restrict__ bmask, int32_t bm_pitch, int32_
     if (w == (n_orders >> 5)) x &= (1u << (n_orders & 31)) - 1u;  // drop the end sentinel
     return x;
   };
-  if (nw <= 128) {
-    // up to four 32-word chunks: one pass over the mask, everything kept in registers
-    uint32_t x[4];
-    int incl[4], tot[4];
-    int nb = 0;
-#pragma unroll
-    for (int ch = 0; ch < 4; ++ch) {
-      x[ch] = word_at(32 * ch + lane);
-      int v = __popc(x[ch]);
-#pragma unroll
-      for (int d = 1; d < 32; d <<= 1) {
-        const int y = __shfl_up_sync(WHP_FULL, v, d);
-        if (lane >= d) v += y;
-      }
-      incl[ch] = v;
-      tot[ch] = __shfl_sync(WHP_FULL, v, 31);
-      nb += tot[ch];
-    }
-    if (lane == 0) {
-      nb_scratch[c] = nb;
-      if (n_batches_out) n_batches_out[c] = nb;
-    }
-    const int target = (int)(((int64_t)lane * nb) >> log2S);  // lane = segment
-    int base = 0;
-#pragma unroll
-    for (int ch = 0; ch < 4; ++ch) {
-      int lo = 0, hi = 31;  // smallest j with base + incl_j > target
-#pragma unroll
-      for (int it = 0; it < 5; ++it) {
-        const int mid = (lo + hi) >> 1;
-        const int im = __shfl_sync(WHP_FULL, incl[ch], mid);
-        if (base + im > target) hi = mid; else lo = mid + 1;
-      }
-      const uint32_t xj = __shfl_sync(WHP_FULL, x[ch], lo);
-      const int ej = __shfl_sync(WHP_FULL, incl[ch] - __popc(x[ch]), lo);
-      if (lane < S && target >= base && target < base + tot[ch]) {
-        uint32_t t = xj;
-        for (int r = target - base - ej; r > 0; --r) t &= t - 1;
-        segstart[c * ss_pitch + lane] = 32 * (32 * ch + lo) + __ffs(t) - 1;
-      }
-      base += tot[ch];
-    }
-    return;
+  // masks of up to 640 words: lane l keeps words 4*W4*l .. 4*W4*(l+1)-1 in registers
+  switch ((nw + 127) >> 7) {
+    case 1: segments_in_registers<1>(bm, bm_pitch, n_orders, nw, lane, S, log2S, c, nb_scratch, n_batches_out, segstart, ss_pitch); return;
+    case 2: segments_in_registers<2>(bm, bm_pitch, n_orders, nw, lane, S, log2S, c, nb_scratch, n_batches_out, segstart, ss_pitch); return;
+    case 3: segments_in_registers<3>(bm, bm_pitch, n_orders, nw, lane, S, log2S, c, nb_scratch, n_batches_out, segstart, ss_pitch); return;
+    case 4: segments_in_registers<4>(bm, bm_pitch, n_orders, nw, lane, S, log2S, c, nb_scratch, n_batches_out, segstart, ss_pitch); return;
+    case 5: segments_in_registers<5>(bm, bm_pitch, n_orders, nw, lane, S, log2S, c, nb_scratch, n_batches_out, segstart, ss_pitch); return;
+    default: break;
   }
   int nb = 0;
   for (int w0 = 0; w0 < nw; w0 += 32) nb += __reduce_add_sync(WHP_FULL, __popc(word_at(w0 + lane)));
