@@ -858,7 +858,7 @@ __device__ __forceinline__ void ldg_four_if(uint4& q, const uint32_t* ptr, bool 
 }
 
 template <bool DEPOT0, int KW, int kPlanes>
-__global__ void __launch_bounds__(KW * kPlanes <= 42 ? 768 : 512, 1)  // counter registers: KW x planes
+__global__ void __launch_bounds__(KW * kPlanes <= 16 ? 768 : 512, 1)  // the four records of a step + KW x planes counters
 whp_sets4_kernel(const whp_tables T, const sets_params P, const uint32_t* __restrict__ pick_f4,
                 const uint16_t* __restrict__ cstream, const uint32_t* __restrict__ bmask,
                 const int32_t* __restrict__ nb_scratch, const int32_t* __restrict__ segstart,
@@ -1573,7 +1573,7 @@ cudaError_t whp_launch_eval_fast(whp_ctx* c, const void* d_perms, int64_t n_cand
   int seg_planes = 1;  // planes of one segment's counters; one more per combine level
   while ((1ll << seg_planes) <= (nb_ub + S - 1) / S) ++seg_planes;
   const int kernel_planes = seg_planes <= 4 ? 4 : seg_planes <= 6 ? 6 : 8;  // the instantiation
-  if (KW * kernel_planes > 42) warps_cap = 16;  // __launch_bounds__ of the register-heavy instantiations
+  if (KW * kernel_planes > (fours ? 16 : 42)) warps_cap = 16;  // __launch_bounds__ of the register-heavy instantiations
   int warps = (int)(avail / priv_per_warp);
   if (warps > warps_cap) warps = warps_cap;
   if (c->dbg_warps >= 1 && c->dbg_warps <= warps) warps = c->dbg_warps;  // WHP_DEBUG_WARPS
