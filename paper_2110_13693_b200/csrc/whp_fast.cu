@@ -71,7 +71,9 @@ __device__ __forceinline__ void dep_trigger() { asm volatile("griddepcontrol.lau
 // conflict-free. The loop is software-pipelined by hand — while the recurrence runs over word w,
 // the order ids of word w+1 leave the tile and their order records are gathered from the table
 // in shared memory — so that a lone warp per scheduler keeps issuing.
-constexpr int kStages = 7;           // tiles (words) in flight per warp
+constexpr int kStages = 6;           // tiles (words) in flight per warp (seven are no faster alone
+                                     // and leave four one-warp blocks 12 KB of an SM's shared memory:
+                                     // with six, two blocks of another stream's kernel fit beside them)
 constexpr int kStagesWide = 5;       // ... of the five-warp block (multi-wave launches, see bounds_shape)
 constexpr int kTileBytes = 32 * 128; // 32 rows x 32 positions x 4 B
 
