@@ -252,6 +252,9 @@ BIG_TABLES = [
     dict(NA=400, S=250, K=200, n_skus=20000, n_orders=12000, qmax=7, C=30, depot=123),  # 7 class words
     dict(NA=1024, S=100, K=64, n_skus=9000, n_orders=30000, qmax=1, C=17, pitch=2),     # one-pick orders
     dict(NA=90, S=4095, K=256, n_skus=9000, n_orders=9000, qmax=13, C=64, spacing=9),   # many fours an order
+    dict(NA=700, S=60, K=17, n_skus=30000, n_orders=10001, qmax=9, C=106, depot=699),   # largest cart, padded plans
+    dict(NA=33, S=9, K=1, n_skus=500, n_orders=600, qmax=255, C=255),                   # 64 fours an order
+    dict(NA=1024, S=4095, K=32, n_skus=60000, n_orders=50000, qmax=2, C=12, spacing=11), # ~6,500 carts a plan
 ]
 
 
